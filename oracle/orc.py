@@ -1,0 +1,275 @@
+"""ctypes wrapper around oracle/orc.c -- CPU ORACLE, TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this module.  It never imports the product package.
+
+`build()` compiles orc.c with gcc into oracle/liborc.so (a few seconds); every
+wrapper below only marshals numpy arrays into the C calls declared in orc.h.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "liborc.so")
+_SRC = os.path.join(_HERE, "orc.c")
+_HDR = os.path.join(_HERE, "orc.h")
+
+PSD_KOLMOGOROV, PSD_VON_KARMAN, PSD_OCEAN_NIKISHOV = 0, 1, 2
+H_FRESNEL, H_ANGULAR_SPECTRUM = 0, 1
+
+
+class _Psd(C.Structure):
+    _fields_ = [("kind", C.c_int), ("L0", C.c_double), ("l0", C.c_double),
+                ("km_coeff", C.c_double), ("chi_T", C.c_double), ("eps", C.c_double),
+                ("w", C.c_double), ("eta", C.c_double)]
+
+
+class _Stats(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("power", "cx", "cy", "sxx", "syy", "sxy", "w2",
+                                           "I_axis", "roi_sumI", "roi_sumI2")] + \
+               [("roi_n", C.c_longlong)]
+
+
+@dataclass
+class Psd:
+    kind: int = PSD_KOLMOGOROV
+    L0: float = 0.0
+    l0: float = 0.0
+    km_coeff: float = 0.0
+    chi_T: float = 0.0
+    eps: float = 0.0
+    w: float = 0.0
+    eta: float = 0.0
+
+    def c(self) -> _Psd:
+        return _Psd(self.kind, self.L0, self.l0, self.km_coeff, self.chi_T, self.eps, self.w, self.eta)
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle (gcc -O2, strict IEEE: no -ffast-math)."""
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_HDR))
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < newest:
+        tmp = _SO + ".tmp%d" % os.getpid()
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _SO)
+    return _SO
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_psd_f.restype = C.c_double
+        _lib.orc_r0.restype = C.c_double
+    return _lib
+
+
+def _p(a, ty=C.c_double):
+    return a.ctypes.data_as(C.POINTER(ty)) if a is not None else None
+
+
+def _c128(a):
+    return np.ascontiguousarray(a, dtype=np.complex128)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _chk(rc, what):
+    if rc != 0:
+        raise RuntimeError(f"oracle {what} failed rc={rc}")
+
+
+# ---- P0 ---------------------------------------------------------------------
+def fft1d(a, sign=-1):
+    a = _c128(a).copy()
+    _chk(lib().orc_fft1d(_p(a), C.c_int(a.shape[-1]), C.c_int(sign)), "fft1d")
+    return a
+
+
+def dft1d_naive(a, sign=-1):
+    a = _c128(a).copy()
+    _chk(lib().orc_dft1d_naive(_p(a), C.c_int(a.shape[-1]), C.c_int(sign)), "dft1d_naive")
+    return a
+
+
+def fft2d(a, sign=-1):
+    a = _c128(a).copy()
+    assert a.ndim == 2 and a.shape[0] == a.shape[1]
+    _chk(lib().orc_fft2d(_p(a), C.c_int(a.shape[0]), C.c_int(sign)), "fft2d")
+    return a
+
+
+# ---- O2 ---------------------------------------------------------------------
+def r0(lam, cn2, dz):
+    return lib().orc_r0(C.c_double(lam), C.c_double(cn2), C.c_double(dz))
+
+
+def psd_f(psd: Psd, lam, cn2, dz, f):
+    pc = psd.c()
+    fn = lib().orc_psd_f
+    f = np.atleast_1d(np.asarray(f, dtype=np.float64))
+    out = np.array([fn(C.byref(pc), C.c_double(lam), C.c_double(cn2), C.c_double(dz), C.c_double(x))
+                    for x in f.ravel()])
+    return out.reshape(f.shape)
+
+
+# ---- O3-O5 ------------------------------------------------------------------
+def make_screens(N, dx, psd: Psd, lam, cn2, dz, n_sh, noise, noise_sh, keep_spectrum=True):
+    """noise: float32 [B][S][N][N][2]; noise_sh: float32 [B][S][n_sh][3][3][2] (or None).
+    Returns (screens f64 [B][S][N][N], spectrum c128 or None, sh_coef c128 or None)."""
+    noise = _f32(noise)
+    B, S = noise.shape[0], noise.shape[1]
+    cn2, dz = _f64(cn2), _f64(dz)
+    assert cn2.shape == (S,) and dz.shape == (S,)
+    screens = np.empty((B, S, N, N), dtype=np.float64)
+    spectrum = np.empty((B, S, N, N), dtype=np.complex128) if keep_spectrum else None
+    sh = np.zeros((B, S, max(n_sh, 1), 3, 3), dtype=np.complex128) if n_sh > 0 else None
+    nsh = _f32(noise_sh) if n_sh > 0 else None
+    pc = psd.c()
+    _chk(lib().orc_make_screens(C.c_int(N), C.c_double(dx), C.byref(pc), C.c_double(lam),
+                                C.c_int(B), C.c_int(S), _p(cn2), _p(dz), C.c_int(n_sh),
+                                _p(noise, C.c_float), _p(nsh, C.c_float),
+                                _p(spectrum), _p(sh), _p(screens)), "make_screens")
+    return screens, spectrum, sh
+
+
+def synthesize(N, dx, n_sh, spectrum, sh_coef):
+    spectrum = _c128(spectrum)
+    B, S = spectrum.shape[0], spectrum.shape[1]
+    sh = _c128(sh_coef) if n_sh > 0 else None
+    screens = np.empty((B, S, N, N), dtype=np.float64)
+    _chk(lib().orc_synthesize(C.c_int(N), C.c_double(dx), C.c_int(B), C.c_int(S), C.c_int(n_sh),
+                              _p(spectrum), _p(sh), _p(screens)), "synthesize")
+    return screens
+
+
+def evolve_screens(N, dx, psd: Psd, lam, cn2, dz, n_sh, a, vx, vy, T, fresh, fresh_sh,
+                   spectrum, sh_coef):
+    """Updates spectrum / sh_coef IN PLACE (must be contiguous c128) and returns the screens."""
+    fresh = _f32(fresh)
+    B, S = fresh.shape[0], fresh.shape[1]
+    assert spectrum.dtype == np.complex128 and spectrum.flags.c_contiguous
+    cn2, dz = _f64(cn2), _f64(dz)
+    screens = np.empty((B, S, N, N), dtype=np.float64)
+    fsh = _f32(fresh_sh) if n_sh > 0 else None
+    if n_sh > 0:
+        assert sh_coef.dtype == np.complex128 and sh_coef.flags.c_contiguous
+    pc = psd.c()
+    _chk(lib().orc_evolve_screens(C.c_int(N), C.c_double(dx), C.byref(pc), C.c_double(lam),
+                                  C.c_int(B), C.c_int(S), _p(cn2), _p(dz), C.c_int(n_sh),
+                                  C.c_double(a), C.c_double(vx), C.c_double(vy), C.c_double(T),
+                                  _p(fresh, C.c_float), _p(fsh, C.c_float),
+                                  _p(spectrum), _p(sh_coef) if n_sh > 0 else None, _p(screens)),
+         "evolve_screens")
+    return screens
+
+
+# ---- O6-O7 ------------------------------------------------------------------
+def _screen_args(screens, B, N, shared):
+    if screens is None:
+        return None, 0, 0
+    screens = _f64(screens)
+    if shared:
+        assert screens.ndim == 3
+        return screens, 0, screens.shape[0]
+    assert screens.ndim == 4 and screens.shape[0] == B
+    return screens, screens.shape[1] * N * N, screens.shape[1]
+
+
+def propagate(N, dx, lam, dz, field, screens=None, shared_screens=False, win_order=0,
+              win_sigma_frac=0.47, n0=1.0, h_kind=H_FRESNEL, return_planes=False):
+    field = _c128(field)
+    B = field.shape[0]
+    dz = _f64(dz)
+    n_steps = dz.shape[0]
+    scr, stride, S = _screen_args(screens, B, N, shared_screens)
+    out = np.empty_like(field)
+    planes = np.empty((B, n_steps, N, N), dtype=np.complex128) if return_planes else None
+    _chk(lib().orc_propagate(C.c_int(N), C.c_double(dx), C.c_double(lam), C.c_double(n0),
+                             C.c_int(B), C.c_int(n_steps), _p(dz), _p(scr), C.c_longlong(stride),
+                             C.c_int(S), C.c_int(win_order), C.c_double(win_sigma_frac),
+                             C.c_int(h_kind), _p(field), _p(out), _p(planes)), "propagate")
+    return (out, planes) if return_planes else out
+
+
+def propagate_adjoint(N, dx, lam, dz, g_out, screens=None, shared_screens=False, win_order=0,
+                      win_sigma_frac=0.47, n0=1.0, h_kind=H_FRESNEL, planes=None):
+    g_out = _c128(g_out)
+    B = g_out.shape[0]
+    dz = _f64(dz)
+    n_steps = dz.shape[0]
+    scr, stride, S = _screen_args(screens, B, N, shared_screens)
+    g_in = np.empty_like(g_out)
+    grad = None
+    if planes is not None:
+        planes = _c128(planes)
+        assert planes.shape == (B, n_steps, N, N)
+        grad = np.zeros((B, max(S, 1), N, N), dtype=np.float64)
+    _chk(lib().orc_propagate_adjoint(C.c_int(N), C.c_double(dx), C.c_double(lam), C.c_double(n0),
+                                     C.c_int(B), C.c_int(n_steps), _p(dz), _p(scr),
+                                     C.c_longlong(stride), C.c_int(S), C.c_int(win_order),
+                                     C.c_double(win_sigma_frac), C.c_int(h_kind),
+                                     _p(g_out), _p(g_in), _p(planes), _p(grad)), "propagate_adjoint")
+    return (g_in, grad) if planes is not None else g_in
+
+
+# ---- O8 ---------------------------------------------------------------------
+STAT_FIELDS = ("power", "cx", "cy", "sxx", "syy", "sxy", "w2", "I_axis", "roi_sumI", "roi_sumI2", "roi_n")
+
+
+def beam_stats(N, dx, field, roi_frac=0.5):
+    field = _c128(field)
+    B = field.shape[0]
+    arr = (_Stats * B)()
+    _chk(lib().orc_beam_stats(C.c_int(N), C.c_double(dx), C.c_int(B), _p(field),
+                              C.c_double(roi_frac), arr), "beam_stats")
+    return [{k: getattr(arr[b], k) for k in STAT_FIELDS} for b in range(B)]
+
+
+def welford(N, field, mean, M2, count):
+    """mean / M2: float64 [N][N] updated in place; returns the new count."""
+    field = _c128(field)
+    cnt = C.c_longlong(count)
+    _chk(lib().orc_welford(C.c_int(N), C.c_int(field.shape[0]), _p(field), _p(mean), _p(M2),
+                           C.byref(cnt)), "welford")
+    return cnt.value
+
+
+# ---- O9 ---------------------------------------------------------------------
+def phase_mul(N, theta, field, sign=1.0):
+    field = _c128(field)
+    theta = _f64(theta)
+    out = np.empty_like(field)
+    _chk(lib().orc_phase_mul(C.c_int(N), C.c_int(field.shape[0]), _p(theta), C.c_double(sign),
+                             _p(field), _p(out)), "phase_mul")
+    return out
+
+
+def dft2_centered(N, field, inverse=False):
+    field = _c128(field)
+    out = np.empty_like(field)
+    _chk(lib().orc_dft2_centered(C.c_int(N), C.c_int(field.shape[0]), C.c_int(int(inverse)),
+                                 _p(field), _p(out)), "dft2_centered")
+    return out
+
+
+def phase_grad(N, g, u):
+    g, u = _c128(g), _c128(u)
+    out = np.empty(g.shape, dtype=np.float64)
+    _chk(lib().orc_phase_grad(C.c_int(N), C.c_int(g.shape[0]), _p(g), _p(u), _p(out)), "phase_grad")
+    return out
