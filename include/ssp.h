@@ -1,0 +1,210 @@
+/*
+ * ssp.h -- C ABI of the B200-native split-step phase-screen propagation library.
+ *
+ * The product boundary.  Every entry point is `extern "C"`, takes plain pointers and
+ * sizes (no torch types) and runs entirely in hand-written sm_100a CUDA kernels; there
+ * is no CPU fallback.  Citations are "PAPER.md:<line>" of the TurPy paper
+ * (arxiv 2604.07248) plus the equation; "Qn" are the readings listed in DESIGN.md
+ * section 3.
+ *
+ * Conventions
+ *   - Grids are square, N a power of two, 8 <= N <= 4096.  Arrays are row-major with x
+ *     fastest: idx = ((b*S + s)*N + iy)*N + ix.  complex64 = interleaved (re, im) fp32.
+ *   - Coordinates x_i = (i - N/2) dx.  Frequencies are in cycles/m in FFT order with the
+ *     negative Nyquist: f_k = k/(N dx) for k < N/2, (k - N)/(N dx) otherwise.
+ *   - Forward DFT X[k] = sum_n x[n] exp(-i 2 pi k n / N), unnormalised.
+ *   - "dev" pointers are device memory of the context's device, 16-byte aligned, owned by
+ *     the caller (allocate them with torch / cudaMalloc); "host" pointers are read during
+ *     the call and not retained.  The library allocates only small tables inside the
+ *     context and frees them in ssp_destroy.
+ *   - Calls enqueue work on the context's stream and return without synchronising,
+ *     except the *_host entry points, which synchronise the stream before returning.
+ *   - Return value: 0 on success, a negative ssp_status otherwise; ssp_last_error gives
+ *     the text.  After an error no output buffer is guaranteed.  No exception crosses
+ *     the ABI.  A context is not thread-safe.
+ */
+#ifndef SSP_H
+#define SSP_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    SSP_OK = 0,
+    SSP_EINVAL = -1,        /* bad argument: N not a power of two or out of range, null
+                               required pointer, S < 0, S > n_steps, a not in [0,1],
+                               lambda <= 0, dz <= 0, misaligned pointer */
+    SSP_EUNSUPPORTED = -2,  /* valid request this build does not implement */
+    SSP_EWORKSPACE = -3,    /* workspace smaller than ssp_workspace_bytes */
+    SSP_ECUDA = -4          /* CUDA runtime / driver error (text in ssp_last_error) */
+} ssp_status;
+
+typedef struct ssp_ctx ssp_ctx; /* opaque; one per (device, stream) */
+
+typedef struct { int N; double dx; } ssp_grid;
+
+typedef enum {
+    SSP_PSD_KOLMOGOROV = 0,     /* Table S1: S17 with L0 -> inf, l0 -> 0 (Q23) */
+    SSP_PSD_VON_KARMAN = 1,     /* modified von Karman, PAPER.md:370 (S17) */
+    SSP_PSD_OCEAN_NIKISHOV = 2  /* Nikishov oceanic spectrum, open literature (Q20) */
+} ssp_psd_kind;
+
+/* Phase PSD parameters.  Atmospheric kinds evaluate S17 with f in cycles/m:
+ *   Phi^f(f) = 0.023 r0^(-5/3) exp(-f^2/fm^2) / (f^2 + f0^2)^(11/6),
+ *   f0 = 1/L0, fm = km_coeff/(2 pi l0) (km_coeff <= 0 -> 2 pi; Q4, Q5),
+ *   r0 = (0.423 k^2 Cn2 dz)^(-3/5), k = 2 pi/lambda (PAPER.md:375 S18; Q16).
+ * Ocean: Phi^f(f) = (2 pi)^3 k^2 dz Phi_n(2 pi f) with Nikishov's Phi_n; cn2 is ignored;
+ *   eta <= 0 -> (nu^3/eps)^(1/4), nu = 1e-6 m^2/s. */
+typedef struct {
+    int kind;                  /* ssp_psd_kind */
+    double L0, l0, km_coeff;   /* von Karman */
+    double chi_T, eps, w, eta; /* ocean */
+} ssp_psd;
+
+/* Super-Gaussian absorbing window applied after every split step (north_star; Q12):
+ *   W = exp(-((x^2 + y^2)/sigma^2)^(order/2)), sigma = sigma_frac N dx; order <= 0 -> off. */
+typedef struct { int order; double sigma_frac; } ssp_window;
+
+/* Per-realisation intensity statistics (PAPER.md:423 S25, :402 S22; O8 in DESIGN.md):
+ *   power = sum I dx^2; (cx, cy) centroid; sxx, syy, sxy central second moments [m^2];
+ *   w2 = sqrt(2 (sxx + syy)) (= w for I ~ exp(-2 r^2/w^2)); I_axis = I[N/2][N/2];
+ *   ROI = [N/2 - h, N/2 + h)^2, h = floor(roi_frac N / 2) (h = 0 -> the pixel N/2):
+ *   roi_sumI, roi_sumI2, roi_n  ->  spatial SI = roi_n roi_sumI2 / roi_sumI^2 - 1. */
+typedef struct {
+    double power, cx, cy, sxx, syy, sxy, w2, I_axis, roi_sumI, roi_sumI2;
+    long long roi_n;
+} ssp_stats;
+
+/* Transfer function of the diffraction step (Q1). */
+typedef enum {
+    SSP_H_FRESNEL = 0,          /* H = exp(-i pi (lambda/n0) dz (fx^2 + fy^2))  (north_star) */
+    SSP_H_ANGULAR_SPECTRUM = 1  /* PAPER.md:96 Eq.6, carrier removed (Q2) -- SSP_EUNSUPPORTED in this build */
+} ssp_h_kind;
+
+/* ---- context ------------------------------------------------------------------- */
+
+/* Create a context bound to `device` and to `cuda_stream` (a cudaStream_t passed as
+ * void*; NULL = the legacy default stream).  Fails with SSP_ECUDA when no CUDA device
+ * is usable.  The stream must outlive the context. */
+int ssp_create(ssp_ctx **out, int device, void *cuda_stream);
+int ssp_destroy(ssp_ctx *ctx);
+/* Text of the last error on this context ("" if none); valid until the next call. */
+const char *ssp_last_error(const ssp_ctx *ctx);
+/* Library version string, e.g. "ssp 0.1 sm_100a". */
+const char *ssp_version(void);
+/* Number of kernels this context has launched since creation (bench bookkeeping). */
+long long ssp_launch_count(const ssp_ctx *ctx);
+
+/* Bytes of device scratch any call on this (grid, B, S) may need; the caller allocates
+ * it once and passes it to every call.  Independent of the context. */
+size_t ssp_workspace_bytes(ssp_grid grid, int B, int S);
+
+/* ---- screens ------------------------------------------------------------------- */
+
+/* Screen generator (PAPER.md:359 S16; :57 Eq.2; :63 Eq.3; :362):
+ *   C[ky][kx] = (a + i b) sqrt(Phi^f(|f|; dz_s)) df,  C[0][0] = 0,  df = 1/(N dx);
+ *   phi_hi    = Re sum_k C[ky][kx] exp(+i 2 pi (kx ix + ky iy)/N)   (unnormalised; Q3, Q6);
+ *   c_pab     = (a + i b) sqrt(Phi^f(|(b-1, a-1)| df_p)) df_p, df_p = df/3^p, p = 1..n_sh (Q7);
+ *   phi_lo    = sum_p sum_{a,b != centre} Re{ c_pab exp(i 2 pi ((b-1) df_p x + (a-1) df_p y)) };
+ *   phi       = phi_hi + phi_lo - mean(phi_lo).
+ * cn2, dz: host [S] (one slab per screen).  d_noise: dev complex64 [B][S][N][N] of
+ * N(0,1)+iN(0,1) draws; d_noise_sh: dev complex64 [B][S][n_sh][3][3] ([a][b], centre
+ * unused), may be NULL when n_sh == 0.  Outputs: d_spectrum dev complex64 [B][S][N][N]
+ * (the stored Fourier spectrum; may be NULL), d_sh_coef dev complex64
+ * [B][S][n_sh][3][3] (may be NULL), d_screens dev fp32 [B][S][N][N] (required).
+ * d_noise may alias d_spectrum.  0 <= n_sh <= 8. */
+int ssp_make_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
+                     int B, int S, const double *cn2, const double *dz, int n_sh,
+                     const float *d_noise, const float *d_noise_sh,
+                     float *d_spectrum, float *d_sh_coef, float *d_screens,
+                     void *d_ws, size_t ws_bytes);
+
+/* Autoregressive evolution on the stored spectrum (PAPER.md:80 Eq.5, :74 Eq.4; Q8-Q10):
+ *   C <- a tau C + sqrt(1 - a^2) C_fresh,  tau = exp(-i 2 pi T (fx vx + fy vy)),
+ * C_fresh built from the fresh noise exactly as in ssp_make_screens; the subharmonic
+ * coefficients follow the same recursion with tau at their fractional frequency; the
+ * screens are then resynthesised.  d_spectrum, d_sh_coef: in-out.  0 <= a <= 1. */
+int ssp_evolve_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
+                       int B, int S, const double *cn2, const double *dz, int n_sh,
+                       double a, double vx, double vy, double T,
+                       const float *d_fresh_noise, const float *d_fresh_noise_sh,
+                       float *d_spectrum, float *d_sh_coef, float *d_screens,
+                       void *d_ws, size_t ws_bytes);
+
+/* ---- propagation --------------------------------------------------------------- */
+
+/* Split-step propagation (Eq.1; step order Q11):
+ *   for j = 1..n_steps:  U <- F^-1{ F{U} H(dz_j) };  if j <= S: U <- U exp(i phi_j);  U <- U W.
+ * dz: host [n_steps].  d_screens: dev fp32, screen j of field b at
+ * d_screens + b*screen_batch_stride + (j-1)*N*N (stride in elements; 0 = one stack shared
+ * by all fields); may be NULL when S == 0.  0 <= S <= n_steps.
+ * d_field_in / d_field_out: dev complex64 [B][N][N]; may alias.
+ * d_planes: optional dev complex64 [B][n_steps][N][N], the field after each complete step
+ * (needed by the adjoint's phase gradient).  d_stats: optional dev ssp_stats[B] of the
+ * output field with ROI fraction roi_frac. */
+int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind,
+                  int B, int n_steps, const double *dz,
+                  const float *d_screens, long long screen_batch_stride, int S,
+                  ssp_window win, const float *d_field_in, float *d_field_out,
+                  float *d_planes, ssp_stats *d_stats, double roi_frac,
+                  void *d_ws, size_t ws_bytes);
+
+/* Adjoint (conjugate transpose) of ssp_propagate (north_star; replaces autograd):
+ *   for j = n_steps..1:  [grad_j = Im(G_j conj(U_j)) if j <= S];  g <- W g;
+ *                        if j <= S: g <- exp(-i phi_j) g;  g <- F^-1{ conj(H(dz_j)) F{g} }.
+ * G_j is the adjoint field arriving at plane j, U_j = d_planes[b][j-1].  Gradient
+ * convention G = dl/dRe U + i dl/dIm U.  d_g_out / d_g_in: dev complex64 [B][N][N]; may
+ * alias.  d_planes and d_phase_grad (dev fp32 [B][S][N][N]) are both given or both NULL. */
+int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind,
+                          int B, int n_steps, const double *dz,
+                          const float *d_screens, long long screen_batch_stride, int S,
+                          ssp_window win, const float *d_g_out, float *d_g_in,
+                          const float *d_planes, float *d_phase_grad,
+                          void *d_ws, size_t ws_bytes);
+
+/* Intensity statistics of B fields (O8).  Optional per-pixel ensemble accumulation by
+ * Welford's algorithm: d_mean, d_M2 dev fp32 [N][N] in-out and *count
+ * (host, in-out) advanced by B; pass all three or none. */
+int ssp_beam_stats(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_field, double roi_frac,
+                   ssp_stats *d_stats, float *d_mean, float *d_M2, long long *count);
+
+/* End-to-end form of ssp_propagate with HOST buffers: copies field and screens to the
+ * device buffers given (d_field [B][N][N] c64, d_screens as above), propagates, copies
+ * the output field and statistics back, and synchronises the stream.  h_* pointers are
+ * host memory (pinned for full copy speed). */
+int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind,
+                       int B, int n_steps, const double *dz,
+                       const float *h_screens, long long screen_batch_stride, int S,
+                       ssp_window win, const float *h_field_in, float *h_field_out,
+                       ssp_stats *h_stats, double roi_frac,
+                       float *d_field, float *d_screens, ssp_stats *d_stats,
+                       void *d_ws, size_t ws_bytes);
+
+/* ---- helpers for mask systems (config 4; O9) ----------------- */
+
+/* out = in exp(i sign theta); theta dev fp32 [N][N] shared by the B fields; in may alias out. */
+int ssp_phase_mul(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_theta, double sign,
+                  const float *d_in, float *d_out);
+/* Lens as a DFT: centred unitary transform F_c = fftshift o fft2 o ifftshift / N
+ * (inverse != 0: its inverse).  in may alias out. */
+int ssp_dft2_centered(ssp_ctx *ctx, ssp_grid grid, int B, int inverse,
+                      const float *d_in, float *d_out, void *d_ws, size_t ws_bytes);
+/* grad[b] = Im(g[b] conj(u[b])), dev fp32 [B][N][N]. */
+int ssp_phase_grad(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_g, const float *d_u,
+                   float *d_grad);
+/* Per field b: d_out[b] = { Re <a,b>, Im <a,b>, sum |a|^2, sum |b|^2 } (doubles),
+ * <a,b> = sum conj(a) b.  d_out: dev double [B][4]. */
+int ssp_inner_products(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_a, const float *d_b,
+                       double *d_out);
+/* out[b] = alpha[b] a[b] + beta[b] b[b] with per-field complex scalars; h_alpha, h_beta:
+ * host double [B][2]; out may alias a or b. */
+int ssp_lincomb(ssp_ctx *ctx, ssp_grid grid, int B, const double *h_alpha, const float *d_a,
+                const double *h_beta, const float *d_b, float *d_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SSP_H */

@@ -1,0 +1,318 @@
+"""Thin ctypes binding of include/ssp.h -- argument marshalling only.
+
+Every function below has the name of the C entry point it calls (minus the `ssp_` prefix) and
+does nothing but turn torch CUDA tensors into device pointers, python lists into host arrays
+and return codes into exceptions.  All arithmetic of the method runs in the library's kernels.
+PyTorch is used for device memory and streams only.  There is no CPU fallback: a missing
+libssp.so, a missing GPU or a non-CUDA tensor raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional, Sequence
+
+import torch
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libssp.so")
+
+PSD_KOLMOGOROV, PSD_VON_KARMAN, PSD_OCEAN_NIKISHOV = 0, 1, 2
+H_FRESNEL, H_ANGULAR_SPECTRUM = 0, 1
+OK, EINVAL, EUNSUPPORTED, EWORKSPACE, ECUDA = 0, -1, -2, -3, -4
+
+# every symbol include/ssp.h declares (tests/test_abi.py checks the header against this list)
+SYMBOLS = (
+    "ssp_create", "ssp_destroy", "ssp_last_error", "ssp_version", "ssp_launch_count",
+    "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_propagate",
+    "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_propagate_host", "ssp_phase_mul",
+    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb",
+)
+
+
+class SspError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"ssp error {code}: {msg}")
+        self.code = code
+
+
+class Grid(C.Structure):
+    _fields_ = [("N", C.c_int), ("dx", C.c_double)]
+
+
+class Psd(C.Structure):
+    _fields_ = [("kind", C.c_int), ("L0", C.c_double), ("l0", C.c_double), ("km_coeff", C.c_double),
+                ("chi_T", C.c_double), ("eps", C.c_double), ("w", C.c_double), ("eta", C.c_double)]
+
+
+class Window(C.Structure):
+    _fields_ = [("order", C.c_int), ("sigma_frac", C.c_double)]
+
+
+class Stats(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("power", "cx", "cy", "sxx", "syy", "sxy", "w2", "I_axis",
+                                           "roi_sumI", "roi_sumI2")] + [("roi_n", C.c_longlong)]
+
+
+STATS_BYTES = C.sizeof(Stats)
+STAT_FIELDS = tuple(n for n, _ in Stats._fields_)
+
+_lib = None
+
+
+def load():
+    """dlopen libssp.so (built in-tree by paper_2604_07248_b200.build).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2604_07248_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    lib.ssp_last_error.restype = C.c_char_p
+    lib.ssp_last_error.argtypes = [C.c_void_p]
+    lib.ssp_version.restype = C.c_char_p
+    lib.ssp_launch_count.restype = C.c_longlong
+    lib.ssp_launch_count.argtypes = [C.c_void_p]
+    lib.ssp_workspace_bytes.restype = C.c_size_t
+    lib.ssp_workspace_bytes.argtypes = [Grid, C.c_int, C.c_int]
+    lib.ssp_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_void_p]
+    lib.ssp_destroy.argtypes = [C.c_void_p]
+    P, D, I, L = C.c_void_p, C.c_double, C.c_int, C.c_longlong
+    lib.ssp_make_screens.argtypes = [P, Grid, C.POINTER(Psd), D, I, I, P, P, I, P, P, P, P, P, P, C.c_size_t]
+    lib.ssp_evolve_screens.argtypes = [P, Grid, C.POINTER(Psd), D, I, I, P, P, I, D, D, D, D, P, P, P, P, P, P,
+                                       C.c_size_t]
+    lib.ssp_propagate.argtypes = [P, Grid, D, D, I, I, I, P, P, L, I, Window, P, P, P, P, D, P, C.c_size_t]
+    lib.ssp_propagate_adjoint.argtypes = [P, Grid, D, D, I, I, I, P, P, L, I, Window, P, P, P, P, P, C.c_size_t]
+    lib.ssp_beam_stats.argtypes = [P, Grid, I, P, D, P, P, P, C.POINTER(L)]
+    lib.ssp_propagate_host.argtypes = [P, Grid, D, D, I, I, I, P, P, L, I, Window, P, P, P, D, P, P, P, P,
+                                       C.c_size_t]
+    lib.ssp_phase_mul.argtypes = [P, Grid, I, P, D, P, P]
+    lib.ssp_dft2_centered.argtypes = [P, Grid, I, I, P, P, P, C.c_size_t]
+    lib.ssp_phase_grad.argtypes = [P, Grid, I, P, P, P]
+    lib.ssp_inner_products.argtypes = [P, Grid, I, P, P, P]
+    lib.ssp_lincomb.argtypes = [P, Grid, I, P, P, P, P, P]
+    _lib = lib
+    return lib
+
+
+def version() -> str:
+    return load().ssp_version().decode()
+
+
+def workspace_bytes(N: int, dx: float, B: int, S: int) -> int:
+    return int(load().ssp_workspace_bytes(Grid(N, dx), B, S))
+
+
+def _dev(t: Optional[torch.Tensor], dtype=None):
+    """Device pointer of a contiguous CUDA tensor (None -> NULL)."""
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise TypeError("ssp: expected a CUDA tensor (no CPU fallback)")
+    if not t.is_contiguous():
+        raise ValueError("ssp: tensor must be contiguous")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"ssp: expected {dtype}, got {t.dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _host_doubles(x: Sequence[float]):
+    arr = (C.c_double * len(x))(*[float(v) for v in x])
+    return arr
+
+
+@dataclass
+class PsdParams:
+    kind: int = PSD_KOLMOGOROV
+    L0: float = 0.0
+    l0: float = 0.0
+    km_coeff: float = 0.0
+    chi_T: float = 0.0
+    eps: float = 0.0
+    w: float = 0.0
+    eta: float = 0.0
+
+    def c(self) -> Psd:
+        return Psd(self.kind, self.L0, self.l0, self.km_coeff, self.chi_T, self.eps, self.w, self.eta)
+
+
+class Context:
+    """ssp_ctx bound to a device and a torch stream (default: the current stream)."""
+
+    def __init__(self, device: int = 0, stream: Optional[torch.cuda.Stream] = None):
+        self._lib = load()
+        if not torch.cuda.is_available():
+            raise RuntimeError("ssp: no CUDA device (there is no CPU fallback)")
+        self.device = device
+        self.stream = stream if stream is not None else torch.cuda.current_stream(device)
+        h = C.c_void_p()
+        rc = self._lib.ssp_create(C.byref(h), device, C.c_void_p(self.stream.cuda_stream))
+        if rc != 0:
+            raise SspError(rc, "ssp_create failed (no usable sm_100 device?)")
+        self._h = h
+        self._ws = None
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.ssp_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _chk(self, rc: int):
+        if rc != 0:
+            raise SspError(rc, self._lib.ssp_last_error(self._h).decode())
+
+    def launch_count(self) -> int:
+        return int(self._lib.ssp_launch_count(self._h))
+
+    def workspace(self, N: int, dx: float, B: int, S: int) -> torch.Tensor:
+        """A cached torch byte buffer of at least ssp_workspace_bytes."""
+        need = max(workspace_bytes(N, dx, B, S), 256)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = torch.empty(need, dtype=torch.uint8, device=f"cuda:{self.device}")
+        return self._ws
+
+    # ---- screens ---------------------------------------------------------------------------
+    def make_screens(self, N, dx, psd: PsdParams, lam, cn2, dz, n_sh, noise, noise_sh=None,
+                     spectrum=None, sh_coef=None, screens=None, ws=None):
+        """noise: complex64 [B][S][N][N]; noise_sh: complex64 [B][S][n_sh][3][3]; returns screens fp32."""
+        B, S = noise.shape[0], noise.shape[1]
+        if screens is None:
+            screens = torch.empty((B, S, N, N), dtype=torch.float32, device=noise.device)
+        ws = self.workspace(N, dx, B, S) if ws is None else ws
+        pc = psd.c()
+        self._chk(self._lib.ssp_make_screens(
+            self._h, Grid(N, dx), C.byref(pc), lam, B, S, _host_doubles(cn2), _host_doubles(dz), n_sh,
+            _dev(noise, torch.complex64), _dev(noise_sh, torch.complex64) if n_sh > 0 else None,
+            _dev(spectrum, torch.complex64), _dev(sh_coef, torch.complex64), _dev(screens, torch.float32),
+            _dev(ws), ws.numel()))
+        return screens
+
+    def evolve_screens(self, N, dx, psd: PsdParams, lam, cn2, dz, n_sh, a, vx, vy, T, fresh, fresh_sh,
+                       spectrum, sh_coef, screens=None, ws=None):
+        B, S = fresh.shape[0], fresh.shape[1]
+        if screens is None:
+            screens = torch.empty((B, S, N, N), dtype=torch.float32, device=fresh.device)
+        ws = self.workspace(N, dx, B, S) if ws is None else ws
+        pc = psd.c()
+        self._chk(self._lib.ssp_evolve_screens(
+            self._h, Grid(N, dx), C.byref(pc), lam, B, S, _host_doubles(cn2), _host_doubles(dz), n_sh,
+            a, vx, vy, T, _dev(fresh, torch.complex64), _dev(fresh_sh, torch.complex64) if n_sh > 0 else None,
+            _dev(spectrum, torch.complex64), _dev(sh_coef, torch.complex64) if n_sh > 0 else None,
+            _dev(screens, torch.float32), _dev(ws), ws.numel()))
+        return screens
+
+    # ---- propagation -----------------------------------------------------------------------
+    @staticmethod
+    def _screen_args(screens, B, N, shared):
+        if screens is None:
+            return None, 0, 0
+        if shared:
+            assert screens.dim() == 3
+            return screens, 0, screens.shape[0]
+        assert screens.dim() == 4 and screens.shape[0] == B
+        return screens, screens.shape[1] * N * N, screens.shape[1]
+
+    def propagate(self, N, dx, lam, dz, field, screens=None, shared_screens=False, win_order=0,
+                  win_sigma_frac=0.47, n0=1.0, h_kind=H_FRESNEL, out=None, planes=None, stats=None,
+                  roi_frac=0.5):
+        """field: complex64 [B][N][N]; screens fp32 [B][S][N][N] (or [S][N][N] shared).
+        planes: optional complex64 [B][n_steps][N][N]; stats: optional uint8 [B*STATS_BYTES]."""
+        B = field.shape[0]
+        scr, stride, S = self._screen_args(screens, B, N, shared_screens)
+        if out is None:
+            out = torch.empty_like(field)
+        self._chk(self._lib.ssp_propagate(
+            self._h, Grid(N, dx), lam, n0, h_kind, B, len(dz), _host_doubles(dz),
+            _dev(scr, torch.float32), stride, S, Window(win_order, win_sigma_frac),
+            _dev(field, torch.complex64), _dev(out, torch.complex64), _dev(planes, torch.complex64),
+            _dev(stats), roi_frac, None, 0))
+        return out
+
+    def propagate_adjoint(self, N, dx, lam, dz, g_out, screens=None, shared_screens=False, win_order=0,
+                          win_sigma_frac=0.47, n0=1.0, h_kind=H_FRESNEL, out=None, planes=None,
+                          phase_grad=None):
+        B = g_out.shape[0]
+        scr, stride, S = self._screen_args(screens, B, N, shared_screens)
+        if out is None:
+            out = torch.empty_like(g_out)
+        self._chk(self._lib.ssp_propagate_adjoint(
+            self._h, Grid(N, dx), lam, n0, h_kind, B, len(dz), _host_doubles(dz),
+            _dev(scr, torch.float32), stride, S, Window(win_order, win_sigma_frac),
+            _dev(g_out, torch.complex64), _dev(out, torch.complex64), _dev(planes, torch.complex64),
+            _dev(phase_grad, torch.float32), None, 0))
+        return out
+
+    def beam_stats(self, N, dx, field, roi_frac=0.5, stats=None, mean=None, M2=None, count=None):
+        """Returns (stats uint8 tensor [B*STATS_BYTES], new count)."""
+        B = field.shape[0]
+        if stats is None:
+            stats = torch.empty(B * STATS_BYTES, dtype=torch.uint8, device=field.device)
+        cnt = C.c_longlong(count if count is not None else 0)
+        self._chk(self._lib.ssp_beam_stats(
+            self._h, Grid(N, dx), B, _dev(field, torch.complex64), roi_frac, _dev(stats),
+            _dev(mean, torch.float32), _dev(M2, torch.float32), C.byref(cnt) if mean is not None else None))
+        return stats, cnt.value
+
+    def propagate_host(self, N, dx, lam, dz, h_field_in, h_field_out, h_screens, shared_screens, S,
+                       win_order, win_sigma_frac, h_stats, roi_frac, d_field, d_screens, d_stats,
+                       n0=1.0, h_kind=H_FRESNEL):
+        """h_*: pinned CPU tensors; d_*: CUDA tensors.  Synchronises the stream."""
+        B = d_field.shape[0]
+        stride = 0 if (shared_screens or S == 0) else S * N * N
+        hp = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+        self._chk(self._lib.ssp_propagate_host(
+            self._h, Grid(N, dx), lam, n0, h_kind, B, len(dz), _host_doubles(dz),
+            hp(h_screens), stride, S, Window(win_order, win_sigma_frac), hp(h_field_in), hp(h_field_out),
+            hp(h_stats), roi_frac, _dev(d_field, torch.complex64), _dev(d_screens, torch.float32),
+            _dev(d_stats), None, 0))
+
+    # ---- helpers ---------------------------------------------------------------------------
+    def phase_mul(self, N, dx, theta, field, sign=1.0, out=None):
+        out = torch.empty_like(field) if out is None else out
+        self._chk(self._lib.ssp_phase_mul(self._h, Grid(N, dx), field.shape[0], _dev(theta, torch.float32),
+                                          sign, _dev(field, torch.complex64), _dev(out, torch.complex64)))
+        return out
+
+    def dft2_centered(self, N, dx, field, inverse=False, out=None):
+        out = torch.empty_like(field) if out is None else out
+        self._chk(self._lib.ssp_dft2_centered(self._h, Grid(N, dx), field.shape[0], int(inverse),
+                                              _dev(field, torch.complex64), _dev(out, torch.complex64), None, 0))
+        return out
+
+    def phase_grad(self, N, dx, g, u, out=None):
+        out = torch.empty(g.shape, dtype=torch.float32, device=g.device) if out is None else out
+        self._chk(self._lib.ssp_phase_grad(self._h, Grid(N, dx), g.shape[0], _dev(g, torch.complex64),
+                                           _dev(u, torch.complex64), _dev(out, torch.float32)))
+        return out
+
+    def inner_products(self, N, dx, a, b, out=None):
+        out = torch.empty((a.shape[0], 4), dtype=torch.float64, device=a.device) if out is None else out
+        self._chk(self._lib.ssp_inner_products(self._h, Grid(N, dx), a.shape[0], _dev(a, torch.complex64),
+                                               _dev(b, torch.complex64), _dev(out, torch.float64)))
+        return out
+
+    def lincomb(self, N, dx, alpha, a, beta, b, out=None):
+        """alpha, beta: python sequences of B complex numbers."""
+        B = a.shape[0]
+        out = torch.empty_like(a) if out is None else out
+        al = _host_doubles([v for z in alpha for v in (complex(z).real, complex(z).imag)])
+        be = _host_doubles([v for z in beta for v in (complex(z).real, complex(z).imag)])
+        self._chk(self._lib.ssp_lincomb(self._h, Grid(N, dx), B, al, _dev(a, torch.complex64), be,
+                                        _dev(b, torch.complex64), _dev(out, torch.complex64)))
+        return out
+
+
+def stats_to_dicts(stats: torch.Tensor):
+    """Decode a device uint8 tensor of ssp_stats records (one D2H copy) into python dicts."""
+    raw = stats.cpu().numpy().tobytes()
+    n = len(raw) // STATS_BYTES
+    arr = (Stats * n).from_buffer_copy(raw)
+    return [{k: getattr(arr[i], k) for k in STAT_FIELDS} for i in range(n)]

@@ -1,0 +1,272 @@
+// ssp_api.cu -- the extern "C" entry points declared in include/ssp.h (context, propagation,
+// adjoint, statistics).  Argument checking and launch sequencing only: every step of the path
+// runs in the kernels of ssp_propagate.cu / ssp_misc.cu.
+#include <cmath>
+#include <cstring>
+
+#include "ssp_internal.h"
+
+using namespace ssp;
+
+static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+extern "C" {
+
+const char *ssp_version(void) { return "ssp 0.1 sm_100a"; }
+
+int ssp_create(ssp_ctx **out, int device, void *cuda_stream)
+{
+    if (!out) return SSP_EINVAL;
+    *out = nullptr;
+    int n = 0;
+    if (cudaGetDeviceCount(&n) != cudaSuccess || n <= 0 || device < 0 || device >= n) return SSP_ECUDA;
+    if (cudaSetDevice(device) != cudaSuccess) return SSP_ECUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return SSP_ECUDA;
+    if (prop.major != 10) return SSP_EUNSUPPORTED; // sm_100a cubins only
+    ssp_ctx *ctx = new ssp_ctx();
+    ctx->device = device;
+    ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    ctx->num_sms = prop.multiProcessorCount;
+    *out = ctx;
+    return SSP_OK;
+}
+
+int ssp_destroy(ssp_ctx *ctx)
+{
+    if (!ctx) return SSP_EINVAL;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    for (auto &kv : ctx->twiddles) cudaFree(kv.second);
+    for (auto &kv : ctx->htables) cudaFree(kv.second);
+    for (auto &kv : ctx->sign_tables) cudaFree(kv.second);
+    for (void *p : ctx->owned) cudaFree(p);
+    if (ctx->scratch) cudaFree(ctx->scratch);
+    delete ctx;
+    return SSP_OK;
+}
+
+const char *ssp_last_error(const ssp_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+long long ssp_launch_count(const ssp_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+} // extern "C"
+
+namespace {
+
+struct PropGeom {
+    int N, B, n_steps, S;
+    double dx, lam_eff;
+    const double *dz;
+};
+
+int check_prop(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind, int B, int n_steps,
+               const double *dz, const float *d_screens, int S, const void *in, const void *out)
+{
+    if (!ctx) return SSP_EINVAL;
+    if (!valid_N(grid.N)) return ctx->fail(SSP_EINVAL, "N=%d is not a power of two in [8, 4096]", grid.N);
+    if (!(grid.dx > 0) || !(lambda > 0) || !(n0 > 0)) return ctx->fail(SSP_EINVAL, "dx, lambda and n0 must be > 0");
+    if (h_kind == SSP_H_ANGULAR_SPECTRUM)
+        return ctx->fail(SSP_EUNSUPPORTED, "angular-spectrum H is not separable; not built yet (DESIGN.md NEXT-3)");
+    if (h_kind != SSP_H_FRESNEL) return ctx->fail(SSP_EINVAL, "unknown h_kind %d", h_kind);
+    if (B < 1 || n_steps < 1 || !dz) return ctx->fail(SSP_EINVAL, "B >= 1, n_steps >= 1 and dz are required");
+    if (S < 0 || S > n_steps) return ctx->fail(SSP_EINVAL, "need 0 <= S <= n_steps (S=%d, n_steps=%d)", S, n_steps);
+    if (S > 0 && !d_screens) return ctx->fail(SSP_EINVAL, "d_screens is null with S=%d", S);
+    for (int j = 0; j < n_steps; ++j)
+        if (!(dz[j] > 0)) return ctx->fail(SSP_EINVAL, "dz[%d] must be > 0", j);
+    if (!in || !out) return ctx->fail(SSP_EINVAL, "field pointers are required");
+    if (!aligned16(in) || !aligned16(out) || !aligned16(d_screens))
+        return ctx->fail(SSP_EINVAL, "device pointers must be 16-byte aligned");
+    return SSP_OK;
+}
+
+void fill_window(RowArgs &r, ssp_window win, int N)
+{
+    r.win_on = (win.order > 0 && win.sigma_frac > 0) ? 1 : 0;
+    if (r.win_on) {
+        const double s = win.sigma_frac * N;
+        r.win_qs = (float)(1.0 / (s * s));
+        r.win_half_order = (float)(0.5 * win.order);
+    }
+}
+
+} // namespace
+
+extern "C" {
+
+int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind,
+                  int B, int n_steps, const double *dz,
+                  const float *d_screens, long long screen_batch_stride, int S,
+                  ssp_window win, const float *d_field_in, float *d_field_out,
+                  float *d_planes, ssp_stats *d_stats, double roi_frac,
+                  void *d_ws, size_t ws_bytes)
+{
+    (void)d_ws; (void)ws_bytes;
+    if (int rc = check_prop(ctx, grid, lambda, n0, h_kind, B, n_steps, dz, d_screens, S, d_field_in, d_field_out))
+        return rc;
+    SSP_CUDA(ctx, cudaSetDevice(ctx->device));
+    const int N = grid.N;
+    const size_t px = (size_t)N * N;
+    const double lam_eff = lambda / n0;
+    const float2 *tw = nullptr;
+    if (int rc = get_twiddles(ctx, N, &tw)) return rc;
+    float2 *u = reinterpret_cast<float2 *>(d_field_out);
+
+    // K4: FFT_x of the input, times hx of step 1
+    const float2 *hx = nullptr;
+    if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[0], 0, 0}, &hx)) return rc;
+    RowArgs r0{};
+    r0.in = reinterpret_cast<const float2 *>(d_field_in);
+    r0.out = u;
+    r0.n_lines = B * N;
+    r0.hx = hx;
+    r0.tw = tw;
+    if (int rc = launch_row(ctx, N, false, true, r0)) return rc;
+
+    for (int j = 1; j <= n_steps; ++j) {
+        // K5: FFT_y -> * hy_j / N^2 -> IFFT_y
+        const float2 *hy = nullptr;
+        if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j - 1], 0, 1}, &hy)) return rc;
+        ColArgs c{};
+        c.in = u; c.out = u; c.B = B; c.hy = hy; c.tw = tw;
+        if (int rc = launch_col_prop(ctx, N, c)) return rc;
+        // K6: IFFT_x -> * exp(i phi_j) W -> [FFT_x -> * hx_{j+1}]
+        RowArgs r{};
+        r.in = u; r.out = u; r.n_lines = B * N; r.tw = tw;
+        if (j <= S) {
+            r.phi = d_screens + (size_t)(j - 1) * px;
+            r.phi_batch_stride = screen_batch_stride;
+            r.phase_sign = 1.f;
+        }
+        fill_window(r, win, N);
+        if (d_planes) {
+            r.plane_out = reinterpret_cast<float2 *>(d_planes) + (size_t)(j - 1) * px;
+            r.plane_stride = (long long)n_steps * (long long)px;
+        }
+        const bool last = (j == n_steps);
+        if (!last) {
+            if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j], 0, 0}, &hx)) return rc;
+            r.hx = hx;
+        }
+        if (int rc = launch_row(ctx, N, true, !last, r)) return rc;
+    }
+    if (d_stats)
+        if (int rc = launch_stats(ctx, N, grid.dx, B, u, roi_frac, d_stats)) return rc;
+    return SSP_OK;
+}
+
+int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind,
+                          int B, int n_steps, const double *dz,
+                          const float *d_screens, long long screen_batch_stride, int S,
+                          ssp_window win, const float *d_g_out, float *d_g_in,
+                          const float *d_planes, float *d_phase_grad,
+                          void *d_ws, size_t ws_bytes)
+{
+    (void)d_ws; (void)ws_bytes;
+    if (int rc = check_prop(ctx, grid, lambda, n0, h_kind, B, n_steps, dz, d_screens, S, d_g_out, d_g_in))
+        return rc;
+    if ((d_planes == nullptr) != (d_phase_grad == nullptr))
+        return ctx->fail(SSP_EINVAL, "d_planes and d_phase_grad must both be given or both be null");
+    SSP_CUDA(ctx, cudaSetDevice(ctx->device));
+    const int N = grid.N;
+    const size_t px = (size_t)N * N;
+    const double lam_eff = lambda / n0;
+    const float2 *tw = nullptr;
+    if (int rc = get_twiddles(ctx, N, &tw)) return rc;
+    float2 *g = reinterpret_cast<float2 *>(d_g_in);
+
+    // pointwise stage of plane j: [grad_j] ; g <- W exp(-i phi_j) g
+    auto plane_stage = [&](RowArgs &r, int j) {
+        if (j <= S) {
+            r.phi = d_screens + (size_t)(j - 1) * px;
+            r.phi_batch_stride = screen_batch_stride;
+            r.phase_sign = -1.f;
+            if (d_phase_grad) {
+                r.plane_in = reinterpret_cast<const float2 *>(d_planes) + (size_t)(j - 1) * px;
+                r.plane_stride = (long long)n_steps * (long long)px;
+                r.grad = d_phase_grad + (size_t)(j - 1) * px;
+                r.grad_stride = (long long)S * (long long)px;
+            }
+        }
+        fill_window(r, win, N);
+    };
+
+    const float2 *hx = nullptr;
+    if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[n_steps - 1], 1, 0}, &hx)) return rc;
+    RowArgs r0{};
+    r0.in = reinterpret_cast<const float2 *>(d_g_out);
+    r0.out = g; r0.n_lines = B * N; r0.hx = hx; r0.tw = tw;
+    plane_stage(r0, n_steps);
+    if (int rc = launch_row(ctx, N, false, true, r0)) return rc;
+
+    for (int j = n_steps; j >= 1; --j) {
+        const float2 *hy = nullptr;
+        if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j - 1], 1, 1}, &hy)) return rc;
+        ColArgs c{};
+        c.in = g; c.out = g; c.B = B; c.hy = hy; c.tw = tw;
+        if (int rc = launch_col_prop(ctx, N, c)) return rc;
+        RowArgs r{};
+        r.in = g; r.out = g; r.n_lines = B * N; r.tw = tw;
+        const bool last = (j == 1);
+        if (!last) {
+            plane_stage(r, j - 1);
+            if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j - 2], 1, 0}, &hx)) return rc;
+            r.hx = hx;
+        }
+        if (int rc = launch_row(ctx, N, true, !last, r)) return rc;
+    }
+    return SSP_OK;
+}
+
+int ssp_beam_stats(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_field, double roi_frac,
+                   ssp_stats *d_stats, float *d_mean, float *d_M2, long long *count)
+{
+    if (!ctx) return SSP_EINVAL;
+    if (!valid_N(grid.N) || !(grid.dx > 0) || B < 1 || !d_field || !aligned16(d_field))
+        return ctx->fail(SSP_EINVAL, "bad grid, batch or field pointer");
+    const int n_opt = (d_mean != nullptr) + (d_M2 != nullptr) + (count != nullptr);
+    if (n_opt != 0 && n_opt != 3) return ctx->fail(SSP_EINVAL, "d_mean, d_M2 and count go together");
+    if (!d_stats && n_opt == 0) return ctx->fail(SSP_EINVAL, "nothing to compute");
+    SSP_CUDA(ctx, cudaSetDevice(ctx->device));
+    const float2 *f = reinterpret_cast<const float2 *>(d_field);
+    if (d_stats)
+        if (int rc = launch_stats(ctx, grid.N, grid.dx, B, f, roi_frac, d_stats)) return rc;
+    if (n_opt == 3) {
+        if (*count < 0) return ctx->fail(SSP_EINVAL, "count must be >= 0");
+        if (int rc = launch_welford(ctx, grid.N, B, f, d_mean, d_M2, *count)) return rc;
+        *count += B;
+    }
+    return SSP_OK;
+}
+
+int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind,
+                       int B, int n_steps, const double *dz,
+                       const float *h_screens, long long screen_batch_stride, int S,
+                       ssp_window win, const float *h_field_in, float *h_field_out,
+                       ssp_stats *h_stats, double roi_frac,
+                       float *d_field, float *d_screens, ssp_stats *d_stats,
+                       void *d_ws, size_t ws_bytes)
+{
+    if (!ctx) return SSP_EINVAL;
+    if (!valid_N(grid.N) || B < 1 || S < 0) return ctx->fail(SSP_EINVAL, "bad grid, batch or S");
+    if (!h_field_in || !h_field_out || !d_field) return ctx->fail(SSP_EINVAL, "field buffers are required");
+    if (S > 0 && (!h_screens || !d_screens)) return ctx->fail(SSP_EINVAL, "screen buffers are required");
+    if (h_stats && !d_stats) return ctx->fail(SSP_EINVAL, "d_stats is required with h_stats");
+    SSP_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t px = (size_t)grid.N * grid.N;
+    SSP_CUDA(ctx, cudaMemcpyAsync(d_field, h_field_in, sizeof(float) * 2 * px * B, cudaMemcpyHostToDevice, ctx->stream));
+    if (S > 0) {
+        const size_t n_scr = (screen_batch_stride == 0) ? (size_t)S * px
+                                                        : (size_t)(B - 1) * (size_t)screen_batch_stride + (size_t)S * px;
+        SSP_CUDA(ctx, cudaMemcpyAsync(d_screens, h_screens, sizeof(float) * n_scr, cudaMemcpyHostToDevice, ctx->stream));
+    }
+    if (int rc = ssp_propagate(ctx, grid, lambda, n0, h_kind, B, n_steps, dz, d_screens, screen_batch_stride, S, win,
+                               d_field, d_field, nullptr, h_stats ? d_stats : nullptr, roi_frac, d_ws, ws_bytes))
+        return rc;
+    SSP_CUDA(ctx, cudaMemcpyAsync(h_field_out, d_field, sizeof(float) * 2 * px * B, cudaMemcpyDeviceToHost, ctx->stream));
+    if (h_stats)
+        SSP_CUDA(ctx, cudaMemcpyAsync(h_stats, d_stats, sizeof(ssp_stats) * B, cudaMemcpyDeviceToHost, ctx->stream));
+    SSP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SSP_OK;
+}
+
+} // extern "C"

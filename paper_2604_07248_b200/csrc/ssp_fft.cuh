@@ -1,0 +1,252 @@
+// ssp_fft.cuh -- in-register complex64 FFT building blocks for sm_100a.
+//
+// A length-N line (row or column of the field) is transformed by T = N/E threads that
+// each hold E points in registers.  N = R1*R2*R3 (mixed radix, each radix <= E): every
+// stage is a set of radix-R butterflies computed entirely in registers with compile-time
+// twiddles; between stages the line is exchanged once through shared memory, multiplied
+// by the inter-stage twiddles W_N^(rho*k) read from a table built in double precision on
+// the host.  With (R1,R2) = (32,32) a 1024-point transform costs ONE shared-memory
+// round trip.
+//
+// Index maps (decimation in frequency, in place; derivation in DESIGN.md section 6):
+//   input  n = n1*(N/R1) + n2*R3 + n3,   output k = k1 + R1*k2 + R1*R2*k3
+//   stage 1: butterfly m=(n2,n3):   A[k1;m]   = sum_n1 x[n1*(N/R1)+m] W_R1^(n1 k1),  *= W_N^(m k1)
+//   stage 2: butterfly (k1,n3):     B[k1,k2;n3] = sum_n2 A[k1;n2,n3] W_R2^(n2 k2),   *= W_N^(R1 n3 k2)
+//   stage 3: butterfly (k1,k2):     X[k]      = sum_n3 B[k1,k2;n3] W_R3^(n3 k3)
+// Register layout "strided by R": thread t holds, for i in [0,E/R), j = t + T*i, the
+// elements  v[i*R + q] <-> line index q*(N/R) + j.  A plan's input layout is strided by
+// R1 and its output layout strided by its last radix, so the plan (R1,R2,R3) followed by
+// the reversed plan (R3,R2,R1) chains register to register with no exchange in between.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <utility>
+
+namespace ssp {
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b)
+{
+    return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+}
+__device__ __forceinline__ float2 cmul_conj(float2 a, float2 b) // a * conj(b)
+{
+    return make_float2(fmaf(a.x, b.x, a.y * b.y), fmaf(a.y, b.x, -a.x * b.y));
+}
+template <bool CONJ>
+__device__ __forceinline__ float2 cmul_c(float2 a, float2 b)
+{
+    return CONJ ? cmul_conj(a, b) : cmul(a, b);
+}
+
+// cos(2 pi k / 32), k = 0..31
+__host__ __device__ constexpr float cos32(int k)
+{
+    constexpr float t[32] = {
+        1.0f, 0.98078528040323043f, 0.92387953251128674f, 0.83146961230254524f,
+        0.70710678118654752f, 0.55557023301960218f, 0.38268343236508977f, 0.19509032201612825f,
+        0.0f, -0.19509032201612825f, -0.38268343236508977f, -0.55557023301960218f,
+        -0.70710678118654752f, -0.83146961230254524f, -0.92387953251128674f, -0.98078528040323043f,
+        -1.0f, -0.98078528040323043f, -0.92387953251128674f, -0.83146961230254524f,
+        -0.70710678118654752f, -0.55557023301960218f, -0.38268343236508977f, -0.19509032201612825f,
+        0.0f, 0.19509032201612825f, 0.38268343236508977f, 0.55557023301960218f,
+        0.70710678118654752f, 0.83146961230254524f, 0.92387953251128674f, 0.98078528040323043f};
+    return t[k & 31];
+}
+__host__ __device__ constexpr float sin32(int k) { return cos32(k - 8); }
+
+// b *= W_R^K with W_R = exp(-/+ i 2 pi / R) (forward / inverse); K, R compile-time.
+template <int R, int K, bool INV>
+__device__ __forceinline__ void mul_w(float2 &b)
+{
+    constexpr int k32 = (K * (32 / R)) & 31;
+    if constexpr (k32 == 0) {
+    } else if constexpr (k32 == 8) { // -i (fwd) / +i (inv)
+        float2 t = b;
+        b = INV ? make_float2(-t.y, t.x) : make_float2(t.y, -t.x);
+    } else if constexpr (k32 == 16) {
+        b = make_float2(-b.x, -b.y);
+    } else if constexpr (k32 == 24) {
+        float2 t = b;
+        b = INV ? make_float2(t.y, -t.x) : make_float2(-t.y, t.x);
+    } else {
+        constexpr float c = cos32(k32);
+        constexpr float s = INV ? sin32(k32) : -sin32(k32);
+        float2 t = b;
+        b = make_float2(fmaf(t.x, c, -t.y * s), fmaf(t.x, s, t.y * c));
+    }
+}
+
+// butterfly (a, b) -> (a + b, (a - b) W_R^K) on v[OFF+K], v[OFF+K+R/2]
+template <int R, int OFF, int K, bool INV>
+__device__ __forceinline__ void bfly(float2 *v)
+{
+    float2 a = v[OFF + K], b = v[OFF + K + R / 2];
+    v[OFF + K] = make_float2(a.x + b.x, a.y + b.y);
+    float2 d = make_float2(a.x - b.x, a.y - b.y);
+    mul_w<R, K, INV>(d);
+    v[OFF + K + R / 2] = d;
+}
+
+template <int R, int OFF, bool INV, int... K>
+__device__ __forceinline__ void dif_level(float2 *v, std::integer_sequence<int, K...>)
+{
+    (bfly<R, OFF, K, INV>(v), ...);
+}
+
+// In-place radix-2 DIF recursion on v[OFF .. OFF+R): leaves X[bitrev(i)] in v[OFF+i].
+template <int R, int OFF, bool INV>
+__device__ __forceinline__ void dif_rec(float2 *v)
+{
+    if constexpr (R >= 2) {
+        dif_level<R, OFF, INV>(v, std::make_integer_sequence<int, R / 2>{});
+        dif_rec<R / 2, OFF, INV>(v);
+        dif_rec<R / 2, OFF + R / 2, INV>(v);
+    }
+}
+
+__host__ __device__ constexpr int bitrev(int i, int R)
+{
+    int r = 0;
+    for (int b = 1; b < R; b <<= 1) {
+        r = (r << 1) | (i & 1);
+        i >>= 1;
+    }
+    return r;
+}
+
+template <int R, int... I>
+__device__ __forceinline__ void unscramble(float2 *v, std::integer_sequence<int, I...>)
+{
+    float2 t[R];
+    ((t[I] = v[bitrev(I, R)]), ...);
+    ((v[I] = t[I]), ...);
+}
+
+// Radix-R DFT of v[0..R) in registers, natural order in and out.  R in {1,2,4,8,16,32}.
+template <int R, bool INV>
+__device__ __forceinline__ void radix(float2 *v)
+{
+    if constexpr (R > 1) {
+        dif_rec<R, 0, INV>(v);
+        unscramble<R>(v, std::make_integer_sequence<int, R>{});
+    }
+}
+
+// ---- plans -----------------------------------------------------------------------
+template <int N> struct Plan;
+template <> struct Plan<8>    { static constexpr int R1 = 8,  R2 = 1,  R3 = 1, E = 8;  };
+template <> struct Plan<16>   { static constexpr int R1 = 16, R2 = 1,  R3 = 1, E = 16; };
+template <> struct Plan<32>   { static constexpr int R1 = 32, R2 = 1,  R3 = 1, E = 32; };
+template <> struct Plan<64>   { static constexpr int R1 = 8,  R2 = 8,  R3 = 1, E = 8;  };
+template <> struct Plan<128>  { static constexpr int R1 = 16, R2 = 8,  R3 = 1, E = 16; };
+template <> struct Plan<256>  { static constexpr int R1 = 16, R2 = 16, R3 = 1, E = 16; };
+template <> struct Plan<512>  { static constexpr int R1 = 32, R2 = 16, R3 = 1, E = 32; };
+template <> struct Plan<1024> { static constexpr int R1 = 32, R2 = 32, R3 = 1, E = 32; };
+template <> struct Plan<2048> { static constexpr int R1 = 32, R2 = 8,  R3 = 8, E = 32; };
+template <> struct Plan<4096> { static constexpr int R1 = 32, R2 = 16, R3 = 8, E = 32; };
+
+template <int N>
+struct PlanInfo {
+    using P = Plan<N>;
+    static constexpr int R1 = P::R1, R2 = P::R2, R3 = P::R3, E = P::E;
+    static constexpr int T = N / E;                        // threads per line
+    static constexpr int NSTAGE = (R2 == 1) ? 1 : (R3 == 1 ? 2 : 3);
+    static constexpr int RL = (NSTAGE == 1) ? R1 : (NSTAGE == 2 ? R2 : R3); // last radix
+    static constexpr int PADQ = N / R1;                    // one pad element per PADQ positions
+    static constexpr int PADQ_REV = N / RL;
+    static constexpr int LINE_ELEMS = N + (R1 > RL ? R1 : RL); // padded line length (either direction)
+    // twiddle tables (forward sign), built on the host in double:
+    //   tw1 [R1][N/R1]:  W_N^(m k1)            tw2 [R2][R3]: W_N^(R1 n3 k2)
+    //   tw1r[RL][N/RL] and tw2r[R2][R1] for the reversed plan (R3|R2, R2, R1)
+    static constexpr int TW1 = 0;
+    static constexpr int TW2 = TW1 + N;
+    static constexpr int TW1R = TW2 + R2 * R3;
+    static constexpr int TW2R = TW1R + N;
+    static constexpr int TW_TOTAL = TW2R + R2 * R1;
+};
+
+// One complete transform of a line held in registers.
+//   DIR_REV = false: plan (R1,R2,R3): input strided by R1, output strided by RL.
+//   DIR_REV = true : plan (RL,..,R1): input strided by RL, output strided by R1.
+// SM: exchange accessor with  st(pos, val), ld(pos), sync()  on UNPADDED positions of this line.
+template <int N, bool DIR_REV, bool INV, class SM>
+__device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 *__restrict__ tw)
+{
+    using PI = PlanInfo<N>;
+    constexpr int E = PI::E, T = PI::T, NS = PI::NSTAGE;
+    constexpr int Ra = DIR_REV ? PI::RL : PI::R1;                        // first radix
+    constexpr int Rb = (NS >= 2) ? (NS == 2 ? (DIR_REV ? PI::R1 : PI::R2) : PI::R2) : 1;
+    constexpr int Rc = (NS == 3) ? (DIR_REV ? PI::R1 : PI::R3) : 1;
+    constexpr int PADQ = N / Ra;
+    const float2 *tw1 = tw + (DIR_REV ? PI::TW1R : PI::TW1);
+    const float2 *tw2 = tw + (DIR_REV ? PI::TW2R : PI::TW2);
+    auto pad = [](int p) { return p + p / PADQ; };
+
+    // ---- stage 1
+    constexpr int M1 = N / Ra;
+#pragma unroll
+    for (int i = 0; i < E / Ra; ++i) {
+        radix<Ra, INV>(v + i * Ra);
+        if constexpr (NS >= 2) {
+            const int m = t + T * i;
+#pragma unroll
+            for (int k = 0; k < Ra; ++k) {
+                float2 x = v[i * Ra + k];
+                if (k > 0) x = cmul_c<INV>(x, __ldg(tw1 + k * M1 + m));
+                sm.st(pad(k * M1 + m), x);
+            }
+        }
+    }
+    if constexpr (NS == 1) return;
+    sm.sync();
+
+    if constexpr (NS == 2) {
+        // ---- stage 2 (last): butterfly j = k1, reads k1*Rb + n2, produces X[k1 + Ra*k2]
+#pragma unroll
+        for (int i = 0; i < E / Rb; ++i) {
+            const int j = t + T * i;
+#pragma unroll
+            for (int n = 0; n < Rb; ++n) v[i * Rb + n] = sm.ld(pad(j * Rb + n));
+            radix<Rb, INV>(v + i * Rb);
+        }
+    } else {
+        // ---- stage 2 (middle): butterfly j = k1*Rc + n3, in place
+#pragma unroll
+        for (int i = 0; i < E / Rb; ++i) {
+            const int j = t + T * i;
+            const int k1 = j / Rc, n3 = j % Rc;
+            const int base = k1 * (Rb * Rc) + n3;
+            float2 *w = v + i * Rb;
+#pragma unroll
+            for (int n = 0; n < Rb; ++n) w[n] = sm.ld(pad(base + n * Rc));
+            radix<Rb, INV>(w);
+#pragma unroll
+            for (int k = 0; k < Rb; ++k) {
+                float2 x = w[k];
+                if (k > 0) x = cmul_c<INV>(x, __ldg(tw2 + k * Rc + n3));
+                sm.st(pad(base + k * Rc), x);
+            }
+        }
+        sm.sync();
+        // ---- stage 3 (last): butterfly j = k1 + Ra*k2, reads k1*Rb*Rc + k2*Rc + n3
+#pragma unroll
+        for (int i = 0; i < E / Rc; ++i) {
+            const int j = t + T * i;
+            const int k1 = j % Ra, k2 = j / Ra;
+            const int base = k1 * (Rb * Rc) + k2 * Rc;
+            float2 *w = v + i * Rc;
+#pragma unroll
+            for (int n = 0; n < Rc; ++n) w[n] = sm.ld(pad(base + n));
+            radix<Rc, INV>(w);
+        }
+    }
+}
+
+// Line index of register element q of butterfly slot i for a layout strided by R.
+template <int N, int R>
+__device__ __forceinline__ int line_index(int t, int i, int q)
+{
+    return q * (N / R) + t + (N / PlanInfo<N>::E) * i;
+}
+
+} // namespace ssp

@@ -1,0 +1,166 @@
+// ssp_internal.h -- context, table caches and kernel launchers shared by the .cu files.
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <map>
+#include <string>
+#include <tuple>
+#include <vector>
+
+#include "../../include/ssp.h"
+
+namespace ssp {
+
+struct HKey {
+    int N;
+    double dx, lam_eff, dz;
+    int conj;      // conj(H)
+    int scaled;    // multiplied by 1/N^2
+    bool operator<(const HKey &o) const
+    {
+        return std::tie(N, dx, lam_eff, dz, conj, scaled) <
+               std::tie(o.N, o.dx, o.lam_eff, o.dz, o.conj, o.scaled);
+    }
+};
+
+} // namespace ssp
+
+struct ssp_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    long long launches = 0;
+    int num_sms = 148;
+    std::map<int, float2 *> twiddles;            // per N, device
+    std::map<ssp::HKey, float2 *> htables;       // 1-D transfer-function tables, device [N]
+    std::map<int, float2 *> sign_tables;         // (-1)^k tables for the centred DFT
+    void *scratch = nullptr;                     // small device scratch (stat accumulators, tables)
+    size_t scratch_bytes = 0;
+    std::vector<void *> owned;                   // misc device allocations freed at destroy
+
+    int fail(int code, const char *fmt, ...)
+    {
+        char buf[512];
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(buf, sizeof buf, fmt, ap);
+        va_end(ap);
+        err = buf;
+        return code;
+    }
+};
+
+#define SSP_CUDA(ctx, call)                                                                  \
+    do {                                                                                     \
+        cudaError_t e_ = (call);                                                             \
+        if (e_ != cudaSuccess)                                                               \
+            return (ctx)->fail(SSP_ECUDA, "%s failed: %s (%s:%d)", #call,                    \
+                               cudaGetErrorString(e_), __FILE__, __LINE__);                  \
+    } while (0)
+
+namespace ssp {
+
+// ---- tables (ssp_tables.cu) ------------------------------------------------------
+int get_twiddles(ssp_ctx *ctx, int N, const float2 **out);
+int get_htable(ssp_ctx *ctx, const HKey &key, const float2 **out);
+int get_sign_table(ssp_ctx *ctx, int N, const float2 **out);
+int ensure_scratch(ssp_ctx *ctx, size_t bytes);
+bool valid_N(int N);
+
+// ---- row / column kernels (ssp_propagate.cu) ---------------------------------------
+struct RowArgs {
+    const float2 *in;
+    float2 *out;
+    int n_lines;                 // B * N
+    // pointwise stage (applied in real space, between the two transforms)
+    const float *phi;            // screen of this step for field 0, or null
+    long long phi_batch_stride;  // elements between fields (0 = shared)
+    float phase_sign;            // +1 forward, -1 adjoint
+    int win_on;
+    float win_qs;                // 1 / (sigma_frac N)^2
+    float win_half_order;        // order / 2
+    float2 *plane_out;           // optional: field after the pointwise stage, field b at + b*plane_stride
+    long long plane_stride;      // elements (float2) between fields
+    const float2 *plane_in;      // optional (adjoint gradient): forward plane
+    float *grad;                 // optional: Im(G conj(U)), field b at + b*grad_stride
+    long long grad_stride;
+    // spectral post-multiply after the second transform
+    const float2 *hx;            // [N] or null
+    // generic pre-multiply on the input line index (centred DFT): [N] or null
+    const float2 *pre;
+    const float2 *pre_line;      // per-line factor pre_line[iy] multiplying the whole line, or null
+    const float2 *tw;
+};
+
+struct ColArgs {
+    const float2 *in;
+    float2 *out;
+    int B;
+    const float2 *hy;            // [N] multiplier between / after the transforms, or null
+    const float2 *tw;
+};
+
+// first: inverse FFT_x before the pointwise stage; second: forward FFT_x after it.
+int launch_row(ssp_ctx *ctx, int N, bool first, bool second, const RowArgs &a);
+// column pass of the propagator: FFT_y -> * hy -> IFFT_y, in place allowed.
+int launch_col_prop(ssp_ctx *ctx, int N, const ColArgs &a);
+// single column transform (inverse != 0: unnormalised inverse) followed by * hy.
+int launch_col_single(ssp_ctx *ctx, int N, bool inverse, const ColArgs &a);
+
+// ---- screens (ssp_screens.cu) ------------------------------------------------------
+struct ScreenFilter {
+    int kind;
+    float f0sq;          // von Karman: 1/L0^2 (0 for Kolmogorov)
+    float inv_fm2_log2e; // von Karman: log2(e) / (2 fm^2)   (0 when l0 == 0)
+    float df;            // 1/(N dx)
+    // ocean
+    float eta, w, two_pi;
+};
+struct ScreenColArgs {
+    const float2 *noise;      // [nscr][N][N]
+    const float2 *old_spec;   // AR: previous spectrum (may alias spec_out), or null
+    float2 *spec_out;         // optional stored spectrum
+    float2 *out;              // column-transformed intermediate [nscr][N][N]
+    int nscr;
+    int g0, S;                // first linear screen index (b*S+s) of this chunk, screens per stack
+    const float *amp;         // per-slab amplitude factor [S] (device): sqrt of the PSD's scalar part * df
+    ScreenFilter flt;
+    float ar_a, ar_g;         // a, sqrt(1-a^2)
+    const float2 *taux, *tauy; // AR tilt tables [N] or null
+    const float2 *tw;
+};
+struct ScreenRowArgs {
+    const float2 *in;         // [nscr][N][N]
+    float *screens;           // [nscr][N][N]
+    int nscr;
+    int n_sh;
+    const float2 *sh_coef;    // [nscr][n_sh][3][3]
+    const float *sh_mean;     // [nscr]
+    const float2 *ex;         // [n_sh][N] exp(i 2 pi df_p x)
+    const float2 *tw;
+};
+int launch_screen_col(ssp_ctx *ctx, int N, const ScreenColArgs &a);
+int launch_screen_row(ssp_ctx *ctx, int N, const ScreenRowArgs &a);
+// subharmonic coefficient update + analytic mean, one block per screen
+int launch_sh_prep(ssp_ctx *ctx, int nscr, int S, int n_sh, const float2 *noise_sh,
+                   const float *amp_sh /*[S][n_sh][9]*/, const float2 *tau_sh /*[n_sh][9] or null*/,
+                   float ar_a, float ar_g, const float2 *old_coef, float2 *coef_out,
+                   const float2 *mfac /*[n_sh][9] Mx*My*/, float *mean_out);
+
+// ---- misc (ssp_misc.cu) ------------------------------------------------------------
+int launch_stats(ssp_ctx *ctx, int N, double dx, int B, const float2 *field, double roi_frac,
+                 ssp_stats *d_stats);
+int launch_welford(ssp_ctx *ctx, int N, int B, const float2 *field, float *mean, float *M2,
+                   long long count0);
+int launch_phase_mul(ssp_ctx *ctx, int N, int B, const float *theta, float sign,
+                     const float2 *in, float2 *out);
+int launch_phase_grad(ssp_ctx *ctx, long long n, const float2 *g, const float2 *u, float *grad);
+int launch_inner(ssp_ctx *ctx, int N, int B, const float2 *a, const float2 *b, double *out);
+int launch_lincomb(ssp_ctx *ctx, int N, int B, const float2 *coef /*dev [B][2] float2*/,
+                   const float2 *a, const float2 *b, float2 *out);
+
+} // namespace ssp

@@ -1,0 +1,235 @@
+// ssp_misc.cu -- statistics reducer (K8) and the small element-wise helpers.
+//
+// K8 (PAPER.md:423 S25, :143; O8): per field, raw intensity moments about the grid
+// centre in pixel units, accumulated per thread in fp64, combined by warp shuffles and one
+// fp64 atomic per warp; a one-thread-per-field finaliser turns them into ssp_stats.
+#include "ssp_internal.h"
+
+namespace ssp {
+
+enum { ACC_I = 0, ACC_X, ACC_Y, ACC_XX, ACC_YY, ACC_XY, ACC_RI, ACC_RI2, ACC_AXIS, ACC_N };
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// grid: (blocks_per_field, B).  Each thread walks float4 pairs (2 pixels) grid-stride.
+__global__ void __launch_bounds__(256) k_stats_accum(const float2 *__restrict__ field, int N, int lo, int hi,
+                                                      double *__restrict__ acc)
+{
+    const int b = blockIdx.y;
+    const size_t px = (size_t)N * N;
+    const float4 *f4 = reinterpret_cast<const float4 *>(field + (size_t)b * px);
+    double a[ACC_N];
+#pragma unroll
+    for (int i = 0; i < ACC_N; ++i) a[i] = 0.0;
+    const int half = N / 2;
+    for (size_t p2 = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p2 < px / 2;
+         p2 += (size_t)gridDim.x * blockDim.x) {
+        const float4 u = __ldg(f4 + p2);
+        const size_t p = 2 * p2;
+        const int iy = (int)(p / N), ix = (int)(p % N);
+        const float I2[2] = {fmaf(u.x, u.x, u.y * u.y), fmaf(u.z, u.z, u.w * u.w)};
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const double I = (double)I2[e];
+            const double x = (double)(ix + e - half), y = (double)(iy - half);
+            a[ACC_I] += I;
+            a[ACC_X] += x * I;
+            a[ACC_Y] += y * I;
+            a[ACC_XX] += x * x * I;
+            a[ACC_YY] += y * y * I;
+            a[ACC_XY] += x * y * I;
+            if (iy >= lo && iy < hi && ix + e >= lo && ix + e < hi) {
+                a[ACC_RI] += I;
+                a[ACC_RI2] += I * I;
+            }
+            if (iy == half && ix + e == half) a[ACC_AXIS] += I;
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < ACC_N; ++i) {
+        const double s = warp_sum(a[i]);
+        if ((threadIdx.x & 31) == 0 && s != 0.0) atomicAdd(acc + (size_t)b * ACC_N + i, s);
+    }
+}
+
+__global__ void k_stats_final(const double *__restrict__ acc, int B, double dx, long long roi_n,
+                              ssp_stats *__restrict__ out)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    const double *a = acc + (size_t)b * ACC_N;
+    ssp_stats s;
+    const double sI = a[ACC_I];
+    s.power = sI * dx * dx;
+    double cx = 0, cy = 0, sxx = 0, syy = 0, sxy = 0;
+    if (sI > 0) {
+        cx = a[ACC_X] / sI;
+        cy = a[ACC_Y] / sI;
+        sxx = a[ACC_XX] / sI - cx * cx;
+        syy = a[ACC_YY] / sI - cy * cy;
+        sxy = a[ACC_XY] / sI - cx * cy;
+    }
+    s.cx = cx * dx;
+    s.cy = cy * dx;
+    s.sxx = sxx * dx * dx;
+    s.syy = syy * dx * dx;
+    s.sxy = sxy * dx * dx;
+    const double tr = s.sxx + s.syy;
+    s.w2 = sqrt(2.0 * (tr > 0 ? tr : 0.0));
+    s.I_axis = a[ACC_AXIS];
+    s.roi_sumI = a[ACC_RI];
+    s.roi_sumI2 = a[ACC_RI2];
+    s.roi_n = roi_n;
+    out[b] = s;
+}
+
+int launch_stats(ssp_ctx *ctx, int N, double dx, int B, const float2 *field, double roi_frac,
+                 ssp_stats *d_stats)
+{
+    if (int rc = ensure_scratch(ctx, sizeof(double) * ACC_N * (size_t)B)) return rc;
+    double *acc = reinterpret_cast<double *>(ctx->scratch);
+    SSP_CUDA(ctx, cudaMemsetAsync(acc, 0, sizeof(double) * ACC_N * (size_t)B, ctx->stream));
+    int h = (int)floor(roi_frac * N / 2.0);
+    int lo = N / 2 - h, hi = N / 2 + h;
+    if (h <= 0) { lo = N / 2; hi = N / 2 + 1; }
+    if (lo < 0) lo = 0;
+    if (hi > N) hi = N;
+    const long long roi_n = (long long)(hi - lo) * (hi - lo);
+    const size_t pairs = (size_t)N * N / 2;
+    int bpf = (int)((pairs + 256 * 8 - 1) / (256 * 8)); // ~16 pixels per thread
+    if (bpf < 1) bpf = 1;
+    k_stats_accum<<<dim3(bpf, B), 256, 0, ctx->stream>>>(field, N, lo, hi, acc);
+    k_stats_final<<<(B + 127) / 128, 128, 0, ctx->stream>>>(acc, B, dx, roi_n, d_stats);
+    ctx->launches += 2;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
+// Welford per pixel, sequential over the B fields of this call.
+__global__ void __launch_bounds__(256) k_welford(const float2 *__restrict__ field, size_t px, int B,
+                                                  float *__restrict__ mean, float *__restrict__ M2, long long count0)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= px) return;
+    float m = mean[i], s = M2[i];
+    for (int b = 0; b < B; ++b) {
+        const float2 u = __ldg(field + (size_t)b * px + i);
+        const float I = fmaf(u.x, u.x, u.y * u.y);
+        const float d = I - m;
+        m += d / (float)(count0 + b + 1);
+        s = fmaf(d, I - m, s);
+    }
+    mean[i] = m;
+    M2[i] = s;
+}
+
+int launch_welford(ssp_ctx *ctx, int N, int B, const float2 *field, float *mean, float *M2, long long count0)
+{
+    const size_t px = (size_t)N * N;
+    k_welford<<<(unsigned)((px + 255) / 256), 256, 0, ctx->stream>>>(field, px, B, mean, M2, count0);
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
+__global__ void __launch_bounds__(256) k_phase_mul(const float *__restrict__ theta, float sign, size_t px, int B,
+                                                    const float2 *in, float2 *out)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= px) return;
+    float s, c;
+    sincosf(__ldg(theta + i), &s, &c); // masks are in [0, 2 pi): the accurate path is cheap enough here
+    s *= sign;
+    for (int b = 0; b < B; ++b) {
+        const float2 u = in[(size_t)b * px + i];
+        out[(size_t)b * px + i] = make_float2(fmaf(u.x, c, -u.y * s), fmaf(u.x, s, u.y * c));
+    }
+}
+
+int launch_phase_mul(ssp_ctx *ctx, int N, int B, const float *theta, float sign, const float2 *in, float2 *out)
+{
+    const size_t px = (size_t)N * N;
+    k_phase_mul<<<(unsigned)((px + 255) / 256), 256, 0, ctx->stream>>>(theta, sign, px, B, in, out);
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
+__global__ void __launch_bounds__(256) k_phase_grad(const float2 *__restrict__ g, const float2 *__restrict__ u,
+                                                     size_t n, float *__restrict__ grad)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float2 a = g[i], b = u[i];
+    grad[i] = a.y * b.x - a.x * b.y;
+}
+
+int launch_phase_grad(ssp_ctx *ctx, long long n, const float2 *g, const float2 *u, float *grad)
+{
+    k_phase_grad<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(g, u, (size_t)n, grad);
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
+// out[b] = { Re<a,b>, Im<a,b>, |a|^2, |b|^2 },  <a,b> = sum conj(a) b
+__global__ void __launch_bounds__(256) k_inner(const float2 *__restrict__ A, const float2 *__restrict__ Bf,
+                                                size_t px, double *__restrict__ out)
+{
+    const int b = blockIdx.y;
+    double r = 0, im = 0, na = 0, nb = 0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < px; i += (size_t)gridDim.x * blockDim.x) {
+        const float2 x = __ldg(A + (size_t)b * px + i), y = __ldg(Bf + (size_t)b * px + i);
+        r += (double)x.x * y.x + (double)x.y * y.y;
+        im += (double)x.x * y.y - (double)x.y * y.x;
+        na += (double)x.x * x.x + (double)x.y * x.y;
+        nb += (double)y.x * y.x + (double)y.y * y.y;
+    }
+    r = warp_sum(r); im = warp_sum(im); na = warp_sum(na); nb = warp_sum(nb);
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(out + 4 * b + 0, r);
+        atomicAdd(out + 4 * b + 1, im);
+        atomicAdd(out + 4 * b + 2, na);
+        atomicAdd(out + 4 * b + 3, nb);
+    }
+}
+
+int launch_inner(ssp_ctx *ctx, int N, int B, const float2 *a, const float2 *b, double *out)
+{
+    const size_t px = (size_t)N * N;
+    SSP_CUDA(ctx, cudaMemsetAsync(out, 0, sizeof(double) * 4 * (size_t)B, ctx->stream));
+    int bpf = (int)((px + 256 * 16 - 1) / (256 * 16));
+    k_inner<<<dim3(bpf, B), 256, 0, ctx->stream>>>(a, b, px, out);
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
+__global__ void __launch_bounds__(256) k_lincomb(const float2 *__restrict__ coef, const float2 *a, const float2 *b,
+                                                  size_t px, float2 *out)
+{
+    const int f = blockIdx.y;
+    const float2 al = coef[2 * f], be = coef[2 * f + 1];
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < px; i += (size_t)gridDim.x * blockDim.x) {
+        const float2 x = a[(size_t)f * px + i], y = b[(size_t)f * px + i];
+        out[(size_t)f * px + i] = make_float2(al.x * x.x - al.y * x.y + be.x * y.x - be.y * y.y,
+                                              al.x * x.y + al.y * x.x + be.x * y.y + be.y * y.x);
+    }
+}
+
+int launch_lincomb(ssp_ctx *ctx, int N, int B, const float2 *coef, const float2 *a, const float2 *b, float2 *out)
+{
+    const size_t px = (size_t)N * N;
+    int bpf = (int)((px + 256 * 4 - 1) / (256 * 4));
+    k_lincomb<<<dim3(bpf, B), 256, 0, ctx->stream>>>(coef, a, b, px, out);
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
+} // namespace ssp

@@ -1,0 +1,226 @@
+// ssp_screens.cu -- phase-screen generator and AR evolver (K1-K3).
+//
+//   k_sh_prep    : subharmonic coefficients c_pab (+ AR recursion) and the analytic mean of phi_lo
+//   k_screen_col : K1 spectral filter / AR prologue fused into K2, the inverse FFT along y
+//   k_screen_row : K3 inverse FFT along x, real part, + subharmonics - mean
+// (PAPER.md:359 S16; :57 Eq.2; :63 Eq.3; :80 Eq.5; :74 Eq.4.)
+#include "ssp_internal.h"
+#include "ssp_lines.cuh"
+
+namespace ssp {
+
+// sqrt of the frequency-dependent part of Phi^f at squared frequency f2 (cycles/m)^2.
+// The scalar part (0.023 r0^-5/3, or the oceanic constants) and df are in the per-slab amplitude.
+__device__ __forceinline__ float psd_shape_sqrt(const ScreenFilter &f, float f2)
+{
+    if (f.kind == SSP_PSD_OCEAN_NIKISHOV) {
+        const float kap = f.two_pi * sqrtf(f2);
+        const float ke = kap * f.eta;
+        const float ke23 = exp2f(0.66666667f * __log2f(ke));
+        const float delta = 8.284f * ke23 * ke23 + 12.978f * ke * ke;
+        const float br = f.w * f.w * __expf(-1.863e-2f * delta) + __expf(-1.9e-4f * delta)
+                         - 2.f * f.w * __expf(-9.41e-3f * delta);
+        return exp2f(-1.8333334f * __log2f(kap)) * sqrtf(fmaxf((1.f + 2.35f * ke23) * br, 0.f));
+    }
+    // von Karman / Kolmogorov: exp(-f2/(2 fm^2)) (f2 + f0^2)^(-11/12)
+    return exp2f(fmaf(-0.91666667f, __log2f(f2 + f.f0sq), -f2 * f.inv_fm2_log2e));
+}
+
+template <int N>
+__global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_screen_col(const ScreenColArgs a)
+{
+    using PI = PlanInfo<N>;
+    using CFG = ColCfg<N>;
+    constexpr int E = PI::E, T = PI::T, C = CFG::C, R1 = PI::R1, RL = PI::RL;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *smem = reinterpret_cast<float2 *>(smem_raw);
+    const int tid = threadIdx.x;
+    const int c = tid % C, t = tid / C;
+    constexpr int GROUPS = N / C;
+    const int scr = blockIdx.x / GROUPS, kx = (blockIdx.x % GROUPS) * C + c;
+    ColSmem<C> sm{smem + c};
+
+    const float amp_s = __ldg(a.amp + (a.g0 + scr) % a.S);
+    const float kxs = (float)((kx < N / 2) ? kx : kx - N);
+    const float df2 = a.flt.df * a.flt.df;
+    const size_t base = (size_t)scr * N * N + kx;
+    const bool ar = a.old_spec != nullptr;
+    float2 tx = make_float2(1.f, 0.f);
+    if (ar && a.taux) tx = __ldg(a.taux + kx);
+
+    float2 v[E];
+#pragma unroll
+    for (int i = 0; i < E / R1; ++i)
+#pragma unroll
+        for (int q = 0; q < R1; ++q) {
+            const int ky = line_index<N, R1>(t, i, q);
+            const float kys = (float)((ky < N / 2) ? ky : ky - N);
+            const float2 nz = a.noise[base + (size_t)ky * N];
+            const float f2 = (kxs * kxs + kys * kys) * df2;
+            float amp = (kx == 0 && ky == 0) ? 0.f : amp_s * psd_shape_sqrt(a.flt, f2);
+            float2 Cv = make_float2(nz.x * amp, nz.y * amp);
+            if (ar) {
+                float2 old = a.old_spec[base + (size_t)ky * N];
+                if (a.taux) old = cmul(old, cmul(tx, __ldg(a.tauy + ky)));
+                Cv = make_float2(fmaf(a.ar_a, old.x, a.ar_g * Cv.x), fmaf(a.ar_a, old.y, a.ar_g * Cv.y));
+            }
+            if (a.spec_out) a.spec_out[base + (size_t)ky * N] = Cv;
+            v[i * R1 + q] = Cv;
+        }
+    fft_line<N, false, true>(v, t, sm, a.tw); // unnormalised inverse along y
+    float2 *dst = a.out + base;
+#pragma unroll
+    for (int i = 0; i < E / RL; ++i)
+#pragma unroll
+        for (int q = 0; q < RL; ++q) dst[(size_t)line_index<N, RL>(t, i, q) * N] = v[i * RL + q];
+}
+
+template <int N>
+__global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_screen_row(const ScreenRowArgs a)
+{
+    using PI = PlanInfo<N>;
+    using CFG = RowCfg<N>;
+    constexpr int E = PI::E, T = PI::T, R1 = PI::R1, RL = PI::RL;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *smem = reinterpret_cast<float2 *>(smem_raw);
+    const int tid = threadIdx.x;
+    const int lib = tid / T, t = tid % T;
+    const long long line = (long long)blockIdx.x * CFG::LPB + lib;
+    const int scr = (int)(line / N), iy = (int)(line % N);
+    RowSmem<CFG::WARP_LOCAL> sm{smem + (size_t)lib * PI::LINE_ELEMS};
+
+    float2 v[E];
+    const float2 *src = a.in + line * N;
+#pragma unroll
+    for (int i = 0; i < E / R1; ++i)
+#pragma unroll
+        for (int q = 0; q < R1; ++q) v[i * R1 + q] = src[line_index<N, R1>(t, i, q)];
+    fft_line<N, false, true>(v, t, sm, a.tw); // unnormalised inverse along x; strided by RL
+
+    float mean = 0.f;
+    if (a.n_sh > 0) {
+        // phi_lo(ix,iy) = sum_p Re( d_p0 conj(ex) + d_p1 + d_p2 ex ),  d_pb = c_p0b conj(ey) + c_p1b + c_p2b ey
+        mean = __ldg(a.sh_mean + scr);
+        for (int p = 0; p < a.n_sh; ++p) {
+            const float2 *cf = a.sh_coef + ((size_t)scr * a.n_sh + p) * 9;
+            const float2 ey = __ldg(a.ex + (size_t)p * N + iy);
+            float2 d[3];
+#pragma unroll
+            for (int bb = 0; bb < 3; ++bb) {
+                const float2 c0 = __ldg(cf + bb), c1 = __ldg(cf + 3 + bb), c2 = __ldg(cf + 6 + bb);
+                const float2 lo = cmul_conj(c0, ey), hi = cmul(c2, ey);
+                d[bb] = make_float2(lo.x + c1.x + hi.x, lo.y + c1.y + hi.y);
+            }
+#pragma unroll
+            for (int i = 0; i < E / RL; ++i)
+#pragma unroll
+                for (int q = 0; q < RL; ++q) {
+                    const float2 ex = __ldg(a.ex + (size_t)p * N + line_index<N, RL>(t, i, q));
+                    // Re(d0 conj(ex)) + Re(d1) + Re(d2 ex)
+                    float r = fmaf(d[0].x, ex.x, d[0].y * ex.y) + d[1].x + fmaf(d[2].x, ex.x, -d[2].y * ex.y);
+                    v[i * RL + q].x += r;
+                }
+        }
+    }
+    float *dst = a.screens + line * N;
+#pragma unroll
+    for (int i = 0; i < E / RL; ++i)
+#pragma unroll
+        for (int q = 0; q < RL; ++q) dst[line_index<N, RL>(t, i, q)] = v[i * RL + q].x - mean;
+}
+
+// one block per screen, one thread per (p, a, b)
+__global__ void __launch_bounds__(96) k_sh_prep(int S, int n_sh, const float2 *__restrict__ noise_sh,
+                                                 const float *__restrict__ amp_sh, const float2 *__restrict__ tau_sh,
+                                                 float ar_a, float ar_g, const float2 *old_coef, float2 *coef_out,
+                                                 const float2 *__restrict__ mfac, float *__restrict__ mean_out)
+{
+    __shared__ float red[96];
+    const int scr = blockIdx.x, i = threadIdx.x, s = scr % S;
+    float contrib = 0.f;
+    if (i < 9 * n_sh) {
+        const size_t idx = (size_t)scr * n_sh * 9 + i;
+        const float amp = __ldg(amp_sh + (size_t)s * n_sh * 9 + i); // 0 at the centre
+        const float2 nz = noise_sh[idx];
+        float2 cv = make_float2(nz.x * amp, nz.y * amp);
+        if (old_coef) {
+            float2 old = old_coef[idx];
+            if (tau_sh) old = cmul(old, __ldg(tau_sh + i));
+            cv = make_float2(fmaf(ar_a, old.x, ar_g * cv.x), fmaf(ar_a, old.y, ar_g * cv.y));
+        }
+        coef_out[idx] = cv;
+        const float2 m = __ldg(mfac + i);
+        contrib = cv.x * m.x - cv.y * m.y;
+    }
+    red[i] = contrib;
+    __syncthreads();
+    if (i == 0) {
+        float sum = 0.f;
+        for (int k = 0; k < 9 * n_sh; ++k) sum += red[k];
+        mean_out[scr] = sum;
+    }
+}
+
+// ---- launchers ------------------------------------------------------------------------
+template <int N>
+static int launch_screen_col_n(ssp_ctx *ctx, const ScreenColArgs &a)
+{
+    using CFG = ColCfg<N>;
+    auto kern = k_screen_col<N>;
+    if (CFG::SMEM > 48 * 1024)
+        SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::SMEM));
+    kern<<<a.nscr * (N / CFG::C), CFG::THREADS, CFG::SMEM, ctx->stream>>>(a);
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
+template <int N>
+static int launch_screen_row_n(ssp_ctx *ctx, const ScreenRowArgs &a)
+{
+    using CFG = RowCfg<N>;
+    auto kern = k_screen_row<N>;
+    if (CFG::SMEM > 48 * 1024)
+        SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::SMEM));
+    kern<<<(unsigned)((long long)a.nscr * N / CFG::LPB), CFG::THREADS, CFG::SMEM, ctx->stream>>>(a);
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
+#define SSP_DISPATCH_N(N_, EXPR)                                   \
+    switch (N_) {                                                  \
+    case 8: { constexpr int NN = 8; return EXPR; }                 \
+    case 16: { constexpr int NN = 16; return EXPR; }               \
+    case 32: { constexpr int NN = 32; return EXPR; }               \
+    case 64: { constexpr int NN = 64; return EXPR; }               \
+    case 128: { constexpr int NN = 128; return EXPR; }             \
+    case 256: { constexpr int NN = 256; return EXPR; }             \
+    case 512: { constexpr int NN = 512; return EXPR; }             \
+    case 1024: { constexpr int NN = 1024; return EXPR; }           \
+    case 2048: { constexpr int NN = 2048; return EXPR; }           \
+    case 4096: { constexpr int NN = 4096; return EXPR; }           \
+    default: return ctx->fail(SSP_EINVAL, "unsupported N=%d", N_); \
+    }
+
+int launch_screen_col(ssp_ctx *ctx, int N, const ScreenColArgs &a)
+{
+    SSP_DISPATCH_N(N, (launch_screen_col_n<NN>(ctx, a)));
+}
+int launch_screen_row(ssp_ctx *ctx, int N, const ScreenRowArgs &a)
+{
+    SSP_DISPATCH_N(N, (launch_screen_row_n<NN>(ctx, a)));
+}
+
+int launch_sh_prep(ssp_ctx *ctx, int nscr, int S, int n_sh, const float2 *noise_sh, const float *amp_sh,
+                   const float2 *tau_sh, float ar_a, float ar_g, const float2 *old_coef, float2 *coef_out,
+                   const float2 *mfac, float *mean_out)
+{
+    k_sh_prep<<<nscr, 96, 0, ctx->stream>>>(S, n_sh, noise_sh, amp_sh, tau_sh, ar_a, ar_g, old_coef, coef_out,
+                                            mfac, mean_out);
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
+} // namespace ssp

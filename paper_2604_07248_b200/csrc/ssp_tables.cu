@@ -1,0 +1,141 @@
+// ssp_tables.cu -- small device tables owned by the context: FFT inter-stage twiddles,
+// 1-D transfer-function tables, sign tables.  All built in double on the host (SURVEY.md
+// section 7, H4: pi*lambda*dz*f^2 reaches hundreds of radians; fp32 device sincos of it
+// would lose the phase), rounded once to fp32 and cached.
+#include <cmath>
+
+#include "ssp_fft.cuh"
+#include "ssp_internal.h"
+
+namespace ssp {
+
+bool valid_N(int N) { return N >= 8 && N <= 4096 && (N & (N - 1)) == 0; }
+
+static int upload(ssp_ctx *ctx, const std::vector<float2> &h, float2 **out)
+{
+    float2 *d = nullptr;
+    SSP_CUDA(ctx, cudaMalloc(&d, h.size() * sizeof(float2)));
+    // pageable source: cudaMemcpyAsync stages it before returning, so `h` may die afterwards
+    cudaError_t e = cudaMemcpyAsync(d, h.data(), h.size() * sizeof(float2), cudaMemcpyHostToDevice, ctx->stream);
+    if (e != cudaSuccess) {
+        cudaFree(d);
+        return ctx->fail(SSP_ECUDA, "table upload failed: %s", cudaGetErrorString(e));
+    }
+    *out = d;
+    return SSP_OK;
+}
+
+static float2 wn(long long e, int N) // exp(-i 2 pi e / N), e reduced mod N first
+{
+    const double kPi = 3.14159265358979323846;
+    e %= N;
+    double ang = -2.0 * kPi * (double)e / (double)N;
+    return make_float2((float)cos(ang), (float)sin(ang));
+}
+
+template <int N>
+static void fill_twiddles(std::vector<float2> &h)
+{
+    using PI = PlanInfo<N>;
+    h.assign(PI::TW_TOTAL, make_float2(1.f, 0.f));
+    // forward plan (R1, R2, R3)
+    for (int k = 0; k < PI::R1; ++k)
+        for (int m = 0; m < N / PI::R1; ++m) h[PI::TW1 + k * (N / PI::R1) + m] = wn((long long)m * k, N);
+    for (int k = 0; k < PI::R2; ++k)
+        for (int n3 = 0; n3 < PI::R3; ++n3) h[PI::TW2 + k * PI::R3 + n3] = wn((long long)PI::R1 * n3 * k, N);
+    // reversed plan (RL, .., R1): first radix RL, third radix R1
+    for (int k = 0; k < PI::RL; ++k)
+        for (int m = 0; m < N / PI::RL; ++m) h[PI::TW1R + k * (N / PI::RL) + m] = wn((long long)m * k, N);
+    for (int k = 0; k < PI::R2; ++k)
+        for (int n3 = 0; n3 < PI::R1; ++n3) h[PI::TW2R + k * PI::R1 + n3] = wn((long long)PI::RL * n3 * k, N);
+}
+
+int get_twiddles(ssp_ctx *ctx, int N, const float2 **out)
+{
+    auto it = ctx->twiddles.find(N);
+    if (it != ctx->twiddles.end()) { *out = it->second; return SSP_OK; }
+    std::vector<float2> h;
+    switch (N) {
+    case 8: fill_twiddles<8>(h); break;
+    case 16: fill_twiddles<16>(h); break;
+    case 32: fill_twiddles<32>(h); break;
+    case 64: fill_twiddles<64>(h); break;
+    case 128: fill_twiddles<128>(h); break;
+    case 256: fill_twiddles<256>(h); break;
+    case 512: fill_twiddles<512>(h); break;
+    case 1024: fill_twiddles<1024>(h); break;
+    case 2048: fill_twiddles<2048>(h); break;
+    case 4096: fill_twiddles<4096>(h); break;
+    default: return ctx->fail(SSP_EINVAL, "unsupported N=%d", N);
+    }
+    float2 *d = nullptr;
+    if (int rc = upload(ctx, h, &d)) return rc;
+    ctx->twiddles[N] = d;
+    *out = d;
+    return SSP_OK;
+}
+
+// h[k] = exp(-+ i pi lam_eff dz f_k^2) [/ N^2], f_k in FFT order (negative Nyquist).
+// The Fresnel kernel is separable: H(kx,ky) = h[kx] h[ky]  (north_star).
+int get_htable(ssp_ctx *ctx, const HKey &key, const float2 **out)
+{
+    auto it = ctx->htables.find(key);
+    if (it != ctx->htables.end()) { *out = it->second; return SSP_OK; }
+    if (ctx->htables.size() > 4096) { // unbounded dz lists: drop the cache rather than grow
+        SSP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        for (auto &kv : ctx->htables) cudaFree(kv.second);
+        ctx->htables.clear();
+    }
+    const double kPi = 3.14159265358979323846;
+    const int N = key.N;
+    std::vector<float2> h(N);
+    const double scale = key.scaled ? 1.0 / ((double)N * (double)N) : 1.0;
+    for (int k = 0; k < N; ++k) {
+        const int ks = (k < N / 2) ? k : k - N;
+        const double f = (double)ks / ((double)N * key.dx);
+        double ang = -kPi * key.lam_eff * key.dz * f * f;
+        ang = fmod(ang, 2.0 * kPi);
+        if (key.conj) ang = -ang;
+        h[k] = make_float2((float)(scale * cos(ang)), (float)(scale * sin(ang)));
+    }
+    float2 *d = nullptr;
+    if (int rc = upload(ctx, h, &d)) return rc;
+    ctx->htables[key] = d;
+    *out = d;
+    return SSP_OK;
+}
+
+// s[k] = (-1)^k: the centred DFT is (-1)^k FFT((-1)^n x) / sqrt(N) per axis (N % 4 == 0).
+int get_sign_table(ssp_ctx *ctx, int N, const float2 **out)
+{
+    auto it = ctx->sign_tables.find(N);
+    if (it != ctx->sign_tables.end()) { *out = it->second; return SSP_OK; }
+    std::vector<float2> h(2 * N);
+    const double s = 1.0 / sqrt((double)N);
+    for (int k = 0; k < N; ++k) {
+        h[k] = make_float2((k & 1) ? -1.f : 1.f, 0.f);             // plain signs
+        h[N + k] = make_float2((float)((k & 1) ? -s : s), 0.f);    // signs / sqrt(N)
+    }
+    float2 *d = nullptr;
+    if (int rc = upload(ctx, h, &d)) return rc;
+    ctx->sign_tables[N] = d;
+    *out = d;
+    return SSP_OK;
+}
+
+int ensure_scratch(ssp_ctx *ctx, size_t bytes)
+{
+    if (bytes <= ctx->scratch_bytes) return SSP_OK;
+    if (ctx->scratch) {
+        SSP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->scratch);
+        ctx->scratch = nullptr;
+        ctx->scratch_bytes = 0;
+    }
+    size_t want = bytes < (1u << 16) ? (1u << 16) : bytes;
+    SSP_CUDA(ctx, cudaMalloc(&ctx->scratch, want));
+    ctx->scratch_bytes = want;
+    return SSP_OK;
+}
+
+} // namespace ssp

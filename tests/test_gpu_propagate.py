@@ -1,0 +1,212 @@
+"""GPU parity: split-step propagation, adjoint and statistics through the C ABI vs the CPU oracle.
+
+Bar (BASELINE.json north_star): per-field relative L2 error <= 2e-5 * log2(N) * screens."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2604_07248_b200 import synth
+from tests.util import rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ssp():
+    import torch
+    from paper_2604_07248_b200 import api, build
+    build.build()
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    ctx = api.Context(0)
+    yield ctx
+    ctx.close()
+
+
+def cu(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def tol(N, n_screens):
+    return 2e-5 * math.log2(N) * max(1, n_screens)
+
+
+def _case(N, B, n_steps, S, seed):
+    dx, lam = 1e-3, 1.0e-6
+    rng = np.random.default_rng(seed)
+    # steps of the order of the aliasing-free distance N dx^2 / lambda, uneven on purpose
+    dz = (N * dx * dx / lam) * (0.1 + 0.3 * rng.random(n_steps))
+    u0 = synth.random_field(N, B, seed)
+    scr = synth.random_screens(N, B, max(S, 1), seed, rms=3.0)[:, :S]
+    return dx, lam, dz, u0, scr
+
+
+@pytest.mark.parametrize("N", [8, 16, 32, 64, 128, 256, 512, 1024])
+def test_propagate_parity_all_plans(ssp, orc, N):
+    """Every FFT plan (1, 2 stages), per-realisation screens, window on, uneven dz."""
+    B, n_steps, S = (3, 3, 3) if N <= 512 else (2, 2, 2)
+    dx, lam, dz, u0, scr = _case(N, B, n_steps, S, N)
+    ref = orc.propagate(N, dx, lam, dz, u0, scr, win_order=16, win_sigma_frac=0.47)
+    out = ssp.propagate(N, dx, lam, list(dz), cu(u0), cu(scr), win_order=16, win_sigma_frac=0.47)
+    err = rel_l2(out.cpu().numpy(), ref)
+    assert err.max() < tol(N, S), err
+    assert err.max() < 5e-6 * n_steps + 1e-6, err        # what fp32 actually delivers
+
+
+@pytest.mark.parametrize("N", [2048, 4096])
+def test_propagate_parity_three_stage_plans(ssp, orc, N):
+    B, n_steps, S = 1, 2, 2
+    dx, lam, dz, u0, scr = _case(N, B, n_steps, S, N)
+    ref = orc.propagate(N, dx, lam, dz, u0, scr, win_order=16, win_sigma_frac=0.47)
+    out = ssp.propagate(N, dx, lam, list(dz), cu(u0), cu(scr), win_order=16, win_sigma_frac=0.47)
+    err = rel_l2(out.cpu().numpy(), ref)
+    assert err.max() < tol(N, S), err
+
+
+def test_propagate_variants(ssp, orc):
+    """In place, shared stack, trailing vacuum step (S = n_steps - 1), no window, n0, planes."""
+    import torch
+    N, B, n_steps = 64, 3, 4
+    dx, lam, dz, u0, scr = _case(N, B, n_steps, 3, 7)
+    # shared stack + trailing vacuum step + refractive index
+    ref = orc.propagate(N, dx, lam, dz, u0, scr[0], shared_screens=True, n0=1.33)
+    d = cu(u0)
+    out = ssp.propagate(N, dx, lam, list(dz), d, cu(scr[0]), shared_screens=True, n0=1.33, out=d)  # in place
+    assert out.data_ptr() == d.data_ptr()
+    assert rel_l2(out.cpu().numpy(), ref).max() < tol(N, 3)
+    # vacuum only (S = 0)
+    ref = orc.propagate(N, dx, lam, dz, u0)
+    out = ssp.propagate(N, dx, lam, list(dz), cu(u0))
+    assert rel_l2(out.cpu().numpy(), ref).max() < tol(N, 1)
+    # saved planes = field after every complete step
+    ref, ref_planes = orc.propagate(N, dx, lam, dz, u0, scr, win_order=8, win_sigma_frac=0.45, return_planes=True)
+    planes = torch.empty((B, n_steps, N, N), dtype=torch.complex64, device="cuda")
+    out = ssp.propagate(N, dx, lam, list(dz), cu(u0), cu(scr), win_order=8, win_sigma_frac=0.45, planes=planes)
+    assert rel_l2(planes.cpu().numpy(), ref_planes).max() < tol(N, 3)
+    assert torch.equal(planes[:, -1], out)
+
+
+def test_config1_full(ssp, orc):
+    """BASELINE.json configs[0] in full: 128^2, 5 von Karman screens + 3 subharmonic levels, 4 realisations,
+    Gaussian beam, super-Gaussian window; received field, beam width, scintillation index."""
+    from paper_2604_07248_b200 import api
+    wl = synth.CONFIGS[1]
+    N, B, S = wl.N, wl.B, wl.S
+    hi, sh = synth.noise_batch(1, 0, B, S, N, wl.n_sh)
+    psd_o = orc.Psd(**wl.psd_dict())
+    scr_ref, _, _ = orc.make_screens(N, wl.dx, psd_o, wl.lam, wl.cn2_list, wl.dz, wl.n_sh, hi, sh)
+    scr32 = scr_ref.astype(np.float32)                       # the same fp32 screens feed both sides
+    u0 = synth.input_field(wl)
+    ref = orc.propagate(N, wl.dx, wl.lam, wl.dz, u0, scr32, win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
+    import torch
+    stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+    out = ssp.propagate(N, wl.dx, wl.lam, list(wl.dz), cu(u0), cu(scr32), win_order=wl.win_order,
+                        win_sigma_frac=wl.win_sigma_frac, stats=stats, roi_frac=0.25)
+    err = rel_l2(out.cpu().numpy(), ref)
+    assert err.max() < tol(N, S), err
+    st_ref = orc.beam_stats(N, wl.dx, ref, roi_frac=0.25)
+    st = api.stats_to_dicts(stats)
+    for a, b in zip(st, st_ref):
+        for k in ("power", "w2", "sxx", "syy", "roi_sumI", "roi_sumI2", "I_axis"):
+            assert abs(a[k] / b[k] - 1) < 1e-4, (k, a[k], b[k])
+        assert abs(a["cx"] - b["cx"]) < 1e-4 * wl.dx * N and abs(a["cy"] - b["cy"]) < 1e-4 * wl.dx * N
+        assert abs(a["sxy"] - b["sxy"]) < 1e-4 * (b["sxx"] + b["syy"])
+        assert a["roi_n"] == b["roi_n"]
+
+
+def test_adjoint_parity_and_gradient(ssp, orc):
+    import torch
+    N, B, n_steps, S = 64, 2, 4, 3
+    dx, lam, dz, u0, scr = _case(N, B, n_steps, S, 21)
+    kw = dict(win_order=8, win_sigma_frac=0.45)
+    out_ref, planes_ref = orc.propagate(N, dx, lam, dz, u0, scr, return_planes=True, **kw)
+    g_out = synth.random_field(N, B, 22)
+    gin_ref, grad_ref = orc.propagate_adjoint(N, dx, lam, dz, g_out, scr, planes=planes_ref.astype(np.complex64), **kw)
+    planes = cu(planes_ref.astype(np.complex64))
+    grad = torch.zeros((B, S, N, N), dtype=torch.float32, device="cuda")
+    gin = ssp.propagate_adjoint(N, dx, lam, list(dz), cu(g_out), cu(scr), planes=planes, phase_grad=grad, **kw)
+    assert rel_l2(gin.cpu().numpy(), gin_ref).max() < tol(N, S)
+    gerr = rel_l2(grad.cpu().numpy(), grad_ref)
+    assert gerr.max() < tol(N, S + 2), gerr
+    # without gradient outputs, in place
+    d = cu(g_out)
+    gin2 = ssp.propagate_adjoint(N, dx, lam, list(dz), d, cu(scr), out=d, **kw)
+    assert rel_l2(gin2.cpu().numpy(), gin_ref).max() < tol(N, S)
+
+
+@pytest.mark.parametrize("N", [32, 256, 1024])
+def test_adjoint_identity_on_gpu(ssp, N):
+    """<A x, y> = <x, A^H y> evaluated entirely on the GPU path (a property that holds at any size)."""
+    B, n_steps, S = 2, 3, 3
+    dx, lam, dz, x, scr = _case(N, B, n_steps, S, 31)
+    y = synth.random_field(N, B, 32)
+    kw = dict(win_order=16, win_sigma_frac=0.47)
+    Ax = ssp.propagate(N, dx, lam, list(dz), cu(x), cu(scr), **kw)
+    AHy = ssp.propagate_adjoint(N, dx, lam, list(dz), cu(y), cu(scr), **kw)
+    ip1 = ssp.inner_products(N, dx, cu(y), Ax).cpu().numpy()       # <y, A x>
+    ip2 = ssp.inner_products(N, dx, AHy, cu(x)).cpu().numpy()      # <A^H y, x>
+    for b in range(B):
+        lhs = complex(ip1[b, 0], ip1[b, 1])
+        rhs = complex(ip2[b, 0], ip2[b, 1])
+        scale = math.sqrt(ip1[b, 2] * ip1[b, 3])
+        assert abs(lhs - rhs) < 2e-6 * n_steps * scale, (lhs, rhs)
+
+
+def test_beam_stats_and_welford(ssp, orc):
+    import torch
+    from paper_2604_07248_b200 import api
+    N, dx, B = 128, 2e-3, 5
+    rng = np.random.default_rng(3)
+    x = synth.coords(N, dx)
+    X, Y = np.meshgrid(x, x)
+    fields = []
+    for b in range(B):
+        x0, y0, wx, wy = rng.normal(0, 0.02), rng.normal(0, 0.02), 0.02 + 0.02 * rng.random(), 0.02 + 0.02 * rng.random()
+        fields.append(np.exp(-((X - x0) / wx) ** 2 - ((Y - y0) / wy) ** 2 + 1j * rng.random() * X * 30))
+    u = (np.stack(fields) + 0.01 * synth.random_field(N, B, 5)).astype(np.complex64)
+    for roi in (0.0, 0.3, 1.0):
+        st_ref = orc.beam_stats(N, dx, u, roi_frac=roi)
+        stats, _ = ssp.beam_stats(N, dx, cu(u), roi_frac=roi)
+        for a, r in zip(api.stats_to_dicts(stats), st_ref):
+            for k in ("power", "w2", "sxx", "syy", "I_axis", "roi_sumI", "roi_sumI2"):
+                assert abs(a[k] / r[k] - 1) < 1e-6, (roi, k, a[k], r[k])
+            for k in ("cx", "cy"):
+                assert abs(a[k] - r[k]) < 1e-7 * dx * N
+            assert abs(a["sxy"] - r["sxy"]) < 1e-6 * (r["sxx"] + r["syy"])
+            assert a["roi_n"] == r["roi_n"]
+    mean = torch.zeros((N, N), dtype=torch.float32, device="cuda")
+    M2 = torch.zeros((N, N), dtype=torch.float32, device="cuda")
+    _, cnt = ssp.beam_stats(N, dx, cu(u[:2]), mean=mean, M2=M2, count=0)
+    _, cnt = ssp.beam_stats(N, dx, cu(u[2:]), mean=mean, M2=M2, count=cnt)
+    m_ref, M2_ref = np.zeros((N, N)), np.zeros((N, N))
+    c_ref = orc.welford(N, u, m_ref, M2_ref, 0)
+    assert cnt == c_ref == B
+    np.testing.assert_allclose(mean.cpu().numpy(), m_ref, rtol=2e-5, atol=1e-7)
+    np.testing.assert_allclose(M2.cpu().numpy(), M2_ref, rtol=2e-4, atol=1e-7)
+
+
+def test_error_codes(ssp):
+    import torch
+    from paper_2604_07248_b200 import api
+    N, dx, lam = 64, 1e-3, 1e-6
+    u = torch.zeros((1, N, N), dtype=torch.complex64, device="cuda")
+    scr = torch.zeros((1, 2, N, N), dtype=torch.float32, device="cuda")
+    with pytest.raises(api.SspError) as e:
+        ssp.propagate(48, dx, lam, [1.0], torch.zeros((1, 48, 48), dtype=torch.complex64, device="cuda"))
+    assert e.value.code == api.EINVAL
+    with pytest.raises(api.SspError) as e:
+        ssp.propagate(N, dx, lam, [1.0], u, scr)                  # S = 2 > n_steps = 1
+    assert e.value.code == api.EINVAL
+    with pytest.raises(api.SspError) as e:
+        ssp.propagate(N, dx, lam, [1.0, -2.0], u)
+    assert e.value.code == api.EINVAL
+    with pytest.raises(api.SspError) as e:
+        ssp.propagate(N, dx, lam, [1.0], u, h_kind=api.H_ANGULAR_SPECTRUM)
+    assert e.value.code == api.EUNSUPPORTED
+    with pytest.raises(api.SspError) as e:
+        ssp.propagate(N, dx, -1.0, [1.0], u)
+    assert e.value.code == api.EINVAL
+    with pytest.raises(TypeError):
+        ssp.propagate(N, dx, lam, [1.0], u.cpu())                # no CPU fallback
+    assert ssp.launch_count() >= 0
