@@ -1,0 +1,343 @@
+#!/usr/bin/env python
+"""bench.py -- whole-hot-path throughput of the split-step phase-screen library on B200.
+
+One "step" = one frame of the temporal workload (BASELINE.json configs[2], 1024^2): evolve every
+screen by one AR step (K1-K3), propagate the field batch through the stack (K4-K6), reduce the
+beam statistics (K8) and run the adjoint propagation (K7).  Metric: split-step screen-steps/s,
+counting forward and adjoint screen-steps; the AR evolution and the statistics are overhead
+inside the timed region.  See DESIGN.md section 7.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--batch B]
+Under torchrun each rank runs its own batch on its own GPU (weak scaling, no data-path collective).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "split-step screen-steps/sec (complex64 N^2 field)"
+UNIT = "screen-steps/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config id (1-5)")
+    ap.add_argument("--batch", type=int, default=0, help="override realisations per GPU")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, reasons, mx = [], set(), None
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx = float(parts[1])
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=mx, reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ---------------------------------------------------------------------------------------------
+# the oracle legs (cpu_baseline and --impl reference): oracle/ as it stands, on the host cores
+# ---------------------------------------------------------------------------------------------
+def oracle_frame(wl, S_s, seed=0, reps=1):
+    """Time `reps` frames of the same path on ONE realisation and S_s screens with the CPU oracle.
+    Returns (seconds per frame, screen-steps per frame)."""
+    import numpy as np
+    from oracle import orc
+    from paper_2604_07248_b200 import synth
+    N = wl.N
+    psd = orc.Psd(**wl.psd_dict())
+    cn2, dz = wl.cn2_list[:S_s], wl.dz[:S_s]
+    frames = synth.noise(wl.cid, seed, 0, S_s, N, wl.n_sh, frames=reps + 1)
+    hi0, sh0 = frames[0]
+    _, spec, shc = orc.make_screens(N, wl.dx, psd, wl.lam, cn2, dz, wl.n_sh, hi0[None], sh0[None])
+    u0 = synth.input_field(wl, 1)
+    a = wl.ar_a if wl.ar_a > 0 else 0.99
+    kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
+    t0 = time.perf_counter()
+    for r in range(reps):
+        hi, sh = frames[r + 1]
+        scr = orc.evolve_screens(N, wl.dx, psd, wl.lam, cn2, dz, wl.n_sh, a, 0.0, 0.0, 0.0, hi[None], sh[None], spec, shc)
+        out = orc.propagate(N, wl.dx, wl.lam, dz, u0, scr, **kw)
+        orc.beam_stats(N, wl.dx, out)
+        orc.propagate_adjoint(N, wl.dx, wl.lam, dz, out, scr, **kw)
+    dt = (time.perf_counter() - t0) / reps
+    return dt, 2 * S_s
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores on a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2604_07248_b200 import synth
+    wl = synth.CONFIGS[args.config]
+    n_frames = args.steps + args.warmup
+    probe, _ = oracle_frame(wl, 1)                       # one screen: sizes the sample
+    budget = 150.0                                       # seconds for the whole run
+    S_s = int(max(1, min(wl.S, budget / max(probe * n_frames, 1e-9))))
+    for _ in range(args.warmup):
+        oracle_frame(wl, S_s)
+    ts = []
+    for _ in range(args.steps):
+        dt, units = oracle_frame(wl, S_s)
+        ts.append(dt)
+    ms = 1e3 * sum(ts) / len(ts)
+    value = units / (ms * 1e-3)
+    sample = f"1 realisation x {S_s} of {wl.S} screens per step (evolve + propagate + stats + adjoint)"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "N": wl.N, "B": 1, "S": S_s, "n_sh": wl.n_sh, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------------
+# the product arm
+# ---------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2604_07248_b200 import api, synth
+    from paper_2604_07248_b200 import build as b
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    if rank == 0:
+        b.build()
+    if world > 1:
+        dist.barrier()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device; the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+
+    wl = synth.CONFIGS[args.config]
+    N, S, n_sh = wl.N, wl.S, wl.n_sh
+    B = args.batch if args.batch > 0 else wl.B           # realisations per GPU (weak scaling)
+    px = N * N
+    ctx = api.Context(local)
+    psd = api.PsdParams(**wl.psd_dict())
+    cn2, dz = list(wl.cn2_list), list(wl.dz)
+    a = wl.ar_a if wl.ar_a > 0 else 0.99
+    kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
+
+    # ---- synthetic inputs resident in HBM (seeded): two full frames of white
+    # noise used alternately as the fresh noise of successive AR steps
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(1234 + rank)
+    def cnoise(*shape):
+        return torch.view_as_complex(torch.randn(*shape, 2, device=dev, generator=gen, dtype=torch.float32))
+    noise = [cnoise(B, S, N, N) for _ in range(2)]
+    noise_sh = [cnoise(B, S, max(n_sh, 1), 3, 3) for _ in range(2)]
+    spectrum = torch.empty((B, S, N, N), dtype=torch.complex64, device=dev)
+    sh_coef = torch.zeros((B, S, max(n_sh, 1), 3, 3), dtype=torch.complex64, device=dev)
+    screens = torch.empty((B, S, N, N), dtype=torch.float32, device=dev)
+    u0 = torch.from_numpy(synth.input_field(wl, B)).to(dev)
+    out = torch.empty_like(u0)
+    gin = torch.empty_like(u0)
+    stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device=dev)
+    ws = ctx.workspace(N, wl.dx, B, S)
+    ctx.make_screens(N, wl.dx, psd, wl.lam, cn2, dz, n_sh, noise[0], noise_sh[0] if n_sh else None,
+                     spectrum=spectrum, sh_coef=sh_coef if n_sh else None, screens=screens, ws=ws)
+
+    def frame(i):
+        ctx.evolve_screens(N, wl.dx, psd, wl.lam, cn2, dz, n_sh, a, 0.0, 0.0, 0.0, noise[i & 1],
+                           noise_sh[i & 1] if n_sh else None, spectrum, sh_coef if n_sh else None,
+                           screens=screens, ws=ws)
+        ctx.propagate(N, wl.dx, wl.lam, dz, u0, screens, out=out, stats=stats, **kw)
+        ctx.propagate_adjoint(N, wl.dx, wl.lam, dz, out, screens, out=gin, **kw)
+
+    def sync_all():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for i in range(args.warmup):
+        frame(i)
+    sync_all()
+
+    # ---- timed region: exactly K steps, CUDA events on the launching stream, per-kernel events on
+    clk = ClockSampler(local) if rank == 0 else None
+    ctx.profile_enable(True)
+    l0 = ctx.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(args.steps):
+        frame(args.warmup + i)
+    e1.record()
+    sync_all()
+    ms_total = e0.elapsed_time(e1)
+    launches = ctx.launch_count() - l0
+    prof = ctx.profile_report()
+    ctx.profile_enable(False)
+    clocks = clk.stop() if clk else None
+    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    units_step = 2 * B * S * world                        # forward + adjoint screen-steps, all ranks
+    value = units_step / (ms_step * 1e-3)
+
+    # ---- roofline of the dominant kernel class (by device time inside the timed region)
+    peak, peak_src = peaks()
+    dom = max(prof.items(), key=lambda kv: kv[1]["ms"]) if prof else (None, None)
+    roof = None
+    if dom[0]:
+        d = dom[1]
+        achieved = d["bytes"] / (d["ms"] * 1e-3) / 1e9
+        traffic = None
+        try:
+            with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as fh:
+                traffic = json.load(fh).get(f"{dom[0]}@{N}")
+        except Exception:
+            pass
+        roof = {"bound": "hbm", "kernel": dom[0], "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "us_per_launch": 1e3 * d["ms"] / d["launches"], "bytes_per_launch": d["bytes"] / d["launches"],
+                "share_of_step": d["ms"] / ms_total}
+    kernels = {k: {"launches": v["launches"], "ms": round(v["ms"], 4),
+                   "GBps": round(v["bytes"] / (v["ms"] * 1e-3) / 1e9, 1)} for k, v in prof.items()}
+    # split-step alone: col + row kernels of propagate and adjoint, 36 B/px per screen-step
+    ss_ms = sum(v["ms"] for k, v in prof.items() if k.startswith(("col_fft", "row_")))
+    ss_bytes = sum(v["bytes"] for k, v in prof.items() if k.startswith(("col_fft", "row_")))
+    split_step = {"screen_steps_per_s": 2 * B * S * args.steps / (ss_ms * 1e-3) if ss_ms else None,
+                  "GBps": ss_bytes / (ss_ms * 1e-3) / 1e9 if ss_ms else None,
+                  "frac_of_peak": ss_bytes / (ss_ms * 1e-3) / 1e9 / peak if ss_ms else None}
+
+    # ---- e2e: the same forward path through ssp_propagate_host with pinned HOST buffers
+    e2e = None
+    if not args.no_e2e:
+        h_in = torch.from_numpy(synth.input_field(wl, B)).pin_memory()
+        h_out = torch.empty_like(h_in).pin_memory()
+        h_scr = screens.cpu().pin_memory()
+        h_st = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8).pin_memory()
+        d_field = torch.empty_like(u0)
+        n_e2e = max(1, min(args.steps, 3))
+        def e2e_step():
+            ctx.propagate_host(N, wl.dx, wl.lam, dz, h_in, h_out, h_scr, False, S, wl.win_order,
+                               wl.win_sigma_frac, h_st, 0.5, d_field, screens, stats)
+        e2e_step()
+        sync_all()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            e2e_step()                                    # synchronises the stream itself
+        dt = (time.perf_counter() - t0) / n_e2e
+        t = torch.tensor([dt], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = float(t.item())
+        e2e = {"value": B * S * world / dt, "unit": UNIT, "what": "forward propagate + stats via ssp_propagate_host",
+               "h2d_bytes_per_step": int(h_in.numel() * 8 + h_scr.numel() * 4),
+               "d2h_bytes_per_step": int(h_out.numel() * 8 + h_st.numel()), "ms_per_step": dt * 1e3}
+
+    # ---- the oracle on the host cores, bounded sample (rank 0, N=1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        S_s = 2 if N >= 1024 else min(S, 5)
+        dt, units = oracle_frame(wl, S_s)
+        cpu = {"value": units / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"1 realisation x {S_s} of {S} screens, one frame (evolve + propagate + stats + adjoint), {dt:.1f} s"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": wl.name, "N": N, "B_per_gpu": B, "S": S, "n_sh": n_sh, "ar_a": a,
+                       "step": "evolve_screens + propagate + beam_stats + propagate_adjoint",
+                       "units_per_step": units_step,
+                       "l2": "inputs larger than L2 (no flush): each step streams > 10 GB"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches) * world, "roofline": roof,
+            "cpu_baseline": cpu, "kernels": kernels, "split_step": split_step,
+        }
+        print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -98,6 +98,13 @@ const char *ssp_version(void);
 /* Number of kernels this context has launched since creation (bench bookkeeping). */
 long long ssp_launch_count(const ssp_ctx *ctx);
 
+/* Per-launch timing for measurement: while enabled, every kernel launch is bracketed by CUDA
+ * events on the context's stream.  ssp_profile_report synchronises the stream, writes one line
+ * per kernel class "name launches total_ms algorithmic_bytes\n" into buf (host) and clears the
+ * records.  Enabling or disabling also clears them. */
+int ssp_profile_enable(ssp_ctx *ctx, int on);
+int ssp_profile_report(ssp_ctx *ctx, char *buf, size_t buf_bytes);
+
 /* Bytes of device scratch any call on this (grid, B, S) may need; the caller allocates
  * it once and passes it to every call.  Independent of the context. */
 size_t ssp_workspace_bytes(ssp_grid grid, int B, int S);

@@ -28,6 +28,7 @@ SYMBOLS = (
     "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_propagate",
     "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_propagate_host", "ssp_phase_mul",
     "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb",
+    "ssp_profile_enable", "ssp_profile_report",
 )
 
 
@@ -93,6 +94,8 @@ def load():
     lib.ssp_phase_grad.argtypes = [P, Grid, I, P, P, P]
     lib.ssp_inner_products.argtypes = [P, Grid, I, P, P, P]
     lib.ssp_lincomb.argtypes = [P, Grid, I, P, P, P, P, P]
+    lib.ssp_profile_enable.argtypes = [P, I]
+    lib.ssp_profile_report.argtypes = [P, C.c_char_p, C.c_size_t]
     _lib = lib
     return lib
 
@@ -168,6 +171,19 @@ class Context:
     def _chk(self, rc: int):
         if rc != 0:
             raise SspError(rc, self._lib.ssp_last_error(self._h).decode())
+
+    def profile_enable(self, on: bool = True):
+        self._chk(self._lib.ssp_profile_enable(self._h, int(on)))
+
+    def profile_report(self) -> dict:
+        """{kernel class: {"launches", "ms", "bytes"}} since the last report; synchronises the stream."""
+        buf = C.create_string_buffer(1 << 16)
+        self._chk(self._lib.ssp_profile_report(self._h, buf, len(buf)))
+        out = {}
+        for line in buf.value.decode().splitlines():
+            name, n, ms, by = line.split()
+            out[name] = {"launches": int(n), "ms": float(ms), "bytes": float(by)}
+        return out
 
     def launch_count(self) -> int:
         return int(self._lib.ssp_launch_count(self._h))

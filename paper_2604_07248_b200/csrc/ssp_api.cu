@@ -41,12 +41,45 @@ int ssp_destroy(ssp_ctx *ctx)
     for (auto &kv : ctx->htables) cudaFree(kv.second);
     for (auto &kv : ctx->sign_tables) cudaFree(kv.second);
     for (void *p : ctx->owned) cudaFree(p);
+    for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
     if (ctx->scratch) cudaFree(ctx->scratch);
     delete ctx;
     return SSP_OK;
 }
 
 const char *ssp_last_error(const ssp_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int ssp_profile_enable(ssp_ctx *ctx, int on)
+{
+    if (!ctx) return SSP_EINVAL;
+    ctx->prof_on = (on != 0);
+    ctx->prof.clear();
+    return SSP_OK;
+}
+
+int ssp_profile_report(ssp_ctx *ctx, char *buf, size_t buf_bytes)
+{
+    if (!ctx || !buf || buf_bytes < 2) return SSP_EINVAL;
+    SSP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    struct Agg { long long n = 0; double ms = 0, bytes = 0; };
+    std::map<std::string, Agg> agg;
+    for (const auto &r : ctx->prof) {
+        float ms = 0.f;
+        SSP_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->prof_events[r.ev], ctx->prof_events[r.ev + 1]));
+        Agg &a = agg[r.name];
+        a.n++; a.ms += ms; a.bytes += r.bytes;
+    }
+    ctx->prof.clear();
+    size_t o = 0;
+    buf[0] = 0;
+    for (const auto &kv : agg) {
+        int w = snprintf(buf + o, buf_bytes - o, "%s %lld %.6f %.0f\n", kv.first.c_str(), kv.second.n, kv.second.ms,
+                         kv.second.bytes);
+        if (w < 0 || (size_t)w >= buf_bytes - o) return ctx->fail(SSP_EINVAL, "profile report buffer too small");
+        o += (size_t)w;
+    }
+    return SSP_OK;
+}
 long long ssp_launch_count(const ssp_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
 } // extern "C"

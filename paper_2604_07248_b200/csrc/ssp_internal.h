@@ -42,6 +42,29 @@ struct ssp_ctx {
     size_t scratch_bytes = 0;
     std::vector<void *> owned;                   // misc device allocations freed at destroy
 
+    // ---- optional per-launch timing with CUDA events on the context's stream (bench.py's roofline)
+    struct ProfRec { const char *name; double bytes; int ev; };
+    bool prof_on = false;
+    std::vector<ProfRec> prof;
+    std::vector<cudaEvent_t> prof_events;        // pool, two per record
+    void prof_begin(const char *name, double alg_bytes)
+    {
+        if (!prof_on) return;
+        const int ev = 2 * (int)prof.size();
+        while ((int)prof_events.size() < ev + 2) {
+            cudaEvent_t e;
+            cudaEventCreate(&e);
+            prof_events.push_back(e);
+        }
+        prof.push_back(ProfRec{name, alg_bytes, ev});
+        cudaEventRecord(prof_events[ev], stream);
+    }
+    void prof_end()
+    {
+        if (!prof_on || prof.empty()) return;
+        cudaEventRecord(prof_events[prof.back().ev + 1], stream);
+    }
+
     int fail(int code, const char *fmt, ...)
     {
         char buf[512];

@@ -103,8 +103,10 @@ int launch_stats(ssp_ctx *ctx, int N, double dx, int B, const float2 *field, dou
     const size_t pairs = (size_t)N * N / 2;
     int bpf = (int)((pairs + 256 * 8 - 1) / (256 * 8)); // ~16 pixels per thread
     if (bpf < 1) bpf = 1;
+    ctx->prof_begin("stats", 8.0 * (double)B * N * N);
     k_stats_accum<<<dim3(bpf, B), 256, 0, ctx->stream>>>(field, N, lo, hi, acc);
     k_stats_final<<<(B + 127) / 128, 128, 0, ctx->stream>>>(acc, B, dx, roi_n, d_stats);
+    ctx->prof_end();
     ctx->launches += 2;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;

@@ -168,7 +168,11 @@ static int launch_row_n(ssp_ctx *ctx, const RowArgs &a)
     if (a.n_lines % CFG::LPB) return ctx->fail(SSP_EINVAL, "row launch: %d lines not a multiple of %d", a.n_lines, CFG::LPB);
     auto kern = k_row<N, FIRST, SECOND>;
     if (int rc = set_smem(ctx, kern, CFG::SMEM)) return rc;
+    // algorithmic bytes: field in + out, + the screen, + saved / read planes and the gradient
+    const double bpp = 16.0 + (a.phi ? 4.0 : 0.0) + (a.plane_out ? 8.0 : 0.0) + (a.grad ? 12.0 : 0.0);
+    ctx->prof_begin(FIRST ? (SECOND ? "row_ifft_pw_fft" : "row_ifft_pw") : "row_pw_fft", bpp * (double)a.n_lines * N);
     kern<<<a.n_lines / CFG::LPB, CFG::THREADS, CFG::SMEM, ctx->stream>>>(a);
+    ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;
@@ -189,7 +193,9 @@ static int launch_col_n(ssp_ctx *ctx, const ColArgs &a)
     using CFG = ColCfg<N>;
     auto kern = k_col<N, MODE>;
     if (int rc = set_smem(ctx, kern, CFG::SMEM)) return rc;
+    ctx->prof_begin(MODE == 0 ? "col_fft_h_ifft" : "col_single", 16.0 * (double)a.B * N * N);
     kern<<<a.B * (N / CFG::C), CFG::THREADS, CFG::SMEM, ctx->stream>>>(a);
+    ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;

@@ -169,7 +169,10 @@ static int launch_screen_col_n(ssp_ctx *ctx, const ScreenColArgs &a)
     auto kern = k_screen_col<N>;
     if (CFG::SMEM > 48 * 1024)
         SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::SMEM));
+    const double bpp = 16.0 + (a.old_spec ? 8.0 : 0.0) + (a.spec_out ? 8.0 : 0.0);
+    ctx->prof_begin("screen_col", bpp * (double)a.nscr * N * N);
     kern<<<a.nscr * (N / CFG::C), CFG::THREADS, CFG::SMEM, ctx->stream>>>(a);
+    ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;
@@ -182,7 +185,9 @@ static int launch_screen_row_n(ssp_ctx *ctx, const ScreenRowArgs &a)
     auto kern = k_screen_row<N>;
     if (CFG::SMEM > 48 * 1024)
         SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::SMEM));
+    ctx->prof_begin("screen_row", 12.0 * (double)a.nscr * N * N);
     kern<<<(unsigned)((long long)a.nscr * N / CFG::LPB), CFG::THREADS, CFG::SMEM, ctx->stream>>>(a);
+    ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;
