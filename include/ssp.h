@@ -122,7 +122,7 @@ size_t ssp_workspace_bytes(ssp_grid grid, int B, int S);
  * unused), may be NULL when n_sh == 0.  Outputs: d_spectrum dev complex64 [B][S][N][N]
  * (the stored Fourier spectrum; may be NULL), d_sh_coef dev complex64
  * [B][S][n_sh][3][3] (may be NULL), d_screens dev fp32 [B][S][N][N] (required).
- * d_noise may alias d_spectrum.  0 <= n_sh <= 8. */
+ * d_noise must not overlap d_spectrum.  0 <= n_sh <= 8. */
 int ssp_make_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
                      int B, int S, const double *cn2, const double *dz, int n_sh,
                      const float *d_noise, const float *d_noise_sh,

@@ -136,6 +136,8 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
     (void)d_ws; (void)ws_bytes;
     if (int rc = check_prop(ctx, grid, lambda, n0, h_kind, B, n_steps, dz, d_screens, S, d_field_in, d_field_out))
         return rc;
+    if (screen_batch_stride < 0 || (screen_batch_stride & 3))
+        return ctx->fail(SSP_EINVAL, "screen_batch_stride must be >= 0 and a multiple of 4 elements");
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));
     const int N = grid.N;
     const size_t px = (size_t)N * N;
@@ -197,6 +199,8 @@ int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0,
     (void)d_ws; (void)ws_bytes;
     if (int rc = check_prop(ctx, grid, lambda, n0, h_kind, B, n_steps, dz, d_screens, S, d_g_out, d_g_in))
         return rc;
+    if (screen_batch_stride < 0 || (screen_batch_stride & 3))
+        return ctx->fail(SSP_EINVAL, "screen_batch_stride must be >= 0 and a multiple of 4 elements");
     if ((d_planes == nullptr) != (d_phase_grad == nullptr))
         return ctx->fail(SSP_EINVAL, "d_planes and d_phase_grad must both be given or both be null");
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));

@@ -13,8 +13,10 @@ struct RowCfg {
     static constexpr int THREADS = (T * N < 256) ? T * N : 256;
     static constexpr int LPB = THREADS / T;                        // lines (rows) per CTA
     static constexpr bool WARP_LOCAL = (T <= 32);                  // a line never spans two warps
-    static constexpr size_t SMEM = (PlanInfo<N>::NSTAGE == 1) ? 0
-        : sizeof(float2) * (size_t)LPB * PlanInfo<N>::LINE_ELEMS;
+    static constexpr size_t SMEM_X = (PlanInfo<N>::NSTAGE == 1) ? 0
+        : sizeof(float2) * (size_t)LPB * PlanInfo<N>::LINE_ELEMS;       // exchange buffers
+    static constexpr size_t SMEM_PHI = sizeof(float) * (size_t)LPB * N; // prefetched screen rows
+    static constexpr size_t SMEM = SMEM_X + SMEM_PHI;
     static constexpr int MIN_BLOCKS = (THREADS * PlanInfo<N>::E >= 8192) ? 2 : 1;
 };
 
@@ -49,6 +51,15 @@ struct ColSmem {
     __device__ __forceinline__ float2 ld(int p) const { return base[p * C]; }
     __device__ __forceinline__ void sync() { __syncthreads(); }
 };
+
+// ---- asynchronous global -> shared copies (LDGSTS), 16 bytes each
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
 
 // ---- pointwise math -----------------------------------------------------------------
 // sin/cos of a phase of any magnitude: Cody-Waite reduction by 2 pi, then the SFU.

@@ -28,6 +28,15 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
     const int b = (int)(line / N), iy = (int)(line % N);
     RowSmem<CFG::WARP_LOCAL> sm{smem + (size_t)lib * PI::LINE_ELEMS};
 
+    // the screen row is streamed from HBM: fetch it asynchronously now, use it after the first transform
+    float *phis = reinterpret_cast<float *>(smem_raw + CFG::SMEM_X) + (size_t)lib * N;
+    if (a.phi) {
+        const float *g = a.phi + b * a.phi_batch_stride + (long long)iy * N;
+#pragma unroll
+        for (int i = 0; i < E / 4; ++i) cp_async16(phis + 4 * (t + T * i), g + 4 * (t + T * i));
+        cp_async_commit();
+    }
+
     float2 v[E];
     constexpr int RIN = FIRST ? PI::R1 : PI::RL;
     {
@@ -52,6 +61,10 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
     constexpr int RL = PI::RL;
     const bool pointwise = a.phi || a.win_on || a.grad || a.plane_out;
     if (pointwise) {
+        if (a.phi) {
+            cp_async_wait_all();
+            sm.sync();
+        }
         const long long pix0 = (long long)iy * N;
         const float yc = (float)(iy - N / 2);
 #pragma unroll
@@ -66,8 +79,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
                 }
                 float mr = 1.f, mi = 0.f;
                 if (a.phi) {
-                    const float ph = __ldg(a.phi + b * a.phi_batch_stride + pix0 + ix);
-                    sincos_reduced(ph, &mi, &mr);
+                    sincos_reduced(phis[ix], &mi, &mr);
                     mi *= a.phase_sign;
                 }
                 if (a.win_on) {

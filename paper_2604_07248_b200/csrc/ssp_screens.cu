@@ -49,24 +49,43 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_s
     if (ar && a.taux) tx = __ldg(a.taux + kx);
 
     float2 v[E];
+    // all noise loads first (independent, in flight together), then filter in registers
+#pragma unroll
+    for (int i = 0; i < E / R1; ++i)
+#pragma unroll
+        for (int q = 0; q < R1; ++q) v[i * R1 + q] = __ldg(a.noise + base + (size_t)line_index<N, R1>(t, i, q) * N);
 #pragma unroll
     for (int i = 0; i < E / R1; ++i)
 #pragma unroll
         for (int q = 0; q < R1; ++q) {
             const int ky = line_index<N, R1>(t, i, q);
             const float kys = (float)((ky < N / 2) ? ky : ky - N);
-            const float2 nz = a.noise[base + (size_t)ky * N];
             const float f2 = (kxs * kxs + kys * kys) * df2;
-            float amp = (kx == 0 && ky == 0) ? 0.f : amp_s * psd_shape_sqrt(a.flt, f2);
-            float2 Cv = make_float2(nz.x * amp, nz.y * amp);
-            if (ar) {
-                float2 old = a.old_spec[base + (size_t)ky * N];
-                if (a.taux) old = cmul(old, cmul(tx, __ldg(a.tauy + ky)));
-                Cv = make_float2(fmaf(a.ar_a, old.x, a.ar_g * Cv.x), fmaf(a.ar_a, old.y, a.ar_g * Cv.y));
-            }
-            if (a.spec_out) a.spec_out[base + (size_t)ky * N] = Cv;
-            v[i * R1 + q] = Cv;
+            const float amp = (kx == 0 && ky == 0) ? 0.f : amp_s * psd_shape_sqrt(a.flt, f2);
+            v[i * R1 + q] = make_float2(v[i * R1 + q].x * amp, v[i * R1 + q].y * amp);
         }
+    if (ar) { // C <- a tau C_old + sqrt(1-a^2) C_fresh, old spectrum loaded in batches of 8
+        constexpr int G = (E < 8) ? E : 8;
+#pragma unroll
+        for (int e0 = 0; e0 < E; e0 += G) {
+            float2 old[G];
+#pragma unroll
+            for (int e = 0; e < G; ++e)
+                old[e] = a.old_spec[base + (size_t)line_index<N, R1>(t, (e0 + e) / R1, (e0 + e) % R1) * N];
+#pragma unroll
+            for (int e = 0; e < G; ++e) {
+                float2 o = old[e];
+                if (a.taux) o = cmul(o, cmul(tx, __ldg(a.tauy + line_index<N, R1>(t, (e0 + e) / R1, (e0 + e) % R1))));
+                v[e0 + e] = make_float2(fmaf(a.ar_a, o.x, a.ar_g * v[e0 + e].x), fmaf(a.ar_a, o.y, a.ar_g * v[e0 + e].y));
+            }
+        }
+    }
+    if (a.spec_out) {
+#pragma unroll
+        for (int i = 0; i < E / R1; ++i)
+#pragma unroll
+            for (int q = 0; q < R1; ++q) a.spec_out[base + (size_t)line_index<N, R1>(t, i, q) * N] = v[i * R1 + q];
+    }
     fft_line<N, false, true>(v, t, sm, a.tw); // unnormalised inverse along y
     float2 *dst = a.out + base;
 #pragma unroll
