@@ -142,8 +142,9 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
     const int N = grid.N;
     const size_t px = (size_t)N * N;
     const double lam_eff = lambda / n0;
-    const float2 *tw = nullptr;
-    if (int rc = get_twiddles(ctx, N, &tw)) return rc;
+    const float2 *tw = nullptr, *twc = nullptr;          // row-plan and column-plan twiddles
+    if (int rc = get_twiddles(ctx, N, 0, &tw)) return rc;
+    if (int rc = get_twiddles(ctx, N, 1, &twc)) return rc;
     float2 *u = reinterpret_cast<float2 *>(d_field_out);
 
     // K4: FFT_x of the input, times hx of step 1
@@ -162,7 +163,7 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
         const float2 *hy = nullptr;
         if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j - 1], 0, 1}, &hy)) return rc;
         ColArgs c{};
-        c.in = u; c.out = u; c.B = B; c.hy = hy; c.tw = tw;
+        c.in = u; c.out = u; c.B = B; c.hy = hy; c.tw = twc;
         if (int rc = launch_col_prop(ctx, N, c)) return rc;
         // K6: IFFT_x -> * exp(i phi_j) W -> [FFT_x -> * hx_{j+1}]
         RowArgs r{};
@@ -207,8 +208,9 @@ int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0,
     const int N = grid.N;
     const size_t px = (size_t)N * N;
     const double lam_eff = lambda / n0;
-    const float2 *tw = nullptr;
-    if (int rc = get_twiddles(ctx, N, &tw)) return rc;
+    const float2 *tw = nullptr, *twc = nullptr;          // row-plan and column-plan twiddles
+    if (int rc = get_twiddles(ctx, N, 0, &tw)) return rc;
+    if (int rc = get_twiddles(ctx, N, 1, &twc)) return rc;
     float2 *g = reinterpret_cast<float2 *>(d_g_in);
 
     // pointwise stage of plane j: [grad_j] ; g <- W exp(-i phi_j) g
@@ -239,7 +241,7 @@ int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0,
         const float2 *hy = nullptr;
         if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j - 1], 1, 1}, &hy)) return rc;
         ColArgs c{};
-        c.in = g; c.out = g; c.B = B; c.hy = hy; c.tw = tw;
+        c.in = g; c.out = g; c.B = B; c.hy = hy; c.tw = twc;
         if (int rc = launch_col_prop(ctx, N, c)) return rc;
         RowArgs r{};
         r.in = g; r.out = g; r.n_lines = B * N; r.tw = tw;

@@ -123,8 +123,9 @@ int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
     const double df = 1.0 / (N * grid.dx);
     const WsLayout L = ws_layout(N, B, S);
     char *ws = reinterpret_cast<char *>(d_ws);
-    const float2 *tw = nullptr;
-    if (int rc = get_twiddles(ctx, N, &tw)) return rc;
+    const float2 *tw = nullptr, *twc = nullptr;          // row-plan and column-plan twiddles
+    if (int rc = get_twiddles(ctx, N, 0, &tw)) return rc;
+    if (int rc = get_twiddles(ctx, N, 1, &twc)) return rc;
     cudaStream_t st = ctx->stream;
 
     // ---- per-slab scalars and 1-D tables (double on the host, fp32 on the device)
@@ -229,7 +230,7 @@ int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
         c.flt = flt;
         c.ar_a = (float)a; c.ar_g = (float)sqrt(1.0 - a * a);
         c.taux = d_taux; c.tauy = d_tauy;
-        c.tw = tw;
+        c.tw = twc;
         if (int rc = launch_screen_col(ctx, N, c)) return rc;
         ScreenRowArgs r{};
         r.in = inter;
@@ -304,8 +305,9 @@ int ssp_dft2_centered(ssp_ctx *ctx, ssp_grid grid, int B, int inverse,
         return ctx->fail(SSP_EINVAL, "bad arguments");
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));
     const int N = grid.N;
-    const float2 *tw = nullptr, *sg = nullptr;
-    if (int rc = get_twiddles(ctx, N, &tw)) return rc;
+    const float2 *tw = nullptr, *twc = nullptr, *sg = nullptr;
+    if (int rc = get_twiddles(ctx, N, 0, &tw)) return rc;
+    if (int rc = get_twiddles(ctx, N, 1, &twc)) return rc;
     if (int rc = get_sign_table(ctx, N, &sg)) return rc;
     // F_c = (-1)^(kx+ky) FFT2( (-1)^(ix+iy) x ) / N; rows carry both input signs, each axis 1/sqrt(N)
     RowArgs r{};
@@ -315,7 +317,7 @@ int ssp_dft2_centered(ssp_ctx *ctx, ssp_grid grid, int B, int inverse,
     r.pre = sg; r.pre_line = sg; r.hx = sg + N; r.tw = tw;
     if (int rc = launch_row(ctx, N, inverse != 0, inverse == 0, r)) return rc;
     ColArgs c{};
-    c.in = r.out; c.out = r.out; c.B = B; c.hy = sg + N; c.tw = tw;
+    c.in = r.out; c.out = r.out; c.B = B; c.hy = sg + N; c.tw = twc;
     return launch_col_single(ctx, N, inverse != 0, c);
 }
 

@@ -35,7 +35,7 @@ struct ssp_ctx {
     std::string err;
     long long launches = 0;
     int num_sms = 148;
-    std::map<int, float2 *> twiddles;            // per N, device
+    std::map<int, float2 *> twiddles;            // per (N, plan variant), device
     std::map<ssp::HKey, float2 *> htables;       // 1-D transfer-function tables, device [N]
     std::map<int, float2 *> sign_tables;         // (-1)^k tables for the centred DFT
     void *scratch = nullptr;                     // small device scratch (stat accumulators, tables)
@@ -88,7 +88,8 @@ struct ssp_ctx {
 namespace ssp {
 
 // ---- tables (ssp_tables.cu) ------------------------------------------------------
-int get_twiddles(ssp_ctx *ctx, int N, const float2 **out);
+// V = 0: row-plan tables, V = 1: column-plan tables (ssp_fft.cuh)
+int get_twiddles(ssp_ctx *ctx, int N, int V, const float2 **out);
 int get_htable(ssp_ctx *ctx, const HKey &key, const float2 **out);
 int get_sign_table(ssp_ctx *ctx, int N, const float2 **out);
 int ensure_scratch(ssp_ctx *ctx, size_t bytes);

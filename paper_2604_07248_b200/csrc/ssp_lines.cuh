@@ -9,38 +9,45 @@ namespace ssp {
 // ---- CTA shapes --------------------------------------------------------------------
 template <int N>
 struct RowCfg {
-    static constexpr int T = PlanInfo<N>::T;
+    static constexpr int V = 0;                                   // plan variant
+    static constexpr int T = PlanInfo<N, 0>::T;
     static constexpr int THREADS = (T * N < 256) ? T * N : 256;
     static constexpr int LPB = THREADS / T;                        // lines (rows) per CTA
     static constexpr bool WARP_LOCAL = (T <= 32);                  // a line never spans two warps
-    static constexpr size_t SMEM_X = (PlanInfo<N>::NSTAGE == 1) ? 0
-        : sizeof(float2) * (size_t)LPB * PlanInfo<N>::LINE_ELEMS;       // exchange buffers
+    static constexpr size_t SMEM_X = (PlanInfo<N, 0>::NSTAGE == 1) ? 0
+        : sizeof(float2) * (size_t)LPB * PlanInfo<N, 0>::LINE_ELEMS;       // exchange buffers
     static constexpr size_t SMEM_PHI = sizeof(float) * (size_t)LPB * N; // prefetched screen rows
     static constexpr size_t SMEM = SMEM_X + SMEM_PHI;
-    static constexpr int MIN_BLOCKS = (THREADS * PlanInfo<N>::E >= 8192) ? 2 : 1;
+    // resident CTAs per SM the register budget is sized for: 512 threads at E = 32, 1024 at E = 16
+    static constexpr int MIN_BLOCKS = (THREADS < 256) ? 1 : (PlanInfo<N, 0>::E >= 32 ? 2 : 4);
 };
 
 template <int N>
 struct ColCfg {
-    static constexpr int T = PlanInfo<N>::T;
+    static constexpr int V = 1;                                   // plan variant
+    static constexpr int T = PlanInfo<N, 1>::T;
     // columns per CTA: 16 columns = 128-byte row segments while the tile fits one SM's
     // shared memory next to a second CTA; wider grids trade segment width for tile height.
     static constexpr int C = (N <= 8) ? 8 : (N <= 512 ? 16 : (N <= 2048 ? 8 : 4));
     static constexpr int THREADS = T * C;
-    static constexpr size_t SMEM = (PlanInfo<N>::NSTAGE == 1) ? 0
-        : sizeof(float2) * (size_t)C * PlanInfo<N>::LINE_ELEMS;
+    static constexpr size_t SMEM = (PlanInfo<N, 1>::NSTAGE == 1) ? 0
+        : sizeof(float2) * (size_t)C * PlanInfo<N, 1>::LINE_ELEMS;
     static constexpr int MIN_BLOCKS = (THREADS <= 256) ? 2 : 1;
 };
 
 // ---- shared-memory exchange accessors -------------------------------------------------
-template <bool WARP_LOCAL>
+// T = threads per line.  A line inside one warp synchronises with __syncwarp; a line spanning
+// several warps uses its own named barrier (id 1 + line-in-CTA), so lines never wait on each other.
+template <int T>
 struct RowSmem {
     float2 *base; // this line's padded buffer
+    int bar_id;
     __device__ __forceinline__ void st(int p, float2 x) { base[p] = x; }
     __device__ __forceinline__ float2 ld(int p) const { return base[p]; }
     __device__ __forceinline__ void sync()
     {
-        if (WARP_LOCAL) __syncwarp(); else __syncthreads();
+        if constexpr (T <= 32) __syncwarp();
+        else asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "n"(T) : "memory");
     }
 };
 

@@ -16,7 +16,7 @@ namespace ssp {
 template <int N, bool FIRST, bool SECOND>
 __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_row(const RowArgs a)
 {
-    using PI = PlanInfo<N>;
+    using PI = PlanInfo<N, 0>;
     using CFG = RowCfg<N>;
     constexpr int E = PI::E, T = PI::T;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
     const int lib = tid / T, t = tid % T;
     const long long line = (long long)blockIdx.x * CFG::LPB + lib;
     const int b = (int)(line / N), iy = (int)(line % N);
-    RowSmem<CFG::WARP_LOCAL> sm{smem + (size_t)lib * PI::LINE_ELEMS};
+    RowSmem<T> sm{smem + (size_t)lib * PI::LINE_ELEMS, 1 + lib};
 
     // the screen row is streamed from HBM: fetch it asynchronously now, use it after the first transform
     float *phis = reinterpret_cast<float *>(smem_raw + CFG::SMEM_X) + (size_t)lib * N;
@@ -44,7 +44,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
 #pragma unroll
         for (int i = 0; i < E / RIN; ++i)
 #pragma unroll
-            for (int q = 0; q < RIN; ++q) v[i * RIN + q] = src[line_index<N, RIN>(t, i, q)];
+            for (int q = 0; q < RIN; ++q) v[i * RIN + q] = src[line_index<N, 0, RIN>(t, i, q)];
     }
     if (a.pre) {
         const float2 pl = a.pre_line ? __ldg(a.pre_line + iy) : make_float2(1.f, 0.f);
@@ -52,10 +52,10 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
         for (int i = 0; i < E / RIN; ++i)
 #pragma unroll
             for (int q = 0; q < RIN; ++q)
-                v[i * RIN + q] = cmul(v[i * RIN + q], cmul(pl, __ldg(a.pre + line_index<N, RIN>(t, i, q))));
+                v[i * RIN + q] = cmul(v[i * RIN + q], cmul(pl, __ldg(a.pre + line_index<N, 0, RIN>(t, i, q))));
     }
 
-    if constexpr (FIRST) fft_line<N, false, true>(v, t, sm, a.tw); // inverse; now strided by RL
+    if constexpr (FIRST) fft_line<N, 0, false, true>(v, t, sm, a.tw); // inverse; now strided by RL
 
     // ---- pointwise stage in real space, layout strided by RL
     constexpr int RL = PI::RL;
@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
         for (int i = 0; i < E / RL; ++i)
 #pragma unroll
             for (int q = 0; q < RL; ++q) {
-                const int ix = line_index<N, RL>(t, i, q);
+                const int ix = line_index<N, 0, RL>(t, i, q);
                 float2 u = v[i * RL + q];
                 if (a.grad) {
                     const float2 U = a.plane_in[b * a.plane_stride + pix0 + ix];
@@ -97,7 +97,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
     constexpr int ROUT = SECOND ? PI::R1 : PI::RL;
     if constexpr (SECOND) {
         if constexpr (FIRST) sm.sync();                  // the exchange buffer is reused
-        fft_line<N, true, false>(v, t, sm, a.tw);        // forward, reversed plan; strided by R1
+        fft_line<N, 0, true, false>(v, t, sm, a.tw);        // forward, reversed plan; strided by R1
     }
     float2 *dst = a.out + line * N;
     if (a.hx) {
@@ -105,14 +105,14 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
         for (int i = 0; i < E / ROUT; ++i)
 #pragma unroll
             for (int q = 0; q < ROUT; ++q) {
-                const int k = line_index<N, ROUT>(t, i, q);
+                const int k = line_index<N, 0, ROUT>(t, i, q);
                 dst[k] = cmul(v[i * ROUT + q], __ldg(a.hx + k));
             }
     } else {
 #pragma unroll
         for (int i = 0; i < E / ROUT; ++i)
 #pragma unroll
-            for (int q = 0; q < ROUT; ++q) dst[line_index<N, ROUT>(t, i, q)] = v[i * ROUT + q];
+            for (int q = 0; q < ROUT; ++q) dst[line_index<N, 0, ROUT>(t, i, q)] = v[i * ROUT + q];
     }
 }
 
@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
 template <int N, int MODE>
 __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_col(const ColArgs a)
 {
-    using PI = PlanInfo<N>;
+    using PI = PlanInfo<N, 1>;
     using CFG = ColCfg<N>;
     constexpr int E = PI::E, T = PI::T, C = CFG::C;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -138,29 +138,29 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_c
 #pragma unroll
     for (int i = 0; i < E / R1; ++i)
 #pragma unroll
-        for (int q = 0; q < R1; ++q) v[i * R1 + q] = src[(size_t)line_index<N, R1>(t, i, q) * N];
+        for (int q = 0; q < R1; ++q) v[i * R1 + q] = src[(size_t)line_index<N, 1, R1>(t, i, q) * N];
 
-    fft_line<N, false, MODE == 2>(v, t, sm, a.tw); // strided by RL
+    fft_line<N, 1, false, MODE == 2>(v, t, sm, a.tw); // strided by RL
     if (a.hy) {
 #pragma unroll
         for (int i = 0; i < E / RL; ++i)
 #pragma unroll
             for (int q = 0; q < RL; ++q)
-                v[i * RL + q] = cmul(v[i * RL + q], __ldg(a.hy + line_index<N, RL>(t, i, q)));
+                v[i * RL + q] = cmul(v[i * RL + q], __ldg(a.hy + line_index<N, 1, RL>(t, i, q)));
     }
     float2 *dst = a.out + (size_t)b * N * N + col;
     if constexpr (MODE == 0) {
         sm.sync();
-        fft_line<N, true, true>(v, t, sm, a.tw);   // inverse, reversed plan; strided by R1
+        fft_line<N, 1, true, true>(v, t, sm, a.tw);   // inverse, reversed plan; strided by R1
 #pragma unroll
         for (int i = 0; i < E / R1; ++i)
 #pragma unroll
-            for (int q = 0; q < R1; ++q) dst[(size_t)line_index<N, R1>(t, i, q) * N] = v[i * R1 + q];
+            for (int q = 0; q < R1; ++q) dst[(size_t)line_index<N, 1, R1>(t, i, q) * N] = v[i * R1 + q];
     } else {
 #pragma unroll
         for (int i = 0; i < E / RL; ++i)
 #pragma unroll
-            for (int q = 0; q < RL; ++q) dst[(size_t)line_index<N, RL>(t, i, q) * N] = v[i * RL + q];
+            for (int q = 0; q < RL; ++q) dst[(size_t)line_index<N, 1, RL>(t, i, q) * N] = v[i * RL + q];
     }
 }
 

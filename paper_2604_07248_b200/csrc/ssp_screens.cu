@@ -29,7 +29,7 @@ __device__ __forceinline__ float psd_shape_sqrt(const ScreenFilter &f, float f2)
 template <int N>
 __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_screen_col(const ScreenColArgs a)
 {
-    using PI = PlanInfo<N>;
+    using PI = PlanInfo<N, 1>;
     using CFG = ColCfg<N>;
     constexpr int E = PI::E, T = PI::T, C = CFG::C, R1 = PI::R1, RL = PI::RL;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -53,12 +53,12 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_s
 #pragma unroll
     for (int i = 0; i < E / R1; ++i)
 #pragma unroll
-        for (int q = 0; q < R1; ++q) v[i * R1 + q] = __ldg(a.noise + base + (size_t)line_index<N, R1>(t, i, q) * N);
+        for (int q = 0; q < R1; ++q) v[i * R1 + q] = __ldg(a.noise + base + (size_t)line_index<N, 1, R1>(t, i, q) * N);
 #pragma unroll
     for (int i = 0; i < E / R1; ++i)
 #pragma unroll
         for (int q = 0; q < R1; ++q) {
-            const int ky = line_index<N, R1>(t, i, q);
+            const int ky = line_index<N, 1, R1>(t, i, q);
             const float kys = (float)((ky < N / 2) ? ky : ky - N);
             const float f2 = (kxs * kxs + kys * kys) * df2;
             const float amp = (kx == 0 && ky == 0) ? 0.f : amp_s * psd_shape_sqrt(a.flt, f2);
@@ -71,11 +71,11 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_s
             float2 old[G];
 #pragma unroll
             for (int e = 0; e < G; ++e)
-                old[e] = a.old_spec[base + (size_t)line_index<N, R1>(t, (e0 + e) / R1, (e0 + e) % R1) * N];
+                old[e] = a.old_spec[base + (size_t)line_index<N, 1, R1>(t, (e0 + e) / R1, (e0 + e) % R1) * N];
 #pragma unroll
             for (int e = 0; e < G; ++e) {
                 float2 o = old[e];
-                if (a.taux) o = cmul(o, cmul(tx, __ldg(a.tauy + line_index<N, R1>(t, (e0 + e) / R1, (e0 + e) % R1))));
+                if (a.taux) o = cmul(o, cmul(tx, __ldg(a.tauy + line_index<N, 1, R1>(t, (e0 + e) / R1, (e0 + e) % R1))));
                 v[e0 + e] = make_float2(fmaf(a.ar_a, o.x, a.ar_g * v[e0 + e].x), fmaf(a.ar_a, o.y, a.ar_g * v[e0 + e].y));
             }
         }
@@ -84,20 +84,20 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_s
 #pragma unroll
         for (int i = 0; i < E / R1; ++i)
 #pragma unroll
-            for (int q = 0; q < R1; ++q) a.spec_out[base + (size_t)line_index<N, R1>(t, i, q) * N] = v[i * R1 + q];
+            for (int q = 0; q < R1; ++q) a.spec_out[base + (size_t)line_index<N, 1, R1>(t, i, q) * N] = v[i * R1 + q];
     }
-    fft_line<N, false, true>(v, t, sm, a.tw); // unnormalised inverse along y
+    fft_line<N, 1, false, true>(v, t, sm, a.tw); // unnormalised inverse along y
     float2 *dst = a.out + base;
 #pragma unroll
     for (int i = 0; i < E / RL; ++i)
 #pragma unroll
-        for (int q = 0; q < RL; ++q) dst[(size_t)line_index<N, RL>(t, i, q) * N] = v[i * RL + q];
+        for (int q = 0; q < RL; ++q) dst[(size_t)line_index<N, 1, RL>(t, i, q) * N] = v[i * RL + q];
 }
 
 template <int N>
 __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_screen_row(const ScreenRowArgs a)
 {
-    using PI = PlanInfo<N>;
+    using PI = PlanInfo<N, 0>;
     using CFG = RowCfg<N>;
     constexpr int E = PI::E, T = PI::T, R1 = PI::R1, RL = PI::RL;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -106,15 +106,15 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_s
     const int lib = tid / T, t = tid % T;
     const long long line = (long long)blockIdx.x * CFG::LPB + lib;
     const int scr = (int)(line / N), iy = (int)(line % N);
-    RowSmem<CFG::WARP_LOCAL> sm{smem + (size_t)lib * PI::LINE_ELEMS};
+    RowSmem<T> sm{smem + (size_t)lib * PI::LINE_ELEMS, 1 + lib};
 
     float2 v[E];
     const float2 *src = a.in + line * N;
 #pragma unroll
     for (int i = 0; i < E / R1; ++i)
 #pragma unroll
-        for (int q = 0; q < R1; ++q) v[i * R1 + q] = src[line_index<N, R1>(t, i, q)];
-    fft_line<N, false, true>(v, t, sm, a.tw); // unnormalised inverse along x; strided by RL
+        for (int q = 0; q < R1; ++q) v[i * R1 + q] = src[line_index<N, 0, R1>(t, i, q)];
+    fft_line<N, 0, false, true>(v, t, sm, a.tw); // unnormalised inverse along x; strided by RL
 
     float mean = 0.f;
     if (a.n_sh > 0) {
@@ -134,7 +134,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_s
             for (int i = 0; i < E / RL; ++i)
 #pragma unroll
                 for (int q = 0; q < RL; ++q) {
-                    const float2 ex = __ldg(a.ex + (size_t)p * N + line_index<N, RL>(t, i, q));
+                    const float2 ex = __ldg(a.ex + (size_t)p * N + line_index<N, 0, RL>(t, i, q));
                     // Re(d0 conj(ex)) + Re(d1) + Re(d2 ex)
                     float r = fmaf(d[0].x, ex.x, d[0].y * ex.y) + d[1].x + fmaf(d[2].x, ex.x, -d[2].y * ex.y);
                     v[i * RL + q].x += r;
@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_s
 #pragma unroll
     for (int i = 0; i < E / RL; ++i)
 #pragma unroll
-        for (int q = 0; q < RL; ++q) dst[line_index<N, RL>(t, i, q)] = v[i * RL + q].x - mean;
+        for (int q = 0; q < RL; ++q) dst[line_index<N, 0, RL>(t, i, q)] = v[i * RL + q].x - mean;
 }
 
 // one block per screen, one thread per (p, a, b)

@@ -33,10 +33,10 @@ static float2 wn(long long e, int N) // exp(-i 2 pi e / N), e reduced mod N firs
     return make_float2((float)cos(ang), (float)sin(ang));
 }
 
-template <int N>
+template <int N, int V>
 static void fill_twiddles(std::vector<float2> &h)
 {
-    using PI = PlanInfo<N>;
+    using PI = PlanInfo<N, V>;
     h.assign(PI::TW_TOTAL, make_float2(1.f, 0.f));
     // forward plan (R1, R2, R3)
     for (int k = 0; k < PI::R1; ++k)
@@ -50,27 +50,28 @@ static void fill_twiddles(std::vector<float2> &h)
         for (int n3 = 0; n3 < PI::R1; ++n3) h[PI::TW2R + k * PI::R1 + n3] = wn((long long)PI::RL * n3 * k, N);
 }
 
-int get_twiddles(ssp_ctx *ctx, int N, const float2 **out)
+int get_twiddles(ssp_ctx *ctx, int N, int V, const float2 **out)
 {
-    auto it = ctx->twiddles.find(N);
+    const int key = 2 * N + (V ? 1 : 0);
+    auto it = ctx->twiddles.find(key);
     if (it != ctx->twiddles.end()) { *out = it->second; return SSP_OK; }
     std::vector<float2> h;
     switch (N) {
-    case 8: fill_twiddles<8>(h); break;
-    case 16: fill_twiddles<16>(h); break;
-    case 32: fill_twiddles<32>(h); break;
-    case 64: fill_twiddles<64>(h); break;
-    case 128: fill_twiddles<128>(h); break;
-    case 256: fill_twiddles<256>(h); break;
-    case 512: fill_twiddles<512>(h); break;
-    case 1024: fill_twiddles<1024>(h); break;
-    case 2048: fill_twiddles<2048>(h); break;
-    case 4096: fill_twiddles<4096>(h); break;
+    case 8: V ? fill_twiddles<8, 1>(h) : fill_twiddles<8, 0>(h); break;
+    case 16: V ? fill_twiddles<16, 1>(h) : fill_twiddles<16, 0>(h); break;
+    case 32: V ? fill_twiddles<32, 1>(h) : fill_twiddles<32, 0>(h); break;
+    case 64: V ? fill_twiddles<64, 1>(h) : fill_twiddles<64, 0>(h); break;
+    case 128: V ? fill_twiddles<128, 1>(h) : fill_twiddles<128, 0>(h); break;
+    case 256: V ? fill_twiddles<256, 1>(h) : fill_twiddles<256, 0>(h); break;
+    case 512: V ? fill_twiddles<512, 1>(h) : fill_twiddles<512, 0>(h); break;
+    case 1024: V ? fill_twiddles<1024, 1>(h) : fill_twiddles<1024, 0>(h); break;
+    case 2048: V ? fill_twiddles<2048, 1>(h) : fill_twiddles<2048, 0>(h); break;
+    case 4096: V ? fill_twiddles<4096, 1>(h) : fill_twiddles<4096, 0>(h); break;
     default: return ctx->fail(SSP_EINVAL, "unsupported N=%d", N);
     }
     float2 *d = nullptr;
     if (int rc = upload(ctx, h, &d)) return rc;
-    ctx->twiddles[N] = d;
+    ctx->twiddles[key] = d;
     *out = d;
     return SSP_OK;
 }
