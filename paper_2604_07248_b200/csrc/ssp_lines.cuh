@@ -79,10 +79,24 @@ __device__ __forceinline__ void sincos_reduced(float x, float *s, float *c)
     *c = __cosf(r);
 }
 
-// super-Gaussian window exp(-(q)^(h)), q = r^2/sigma^2 (q = 0 -> 1)
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float lg2_approx(float x)
+{
+    float y;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// super-Gaussian window exp(-(q)^(h)), q = r^2/sigma^2: three SFU ops, no special-case fix-ups
+// (q = 0: lg2 -> -inf, ex2 -> 0, exp(-0) = 1).
 __device__ __forceinline__ float window_amp(float q, float h)
 {
-    return __expf(-__powf(q, h));
+    return ex2_approx(-1.4426950408889634f * ex2_approx(h * lg2_approx(q)));
 }
 
 } // namespace ssp
