@@ -133,9 +133,10 @@ __device__ __forceinline__ void radix(float2 *v)
 }
 
 // ---- plans -----------------------------------------------------------------------
-// V = 0 ("row" variant): for N >= 1024 symmetric three-stage plans with 16 points per thread
-//   (about 64 registers) so that 32 warps fit one SM and a line synchronises on its own named
-//   barrier; measured on B200 the row kernel went from 2937 to 3441 GB/s with it.
+// V = 0 ("row" variant): plans whose first and last radix agree wherever one exists, so that the
+//   row kernel can run one forward-transform body twice (ssp_kernels.cuh).  N = 1024 is 32 x 32 with
+//   one warp per row (a single exchange, __syncwarp only); N >= 2048 are three-stage plans with 16
+//   points per thread and a named barrier per row.
 // V = 1 ("column" variant): 32 points per thread and as few exchanges as possible, because a
 //   column tile synchronises the whole CTA at every exchange (E = 16 measured 2664 vs 3388 GB/s).
 template <int N, int V> struct Plan;
@@ -148,7 +149,7 @@ SSP_PLAN(64, 0, 8, 8, 1, 8);       SSP_PLAN(64, 1, 8, 8, 1, 8);
 SSP_PLAN(128, 0, 16, 8, 1, 16);    SSP_PLAN(128, 1, 16, 8, 1, 16);
 SSP_PLAN(256, 0, 16, 16, 1, 16);   SSP_PLAN(256, 1, 16, 16, 1, 16);
 SSP_PLAN(512, 0, 32, 16, 1, 32);   SSP_PLAN(512, 1, 32, 16, 1, 32);
-SSP_PLAN(1024, 0, 16, 4, 16, 16);  SSP_PLAN(1024, 1, 32, 32, 1, 32);
+SSP_PLAN(1024, 0, 32, 32, 1, 32);   SSP_PLAN(1024, 1, 32, 32, 1, 32);
 SSP_PLAN(2048, 0, 16, 8, 16, 16);  SSP_PLAN(2048, 1, 32, 8, 8, 32);
 SSP_PLAN(4096, 0, 16, 16, 16, 16); SSP_PLAN(4096, 1, 32, 16, 8, 32);
 #undef SSP_PLAN

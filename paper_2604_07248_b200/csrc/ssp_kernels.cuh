@@ -1,0 +1,227 @@
+// ssp_kernels.cuh -- row and column kernels of the fused split step (K4-K7).
+//
+//   k_row<N,FIRST,SECOND,EXTRA>:  [IFFT_x] -> * exp(+-i phi) W [-> save plane / phase gradient]
+//                                 -> [FFT_x] -> * hx(next step)                  (Eq.1)
+//   k_col<N,MODE>:                FFT_y -> * hy/N^2 -> IFFT_y on a tile of C columns (register loads)
+//   k_col_tma<N>:                 the same pass with the tile moved by TMA (ssp_col_tma.cuh)
+//
+// One split step = one column + one row launch = two HBM round trips of the field plus one
+// fp32 read of the screen: 36 B/px.  H is separable for the Fresnel
+// kernel, H = hx[kx] hy[ky], both 1-D tables built in double on the host.
+//
+// Inverse transforms run the FORWARD code on re/im-swapped data: with s(a+ib) = b+ia,
+// IFFT(x) = s(FFT(s(x))), and the swap is register renaming.  For plans whose first and last
+// radix agree the output layout of a transform equals its input layout, so IFFT -> pointwise
+// -> FFT is one forward-transform body executed twice in a rolled loop: half the code, which
+// matters because the unrolled butterflies otherwise overflow the 32 KB instruction cache.
+#pragma once
+
+#include "ssp_internal.h"
+#include "ssp_lines.cuh"
+
+namespace ssp {
+
+template <bool SWAP>
+__device__ __forceinline__ float2 swap_if(float2 x) { return SWAP ? make_float2(x.y, x.x) : x; }
+
+// Pointwise stage in real space on a line held in the layout strided by RL.
+template <int N, int RL, int E, int T, bool EXTRA>
+__device__ __forceinline__ void row_pointwise(float2 *v, const RowArgs &a, const float *phis, int t, int b, int iy)
+{
+    const long long pix0 = (long long)iy * N;
+    const float yc = (float)(iy - N / 2);
+    const float y2 = yc * yc * a.win_qs;
+    const float xf = (float)(t - N / 2);
+#pragma unroll
+    for (int i = 0; i < E / RL; ++i)
+#pragma unroll
+        for (int q = 0; q < RL; ++q) {
+            const int off = q * (N / RL) + T * i;                 // ix = t + off, off compile-time
+            float2 u = v[i * RL + q];
+            if constexpr (EXTRA) {
+                if (a.grad) {
+                    const float2 U = a.plane_in[b * a.plane_stride + pix0 + t + off];
+                    a.grad[b * a.grad_stride + pix0 + t + off] = u.y * U.x - u.x * U.y; // Im(G conj(U))
+                }
+            }
+            float mr = 1.f, mi = 0.f;
+            if (a.phi) {
+                sincos_reduced(phis[t + off], &mi, &mr);
+                mi *= a.phase_sign;
+            }
+            if (a.win_on) {
+                const float xc = xf + (float)off;
+                const float amp = window_amp(fmaf(xc * xc, a.win_qs, y2), a.win_half_order);
+                mr *= amp;
+                mi *= amp;
+            }
+            u = cmul(u, make_float2(mr, mi));
+            if constexpr (EXTRA) {
+                if (a.plane_out) a.plane_out[b * a.plane_stride + pix0 + t + off] = u;
+            }
+            v[i * RL + q] = u;
+        }
+}
+
+template <int N, bool FIRST, bool SECOND, bool EXTRA>
+__global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_row(const RowArgs a)
+{
+    using PI = PlanInfo<N, 0>;
+    using CFG = RowCfg<N>;
+    constexpr int E = PI::E, T = PI::T, R1 = PI::R1, RL = PI::RL;
+    constexpr bool SYM = (R1 == RL);                              // output layout == input layout
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *smem = reinterpret_cast<float2 *>(smem_raw);
+
+    const int tid = threadIdx.x;
+    const int lib = tid / T, t = tid % T;
+    const long long line = (long long)blockIdx.x * CFG::LPB + lib;
+    const int b = (int)(line / N), iy = (int)(line % N);
+    RowSmem<T> sm{smem + (size_t)lib * PI::LINE_ELEMS, 1 + lib};
+
+    // the screen row is streamed from HBM: fetch it asynchronously now, use it after the first transform
+    float *phis = reinterpret_cast<float *>(smem_raw + CFG::SMEM_X) + (size_t)lib * N;
+    if (a.phi) {
+        const float *g = a.phi + b * a.phi_batch_stride + (long long)iy * N;
+#pragma unroll
+        for (int i = 0; i < E / 4; ++i) cp_async16(phis + 4 * (t + T * i), g + 4 * (t + T * i));
+        cp_async_commit();
+    }
+    const bool pointwise = a.phi || a.win_on || (EXTRA && (a.grad || a.plane_out));
+
+    float2 v[E];
+    // FIRST (an inverse transform comes first) loads re/im-swapped when the forward code runs it
+    constexpr bool SWAP_IN = FIRST && SYM;
+    constexpr int RIN = (FIRST || SYM) ? R1 : RL;
+    {
+        const float2 *src = a.in + line * N;
+#pragma unroll
+        for (int i = 0; i < E / RIN; ++i)
+#pragma unroll
+            for (int q = 0; q < RIN; ++q) {
+                float2 x = src[line_index<N, 0, RIN>(t, i, q)];
+                if constexpr (EXTRA) {
+                    if (a.pre) {
+                        const float2 pl = a.pre_line ? __ldg(a.pre_line + iy) : make_float2(1.f, 0.f);
+                        x = cmul(x, cmul(pl, __ldg(a.pre + line_index<N, 0, RIN>(t, i, q))));
+                    }
+                }
+                v[i * RIN + q] = swap_if<SWAP_IN>(x);
+            }
+    }
+    auto wait_phi = [&]() {
+        if (a.phi) {
+            cp_async_wait_all();
+            sm.sync();
+        }
+    };
+
+    constexpr int ROUT = SYM ? R1 : (SECOND ? R1 : RL);
+    if constexpr (SYM) {
+        if constexpr (FIRST && SECOND) {
+#pragma unroll 1
+            for (int pass = 0; pass < 2; ++pass) {
+                fft_line<N, 0, false, false>(v, t, sm, a.tw);
+                if (pass == 0) {
+#pragma unroll
+                    for (int e = 0; e < E; ++e) v[e] = swap_if<true>(v[e]);
+                    if (pointwise) {
+                        wait_phi();
+                        row_pointwise<N, RL, E, T, EXTRA>(v, a, phis, t, b, iy);
+                    }
+                    sm.sync();                                    // the exchange buffer is reused
+                }
+            }
+        } else if constexpr (FIRST) {
+            fft_line<N, 0, false, false>(v, t, sm, a.tw);
+#pragma unroll
+            for (int e = 0; e < E; ++e) v[e] = swap_if<true>(v[e]);
+            if (pointwise) {
+                wait_phi();
+                row_pointwise<N, RL, E, T, EXTRA>(v, a, phis, t, b, iy);
+            }
+        } else {
+            if (pointwise) {
+                wait_phi();
+                row_pointwise<N, RL, E, T, EXTRA>(v, a, phis, t, b, iy);
+            }
+            fft_line<N, 0, false, false>(v, t, sm, a.tw);
+        }
+    } else {
+        if constexpr (FIRST) fft_line<N, 0, false, true>(v, t, sm, a.tw); // inverse; now strided by RL
+        if (pointwise) {
+            wait_phi();
+            row_pointwise<N, RL, E, T, EXTRA>(v, a, phis, t, b, iy);
+        }
+        if constexpr (SECOND) {
+            if constexpr (FIRST) sm.sync();                       // the exchange buffer is reused
+            fft_line<N, 0, true, false>(v, t, sm, a.tw);          // forward, reversed plan; strided by R1
+        }
+    }
+
+    float2 *dst = a.out + line * N;
+    if (a.hx) {
+#pragma unroll
+        for (int i = 0; i < E / ROUT; ++i)
+#pragma unroll
+            for (int q = 0; q < ROUT; ++q) {
+                const int k = line_index<N, 0, ROUT>(t, i, q);
+                dst[k] = cmul(v[i * ROUT + q], __ldg(a.hx + k));
+            }
+    } else {
+#pragma unroll
+        for (int i = 0; i < E / ROUT; ++i)
+#pragma unroll
+            for (int q = 0; q < ROUT; ++q) dst[line_index<N, 0, ROUT>(t, i, q)] = v[i * ROUT + q];
+    }
+}
+
+// MODE 0: FFT_y -> * hy -> IFFT_y.  MODE 1: FFT_y -> * hy.  MODE 2: unnormalised IFFT_y -> * hy.
+template <int N, int MODE>
+__global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_col(const ColArgs a)
+{
+    using PI = PlanInfo<N, 1>;
+    using CFG = ColCfg<N>;
+    constexpr int E = PI::E, T = PI::T, C = CFG::C;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2 *smem = reinterpret_cast<float2 *>(smem_raw);
+
+    const int tid = threadIdx.x;
+    const int c = tid % C, t = tid / C;
+    constexpr int GROUPS = N / C;
+    const int b = blockIdx.x / GROUPS, col = (blockIdx.x % GROUPS) * C + c;
+    ColSmem<C> sm{smem + c};
+
+    float2 v[E];
+    constexpr int R1 = PI::R1, RL = PI::RL;
+    const float2 *src = a.in + (size_t)b * N * N + col;
+#pragma unroll
+    for (int i = 0; i < E / R1; ++i)
+#pragma unroll
+        for (int q = 0; q < R1; ++q) v[i * R1 + q] = src[(size_t)line_index<N, 1, R1>(t, i, q) * N];
+
+    fft_line<N, 1, false, MODE == 2>(v, t, sm, a.tw); // strided by RL
+    if (a.hy) {
+#pragma unroll
+        for (int i = 0; i < E / RL; ++i)
+#pragma unroll
+            for (int q = 0; q < RL; ++q)
+                v[i * RL + q] = cmul(v[i * RL + q], __ldg(a.hy + line_index<N, 1, RL>(t, i, q)));
+    }
+    float2 *dst = a.out + (size_t)b * N * N + col;
+    if constexpr (MODE == 0) {
+        sm.sync();
+        fft_line<N, 1, true, true>(v, t, sm, a.tw);   // inverse, reversed plan; strided by R1
+#pragma unroll
+        for (int i = 0; i < E / R1; ++i)
+#pragma unroll
+            for (int q = 0; q < R1; ++q) dst[(size_t)line_index<N, 1, R1>(t, i, q) * N] = v[i * R1 + q];
+    } else {
+#pragma unroll
+        for (int i = 0; i < E / RL; ++i)
+#pragma unroll
+            for (int q = 0; q < RL; ++q) dst[(size_t)line_index<N, 1, RL>(t, i, q) * N] = v[i * RL + q];
+    }
+}
+
+} // namespace ssp

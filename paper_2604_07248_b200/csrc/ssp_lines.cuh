@@ -7,19 +7,32 @@
 namespace ssp {
 
 // ---- CTA shapes --------------------------------------------------------------------
+// Row-kernel CTA size and resident CTAs per SM the register budget is sized for.  Default: 256
+// threads, 512 resident threads at E = 32 and 1024 at E = 16.  N = 1024 (one warp per row, 32 points
+// per thread) measured best on B200 with 168 registers: 3 CTAs of 4 rows (profiles/r01_notes.md).
+template <int N>
+struct RowTune {
+    static constexpr int MAX_THREADS = 256;
+    static constexpr int MIN_BLOCKS = (PlanInfo<N, 0>::E >= 32) ? 2 : 4;
+};
+template <>
+struct RowTune<1024> {
+    static constexpr int MAX_THREADS = 128;
+    static constexpr int MIN_BLOCKS = 3;
+};
+
 template <int N>
 struct RowCfg {
     static constexpr int V = 0;                                   // plan variant
     static constexpr int T = PlanInfo<N, 0>::T;
-    static constexpr int THREADS = (T * N < 256) ? T * N : 256;
+    static constexpr int THREADS = (T * N < RowTune<N>::MAX_THREADS) ? T * N : RowTune<N>::MAX_THREADS;
     static constexpr int LPB = THREADS / T;                        // lines (rows) per CTA
     static constexpr bool WARP_LOCAL = (T <= 32);                  // a line never spans two warps
     static constexpr size_t SMEM_X = (PlanInfo<N, 0>::NSTAGE == 1) ? 0
         : sizeof(float2) * (size_t)LPB * PlanInfo<N, 0>::LINE_ELEMS;       // exchange buffers
     static constexpr size_t SMEM_PHI = sizeof(float) * (size_t)LPB * N; // prefetched screen rows
     static constexpr size_t SMEM = SMEM_X + SMEM_PHI;
-    // resident CTAs per SM the register budget is sized for: 512 threads at E = 32, 1024 at E = 16
-    static constexpr int MIN_BLOCKS = (THREADS < 256) ? 1 : (PlanInfo<N, 0>::E >= 32 ? 2 : 4);
+    static constexpr int MIN_BLOCKS = (THREADS < RowTune<N>::MAX_THREADS) ? 1 : RowTune<N>::MIN_BLOCKS;
 };
 
 template <int N>

@@ -8,161 +8,9 @@
 // One split step = one k_col + one k_row launch = two HBM round trips of the field plus one
 // fp32 read of the screen: 36 B/px.  H is separable for the Fresnel
 // kernel, H = hx[kx] hy[ky], both 1-D tables built in double on the host.
-#include "ssp_internal.h"
-#include "ssp_lines.cuh"
+#include "ssp_kernels.cuh"
 
 namespace ssp {
-
-template <int N, bool FIRST, bool SECOND>
-__global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_row(const RowArgs a)
-{
-    using PI = PlanInfo<N, 0>;
-    using CFG = RowCfg<N>;
-    constexpr int E = PI::E, T = PI::T;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2 *smem = reinterpret_cast<float2 *>(smem_raw);
-
-    const int tid = threadIdx.x;
-    const int lib = tid / T, t = tid % T;
-    const long long line = (long long)blockIdx.x * CFG::LPB + lib;
-    const int b = (int)(line / N), iy = (int)(line % N);
-    RowSmem<T> sm{smem + (size_t)lib * PI::LINE_ELEMS, 1 + lib};
-
-    // the screen row is streamed from HBM: fetch it asynchronously now, use it after the first transform
-    float *phis = reinterpret_cast<float *>(smem_raw + CFG::SMEM_X) + (size_t)lib * N;
-    if (a.phi) {
-        const float *g = a.phi + b * a.phi_batch_stride + (long long)iy * N;
-#pragma unroll
-        for (int i = 0; i < E / 4; ++i) cp_async16(phis + 4 * (t + T * i), g + 4 * (t + T * i));
-        cp_async_commit();
-    }
-
-    float2 v[E];
-    constexpr int RIN = FIRST ? PI::R1 : PI::RL;
-    {
-        const float2 *src = a.in + line * N;
-#pragma unroll
-        for (int i = 0; i < E / RIN; ++i)
-#pragma unroll
-            for (int q = 0; q < RIN; ++q) v[i * RIN + q] = src[line_index<N, 0, RIN>(t, i, q)];
-    }
-    if (a.pre) {
-        const float2 pl = a.pre_line ? __ldg(a.pre_line + iy) : make_float2(1.f, 0.f);
-#pragma unroll
-        for (int i = 0; i < E / RIN; ++i)
-#pragma unroll
-            for (int q = 0; q < RIN; ++q)
-                v[i * RIN + q] = cmul(v[i * RIN + q], cmul(pl, __ldg(a.pre + line_index<N, 0, RIN>(t, i, q))));
-    }
-
-    if constexpr (FIRST) fft_line<N, 0, false, true>(v, t, sm, a.tw); // inverse; now strided by RL
-
-    // ---- pointwise stage in real space, layout strided by RL
-    constexpr int RL = PI::RL;
-    const bool pointwise = a.phi || a.win_on || a.grad || a.plane_out;
-    if (pointwise) {
-        if (a.phi) {
-            cp_async_wait_all();
-            sm.sync();
-        }
-        const long long pix0 = (long long)iy * N;
-        const float yc = (float)(iy - N / 2);
-#pragma unroll
-        for (int i = 0; i < E / RL; ++i)
-#pragma unroll
-            for (int q = 0; q < RL; ++q) {
-                const int ix = line_index<N, 0, RL>(t, i, q);
-                float2 u = v[i * RL + q];
-                if (a.grad) {
-                    const float2 U = a.plane_in[b * a.plane_stride + pix0 + ix];
-                    a.grad[b * a.grad_stride + pix0 + ix] = u.y * U.x - u.x * U.y; // Im(G conj(U))
-                }
-                float mr = 1.f, mi = 0.f;
-                if (a.phi) {
-                    sincos_reduced(phis[ix], &mi, &mr);
-                    mi *= a.phase_sign;
-                }
-                if (a.win_on) {
-                    const float xc = (float)(ix - N / 2);
-                    const float amp = window_amp((xc * xc + yc * yc) * a.win_qs, a.win_half_order);
-                    mr *= amp;
-                    mi *= amp;
-                }
-                u = cmul(u, make_float2(mr, mi));
-                if (a.plane_out) a.plane_out[b * a.plane_stride + pix0 + ix] = u;
-                v[i * RL + q] = u;
-            }
-    }
-
-    constexpr int ROUT = SECOND ? PI::R1 : PI::RL;
-    if constexpr (SECOND) {
-        if constexpr (FIRST) sm.sync();                  // the exchange buffer is reused
-        fft_line<N, 0, true, false>(v, t, sm, a.tw);        // forward, reversed plan; strided by R1
-    }
-    float2 *dst = a.out + line * N;
-    if (a.hx) {
-#pragma unroll
-        for (int i = 0; i < E / ROUT; ++i)
-#pragma unroll
-            for (int q = 0; q < ROUT; ++q) {
-                const int k = line_index<N, 0, ROUT>(t, i, q);
-                dst[k] = cmul(v[i * ROUT + q], __ldg(a.hx + k));
-            }
-    } else {
-#pragma unroll
-        for (int i = 0; i < E / ROUT; ++i)
-#pragma unroll
-            for (int q = 0; q < ROUT; ++q) dst[line_index<N, 0, ROUT>(t, i, q)] = v[i * ROUT + q];
-    }
-}
-
-// MODE 0: FFT_y -> * hy -> IFFT_y.  MODE 1: FFT_y -> * hy.  MODE 2: unnormalised IFFT_y -> * hy.
-template <int N, int MODE>
-__global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_col(const ColArgs a)
-{
-    using PI = PlanInfo<N, 1>;
-    using CFG = ColCfg<N>;
-    constexpr int E = PI::E, T = PI::T, C = CFG::C;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2 *smem = reinterpret_cast<float2 *>(smem_raw);
-
-    const int tid = threadIdx.x;
-    const int c = tid % C, t = tid / C;
-    constexpr int GROUPS = N / C;
-    const int b = blockIdx.x / GROUPS, col = (blockIdx.x % GROUPS) * C + c;
-    ColSmem<C> sm{smem + c};
-
-    float2 v[E];
-    constexpr int R1 = PI::R1, RL = PI::RL;
-    const float2 *src = a.in + (size_t)b * N * N + col;
-#pragma unroll
-    for (int i = 0; i < E / R1; ++i)
-#pragma unroll
-        for (int q = 0; q < R1; ++q) v[i * R1 + q] = src[(size_t)line_index<N, 1, R1>(t, i, q) * N];
-
-    fft_line<N, 1, false, MODE == 2>(v, t, sm, a.tw); // strided by RL
-    if (a.hy) {
-#pragma unroll
-        for (int i = 0; i < E / RL; ++i)
-#pragma unroll
-            for (int q = 0; q < RL; ++q)
-                v[i * RL + q] = cmul(v[i * RL + q], __ldg(a.hy + line_index<N, 1, RL>(t, i, q)));
-    }
-    float2 *dst = a.out + (size_t)b * N * N + col;
-    if constexpr (MODE == 0) {
-        sm.sync();
-        fft_line<N, 1, true, true>(v, t, sm, a.tw);   // inverse, reversed plan; strided by R1
-#pragma unroll
-        for (int i = 0; i < E / R1; ++i)
-#pragma unroll
-            for (int q = 0; q < R1; ++q) dst[(size_t)line_index<N, 1, R1>(t, i, q) * N] = v[i * R1 + q];
-    } else {
-#pragma unroll
-        for (int i = 0; i < E / RL; ++i)
-#pragma unroll
-            for (int q = 0; q < RL; ++q) dst[(size_t)line_index<N, 1, RL>(t, i, q) * N] = v[i * RL + q];
-    }
-}
 
 // ---- launchers ------------------------------------------------------------------------
 template <class K>
@@ -173,12 +21,12 @@ static int set_smem(ssp_ctx *ctx, K kernel, size_t bytes)
     return SSP_OK;
 }
 
-template <int N, bool FIRST, bool SECOND>
-static int launch_row_n(ssp_ctx *ctx, const RowArgs &a)
+template <int N, bool FIRST, bool SECOND, bool EXTRA>
+static int launch_row_x(ssp_ctx *ctx, const RowArgs &a)
 {
     using CFG = RowCfg<N>;
     if (a.n_lines % CFG::LPB) return ctx->fail(SSP_EINVAL, "row launch: %d lines not a multiple of %d", a.n_lines, CFG::LPB);
-    auto kern = k_row<N, FIRST, SECOND>;
+    auto kern = k_row<N, FIRST, SECOND, EXTRA>;
     if (int rc = set_smem(ctx, kern, CFG::SMEM)) return rc;
     // algorithmic bytes: field in + out, + the screen, + saved / read planes and the gradient
     const double bpp = 16.0 + (a.phi ? 4.0 : 0.0) + (a.plane_out ? 8.0 : 0.0) + (a.grad ? 12.0 : 0.0);
@@ -188,6 +36,14 @@ static int launch_row_n(ssp_ctx *ctx, const RowArgs &a)
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;
+}
+
+// EXTRA = saved planes, phase gradient or the input pre-multiply are compiled in
+template <int N, bool FIRST, bool SECOND>
+static int launch_row_n(ssp_ctx *ctx, const RowArgs &a)
+{
+    if (a.grad || a.plane_out || a.pre) return launch_row_x<N, FIRST, SECOND, true>(ctx, a);
+    return launch_row_x<N, FIRST, SECOND, false>(ctx, a);
 }
 
 template <int N>
