@@ -1,0 +1,165 @@
+// ssp_col_tma.cuh -- column pass of the split step with the tile moved by TMA (K5).
+//
+// A tile is C adjacent columns x N rows of one field.  Persistent CTAs walk the tiles with two
+// shared-memory buffers each: while tile i is transformed (FFT_y -> * hy/N^2 -> IFFT_y, PAPER.md:37
+// Eq.1) in buffer i&1, the TMA engine loads tile i+1 into the other buffer, and the result of tile
+// i leaves through a TMA store from the buffer it was computed in.  No global load or store is
+// issued by the threads, so the column kernel neither queues on the LSU nor exposes DRAM latency.
+// The buffer is used three ways in turn: dense [row][C] tile written by TMA, padded exchange
+// buffer of the in-register FFT (ssp_fft.cuh), dense result tile read by TMA.
+#pragma once
+
+#include <cuda.h>
+
+#include "ssp_internal.h"
+#include "ssp_lines.cuh"
+
+namespace ssp {
+
+// ---- mbarrier / bulk-tensor copy wrappers (PTX ISA: mbarrier, cp.async.bulk.tensor) ------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        " @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void *dst, const CUtensorMap *tm, int x, int y, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(smem_u32(dst)), "l"(tm), "r"(x), "r"(y), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap *tm, int x, int y, const void *src)
+{
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
+                 ::"l"(tm), "r"(x), "r"(y), "r"(smem_u32(src)) : "memory");
+}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+
+// ---- CTA shape ---------------------------------------------------------------------------------
+template <int N>
+struct ColTmaCfg {
+    static constexpr int T = PlanInfo<N, 1>::T;
+    static constexpr int C = 4;                                       // 32-byte row segments per box
+    static constexpr int THREADS = T * C;
+    static constexpr int MIN_BLOCKS = 3;
+    static constexpr int BOX_ROWS = (N < 256) ? N : 256;              // TMA box dimensions are <= 256
+    static constexpr int BOXES = N / BOX_ROWS;
+    static constexpr int BUF_ELEMS = C * PlanInfo<N, 1>::LINE_ELEMS;  // float2 per buffer (padded exchange)
+    static constexpr size_t SMEM = 2 * sizeof(float2) * BUF_ELEMS + 16;
+    static constexpr unsigned TILE_BYTES = (unsigned)(sizeof(float2) * C * N);
+};
+
+struct ColTmaArgs {
+    const float2 *hy;            // [N] multiplier between the transforms
+    const float2 *tw;            // column-plan twiddles
+    int ntiles;                  // B * N / C
+};
+
+// FFT_y -> * hy -> IFFT_y.  tm_in / tm_out describe the [B*N rows][2N floats] field buffers.
+template <int N>
+__global__ void __launch_bounds__(ColTmaCfg<N>::THREADS, ColTmaCfg<N>::MIN_BLOCKS)
+k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_out, const ColTmaArgs a)
+{
+    using PI = PlanInfo<N, 1>;
+    using CFG = ColTmaCfg<N>;
+    constexpr int E = PI::E, C = CFG::C, R1 = PI::R1, RL = PI::RL;
+    constexpr bool SYM = (R1 == RL);
+    constexpr int GROUPS = N / C;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float2 *sbuf = reinterpret_cast<float2 *>(smem_raw);
+    unsigned long long *full = reinterpret_cast<unsigned long long *>(smem_raw + 2 * sizeof(float2) * CFG::BUF_ELEMS);
+    const int tid = threadIdx.x, c = tid % C, t = tid / C;
+
+    auto issue_load = [&](int tile, int buf) {
+        const int b = tile / GROUPS, col0 = (tile % GROUPS) * C;
+        mbar_expect_tx(&full[buf], CFG::TILE_BYTES);
+#pragma unroll
+        for (int j = 0; j < CFG::BOXES; ++j)
+            tma_load_2d(sbuf + buf * CFG::BUF_ELEMS + j * CFG::BOX_ROWS * C, &tm_in, 2 * col0, b * N + j * CFG::BOX_ROWS,
+                        &full[buf]);
+    };
+    if (tid == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        fence_mbar_init();
+        if ((int)blockIdx.x < a.ntiles) issue_load(blockIdx.x, 0);
+    }
+    __syncthreads();
+
+    int it = 0;
+    for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x, ++it) {
+        const int cur = it & 1;
+        float2 *tile_s = sbuf + cur * CFG::BUF_ELEMS;
+        ColSmem<C> sm{tile_s + c};
+        mbar_wait(&full[cur], (it >> 1) & 1);
+        float2 v[E];
+#pragma unroll
+        for (int i = 0; i < E / R1; ++i)
+#pragma unroll
+            for (int q = 0; q < R1; ++q) v[i * R1 + q] = tile_s[line_index<N, 1, R1>(t, i, q) * C + c];
+        __syncthreads();                                          // the tile is in registers: the buffer is free
+        if (tid == 0 && tile + (int)gridDim.x < a.ntiles) {
+            tma_store_wait_read();                                // the store of tile it-1 has released the other buffer
+            issue_load(tile + gridDim.x, cur ^ 1);
+        }
+        if constexpr (SYM) {
+            // pass 0: forward; * hy, leaving the product re/im-swapped; pass 1: forward on swapped data = inverse
+#pragma unroll 1
+            for (int pass = 0; pass < 2; ++pass) {
+                fft_line<N, 1, false, false, true>(v, t, sm, a.tw);
+                if (pass == 0) {
+#pragma unroll
+                    for (int i = 0; i < E / RL; ++i)
+#pragma unroll
+                        for (int q = 0; q < RL; ++q) {
+                            const float2 h = __ldg(a.hy + line_index<N, 1, RL>(t, i, q)), x = v[i * RL + q];
+                            v[i * RL + q] = make_float2(fmaf(x.x, h.y, x.y * h.x), fmaf(x.x, h.x, -x.y * h.y));
+                        }
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < E / R1; ++i)
+#pragma unroll
+                for (int q = 0; q < R1; ++q) {
+                    const float2 x = v[i * R1 + q];
+                    tile_s[line_index<N, 1, R1>(t, i, q) * C + c] = make_float2(x.y, x.x);
+                }
+        } else {
+            fft_line<N, 1, false, false, true>(v, t, sm, a.tw);   // strided by RL
+#pragma unroll
+            for (int i = 0; i < E / RL; ++i)
+#pragma unroll
+                for (int q = 0; q < RL; ++q)
+                    v[i * RL + q] = cmul(v[i * RL + q], __ldg(a.hy + line_index<N, 1, RL>(t, i, q)));
+            fft_line<N, 1, true, true, true>(v, t, sm, a.tw);     // inverse, reversed plan; strided by R1
+#pragma unroll
+            for (int i = 0; i < E / R1; ++i)
+#pragma unroll
+                for (int q = 0; q < R1; ++q) tile_s[line_index<N, 1, R1>(t, i, q) * C + c] = v[i * R1 + q];
+        }
+        fence_proxy_async();                                      // generic-proxy writes visible to the TMA store
+        __syncthreads();
+        if (tid == 0) {
+            const int b = tile / GROUPS, col0 = (tile % GROUPS) * C;
+#pragma unroll
+            for (int j = 0; j < CFG::BOXES; ++j)
+                tma_store_2d(&tm_out, 2 * col0, b * N + j * CFG::BOX_ROWS, tile_s + j * CFG::BOX_ROWS * C);
+            tma_store_commit();
+        }
+    }
+    if (tid == 0) tma_store_wait_read();
+}
+
+} // namespace ssp

@@ -177,8 +177,11 @@ struct PlanInfo {
 // One complete transform of a line held in registers.
 //   DIR_REV = false: plan (R1,R2,R3): input strided by R1, output strided by RL.
 //   DIR_REV = true : plan (RL,..,R1): input strided by RL, output strided by R1.
-// SM: exchange accessor with  st(pos, val), ld(pos), sync()  on UNPADDED positions of this line.
-template <int N, int V, bool DIR_REV, bool INV, class SM>
+// SM: exchange accessor with  st(pos, val), ld(pos), sync()  on padded positions of this line.
+// TAIL_SYNC: synchronise right after the last exchange has been read, so that the caller may reuse
+// the buffer at once.  A barrier placed there is cheap (the threads have just left the previous one);
+// the same barrier after the last butterflies would re-align threads that have drifted apart.
+template <int N, int V, bool DIR_REV, bool INV, bool TAIL_SYNC = false, class SM>
 __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 *__restrict__ tw)
 {
     using PI = PlanInfo<N, V>;
@@ -189,7 +192,9 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 
     constexpr int PADQ = N / Ra;
     const float2 *tw1 = tw + (DIR_REV ? PI::TW1R : PI::TW1);
     const float2 *tw2 = tw + (DIR_REV ? PI::TW2R : PI::TW2);
-    auto pad = [](int p) { return p + p / PADQ; };
+    // padded position of line index k1 * PADQ + r, r < PADQ: one pad element per PADQ positions.  Written
+    // with k1 explicit so that no division of a run-time index is left in the address arithmetic.
+    constexpr int PITCH = PADQ + 1;
 
     // ---- stage 1
     constexpr int M1 = N / Ra;
@@ -202,7 +207,7 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 
             for (int k = 0; k < Ra; ++k) {
                 float2 x = v[i * Ra + k];
                 if (k > 0) x = cmul_c<INV>(x, __ldg(tw1 + k * M1 + m));
-                sm.st(pad(k * M1 + m), x);
+                sm.st(k * PITCH + m, x);
             }
         }
     }
@@ -215,9 +220,11 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 
         for (int i = 0; i < E / Rb; ++i) {
             const int j = t + T * i;
 #pragma unroll
-            for (int n = 0; n < Rb; ++n) v[i * Rb + n] = sm.ld(pad(j * Rb + n));
-            radix<Rb, INV>(v + i * Rb);
+            for (int n = 0; n < Rb; ++n) v[i * Rb + n] = sm.ld(j * PITCH + n);
         }
+        if constexpr (TAIL_SYNC) sm.sync();
+#pragma unroll
+        for (int i = 0; i < E / Rb; ++i) radix<Rb, INV>(v + i * Rb);
     } else {
         // ---- stage 2 (middle): butterfly j = k1 + Ra*n3 (k1 fastest: with the pitch N/Ra + 1 the
         // 16 lanes of a half warp hit 16 different bank pairs), in place
@@ -225,16 +232,16 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 
         for (int i = 0; i < E / Rb; ++i) {
             const int j = t + T * i;
             const int k1 = j % Ra, n3 = j / Ra;
-            const int base = k1 * (Rb * Rc) + n3;
+            const int base = k1 * PITCH + n3;
             float2 *w = v + i * Rb;
 #pragma unroll
-            for (int n = 0; n < Rb; ++n) w[n] = sm.ld(pad(base + n * Rc));
+            for (int n = 0; n < Rb; ++n) w[n] = sm.ld(base + n * Rc);
             radix<Rb, INV>(w);
 #pragma unroll
             for (int k = 0; k < Rb; ++k) {
                 float2 x = w[k];
                 if (k > 0) x = cmul_c<INV>(x, __ldg(tw2 + k * Rc + n3));
-                sm.st(pad(base + k * Rc), x);
+                sm.st(base + k * Rc, x);
             }
         }
         sm.sync();
@@ -243,12 +250,14 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 
         for (int i = 0; i < E / Rc; ++i) {
             const int j = t + T * i;
             const int k1 = j % Ra, k2 = j / Ra;
-            const int base = k1 * (Rb * Rc) + k2 * Rc;
+            const int base = k1 * PITCH + k2 * Rc;
             float2 *w = v + i * Rc;
 #pragma unroll
-            for (int n = 0; n < Rc; ++n) w[n] = sm.ld(pad(base + n));
-            radix<Rc, INV>(w);
+            for (int n = 0; n < Rc; ++n) w[n] = sm.ld(base + n);
         }
+        if constexpr (TAIL_SYNC) sm.sync();
+#pragma unroll
+        for (int i = 0; i < E / Rc; ++i) radix<Rc, INV>(v + i * Rc);
     }
 }
 

@@ -1,6 +1,7 @@
 // ssp_internal.h -- context, table caches and kernel launchers shared by the .cu files.
 #pragma once
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <cstdarg>
@@ -41,6 +42,7 @@ struct ssp_ctx {
     void *scratch = nullptr;                     // small device scratch (stat accumulators, tables)
     size_t scratch_bytes = 0;
     std::vector<void *> owned;                   // misc device allocations freed at destroy
+    void *encode_tiled = nullptr;                // cuTensorMapEncodeTiled, resolved through the runtime
 
     // ---- optional per-launch timing with CUDA events on the context's stream (bench.py's roofline)
     struct ProfRec { const char *name; double bytes; int ev; };
@@ -93,6 +95,10 @@ int get_twiddles(ssp_ctx *ctx, int N, int V, const float2 **out);
 int get_htable(ssp_ctx *ctx, const HKey &key, const float2 **out);
 int get_sign_table(ssp_ctx *ctx, int N, const float2 **out);
 int ensure_scratch(ssp_ctx *ctx, size_t bytes);
+// TMA descriptor of a row-major buffer of complex64: `cols` elements per row, `rows` rows, boxes of
+// box_cols x box_rows elements (no swizzle).  Encoded on the host for every call: the buffers are the caller's.
+int make_tmap_c64(ssp_ctx *ctx, const void *base, size_t cols, size_t rows, int box_cols, int box_rows,
+                  CUtensorMap *out);
 bool valid_N(int N);
 
 // ---- row / column kernels (ssp_propagate.cu) ---------------------------------------

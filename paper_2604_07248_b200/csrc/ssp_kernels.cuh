@@ -121,7 +121,10 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
         if constexpr (FIRST && SECOND) {
 #pragma unroll 1
             for (int pass = 0; pass < 2; ++pass) {
-                fft_line<N, 0, false, false>(v, t, sm, a.tw);
+                // the exchange buffer is reused by the next pass: a row spanning several warps synchronises
+                // right after its last exchange read (TAIL), a warp-local row after the pointwise stage
+                constexpr bool TAIL = (T > 32);
+                fft_line<N, 0, false, false, TAIL>(v, t, sm, a.tw);
                 if (pass == 0) {
 #pragma unroll
                     for (int e = 0; e < E; ++e) v[e] = swap_if<true>(v[e]);
@@ -129,7 +132,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
                         wait_phi();
                         row_pointwise<N, RL, E, T, EXTRA>(v, a, phis, t, b, iy);
                     }
-                    sm.sync();                                    // the exchange buffer is reused
+                    if constexpr (!TAIL) sm.sync();
                 }
             }
         } else if constexpr (FIRST) {
@@ -148,15 +151,12 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
             fft_line<N, 0, false, false>(v, t, sm, a.tw);
         }
     } else {
-        if constexpr (FIRST) fft_line<N, 0, false, true>(v, t, sm, a.tw); // inverse; now strided by RL
+        if constexpr (FIRST) fft_line<N, 0, false, true, SECOND>(v, t, sm, a.tw); // inverse; now strided by RL
         if (pointwise) {
             wait_phi();
             row_pointwise<N, RL, E, T, EXTRA>(v, a, phis, t, b, iy);
         }
-        if constexpr (SECOND) {
-            if constexpr (FIRST) sm.sync();                       // the exchange buffer is reused
-            fft_line<N, 0, true, false>(v, t, sm, a.tw);          // forward, reversed plan; strided by R1
-        }
+        if constexpr (SECOND) fft_line<N, 0, true, false>(v, t, sm, a.tw); // forward, reversed plan; strided by R1
     }
 
     float2 *dst = a.out + line * N;
@@ -200,7 +200,7 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_c
 #pragma unroll
         for (int q = 0; q < R1; ++q) v[i * R1 + q] = src[(size_t)line_index<N, 1, R1>(t, i, q) * N];
 
-    fft_line<N, 1, false, MODE == 2>(v, t, sm, a.tw); // strided by RL
+    fft_line<N, 1, false, MODE == 2, MODE == 0>(v, t, sm, a.tw); // strided by RL
     if (a.hy) {
 #pragma unroll
         for (int i = 0; i < E / RL; ++i)
@@ -210,7 +210,6 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_c
     }
     float2 *dst = a.out + (size_t)b * N * N + col;
     if constexpr (MODE == 0) {
-        sm.sync();
         fft_line<N, 1, true, true>(v, t, sm, a.tw);   // inverse, reversed plan; strided by R1
 #pragma unroll
         for (int i = 0; i < E / R1; ++i)

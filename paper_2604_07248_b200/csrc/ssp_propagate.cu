@@ -9,6 +9,7 @@
 // fp32 read of the screen: 36 B/px.  H is separable for the Fresnel
 // kernel, H = hx[kx] hy[ky], both 1-D tables built in double on the host.
 #include "ssp_kernels.cuh"
+#include "ssp_col_tma.cuh"
 
 namespace ssp {
 
@@ -89,8 +90,30 @@ int launch_row(ssp_ctx *ctx, int N, bool first, bool second, const RowArgs &a)
     SSP_DISPATCH_N(N, (launch_row_sel<NN>(ctx, first, second, a)));
 }
 
+// TMA-fed persistent column kernel (ssp_col_tma.cuh)
+template <int N>
+static int launch_col_tma_n(ssp_ctx *ctx, const ColArgs &a)
+{
+    using CFG = ColTmaCfg<N>;
+    auto kern = k_col_tma<N>;
+    CUtensorMap tm_in, tm_out;
+    if (int rc = make_tmap_c64(ctx, a.in, N, (size_t)a.B * N, CFG::C, CFG::BOX_ROWS, &tm_in)) return rc;
+    if (int rc = make_tmap_c64(ctx, a.out, N, (size_t)a.B * N, CFG::C, CFG::BOX_ROWS, &tm_out)) return rc;
+    if (int rc = set_smem(ctx, kern, CFG::SMEM)) return rc;
+    const int ntiles = a.B * (N / CFG::C);
+    const int resident = ctx->num_sms * CFG::MIN_BLOCKS;
+    ColTmaArgs ta{a.hy, a.tw, ntiles};
+    ctx->prof_begin("col_fft_h_ifft", 16.0 * (double)a.B * N * N);
+    kern<<<ntiles < resident ? ntiles : resident, CFG::THREADS, CFG::SMEM, ctx->stream>>>(tm_in, tm_out, ta);
+    ctx->prof_end();
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
 int launch_col_prop(ssp_ctx *ctx, int N, const ColArgs &a)
 {
+    if (N == 1024 && a.hy) return launch_col_tma_n<1024>(ctx, a);
     SSP_DISPATCH_N(N, (launch_col_n<NN, 0>(ctx, a)));
 }
 

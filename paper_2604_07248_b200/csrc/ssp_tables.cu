@@ -124,6 +124,34 @@ int get_sign_table(ssp_ctx *ctx, int N, const float2 **out)
     return SSP_OK;
 }
 
+typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int make_tmap_c64(ssp_ctx *ctx, const void *base, size_t cols, size_t rows, int box_cols, int box_rows,
+                  CUtensorMap *out)
+{
+    if (!ctx->encode_tiled) {
+        cudaDriverEntryPointQueryResult q;
+        void *p = nullptr;
+        SSP_CUDA(ctx, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q));
+        if (!p || q != cudaDriverEntryPointSuccess)
+            return ctx->fail(SSP_EUNSUPPORTED, "the driver does not export cuTensorMapEncodeTiled");
+        ctx->encode_tiled = p;
+    }
+    // complex64 as pairs of fp32: the inner dimension counts floats
+    const cuuint64_t dims[2] = {(cuuint64_t)cols * 2, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)cols * sizeof(float2)};
+    const cuuint32_t box[2] = {(cuuint32_t)box_cols * 2, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = reinterpret_cast<encode_tiled_fn>(ctx->encode_tiled)(
+        out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void *>(base), dims, strides, box, estr,
+        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return ctx->fail(SSP_ECUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    return SSP_OK;
+}
+
 int ensure_scratch(ssp_ctx *ctx, size_t bytes)
 {
     if (bytes <= ctx->scratch_bytes) return SSP_OK;
