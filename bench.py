@@ -31,7 +31,7 @@ UNIT = "screen-steps/s"
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config id (1-5)")
@@ -50,9 +50,24 @@ def peaks():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def ncu_traffic(kernel_class, N):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full`
+    capture (profiles/ncu_traffic.csv: class,N,bytes,source), or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as fh:
+            for line in fh:
+                p = [x.strip() for x in line.split(",")]
+                if len(p) >= 3 and p[0] == kernel_class and p[1] == str(N):
+                    return float(p[2])
+    except Exception:
+        pass
+    return None
+
+
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms; started before the warm-up so that the
+    tool is already running when the timed region starts, samples outside [t0, t1] are dropped."""
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
@@ -61,12 +76,13 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                       "--format=csv,noheader,nounits", "-lms", "50"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
 
-    def stop(self):
+    def stop(self, t0=None, t1=None):
+        import datetime
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         if self.p is None:
             return out
@@ -81,7 +97,14 @@ class ClockSampler:
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for line in self.f.read().splitlines():
             parts = [x.strip() for x in line.split(",")]
-            if len(parts) < 7:
+            if len(parts) < 8:
+                continue
+            try:
+                ts = datetime.datetime.strptime(parts[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+            except ValueError:
+                continue
+            parts = parts[1:]
+            if t0 is not None and not (t0 - 0.05 <= ts <= t1 + 0.05):
                 continue
             try:
                 sm.append(float(parts[0]))
@@ -226,12 +249,13 @@ def run_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
+    clk = ClockSampler(local) if rank == 0 else None
     for i in range(args.warmup):
         frame(i)
     sync_all()
 
     # ---- timed region: exactly K steps, CUDA events on the launching stream, per-kernel events on
-    clk = ClockSampler(local) if rank == 0 else None
+    wall0 = time.time()
     ctx.profile_enable(True)
     l0 = ctx.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -240,11 +264,12 @@ def run_ours(args):
         frame(args.warmup + i)
     e1.record()
     sync_all()
+    wall1 = time.time()
     ms_total = e0.elapsed_time(e1)
     launches = ctx.launch_count() - l0
     prof = ctx.profile_report()
     ctx.profile_enable(False)
-    clocks = clk.stop() if clk else None
+    clocks = clk.stop(wall0, wall1) if clk else None
     t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -261,11 +286,7 @@ def run_ours(args):
         d = dom[1]
         achieved = d["bytes"] / (d["ms"] * 1e-3) / 1e9
         traffic = None
-        try:
-            with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as fh:
-                traffic = json.load(fh).get(f"{dom[0]}@{N}")
-        except Exception:
-            pass
+        traffic = ncu_traffic(dom[0], N)
         roof = {"bound": "hbm", "kernel": dom[0], "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                 "us_per_launch": 1e3 * d["ms"] / d["launches"], "bytes_per_launch": d["bytes"] / d["launches"],

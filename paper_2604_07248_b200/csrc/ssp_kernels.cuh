@@ -1,6 +1,6 @@
 // ssp_kernels.cuh -- row and column kernels of the fused split step (K4-K7).
 //
-//   k_row<N,FIRST,SECOND,EXTRA>:  [IFFT_x] -> * exp(+-i phi) W [-> save plane / phase gradient]
+//   k_row<N,FIRST,SECOND,GENERIC>:  [IFFT_x] -> * exp(+-i phi) W [-> save plane / phase gradient]
 //                                 -> [FFT_x] -> * hx(next step)                  (Eq.1)
 //   k_col<N,MODE>:                FFT_y -> * hy/N^2 -> IFFT_y on a tile of C columns (register loads)
 //   k_col_tma<N>:                 the same pass with the tile moved by TMA (ssp_col_tma.cuh)
@@ -24,8 +24,12 @@ namespace ssp {
 template <bool SWAP>
 __device__ __forceinline__ float2 swap_if(float2 x) { return SWAP ? make_float2(x.y, x.x) : x; }
 
-// Pointwise stage in real space on a line held in the layout strided by RL.
-template <int N, int RL, int E, int T, bool EXTRA>
+// Pointwise stage in real space on a line held in the layout strided by RL.  SWAPPED: the registers
+// hold the field re/im-swapped (it came out of an inverse transform run by the forward code); the
+// result is in plain form either way.  GENERIC = false is the common split step (screen and window
+// both present, nothing saved): no per-element flag tests in the unrolled body.  GENERIC = true reads
+// the run-time flags: optional screen / window, saved planes, phase gradient.
+template <int N, int RL, int E, int T, bool GENERIC, bool SWAPPED>
 __device__ __forceinline__ void row_pointwise(float2 *v, const RowArgs &a, const float *phis, int t, int b, int iy)
 {
     const long long pix0 = (long long)iy * N;
@@ -37,33 +41,33 @@ __device__ __forceinline__ void row_pointwise(float2 *v, const RowArgs &a, const
 #pragma unroll
         for (int q = 0; q < RL; ++q) {
             const int off = q * (N / RL) + T * i;                 // ix = t + off, off compile-time
-            float2 u = v[i * RL + q];
-            if constexpr (EXTRA) {
+            const float2 u = swap_if<SWAPPED>(v[i * RL + q]);
+            if constexpr (GENERIC) {
                 if (a.grad) {
                     const float2 U = a.plane_in[b * a.plane_stride + pix0 + t + off];
                     a.grad[b * a.grad_stride + pix0 + t + off] = u.y * U.x - u.x * U.y; // Im(G conj(U))
                 }
             }
             float mr = 1.f, mi = 0.f;
-            if (a.phi) {
+            if (!GENERIC || a.phi) {
                 sincos_reduced(phis[t + off], &mi, &mr);
                 mi *= a.phase_sign;
             }
-            if (a.win_on) {
+            if (!GENERIC || a.win_on) {
                 const float xc = xf + (float)off;
                 const float amp = window_amp(fmaf(xc * xc, a.win_qs, y2), a.win_half_order);
                 mr *= amp;
                 mi *= amp;
             }
-            u = cmul(u, make_float2(mr, mi));
-            if constexpr (EXTRA) {
-                if (a.plane_out) a.plane_out[b * a.plane_stride + pix0 + t + off] = u;
+            const float2 r = cmul(u, make_float2(mr, mi));
+            if constexpr (GENERIC) {
+                if (a.plane_out) a.plane_out[b * a.plane_stride + pix0 + t + off] = r;
             }
-            v[i * RL + q] = u;
+            v[i * RL + q] = r;
         }
 }
 
-template <int N, bool FIRST, bool SECOND, bool EXTRA>
+template <int N, bool FIRST, bool SECOND, bool GENERIC>
 __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_row(const RowArgs a)
 {
     using PI = PlanInfo<N, 0>;
@@ -81,13 +85,13 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
 
     // the screen row is streamed from HBM: fetch it asynchronously now, use it after the first transform
     float *phis = reinterpret_cast<float *>(smem_raw + CFG::SMEM_X) + (size_t)lib * N;
-    if (a.phi) {
+    if (!GENERIC || a.phi) {
         const float *g = a.phi + b * a.phi_batch_stride + (long long)iy * N;
 #pragma unroll
         for (int i = 0; i < E / 4; ++i) cp_async16(phis + 4 * (t + T * i), g + 4 * (t + T * i));
         cp_async_commit();
     }
-    const bool pointwise = a.phi || a.win_on || (EXTRA && (a.grad || a.plane_out));
+    const bool pointwise = !GENERIC || a.phi || a.win_on || a.grad || a.plane_out;
 
     float2 v[E];
     // FIRST (an inverse transform comes first) loads re/im-swapped when the forward code runs it
@@ -100,7 +104,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
 #pragma unroll
             for (int q = 0; q < RIN; ++q) {
                 float2 x = src[line_index<N, 0, RIN>(t, i, q)];
-                if constexpr (EXTRA) {
+                if constexpr (GENERIC) {
                     if (a.pre) {
                         const float2 pl = a.pre_line ? __ldg(a.pre_line + iy) : make_float2(1.f, 0.f);
                         x = cmul(x, cmul(pl, __ldg(a.pre + line_index<N, 0, RIN>(t, i, q))));
@@ -110,7 +114,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
             }
     }
     auto wait_phi = [&]() {
-        if (a.phi) {
+        if (!GENERIC || a.phi) {
             cp_async_wait_all();
             sm.sync();
         }
@@ -126,27 +130,19 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
                 constexpr bool TAIL = (T > 32);
                 fft_line<N, 0, false, false, TAIL>(v, t, sm, a.tw);
                 if (pass == 0) {
-#pragma unroll
-                    for (int e = 0; e < E; ++e) v[e] = swap_if<true>(v[e]);
-                    if (pointwise) {
-                        wait_phi();
-                        row_pointwise<N, RL, E, T, EXTRA>(v, a, phis, t, b, iy);
-                    }
+                    wait_phi();
+                    row_pointwise<N, RL, E, T, GENERIC, true>(v, a, phis, t, b, iy);
                     if constexpr (!TAIL) sm.sync();
                 }
             }
         } else if constexpr (FIRST) {
             fft_line<N, 0, false, false>(v, t, sm, a.tw);
-#pragma unroll
-            for (int e = 0; e < E; ++e) v[e] = swap_if<true>(v[e]);
-            if (pointwise) {
-                wait_phi();
-                row_pointwise<N, RL, E, T, EXTRA>(v, a, phis, t, b, iy);
-            }
+            wait_phi();
+            row_pointwise<N, RL, E, T, GENERIC, true>(v, a, phis, t, b, iy);
         } else {
             if (pointwise) {
                 wait_phi();
-                row_pointwise<N, RL, E, T, EXTRA>(v, a, phis, t, b, iy);
+                row_pointwise<N, RL, E, T, GENERIC, false>(v, a, phis, t, b, iy);
             }
             fft_line<N, 0, false, false>(v, t, sm, a.tw);
         }
@@ -154,7 +150,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
         if constexpr (FIRST) fft_line<N, 0, false, true, SECOND>(v, t, sm, a.tw); // inverse; now strided by RL
         if (pointwise) {
             wait_phi();
-            row_pointwise<N, RL, E, T, EXTRA>(v, a, phis, t, b, iy);
+            row_pointwise<N, RL, E, T, GENERIC, false>(v, a, phis, t, b, iy);
         }
         if constexpr (SECOND) fft_line<N, 0, true, false>(v, t, sm, a.tw); // forward, reversed plan; strided by R1
     }

@@ -22,12 +22,12 @@ static int set_smem(ssp_ctx *ctx, K kernel, size_t bytes)
     return SSP_OK;
 }
 
-template <int N, bool FIRST, bool SECOND, bool EXTRA>
+template <int N, bool FIRST, bool SECOND, bool GENERIC>
 static int launch_row_x(ssp_ctx *ctx, const RowArgs &a)
 {
     using CFG = RowCfg<N>;
     if (a.n_lines % CFG::LPB) return ctx->fail(SSP_EINVAL, "row launch: %d lines not a multiple of %d", a.n_lines, CFG::LPB);
-    auto kern = k_row<N, FIRST, SECOND, EXTRA>;
+    auto kern = k_row<N, FIRST, SECOND, GENERIC>;
     if (int rc = set_smem(ctx, kern, CFG::SMEM)) return rc;
     // algorithmic bytes: field in + out, + the screen, + saved / read planes and the gradient
     const double bpp = 16.0 + (a.phi ? 4.0 : 0.0) + (a.plane_out ? 8.0 : 0.0) + (a.grad ? 12.0 : 0.0);
@@ -39,12 +39,14 @@ static int launch_row_x(ssp_ctx *ctx, const RowArgs &a)
     return SSP_OK;
 }
 
-// EXTRA = saved planes, phase gradient or the input pre-multiply are compiled in
+// the common split step (screen and window present, nothing saved, no pre-multiply) has its own
+// instantiation without run-time flag tests; everything else takes the generic one
 template <int N, bool FIRST, bool SECOND>
 static int launch_row_n(ssp_ctx *ctx, const RowArgs &a)
 {
-    if (a.grad || a.plane_out || a.pre) return launch_row_x<N, FIRST, SECOND, true>(ctx, a);
-    return launch_row_x<N, FIRST, SECOND, false>(ctx, a);
+    const bool common = a.phi && a.win_on && !a.grad && !a.plane_out && !a.pre;
+    if (common) return launch_row_x<N, FIRST, SECOND, false>(ctx, a);
+    return launch_row_x<N, FIRST, SECOND, true>(ctx, a);
 }
 
 template <int N>
