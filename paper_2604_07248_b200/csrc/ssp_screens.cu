@@ -6,14 +6,16 @@
 // (PAPER.md:359 S16; :57 Eq.2; :63 Eq.3; :80 Eq.5; :74 Eq.4.)
 #include "ssp_internal.h"
 #include "ssp_lines.cuh"
+#include "ssp_col_tma.cuh"
 
 namespace ssp {
 
 // sqrt of the frequency-dependent part of Phi^f at squared frequency f2 (cycles/m)^2.
 // The scalar part (0.023 r0^-5/3, or the oceanic constants) and df are in the per-slab amplitude.
-__device__ __forceinline__ float psd_shape_sqrt(const ScreenFilter &f, float f2)
+template <bool OCEAN>
+__device__ __forceinline__ float psd_shape_sqrt_k(const ScreenFilter &f, float f2)
 {
-    if (f.kind == SSP_PSD_OCEAN_NIKISHOV) {
+    if constexpr (OCEAN) {
         const float kap = f.two_pi * sqrtf(f2);
         const float ke = kap * f.eta;
         const float ke23 = exp2f(0.66666667f * __log2f(ke));
@@ -24,6 +26,10 @@ __device__ __forceinline__ float psd_shape_sqrt(const ScreenFilter &f, float f2)
     }
     // von Karman / Kolmogorov: exp(-f2/(2 fm^2)) (f2 + f0^2)^(-11/12)
     return exp2f(fmaf(-0.91666667f, __log2f(f2 + f.f0sq), -f2 * f.inv_fm2_log2e));
+}
+__device__ __forceinline__ float psd_shape_sqrt(const ScreenFilter &f, float f2)
+{
+    return (f.kind == SSP_PSD_OCEAN_NIKISHOV) ? psd_shape_sqrt_k<true>(f, f2) : psd_shape_sqrt_k<false>(f, f2);
 }
 
 template <int N>
@@ -92,6 +98,93 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_s
     for (int i = 0; i < E / RL; ++i)
 #pragma unroll
         for (int q = 0; q < RL; ++q) dst[(size_t)line_index<N, 1, RL>(t, i, q) * N] = v[i * RL + q];
+}
+
+// K1+K2 with the tiles moved by TMA: noise (and the old spectrum) arrive as C-column boxes in two
+// shared-memory buffers, the new spectrum leaves from the buffer the old one came in, the column
+// transform exchanges through the noise buffer and its result leaves from there.  Same arithmetic,
+// element for element, as k_screen_col; no global load or store is issued by the threads.
+template <int N, bool OCEAN, bool AR, bool TILT>
+__global__ void __launch_bounds__(ColTmaCfg<N>::THREADS, ColTmaCfg<N>::MIN_BLOCKS)
+k_screen_col_tma(const __grid_constant__ CUtensorMap tm_noise, const __grid_constant__ CUtensorMap tm_spec,
+                 const __grid_constant__ CUtensorMap tm_out, const ScreenColArgs a)
+{
+    using PI = PlanInfo<N, 1>;
+    using CFG = ColTmaCfg<N>;
+    constexpr int E = PI::E, C = CFG::C, R1 = PI::R1;
+    constexpr int GROUPS = N / C;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float2 *buf_x = reinterpret_cast<float2 *>(smem_raw);                 // noise -> exchange -> result
+    float2 *buf_s = buf_x + CFG::BUF_ELEMS;                               // old spectrum -> new spectrum
+    unsigned long long *full = reinterpret_cast<unsigned long long *>(smem_raw + 2 * sizeof(float2) * CFG::BUF_ELEMS);
+    const int tid = threadIdx.x, c = tid % C, t = tid / C;
+    const int scr = blockIdx.x / GROUPS, col0 = (blockIdx.x % GROUPS) * C, kx = col0 + c;
+    constexpr bool ar = AR;
+
+    if (tid == 0) {
+        mbar_init(full, 1);
+        fence_mbar_init();
+        mbar_expect_tx(full, ar ? 2 * CFG::TILE_BYTES : CFG::TILE_BYTES);
+#pragma unroll
+        for (int j = 0; j < CFG::BOXES; ++j)
+            tma_load_2d(buf_x + j * CFG::BOX_ROWS * C, &tm_noise, 2 * col0, scr * N + j * CFG::BOX_ROWS, full);
+        if (ar) {
+#pragma unroll
+            for (int j = 0; j < CFG::BOXES; ++j)
+                tma_load_2d(buf_s + j * CFG::BOX_ROWS * C, &tm_spec, 2 * col0, scr * N + j * CFG::BOX_ROWS, full);
+        }
+    }
+    const float amp_s = __ldg(a.amp + (a.g0 + scr) % a.S);
+    const float kxs = (float)((kx < N / 2) ? kx : kx - N);
+    const float df2 = a.flt.df * a.flt.df;
+    float2 tx = make_float2(1.f, 0.f);
+    if constexpr (TILT) tx = __ldg(a.taux + kx);
+    __syncthreads();
+    mbar_wait(full, 0);
+
+    float2 v[E];
+#pragma unroll
+    for (int i = 0; i < E / R1; ++i)
+#pragma unroll
+        for (int q = 0; q < R1; ++q) {
+            const int ky = line_index<N, 1, R1>(t, i, q);
+            const float2 nz = buf_x[ky * C + c];
+            const float kys = (float)((ky < N / 2) ? ky : ky - N);
+            const float f2 = (kxs * kxs + kys * kys) * df2;
+            const float amp = (kx == 0 && ky == 0) ? 0.f : amp_s * psd_shape_sqrt_k<OCEAN>(a.flt, f2);
+            float2 x = make_float2(nz.x * amp, nz.y * amp);
+            if constexpr (AR) { // C <- a tau C_old + sqrt(1-a^2) C_fresh
+                float2 o = buf_s[ky * C + c];
+                if constexpr (TILT) o = cmul(o, cmul(tx, __ldg(a.tauy + ky)));
+                x = make_float2(fmaf(a.ar_a, o.x, a.ar_g * x.x), fmaf(a.ar_a, o.y, a.ar_g * x.y));
+            }
+            if (a.spec_out) buf_s[ky * C + c] = x;                        // same owner as the read above
+            v[i * R1 + q] = x;
+        }
+    fence_proxy_async();
+    __syncthreads();                                                      // tiles consumed, new spectrum complete
+    if (tid == 0 && a.spec_out) {
+#pragma unroll
+        for (int j = 0; j < CFG::BOXES; ++j)
+            tma_store_2d(&tm_spec, 2 * col0, scr * N + j * CFG::BOX_ROWS, buf_s + j * CFG::BOX_ROWS * C);
+        tma_store_commit();
+    }
+    ColSmem<C> sm{buf_x + c};
+    fft_line<N, 1, false, true, true>(v, t, sm, a.tw);                    // unnormalised inverse along y
+    constexpr int RL = PI::RL;
+#pragma unroll
+    for (int i = 0; i < E / RL; ++i)
+#pragma unroll
+        for (int q = 0; q < RL; ++q) buf_x[line_index<N, 1, RL>(t, i, q) * C + c] = v[i * RL + q];
+    fence_proxy_async();
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+        for (int j = 0; j < CFG::BOXES; ++j)
+            tma_store_2d(&tm_out, 2 * col0, scr * N + j * CFG::BOX_ROWS, buf_x + j * CFG::BOX_ROWS * C);
+        tma_store_commit();
+        tma_store_wait_read();
+    }
 }
 
 template <int N>
@@ -197,6 +290,39 @@ static int launch_screen_col_n(ssp_ctx *ctx, const ScreenColArgs &a)
     return SSP_OK;
 }
 
+template <int N, bool OCEAN, bool AR, bool TILT>
+static int launch_screen_col_tma_x(ssp_ctx *ctx, const ScreenColArgs &a)
+{
+    using CFG = ColTmaCfg<N>;
+    auto kern = k_screen_col_tma<N, OCEAN, AR, TILT>;
+    const size_t rows = (size_t)a.nscr * N;
+    CUtensorMap tm_noise, tm_spec, tm_out;
+    if (int rc = make_tmap_c64(ctx, a.noise, N, rows, CFG::C, CFG::BOX_ROWS, &tm_noise)) return rc;
+    const void *spec = a.spec_out ? (const void *)a.spec_out : (const void *)a.old_spec;
+    if (int rc = make_tmap_c64(ctx, spec ? spec : (const void *)a.noise, N, rows, CFG::C, CFG::BOX_ROWS, &tm_spec)) return rc;
+    if (int rc = make_tmap_c64(ctx, a.out, N, rows, CFG::C, CFG::BOX_ROWS, &tm_out)) return rc;
+    SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::SMEM));
+    const double bpp = 16.0 + (a.old_spec ? 8.0 : 0.0) + (a.spec_out ? 8.0 : 0.0);
+    ctx->prof_begin("screen_col", bpp * (double)a.nscr * N * N);
+    kern<<<a.nscr * (N / CFG::C), CFG::THREADS, CFG::SMEM, ctx->stream>>>(tm_noise, tm_spec, tm_out, a);
+    ctx->prof_end();
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
+template <int N>
+static int launch_screen_col_tma_n(ssp_ctx *ctx, const ScreenColArgs &a)
+{
+    const bool ocean = a.flt.kind == SSP_PSD_OCEAN_NIKISHOV, ar = a.old_spec != nullptr, tilt = ar && a.taux;
+    if (ocean) {
+        if (!ar) return launch_screen_col_tma_x<N, true, false, false>(ctx, a);
+        return tilt ? launch_screen_col_tma_x<N, true, true, true>(ctx, a) : launch_screen_col_tma_x<N, true, true, false>(ctx, a);
+    }
+    if (!ar) return launch_screen_col_tma_x<N, false, false, false>(ctx, a);
+    return tilt ? launch_screen_col_tma_x<N, false, true, true>(ctx, a) : launch_screen_col_tma_x<N, false, true, false>(ctx, a);
+}
+
 template <int N>
 static int launch_screen_row_n(ssp_ctx *ctx, const ScreenRowArgs &a)
 {
@@ -229,6 +355,8 @@ static int launch_screen_row_n(ssp_ctx *ctx, const ScreenRowArgs &a)
 
 int launch_screen_col(ssp_ctx *ctx, int N, const ScreenColArgs &a)
 {
+    // the TMA kernel keeps the stored spectrum in place: an old spectrum elsewhere takes the register-load kernel
+    if (N == 1024 && (!a.old_spec || !a.spec_out || a.old_spec == a.spec_out)) return launch_screen_col_tma_n<1024>(ctx, a);
     SSP_DISPATCH_N(N, (launch_screen_col_n<NN>(ctx, a)));
 }
 int launch_screen_row(ssp_ctx *ctx, int N, const ScreenRowArgs &a)
