@@ -209,10 +209,12 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_s
         for (int q = 0; q < R1; ++q) v[i * R1 + q] = src[line_index<N, 0, R1>(t, i, q)];
     fft_line<N, 0, false, true>(v, t, sm, a.tw); // unnormalised inverse along x; strided by RL
 
-    float mean = 0.f;
+    // phi_lo(ix,iy) = sum_p Re( d_p0 conj(ex) + d_p1 + d_p2 ex ),  d_pb = c_p0b conj(ey) + c_p1b + c_p2b ey
+    //              = sum_p [ (Re d_p0 + Re d_p2) cos_p(ix) + (Im d_p0 - Im d_p2) sin_p(ix) + Re d_p1 ]:
+    // two FMAs per level and pixel; the ix-independent terms and the analytic mean go into one constant.
+    float cst = 0.f;
     if (a.n_sh > 0) {
-        // phi_lo(ix,iy) = sum_p Re( d_p0 conj(ex) + d_p1 + d_p2 ex ),  d_pb = c_p0b conj(ey) + c_p1b + c_p2b ey
-        mean = __ldg(a.sh_mean + scr);
+        cst = -__ldg(a.sh_mean + scr);
         for (int p = 0; p < a.n_sh; ++p) {
             const float2 *cf = a.sh_coef + ((size_t)scr * a.n_sh + p) * 9;
             const float2 ey = __ldg(a.ex + (size_t)p * N + iy);
@@ -223,14 +225,15 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_s
                 const float2 lo = cmul_conj(c0, ey), hi = cmul(c2, ey);
                 d[bb] = make_float2(lo.x + c1.x + hi.x, lo.y + c1.y + hi.y);
             }
+            const float ca = d[0].x + d[2].x, sa = d[0].y - d[2].y;
+            cst += d[1].x;
+            const float2 *exp_ = a.ex + (size_t)p * N + t;
 #pragma unroll
             for (int i = 0; i < E / RL; ++i)
 #pragma unroll
                 for (int q = 0; q < RL; ++q) {
-                    const float2 ex = __ldg(a.ex + (size_t)p * N + line_index<N, 0, RL>(t, i, q));
-                    // Re(d0 conj(ex)) + Re(d1) + Re(d2 ex)
-                    float r = fmaf(d[0].x, ex.x, d[0].y * ex.y) + d[1].x + fmaf(d[2].x, ex.x, -d[2].y * ex.y);
-                    v[i * RL + q].x += r;
+                    const float2 ex = __ldg(exp_ + (line_index<N, 0, RL>(t, i, q) - t));
+                    v[i * RL + q].x = fmaf(ca, ex.x, fmaf(sa, ex.y, v[i * RL + q].x));
                 }
         }
     }
@@ -238,7 +241,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_s
 #pragma unroll
     for (int i = 0; i < E / RL; ++i)
 #pragma unroll
-        for (int q = 0; q < RL; ++q) dst[line_index<N, 0, RL>(t, i, q)] = v[i * RL + q].x - mean;
+        for (int q = 0; q < RL; ++q) dst[line_index<N, 0, RL>(t, i, q)] = v[i * RL + q].x + cst;
 }
 
 // one block per screen, one thread per (p, a, b)
