@@ -1,0 +1,209 @@
+"""GPU parity on BASELINE.json configs 2-5 (slices the fp64 oracle finishes in tens of seconds; config 1
+runs in full in test_gpu_propagate.py) and on the bench launch configuration at full size.
+
+Slices (stated per test): the grid, geometry, medium, beam and batch layout are the
+config's own; what is cut is the number of realisations and, for 2048^2 / 4096^2, the number of screens.
+Bar: per-field relative L2 <= 2e-5 log2(N) screens (north_star); screens 2e-5 log2(N) each."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2604_07248_b200 import synth
+from tests.util import rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ssp():
+    import torch
+    from paper_2604_07248_b200 import api, build
+    build.build()
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    ctx = api.Context(0)
+    yield ctx
+    ctx.close()
+
+
+def cu(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def c64(a):
+    return np.ascontiguousarray(a).view(np.complex64)[..., 0]
+
+
+def tol(N, n):
+    return 2e-5 * math.log2(N) * max(1, n)
+
+
+def _psd(wl, orc):
+    from paper_2604_07248_b200 import api
+    return orc.Psd(**wl.psd_dict()), api.PsdParams(**wl.psd_dict())
+
+
+def _check_stats(st, st_ref, wl):
+    for a, b in zip(st, st_ref):
+        for k in ("power", "w2", "sxx", "syy", "roi_sumI", "roi_sumI2", "I_axis"):
+            assert abs(a[k] / b[k] - 1) < 1e-4, (k, a[k], b[k])
+        assert abs(a["cx"] - b["cx"]) < 1e-4 * wl.dx * wl.N and abs(a["cy"] - b["cy"]) < 1e-4 * wl.dx * wl.N
+        assert a["roi_n"] == b["roi_n"]
+
+
+def test_config2_scintillation_sweep_slice(ssp, orc):
+    """configs[1]: 512^2 plane wave, 10 Kolmogorov screens, Cn2 in {1e-15, 1e-14, 1e-13}; slice = 2 of the 64
+    realisations per Cn2.  Screens, received field and the ROI sums behind the scintillation index."""
+    import torch
+    from paper_2604_07248_b200 import api
+    wl = synth.CONFIGS[2]
+    N, S, B = wl.N, wl.S, 2
+    po, pg = _psd(wl, orc)
+    u0 = synth.input_field(wl, B)
+    for ic, cn2 in enumerate(wl.cn2_sweep):
+        hi, sh = synth.noise_batch(2, ic, B, S, N, 0)
+        cn2s = np.full(S, cn2)
+        scr_ref, _, _ = orc.make_screens(N, wl.dx, po, wl.lam, cn2s, wl.dz, 0, hi, sh, keep_spectrum=False)
+        scr = ssp.make_screens(N, wl.dx, pg, wl.lam, list(cn2s), list(wl.dz), 0, cu(c64(hi)))
+        assert rel_l2(scr.cpu().numpy(), scr_ref).max() < tol(N, 1)
+        scr32 = scr_ref.astype(np.float32)                    # identical fp32 screens feed both propagators
+        kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
+        ref = orc.propagate(N, wl.dx, wl.lam, wl.dz, u0, scr32, **kw)
+        stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+        out = ssp.propagate(N, wl.dx, wl.lam, list(wl.dz), cu(u0), cu(scr32), stats=stats, roi_frac=0.5, **kw)
+        err = rel_l2(out.cpu().numpy(), ref)
+        assert err.max() < tol(N, S), (cn2, err)
+        _check_stats(api.stats_to_dicts(stats), orc.beam_stats(N, wl.dx, ref, roi_frac=0.5), wl)
+
+
+def test_config3_temporal_slice(ssp, orc):
+    """configs[2]: 1024^2, 20 von Karman screens + 3 subharmonic levels, AR a = 0.99, Gaussian beam; slice = 1 of
+    the 32 stacks, 2 of the 100 time steps.  Per frame: evolved screens, received field, beam width."""
+    import torch
+    from paper_2604_07248_b200 import api
+    wl = synth.CONFIGS[3]
+    N, S, B = wl.N, wl.S, 1
+    po, pg = _psd(wl, orc)
+    frames = synth.noise(3, 0, 0, S, N, wl.n_sh, frames=3)
+    hi0, sh0 = frames[0]
+    _, spec_ref, shc_ref = orc.make_screens(N, wl.dx, po, wl.lam, wl.cn2_list, wl.dz, wl.n_sh, hi0[None], sh0[None])
+    spec = torch.empty((B, S, N, N), dtype=torch.complex64, device="cuda")
+    shc = torch.zeros((B, S, wl.n_sh, 3, 3), dtype=torch.complex64, device="cuda")
+    ssp.make_screens(N, wl.dx, pg, wl.lam, list(wl.cn2_list), list(wl.dz), wl.n_sh, cu(c64(hi0[None])), cu(c64(sh0[None])),
+                     spectrum=spec, sh_coef=shc)
+    u0 = synth.input_field(wl, B)
+    kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
+    for t in (1, 2):
+        hi, sh = frames[t]
+        scr_ref = orc.evolve_screens(N, wl.dx, po, wl.lam, wl.cn2_list, wl.dz, wl.n_sh, wl.ar_a, 0, 0, 0, hi[None], sh[None],
+                                     spec_ref, shc_ref)
+        scr = ssp.evolve_screens(N, wl.dx, pg, wl.lam, list(wl.cn2_list), list(wl.dz), wl.n_sh, wl.ar_a, 0, 0, 0,
+                                 cu(c64(hi[None])), cu(c64(sh[None])), spec, shc)
+        err = rel_l2(scr.cpu().numpy(), scr_ref)
+        assert err.max() < tol(N, t + 1), (t, err)
+    scr32 = scr_ref.astype(np.float32)
+    ref = orc.propagate(N, wl.dx, wl.lam, wl.dz, u0, scr32, **kw)
+    stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+    out = ssp.propagate(N, wl.dx, wl.lam, list(wl.dz), cu(u0), cu(scr32), stats=stats, roi_frac=0.25, **kw)
+    assert rel_l2(out.cpu().numpy(), ref).max() < tol(N, S)
+    _check_stats(api.stats_to_dicts(stats), orc.beam_stats(N, wl.dx, ref, roi_frac=0.25), wl)
+
+
+def test_config4_forward_adjoint_masks_slice(ssp, orc):
+    """configs[3]: 2048^2, Kolmogorov Cn2 = 1e-13 screens at dz = L/30, Gaussian beam, two uniform-random phase
+    masks (receiver pupil, Fourier plane of a 2f system), Gaussian-overlap loss and its gradients w.r.t. both
+    masks and every screen via the adjoint split step.  Slice = 1 of 8 fields, the first 3 of the 30 screens."""
+    from tests import o9
+    wl = synth.CONFIGS[4]
+    N, S, B = wl.N, 3, 1
+    po, pg = _psd(wl, orc)
+    dz, cn2 = wl.dz[:S], wl.cn2_list[:S]
+    hi, sh = synth.noise_batch(4, 0, B, S, N, 0)
+    scr_ref, _, _ = orc.make_screens(N, wl.dx, po, wl.lam, cn2, dz, 0, hi, sh, keep_spectrum=False)
+    scr = ssp.make_screens(N, wl.dx, pg, wl.lam, list(cn2), list(dz), 0, cu(c64(hi)))
+    assert rel_l2(scr.cpu().numpy(), scr_ref).max() < tol(N, 1)
+    scr32 = scr_ref.astype(np.float32)
+    th = synth.phase_masks(0, N, 2)
+    u0 = synth.input_field(wl, B)
+    kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
+    ref = o9.oracle_chain(orc, N, wl.dx, wl.lam, dz, u0, scr32, th[0], th[1], kw)
+    got = o9.gpu_chain(ssp, N, wl.dx, wl.lam, dz, u0, scr32, th[0], th[1], kw)
+    assert rel_l2(got["V5"].cpu().numpy(), ref["V5"]).max() < tol(N, S + 2)
+    assert abs(got["loss"][0] - ref["loss"][0]) < 1e-4 * max(ref["loss"][0], 1e-3), (got["loss"], ref["loss"])
+    assert rel_l2(got["G0"].cpu().numpy(), ref["G0"]).max() < tol(N, 2 * S + 4)
+    for k in ("g_th1", "g_th2"):
+        assert rel_l2(got[k].cpu().numpy(), ref[k]).max() < tol(N, 2 * S + 4), k
+    gerr = rel_l2(got["g_phi"].cpu().numpy(), ref["g_phi"])
+    assert gerr.max() < tol(N, 2 * S + 4), gerr
+
+
+def test_config5_ocean_slice(ssp, orc):
+    """configs[4]: 4096^2, Nikishov oceanic spectrum with 4 subharmonic levels, Gaussian beam w0 = 5 mm,
+    dz = L/20; slice = 1 of 2 fields, the first 2 of the 20 screens.  Screens, received field, beam statistics."""
+    import torch
+    from paper_2604_07248_b200 import api
+    wl = synth.CONFIGS[5]
+    N, S, B = wl.N, 2, 1
+    po, pg = _psd(wl, orc)
+    dz, cn2 = wl.dz[:S], wl.cn2_list[:S]
+    hi, sh = synth.noise_batch(5, 0, B, S, N, wl.n_sh)
+    scr_ref, _, _ = orc.make_screens(N, wl.dx, po, wl.lam, cn2, dz, wl.n_sh, hi, sh, keep_spectrum=False)
+    scr = ssp.make_screens(N, wl.dx, pg, wl.lam, list(cn2), list(dz), wl.n_sh, cu(c64(hi)), cu(c64(sh)))
+    assert rel_l2(scr.cpu().numpy(), scr_ref).max() < tol(N, 1)
+    scr32 = scr_ref.astype(np.float32)
+    u0 = synth.input_field(wl, B)
+    kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
+    ref = orc.propagate(N, wl.dx, wl.lam, dz, u0, scr32, **kw)
+    stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+    out = ssp.propagate(N, wl.dx, wl.lam, list(dz), cu(u0), cu(scr32), stats=stats, roi_frac=0.25, **kw)
+    assert rel_l2(out.cpu().numpy(), ref).max() < tol(N, S)
+    _check_stats(api.stats_to_dicts(stats), orc.beam_stats(N, wl.dx, ref, roi_frac=0.25), wl)
+
+
+def test_bench_launch_configuration_full_size(ssp, orc):
+    """The launch configuration bench.py times (config 3 in full: 1024^2, B = 32 stacks of 20 screens, one AR
+    frame): realisation 17 of the batch is checked against the oracle run on that realisation alone (screens,
+    received field, adjoint field); properties that hold at any size cover the rest of the batch."""
+    import torch
+    from paper_2604_07248_b200 import api
+    wl = synth.CONFIGS[3]
+    N, S, B, b_s = wl.N, wl.S, wl.B, 17
+    po, pg = _psd(wl, orc)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(7)
+    noise = [torch.view_as_complex(torch.randn(B, S, N, N, 2, device="cuda", generator=gen)) for _ in range(2)]
+    noise_sh = [torch.view_as_complex(torch.randn(B, S, wl.n_sh, 3, 3, 2, device="cuda", generator=gen)) for _ in range(2)]
+    spec = torch.empty((B, S, N, N), dtype=torch.complex64, device="cuda")
+    shc = torch.zeros((B, S, wl.n_sh, 3, 3), dtype=torch.complex64, device="cuda")
+    cn2, dz = list(wl.cn2_list), list(wl.dz)
+    ssp.make_screens(N, wl.dx, pg, wl.lam, cn2, dz, wl.n_sh, noise[0], noise_sh[0], spectrum=spec, sh_coef=shc)
+    scr = ssp.evolve_screens(N, wl.dx, pg, wl.lam, cn2, dz, wl.n_sh, wl.ar_a, 0, 0, 0, noise[1], noise_sh[1], spec, shc)
+    # the oracle consumes the same white noise (as drawn on the device, copied back) for realisation b_s
+    f2 = lambda t: np.ascontiguousarray(torch.view_as_real(t[b_s:b_s + 1]).cpu().numpy())
+    _, spec_ref, shc_ref = orc.make_screens(N, wl.dx, po, wl.lam, wl.cn2_list, wl.dz, wl.n_sh, f2(noise[0]), f2(noise_sh[0]))
+    scr_ref = orc.evolve_screens(N, wl.dx, po, wl.lam, wl.cn2_list, wl.dz, wl.n_sh, wl.ar_a, 0, 0, 0, f2(noise[1]),
+                                 f2(noise_sh[1]), spec_ref, shc_ref)
+    assert rel_l2(scr[b_s:b_s + 1].cpu().numpy(), scr_ref).max() < tol(N, 2)
+    u0 = synth.input_field(wl, B)
+    kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
+    stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+    out = ssp.propagate(N, wl.dx, wl.lam, dz, cu(u0), scr, stats=stats, roi_frac=0.25, **kw)
+    gin = ssp.propagate_adjoint(N, wl.dx, wl.lam, dz, out, scr, **kw)
+    scr32 = scr[b_s:b_s + 1].cpu().numpy()                    # the GPU's own fp32 screens of that realisation
+    ref = orc.propagate(N, wl.dx, wl.lam, wl.dz, u0[b_s:b_s + 1], scr32, **kw)
+    assert rel_l2(out[b_s:b_s + 1].cpu().numpy(), ref).max() < tol(N, S)
+    gref = orc.propagate_adjoint(N, wl.dx, wl.lam, wl.dz, out[b_s:b_s + 1].cpu().numpy(), scr32, **kw)
+    assert rel_l2(gin[b_s:b_s + 1].cpu().numpy(), gref).max() < tol(N, S)
+    _check_stats(api.stats_to_dicts(stats)[b_s:b_s + 1], orc.beam_stats(N, wl.dx, ref, roi_frac=0.25), wl)
+    # any size: <A x, y> = <x, A^H y> per realisation with y = A x, and power never grows (|H| = 1, |W| <= 1)
+    ip1 = ssp.inner_products(N, wl.dx, out, out).cpu().numpy()          # <Ax, Ax>
+    ip2 = ssp.inner_products(N, wl.dx, gin, cu(u0)).cpu().numpy()       # <A^H A x, x>
+    p0 = ssp.inner_products(N, wl.dx, cu(u0), cu(u0)).cpu().numpy()[:, 2]
+    for b in range(B):
+        assert abs(ip1[b, 0] - ip2[b, 0]) < 2e-6 * S * ip1[b, 0], (b, ip1[b], ip2[b])
+        assert abs(ip2[b, 1]) < 2e-6 * S * ip1[b, 0]
+        assert ip1[b, 2] <= p0[b] * (1 + 1e-5)
+    # distinct noise per realisation gives distinct fields; all finite
+    assert torch.isfinite(torch.view_as_real(out)).all()
+    assert not torch.equal(out[0], out[1])

@@ -1,0 +1,42 @@
+"""Pin of the config-4 mask-system composition (tests/o9.py, O9) on the CPU oracle: every gradient
+the chain returns equals a central finite difference of the loss (P8 extended to the whole system)."""
+import numpy as np
+
+from paper_2604_07248_b200 import synth
+from tests import o9
+
+
+def _loss(orc, N, dx, lam, dz, u0, scr, th1, th2, kw):
+    V1 = orc.propagate(N, dx, lam, dz, u0, scr, **kw)
+    T = orc.propagate(N, dx, lam, dz, u0, None, **kw)
+    V5 = orc.dft2_centered(N, orc.phase_mul(N, th2, orc.dft2_centered(N, orc.phase_mul(N, th1, V1))), inverse=True)
+    c = np.vdot(T[0], V5[0])
+    return 1.0 - abs(c) ** 2 / (np.vdot(T[0], T[0]).real * np.vdot(V5[0], V5[0]).real)
+
+
+def test_o9_gradients_match_finite_differences(orc):
+    N, dx, lam = 16, 1e-3, 1e-6
+    dz = np.array([3.0, 5.0, 4.0])
+    kw = dict(win_order=8, win_sigma_frac=0.45)
+    u0 = synth.gaussian_beam(N, dx, 4e-3, 1).astype(np.complex128)
+    scr = synth.random_screens(N, 1, 3, 5, rms=1.0).astype(np.float64)
+    th = synth.phase_masks(0, N, 2).astype(np.float64)
+    r = o9.oracle_chain(orc, N, dx, lam, dz, u0, scr, th[0], th[1], kw)
+    assert 0.0 < r["loss"][0] < 1.0
+    rng = np.random.default_rng(0)
+    h = 1e-6
+    for what in ("th1", "th2", "phi0", "phi2"):
+        for _ in range(4):
+            iy, ix = rng.integers(2, N - 2, 2)
+            t1p, t1m, t2p, t2m, sp, sm_ = th[0].copy(), th[0].copy(), th[1].copy(), th[1].copy(), scr.copy(), scr.copy()
+            if what == "th1":
+                t1p[iy, ix] += h; t1m[iy, ix] -= h; g = r["g_th1"][0, iy, ix]
+            elif what == "th2":
+                t2p[iy, ix] += h; t2m[iy, ix] -= h; g = r["g_th2"][0, iy, ix]
+            else:
+                s = int(what[-1])
+                sp[0, s, iy, ix] += h; sm_[0, s, iy, ix] -= h; g = r["g_phi"][0, s, iy, ix]
+            fd = (_loss(orc, N, dx, lam, dz, u0, sp, t1p, t2p, kw) - _loss(orc, N, dx, lam, dz, u0, sm_, t1m, t2m, kw)) / (2 * h)
+            assert abs(fd - g) < 1e-6 * max(1e-3, abs(g)) + 1e-9, (what, iy, ix, fd, g)
+    # mask 1 and the last screen share a plane: their gradients are the same map
+    np.testing.assert_allclose(r["g_th1"][0], r["g_phi"][0, 2], rtol=1e-9, atol=1e-14)
