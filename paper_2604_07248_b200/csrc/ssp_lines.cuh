@@ -9,7 +9,7 @@ namespace ssp {
 // ---- CTA shapes --------------------------------------------------------------------
 // Row-kernel CTA size and resident CTAs per SM the register budget is sized for.  Default: 256
 // threads, 512 resident threads at E = 32 and 1024 at E = 16.  N = 1024 (one warp per row, 32 points
-// per thread) measured best on B200 with 168 registers: 3 CTAs of 4 rows (profiles/r01_notes.md).
+// per thread) measured best on B200 with 168 registers: 3 CTAs of 4 rows.
 template <int N>
 struct RowTune {
     static constexpr int MAX_THREADS = 256;
