@@ -123,9 +123,9 @@ int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
     const double df = 1.0 / (N * grid.dx);
     const WsLayout L = ws_layout(N, B, S);
     char *ws = reinterpret_cast<char *>(d_ws);
-    const float2 *tw = nullptr, *twc = nullptr;          // row-plan and column-plan twiddles
+    const float2 *tw = nullptr, *twc = nullptr;          // row-plan and screen-column-plan twiddles
     if (int rc = get_twiddles(ctx, N, 0, &tw)) return rc;
-    if (int rc = get_twiddles(ctx, N, 1, &twc)) return rc;
+    if (int rc = get_twiddles(ctx, N, screen_col_plan_variant(N), &twc)) return rc;
     cudaStream_t st = ctx->stream;
 
     // ---- per-slab scalars and 1-D tables (double on the host, fp32 on the device)

@@ -48,16 +48,47 @@ __device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk
 __device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 
 // ---- CTA shape ---------------------------------------------------------------------------------
+// C columns per tile (TMA rows of 8 C bytes, at least 16), NBUF shared-memory buffers per CTA (2: persistent
+// CTAs, the load of the next tile overlaps the transform; 1: one tile per CTA), resident CTAs per SM.
+template <int N>
+struct ColTmaTune { static constexpr int C = 4, NBUF = 2, MIN_BLOCKS = 3; static constexpr bool ENABLED = false; };
+template <> struct ColTmaTune<512> { static constexpr int C = 8, NBUF = 2, MIN_BLOCKS = 3; static constexpr bool ENABLED = true; };
+template <> struct ColTmaTune<1024> { static constexpr int C = 4, NBUF = 2, MIN_BLOCKS = 3; static constexpr bool ENABLED = true; };
+template <> struct ColTmaTune<2048> { static constexpr int C = 4, NBUF = 1, MIN_BLOCKS = 2; static constexpr bool ENABLED = true; };
+template <> struct ColTmaTune<4096> { static constexpr int C = 2, NBUF = 1, MIN_BLOCKS = 2; static constexpr bool ENABLED = true; };
+
 template <int N>
 struct ColTmaCfg {
     static constexpr int T = PlanInfo<N, 1>::T;
-    static constexpr int C = 4;                                       // 32-byte row segments per box
+    static constexpr int C = ColTmaTune<N>::C;
+    static constexpr int NBUF = ColTmaTune<N>::NBUF;
     static constexpr int THREADS = T * C;
-    static constexpr int MIN_BLOCKS = 3;
+    static constexpr int MIN_BLOCKS = ColTmaTune<N>::MIN_BLOCKS;
     static constexpr int BOX_ROWS = (N < 256) ? N : 256;              // TMA box dimensions are <= 256
     static constexpr int BOXES = N / BOX_ROWS;
     static constexpr int BUF_ELEMS = C * PlanInfo<N, 1>::LINE_ELEMS;  // float2 per buffer (padded exchange)
-    static constexpr size_t SMEM = 2 * sizeof(float2) * BUF_ELEMS + 16;
+    static constexpr size_t SMEM = NBUF * sizeof(float2) * BUF_ELEMS + 16;
+    static constexpr unsigned TILE_BYTES = (unsigned)(sizeof(float2) * C * N);
+};
+
+// Screen generator (K1+K2): one tile per CTA, one buffer (noise -> exchange -> result) plus a second one only
+// when a spectrum is read or kept (old spectrum -> new spectrum).
+template <int N>
+struct ScreenColTmaTune { static constexpr int C = 4, MIN_BLOCKS = 3; static constexpr bool ENABLED = false; };
+template <> struct ScreenColTmaTune<512> { static constexpr int C = 8, MIN_BLOCKS = 3; static constexpr bool ENABLED = true; };
+template <> struct ScreenColTmaTune<1024> { static constexpr int C = 4, MIN_BLOCKS = 3; static constexpr bool ENABLED = true; };
+
+template <int N>
+struct ScreenColTmaCfg {
+    static constexpr int T = PlanInfo<N, 1>::T;
+    static constexpr int C = ScreenColTmaTune<N>::C;
+    static constexpr int THREADS = T * C;
+    static constexpr int MIN_BLOCKS = ScreenColTmaTune<N>::MIN_BLOCKS;
+    static constexpr int BOX_ROWS = (N < 256) ? N : 256;
+    static constexpr int BOXES = N / BOX_ROWS;
+    static constexpr int BUF_ELEMS = C * PlanInfo<N, 1>::LINE_ELEMS;
+    static constexpr size_t HEAD = 128;                               // mbarrier, keeps the buffers 128-byte aligned
+    static constexpr size_t smem(int nbuf) { return HEAD + (size_t)nbuf * sizeof(float2) * BUF_ELEMS; }
     static constexpr unsigned TILE_BYTES = (unsigned)(sizeof(float2) * C * N);
 };
 
@@ -79,7 +110,7 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
     constexpr int GROUPS = N / C;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *sbuf = reinterpret_cast<float2 *>(smem_raw);
-    unsigned long long *full = reinterpret_cast<unsigned long long *>(smem_raw + 2 * sizeof(float2) * CFG::BUF_ELEMS);
+    unsigned long long *full = reinterpret_cast<unsigned long long *>(smem_raw + CFG::NBUF * sizeof(float2) * CFG::BUF_ELEMS);
     const int tid = threadIdx.x, c = tid % C, t = tid / C;
 
     auto issue_load = [&](int tile, int buf) {
@@ -100,17 +131,17 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
 
     int it = 0;
     for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x, ++it) {
-        const int cur = it & 1;
+        const int cur = (CFG::NBUF == 2) ? (it & 1) : 0;          // NBUF == 1: one tile per CTA (grid = tiles)
         float2 *tile_s = sbuf + cur * CFG::BUF_ELEMS;
         ColSmem<C> sm{tile_s + c};
-        mbar_wait(&full[cur], (it >> 1) & 1);
+        mbar_wait(&full[cur], (CFG::NBUF == 2) ? ((it >> 1) & 1) : (it & 1));
         float2 v[E];
 #pragma unroll
         for (int i = 0; i < E / R1; ++i)
 #pragma unroll
             for (int q = 0; q < R1; ++q) v[i * R1 + q] = tile_s[line_index<N, 1, R1>(t, i, q) * C + c];
         __syncthreads();                                          // the tile is in registers: the buffer is free
-        if (tid == 0 && tile + (int)gridDim.x < a.ntiles) {
+        if (CFG::NBUF == 2 && tid == 0 && tile + (int)gridDim.x < a.ntiles) {
             tma_store_wait_read();                                // the store of tile it-1 has released the other buffer
             issue_load(tile + gridDim.x, cur ^ 1);
         }

@@ -174,6 +174,7 @@ struct ScreenRowArgs {
     const float2 *tw;
 };
 int launch_screen_col(ssp_ctx *ctx, int N, const ScreenColArgs &a);
+int screen_col_plan_variant(int N);   // plan variant (ssp_fft.cuh) whose twiddles launch_screen_col expects in a.tw
 int launch_screen_row(ssp_ctx *ctx, int N, const ScreenRowArgs &a);
 // subharmonic coefficient update + analytic mean, one block per screen
 int launch_sh_prep(ssp_ctx *ctx, int nscr, int S, int n_sh, const float2 *noise_sh,

@@ -20,6 +20,10 @@ struct RowTune<1024> {
     static constexpr int MAX_THREADS = 128;
     static constexpr int MIN_BLOCKS = 3;
 };
+template <>
+struct RowTune<2048> : RowTune<1024> {};
+template <>
+struct RowTune<4096> : RowTune<1024> {};
 
 template <int N>
 struct RowCfg {
@@ -35,16 +39,16 @@ struct RowCfg {
     static constexpr int MIN_BLOCKS = (THREADS < RowTune<N>::MAX_THREADS) ? 1 : RowTune<N>::MIN_BLOCKS;
 };
 
-template <int N>
+template <int N, int V_ = 1>
 struct ColCfg {
-    static constexpr int V = 1;                                   // plan variant
-    static constexpr int T = PlanInfo<N, 1>::T;
+    static constexpr int V = V_;                                  // plan variant
+    static constexpr int T = PlanInfo<N, V_>::T;
     // columns per CTA: 16 columns = 128-byte row segments while the tile fits one SM's
     // shared memory next to a second CTA; wider grids trade segment width for tile height.
     static constexpr int C = (N <= 8) ? 8 : (N <= 512 ? 16 : (N <= 2048 ? 8 : 4));
     static constexpr int THREADS = T * C;
-    static constexpr size_t SMEM = (PlanInfo<N, 1>::NSTAGE == 1) ? 0
-        : sizeof(float2) * (size_t)C * PlanInfo<N, 1>::LINE_ELEMS;
+    static constexpr size_t SMEM = (PlanInfo<N, V_>::NSTAGE == 1) ? 0
+        : sizeof(float2) * (size_t)C * PlanInfo<N, V_>::LINE_ELEMS;
     static constexpr int MIN_BLOCKS = (THREADS <= 256) ? 2 : 1;
 };
 

@@ -104,9 +104,11 @@ static int launch_col_tma_n(ssp_ctx *ctx, const ColArgs &a)
     if (int rc = set_smem(ctx, kern, CFG::SMEM)) return rc;
     const int ntiles = a.B * (N / CFG::C);
     const int resident = ctx->num_sms * CFG::MIN_BLOCKS;
+    // two buffers: persistent CTAs walk the tiles; one buffer: one tile per CTA
+    const int grid = (CFG::NBUF == 2 && ntiles > resident) ? resident : ntiles;
     ColTmaArgs ta{a.hy, a.tw, ntiles};
     ctx->prof_begin("col_fft_h_ifft", 16.0 * (double)a.B * N * N);
-    kern<<<ntiles < resident ? ntiles : resident, CFG::THREADS, CFG::SMEM, ctx->stream>>>(tm_in, tm_out, ta);
+    kern<<<grid, CFG::THREADS, CFG::SMEM, ctx->stream>>>(tm_in, tm_out, ta);
     ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
@@ -115,7 +117,12 @@ static int launch_col_tma_n(ssp_ctx *ctx, const ColArgs &a)
 
 int launch_col_prop(ssp_ctx *ctx, int N, const ColArgs &a)
 {
-    if (N == 1024 && a.hy) return launch_col_tma_n<1024>(ctx, a);
+    if (a.hy) {
+        if (N == 512) return launch_col_tma_n<512>(ctx, a);
+        if (N == 1024) return launch_col_tma_n<1024>(ctx, a);
+        if (N == 2048) return launch_col_tma_n<2048>(ctx, a);
+        if (N == 4096) return launch_col_tma_n<4096>(ctx, a);
+    }
     SSP_DISPATCH_N(N, (launch_col_n<NN, 0>(ctx, a)));
 }
 

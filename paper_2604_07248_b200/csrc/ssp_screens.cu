@@ -33,10 +33,10 @@ __device__ __forceinline__ float psd_shape_sqrt(const ScreenFilter &f, float f2)
 }
 
 template <int N>
-__global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_screen_col(const ScreenColArgs a)
+__global__ void __launch_bounds__(ColCfg<N, 2>::THREADS, ColCfg<N, 2>::MIN_BLOCKS) k_screen_col(const ScreenColArgs a)
 {
-    using PI = PlanInfo<N, 1>;
-    using CFG = ColCfg<N>;
+    using PI = PlanInfo<N, 2>;
+    using CFG = ColCfg<N, 2>;
     constexpr int E = PI::E, T = PI::T, C = CFG::C, R1 = PI::R1, RL = PI::RL;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *smem = reinterpret_cast<float2 *>(smem_raw);
@@ -59,12 +59,12 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_s
 #pragma unroll
     for (int i = 0; i < E / R1; ++i)
 #pragma unroll
-        for (int q = 0; q < R1; ++q) v[i * R1 + q] = __ldg(a.noise + base + (size_t)line_index<N, 1, R1>(t, i, q) * N);
+        for (int q = 0; q < R1; ++q) v[i * R1 + q] = __ldg(a.noise + base + (size_t)line_index<N, 2, R1>(t, i, q) * N);
 #pragma unroll
     for (int i = 0; i < E / R1; ++i)
 #pragma unroll
         for (int q = 0; q < R1; ++q) {
-            const int ky = line_index<N, 1, R1>(t, i, q);
+            const int ky = line_index<N, 2, R1>(t, i, q);
             const float kys = (float)((ky < N / 2) ? ky : ky - N);
             const float f2 = (kxs * kxs + kys * kys) * df2;
             const float amp = (kx == 0 && ky == 0) ? 0.f : amp_s * psd_shape_sqrt(a.flt, f2);
@@ -77,11 +77,11 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_s
             float2 old[G];
 #pragma unroll
             for (int e = 0; e < G; ++e)
-                old[e] = a.old_spec[base + (size_t)line_index<N, 1, R1>(t, (e0 + e) / R1, (e0 + e) % R1) * N];
+                old[e] = a.old_spec[base + (size_t)line_index<N, 2, R1>(t, (e0 + e) / R1, (e0 + e) % R1) * N];
 #pragma unroll
             for (int e = 0; e < G; ++e) {
                 float2 o = old[e];
-                if (a.taux) o = cmul(o, cmul(tx, __ldg(a.tauy + line_index<N, 1, R1>(t, (e0 + e) / R1, (e0 + e) % R1))));
+                if (a.taux) o = cmul(o, cmul(tx, __ldg(a.tauy + line_index<N, 2, R1>(t, (e0 + e) / R1, (e0 + e) % R1))));
                 v[e0 + e] = make_float2(fmaf(a.ar_a, o.x, a.ar_g * v[e0 + e].x), fmaf(a.ar_a, o.y, a.ar_g * v[e0 + e].y));
             }
         }
@@ -90,14 +90,14 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_s
 #pragma unroll
         for (int i = 0; i < E / R1; ++i)
 #pragma unroll
-            for (int q = 0; q < R1; ++q) a.spec_out[base + (size_t)line_index<N, 1, R1>(t, i, q) * N] = v[i * R1 + q];
+            for (int q = 0; q < R1; ++q) a.spec_out[base + (size_t)line_index<N, 2, R1>(t, i, q) * N] = v[i * R1 + q];
     }
-    fft_line<N, 1, false, true>(v, t, sm, a.tw); // unnormalised inverse along y
+    fft_line<N, 2, false, true>(v, t, sm, a.tw); // unnormalised inverse along y
     float2 *dst = a.out + base;
 #pragma unroll
     for (int i = 0; i < E / RL; ++i)
 #pragma unroll
-        for (int q = 0; q < RL; ++q) dst[(size_t)line_index<N, 1, RL>(t, i, q) * N] = v[i * RL + q];
+        for (int q = 0; q < RL; ++q) dst[(size_t)line_index<N, 2, RL>(t, i, q) * N] = v[i * RL + q];
 }
 
 // K1+K2 with the tiles moved by TMA: noise (and the old spectrum) arrive as C-column boxes in two
@@ -105,18 +105,18 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_s
 // transform exchanges through the noise buffer and its result leaves from there.  Same arithmetic,
 // element for element, as k_screen_col; no global load or store is issued by the threads.
 template <int N, bool OCEAN, bool AR, bool TILT>
-__global__ void __launch_bounds__(ColTmaCfg<N>::THREADS, ColTmaCfg<N>::MIN_BLOCKS)
+__global__ void __launch_bounds__(ScreenColTmaCfg<N>::THREADS, ScreenColTmaCfg<N>::MIN_BLOCKS)
 k_screen_col_tma(const __grid_constant__ CUtensorMap tm_noise, const __grid_constant__ CUtensorMap tm_spec,
                  const __grid_constant__ CUtensorMap tm_out, const ScreenColArgs a)
 {
     using PI = PlanInfo<N, 1>;
-    using CFG = ColTmaCfg<N>;
+    using CFG = ScreenColTmaCfg<N>;
     constexpr int E = PI::E, C = CFG::C, R1 = PI::R1;
     constexpr int GROUPS = N / C;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float2 *buf_x = reinterpret_cast<float2 *>(smem_raw);                 // noise -> exchange -> result
-    float2 *buf_s = buf_x + CFG::BUF_ELEMS;                               // old spectrum -> new spectrum
-    unsigned long long *full = reinterpret_cast<unsigned long long *>(smem_raw + 2 * sizeof(float2) * CFG::BUF_ELEMS);
+    unsigned long long *full = reinterpret_cast<unsigned long long *>(smem_raw);
+    float2 *buf_x = reinterpret_cast<float2 *>(smem_raw + CFG::HEAD);     // noise -> exchange -> result
+    float2 *buf_s = buf_x + CFG::BUF_ELEMS;                               // old -> new spectrum (present iff used)
     const int tid = threadIdx.x, c = tid % C, t = tid / C;
     const int scr = blockIdx.x / GROUPS, col0 = (blockIdx.x % GROUPS) * C, kx = col0 + c;
     constexpr bool ar = AR;
@@ -280,7 +280,7 @@ __global__ void __launch_bounds__(96) k_sh_prep(int S, int n_sh, const float2 *_
 template <int N>
 static int launch_screen_col_n(ssp_ctx *ctx, const ScreenColArgs &a)
 {
-    using CFG = ColCfg<N>;
+    using CFG = ColCfg<N, 2>;
     auto kern = k_screen_col<N>;
     if (CFG::SMEM > 48 * 1024)
         SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::SMEM));
@@ -296,18 +296,19 @@ static int launch_screen_col_n(ssp_ctx *ctx, const ScreenColArgs &a)
 template <int N, bool OCEAN, bool AR, bool TILT>
 static int launch_screen_col_tma_x(ssp_ctx *ctx, const ScreenColArgs &a)
 {
-    using CFG = ColTmaCfg<N>;
+    using CFG = ScreenColTmaCfg<N>;
     auto kern = k_screen_col_tma<N, OCEAN, AR, TILT>;
+    const size_t smem = CFG::smem((a.old_spec || a.spec_out) ? 2 : 1);
     const size_t rows = (size_t)a.nscr * N;
     CUtensorMap tm_noise, tm_spec, tm_out;
     if (int rc = make_tmap_c64(ctx, a.noise, N, rows, CFG::C, CFG::BOX_ROWS, &tm_noise)) return rc;
     const void *spec = a.spec_out ? (const void *)a.spec_out : (const void *)a.old_spec;
     if (int rc = make_tmap_c64(ctx, spec ? spec : (const void *)a.noise, N, rows, CFG::C, CFG::BOX_ROWS, &tm_spec)) return rc;
     if (int rc = make_tmap_c64(ctx, a.out, N, rows, CFG::C, CFG::BOX_ROWS, &tm_out)) return rc;
-    SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::SMEM));
+    SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::smem(2)));
     const double bpp = 16.0 + (a.old_spec ? 8.0 : 0.0) + (a.spec_out ? 8.0 : 0.0);
     ctx->prof_begin("screen_col", bpp * (double)a.nscr * N * N);
-    kern<<<a.nscr * (N / CFG::C), CFG::THREADS, CFG::SMEM, ctx->stream>>>(tm_noise, tm_spec, tm_out, a);
+    kern<<<a.nscr * (N / CFG::C), CFG::THREADS, smem, ctx->stream>>>(tm_noise, tm_spec, tm_out, a);
     ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
@@ -356,10 +357,16 @@ static int launch_screen_row_n(ssp_ctx *ctx, const ScreenRowArgs &a)
     default: return ctx->fail(SSP_EINVAL, "unsupported N=%d", N_); \
     }
 
+// the TMA generator runs the column plan (V = 1), the register-load one its own (V = 2); they differ at N >= 2048
+int screen_col_plan_variant(int N) { return (N == 512 || N == 1024) ? 1 : 2; }
+
 int launch_screen_col(ssp_ctx *ctx, int N, const ScreenColArgs &a)
 {
     // the TMA kernel keeps the stored spectrum in place: an old spectrum elsewhere takes the register-load kernel
-    if (N == 1024 && (!a.old_spec || !a.spec_out || a.old_spec == a.spec_out)) return launch_screen_col_tma_n<1024>(ctx, a);
+    if (!a.old_spec || !a.spec_out || a.old_spec == a.spec_out) {
+        if (N == 512) return launch_screen_col_tma_n<512>(ctx, a);
+        if (N == 1024) return launch_screen_col_tma_n<1024>(ctx, a);
+    }
     SSP_DISPATCH_N(N, (launch_screen_col_n<NN>(ctx, a)));
 }
 int launch_screen_row(ssp_ctx *ctx, int N, const ScreenRowArgs &a)

@@ -52,21 +52,21 @@ static void fill_twiddles(std::vector<float2> &h)
 
 int get_twiddles(ssp_ctx *ctx, int N, int V, const float2 **out)
 {
-    const int key = 2 * N + (V ? 1 : 0);
+    const int key = 4 * N + V;
     auto it = ctx->twiddles.find(key);
     if (it != ctx->twiddles.end()) { *out = it->second; return SSP_OK; }
     std::vector<float2> h;
     switch (N) {
-    case 8: V ? fill_twiddles<8, 1>(h) : fill_twiddles<8, 0>(h); break;
-    case 16: V ? fill_twiddles<16, 1>(h) : fill_twiddles<16, 0>(h); break;
-    case 32: V ? fill_twiddles<32, 1>(h) : fill_twiddles<32, 0>(h); break;
-    case 64: V ? fill_twiddles<64, 1>(h) : fill_twiddles<64, 0>(h); break;
-    case 128: V ? fill_twiddles<128, 1>(h) : fill_twiddles<128, 0>(h); break;
-    case 256: V ? fill_twiddles<256, 1>(h) : fill_twiddles<256, 0>(h); break;
-    case 512: V ? fill_twiddles<512, 1>(h) : fill_twiddles<512, 0>(h); break;
-    case 1024: V ? fill_twiddles<1024, 1>(h) : fill_twiddles<1024, 0>(h); break;
-    case 2048: V ? fill_twiddles<2048, 1>(h) : fill_twiddles<2048, 0>(h); break;
-    case 4096: V ? fill_twiddles<4096, 1>(h) : fill_twiddles<4096, 0>(h); break;
+    case 8: V == 2 ? fill_twiddles<8, 2>(h) : (V ? fill_twiddles<8, 1>(h) : fill_twiddles<8, 0>(h)); break;
+    case 16: V == 2 ? fill_twiddles<16, 2>(h) : (V ? fill_twiddles<16, 1>(h) : fill_twiddles<16, 0>(h)); break;
+    case 32: V == 2 ? fill_twiddles<32, 2>(h) : (V ? fill_twiddles<32, 1>(h) : fill_twiddles<32, 0>(h)); break;
+    case 64: V == 2 ? fill_twiddles<64, 2>(h) : (V ? fill_twiddles<64, 1>(h) : fill_twiddles<64, 0>(h)); break;
+    case 128: V == 2 ? fill_twiddles<128, 2>(h) : (V ? fill_twiddles<128, 1>(h) : fill_twiddles<128, 0>(h)); break;
+    case 256: V == 2 ? fill_twiddles<256, 2>(h) : (V ? fill_twiddles<256, 1>(h) : fill_twiddles<256, 0>(h)); break;
+    case 512: V == 2 ? fill_twiddles<512, 2>(h) : (V ? fill_twiddles<512, 1>(h) : fill_twiddles<512, 0>(h)); break;
+    case 1024: V == 2 ? fill_twiddles<1024, 2>(h) : (V ? fill_twiddles<1024, 1>(h) : fill_twiddles<1024, 0>(h)); break;
+    case 2048: V == 2 ? fill_twiddles<2048, 2>(h) : (V ? fill_twiddles<2048, 1>(h) : fill_twiddles<2048, 0>(h)); break;
+    case 4096: V == 2 ? fill_twiddles<4096, 2>(h) : (V ? fill_twiddles<4096, 1>(h) : fill_twiddles<4096, 0>(h)); break;
     default: return ctx->fail(SSP_EINVAL, "unsupported N=%d", N);
     }
     float2 *d = nullptr;
