@@ -36,6 +36,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config id (1-5)")
     ap.add_argument("--batch", type=int, default=0, help="override realisations per GPU")
+    ap.add_argument("--h-kind", default="fresnel", choices=["fresnel", "angular"],
+                    help="transfer function: north_star's Fresnel form (default) or the paper's angular spectrum")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -215,7 +217,8 @@ def run_ours(args):
     psd = api.PsdParams(**wl.psd_dict())
     cn2, dz = list(wl.cn2_list), list(wl.dz)
     a = wl.ar_a if wl.ar_a > 0 else 0.99
-    kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
+    kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac,
+              h_kind=api.H_ANGULAR_SPECTRUM if args.h_kind == "angular" else api.H_FRESNEL)
 
     # ---- synthetic inputs resident in HBM (seeded): two full frames of white
     # noise used alternately as the fresh noise of successive AR steps
@@ -311,7 +314,7 @@ def run_ours(args):
         n_e2e = max(1, min(args.steps, 3))
         def e2e_step():
             ctx.propagate_host(N, wl.dx, wl.lam, dz, h_in, h_out, h_scr, False, S, wl.win_order,
-                               wl.win_sigma_frac, h_st, 0.5, d_field, screens, stats)
+                               wl.win_sigma_frac, h_st, 0.5, d_field, screens, stats, h_kind=kw["h_kind"])
         e2e_step()
         sync_all()
         t0 = time.perf_counter()
@@ -339,7 +342,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": wl.name, "N": N, "B_per_gpu": B, "S": S, "n_sh": n_sh, "ar_a": a,
+            "config": {"workload": wl.name, "N": N, "B_per_gpu": B, "S": S, "n_sh": n_sh, "ar_a": a, "h_kind": args.h_kind,
                        "step": "evolve_screens + propagate + beam_stats + propagate_adjoint",
                        "units_per_step": units_step,
                        "l2": "inputs larger than L2 (no flush): each step streams > 10 GB"},

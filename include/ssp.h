@@ -81,7 +81,9 @@ typedef struct {
 /* Transfer function of the diffraction step (Q1). */
 typedef enum {
     SSP_H_FRESNEL = 0,          /* H = exp(-i pi (lambda/n0) dz (fx^2 + fy^2))  (north_star) */
-    SSP_H_ANGULAR_SPECTRUM = 1  /* PAPER.md:96 Eq.6, carrier removed (Q2) -- SSP_EUNSUPPORTED in this build */
+    SSP_H_ANGULAR_SPECTRUM = 1  /* PAPER.md:96 Eq.6, carrier removed (Q2): H = exp(i dz (sqrt(km^2 - kappa^2) - km)),
+                                   km = 2 pi n0 / lambda, kappa = 2 pi |f|; evanescent bins -> 0.  Not separable: the
+                                   context caches one complex64 map [N][N] per distinct (dz, conj) */
 } ssp_h_kind;
 
 /* ---- context ------------------------------------------------------------------- */

@@ -39,6 +39,7 @@ int ssp_destroy(ssp_ctx *ctx)
     cudaStreamSynchronize(ctx->stream);
     for (auto &kv : ctx->twiddles) cudaFree(kv.second);
     for (auto &kv : ctx->htables) cudaFree(kv.second);
+    for (auto &kv : ctx->h2d_tables) cudaFree(kv.second);
     for (auto &kv : ctx->sign_tables) cudaFree(kv.second);
     for (void *p : ctx->owned) cudaFree(p);
     for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
@@ -98,9 +99,7 @@ int check_prop(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind
     if (!ctx) return SSP_EINVAL;
     if (!valid_N(grid.N)) return ctx->fail(SSP_EINVAL, "N=%d is not a power of two in [8, 4096]", grid.N);
     if (!(grid.dx > 0) || !(lambda > 0) || !(n0 > 0)) return ctx->fail(SSP_EINVAL, "dx, lambda and n0 must be > 0");
-    if (h_kind == SSP_H_ANGULAR_SPECTRUM)
-        return ctx->fail(SSP_EUNSUPPORTED, "angular-spectrum H is not separable; not built yet (DESIGN.md NEXT-3)");
-    if (h_kind != SSP_H_FRESNEL) return ctx->fail(SSP_EINVAL, "unknown h_kind %d", h_kind);
+    if (h_kind != SSP_H_FRESNEL && h_kind != SSP_H_ANGULAR_SPECTRUM) return ctx->fail(SSP_EINVAL, "unknown h_kind %d", h_kind);
     if (B < 1 || n_steps < 1 || !dz) return ctx->fail(SSP_EINVAL, "B >= 1, n_steps >= 1 and dz are required");
     if (S < 0 || S > n_steps) return ctx->fail(SSP_EINVAL, "need 0 <= S <= n_steps (S=%d, n_steps=%d)", S, n_steps);
     if (S > 0 && !d_screens) return ctx->fail(SSP_EINVAL, "d_screens is null with S=%d", S);
@@ -147,9 +146,13 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
     if (int rc = get_twiddles(ctx, N, 1, &twc)) return rc;
     float2 *u = reinterpret_cast<float2 *>(d_field_out);
 
+    // Fresnel: H = hx[kx] hy[ky], hx applied by the row kernels, hy by the column kernel.
+    // Angular spectrum: H(ky,kx) is not separable; the column kernel applies the whole map, the rows none.
+    const bool as = (h_kind == SSP_H_ANGULAR_SPECTRUM);
     // K4: FFT_x of the input, times hx of step 1
     const float2 *hx = nullptr;
-    if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[0], 0, 0}, &hx)) return rc;
+    if (!as)
+        if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[0], 0, 0}, &hx)) return rc;
     RowArgs r0{};
     r0.in = reinterpret_cast<const float2 *>(d_field_in);
     r0.out = u;
@@ -160,10 +163,11 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
 
     for (int j = 1; j <= n_steps; ++j) {
         // K5: FFT_y -> * hy_j / N^2 -> IFFT_y
-        const float2 *hy = nullptr;
-        if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j - 1], 0, 1}, &hy)) return rc;
+        const float2 *hy = nullptr, *h2d = nullptr;
+        if (as) { if (int rc = get_h2d_table(ctx, HKey{N, grid.dx, lam_eff, dz[j - 1], 0, 1}, &h2d)) return rc; }
+        else if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j - 1], 0, 1}, &hy)) return rc;
         ColArgs c{};
-        c.in = u; c.out = u; c.B = B; c.hy = hy; c.tw = twc;
+        c.in = u; c.out = u; c.B = B; c.hy = hy; c.h2d = h2d; c.tw = twc;
         if (int rc = launch_col_prop(ctx, N, c)) return rc;
         // K6: IFFT_x -> * exp(i phi_j) W -> [FFT_x -> * hx_{j+1}]
         RowArgs r{};
@@ -179,7 +183,7 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
             r.plane_stride = (long long)n_steps * (long long)px;
         }
         const bool last = (j == n_steps);
-        if (!last) {
+        if (!last && !as) {
             if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j], 0, 0}, &hx)) return rc;
             r.hx = hx;
         }
@@ -229,8 +233,10 @@ int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0,
         fill_window(r, win, N);
     };
 
+    const bool as = (h_kind == SSP_H_ANGULAR_SPECTRUM);
     const float2 *hx = nullptr;
-    if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[n_steps - 1], 1, 0}, &hx)) return rc;
+    if (!as)
+        if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[n_steps - 1], 1, 0}, &hx)) return rc;
     RowArgs r0{};
     r0.in = reinterpret_cast<const float2 *>(d_g_out);
     r0.out = g; r0.n_lines = B * N; r0.hx = hx; r0.tw = tw;
@@ -238,18 +244,21 @@ int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0,
     if (int rc = launch_row(ctx, N, false, true, r0)) return rc;
 
     for (int j = n_steps; j >= 1; --j) {
-        const float2 *hy = nullptr;
-        if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j - 1], 1, 1}, &hy)) return rc;
+        const float2 *hy = nullptr, *h2d = nullptr;
+        if (as) { if (int rc = get_h2d_table(ctx, HKey{N, grid.dx, lam_eff, dz[j - 1], 1, 1}, &h2d)) return rc; }
+        else if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j - 1], 1, 1}, &hy)) return rc;
         ColArgs c{};
-        c.in = g; c.out = g; c.B = B; c.hy = hy; c.tw = twc;
+        c.in = g; c.out = g; c.B = B; c.hy = hy; c.h2d = h2d; c.tw = twc;
         if (int rc = launch_col_prop(ctx, N, c)) return rc;
         RowArgs r{};
         r.in = g; r.out = g; r.n_lines = B * N; r.tw = tw;
         const bool last = (j == 1);
         if (!last) {
             plane_stage(r, j - 1);
-            if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j - 2], 1, 0}, &hx)) return rc;
-            r.hx = hx;
+            if (!as) {
+                if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j - 2], 1, 0}, &hx)) return rc;
+                r.hx = hx;
+            }
         }
         if (int rc = launch_row(ctx, N, true, !last, r)) return rc;
     }

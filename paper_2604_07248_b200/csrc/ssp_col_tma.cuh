@@ -93,13 +93,14 @@ struct ScreenColTmaCfg {
 };
 
 struct ColTmaArgs {
-    const float2 *hy;            // [N] multiplier between the transforms
+    const float2 *hy;            // [N] multiplier between the transforms (separable H), or
+    const float2 *h2d;           // tile-major [N/C][N][C] multiplier H(ky,kx) when H2D (non-separable H)
     const float2 *tw;            // column-plan twiddles
     int ntiles;                  // B * N / C
 };
 
 // FFT_y -> * hy -> IFFT_y.  tm_in / tm_out describe the [B*N rows][2N floats] field buffers.
-template <int N>
+template <int N, bool H2D>
 __global__ void __launch_bounds__(ColTmaCfg<N>::THREADS, ColTmaCfg<N>::MIN_BLOCKS)
 k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_out, const ColTmaArgs a)
 {
@@ -141,6 +142,9 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
 #pragma unroll
             for (int q = 0; q < R1; ++q) v[i * R1 + q] = tile_s[line_index<N, 1, R1>(t, i, q) * C + c];
         __syncthreads();                                          // the tile is in registers: the buffer is free
+        // multiplier of element (ky, this thread's column): hy[ky], or H(ky,kx) read through L1/L2
+        const float2 *hcol = H2D ? a.h2d + (size_t)(tile % GROUPS) * N * C + c : a.hy;
+        constexpr int HS = H2D ? C : 1;                           // stride of ky in the multiplier table
         if (CFG::NBUF == 2 && tid == 0 && tile + (int)gridDim.x < a.ntiles) {
             tma_store_wait_read();                                // the store of tile it-1 has released the other buffer
             issue_load(tile + gridDim.x, cur ^ 1);
@@ -155,7 +159,7 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
                     for (int i = 0; i < E / RL; ++i)
 #pragma unroll
                         for (int q = 0; q < RL; ++q) {
-                            const float2 h = __ldg(a.hy + line_index<N, 1, RL>(t, i, q)), x = v[i * RL + q];
+                            const float2 h = __ldg(hcol + (size_t)line_index<N, 1, RL>(t, i, q) * HS), x = v[i * RL + q];
                             v[i * RL + q] = make_float2(fmaf(x.x, h.y, x.y * h.x), fmaf(x.x, h.x, -x.y * h.y));
                         }
                 }
@@ -173,7 +177,7 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
             for (int i = 0; i < E / RL; ++i)
 #pragma unroll
                 for (int q = 0; q < RL; ++q)
-                    v[i * RL + q] = cmul(v[i * RL + q], __ldg(a.hy + line_index<N, 1, RL>(t, i, q)));
+                    v[i * RL + q] = cmul(v[i * RL + q], __ldg(hcol + (size_t)line_index<N, 1, RL>(t, i, q) * HS));
             fft_line<N, 1, true, true, true>(v, t, sm, a.tw);     // inverse, reversed plan; strided by R1
 #pragma unroll
             for (int i = 0; i < E / R1; ++i)

@@ -38,6 +38,8 @@ struct ssp_ctx {
     int num_sms = 148;
     std::map<int, float2 *> twiddles;            // per (N, plan variant), device
     std::map<ssp::HKey, float2 *> htables;       // 1-D transfer-function tables, device [N]
+    std::map<ssp::HKey, float2 *> h2d_tables;    // 2-D transfer functions [N][N] (angular spectrum), device
+    size_t h2d_bytes = 0;
     std::map<int, float2 *> sign_tables;         // (-1)^k tables for the centred DFT
     void *scratch = nullptr;                     // small device scratch (stat accumulators, tables)
     size_t scratch_bytes = 0;
@@ -93,6 +95,10 @@ namespace ssp {
 // V = 0: row-plan tables, V = 1: column-plan tables (ssp_fft.cuh)
 int get_twiddles(ssp_ctx *ctx, int N, int V, const float2 **out);
 int get_htable(ssp_ctx *ctx, const HKey &key, const float2 **out);
+// Angular-spectrum transfer function H(ky,kx)/N^2 as a complex64 map [N][N] (Eq.6, carrier removed,
+// evanescent bins 0), evaluated once per (grid, lambda/n0, dz, conj) in double on the device and cached
+// (8 N^2 bytes each, L2-resident at N <= 1024; the cache is dropped when it passes 1 GiB).
+int get_h2d_table(ssp_ctx *ctx, const HKey &key, const float2 **out);
 int get_sign_table(ssp_ctx *ctx, int N, const float2 **out);
 int ensure_scratch(ssp_ctx *ctx, size_t bytes);
 // TMA descriptor of a row-major buffer of complex64: `cols` elements per row, `rows` rows, boxes of
@@ -131,6 +137,8 @@ struct ColArgs {
     float2 *out;
     int B;
     const float2 *hy;            // [N] multiplier between / after the transforms, or null
+    const float2 *h2d;           // multiplier H(ky,kx) used instead of hy (non-separable H), tile-major
+                                 // [N/C][N][C] with C = col_tile_width(N), or null
     const float2 *tw;
 };
 
@@ -187,6 +195,8 @@ int launch_stats(ssp_ctx *ctx, int N, double dx, int B, const float2 *field, dou
                  ssp_stats *d_stats);
 int launch_welford(ssp_ctx *ctx, int N, int B, const float2 *field, float *mean, float *M2,
                    long long count0);
+int launch_h2d_table(ssp_ctx *ctx, int N, int C, double dx, double lam_eff, double dz, int conj, float2 *out);
+int col_tile_width(int N);     // columns per tile of the kernel launch_col_prop picks for N (layout of the H map)
 int launch_phase_mul(ssp_ctx *ctx, int N, int B, const float *theta, float sign,
                      const float2 *in, float2 *out);
 int launch_phase_grad(ssp_ctx *ctx, long long n, const float2 *g, const float2 *u, float *grad);

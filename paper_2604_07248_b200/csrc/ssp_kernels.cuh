@@ -197,7 +197,13 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_c
         for (int q = 0; q < R1; ++q) v[i * R1 + q] = src[(size_t)line_index<N, 1, R1>(t, i, q) * N];
 
     fft_line<N, 1, false, MODE == 2, MODE == 0>(v, t, sm, a.tw); // strided by RL
-    if (a.hy) {
+    if (a.h2d) { // non-separable H(ky,kx)
+#pragma unroll
+        for (int i = 0; i < E / RL; ++i)
+#pragma unroll
+            for (int q = 0; q < RL; ++q)
+                v[i * RL + q] = cmul(v[i * RL + q], __ldg(a.h2d + ((size_t)(col / C) * N + line_index<N, 1, RL>(t, i, q)) * C + c));
+    } else if (a.hy) {
 #pragma unroll
         for (int i = 0; i < E / RL; ++i)
 #pragma unroll

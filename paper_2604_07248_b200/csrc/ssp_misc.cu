@@ -153,6 +153,41 @@ __global__ void __launch_bounds__(256) k_phase_mul(const float *__restrict__ the
     }
 }
 
+// Angular-spectrum transfer function (Eq.6 without the carrier, Q2), scaled by 1/N^2:
+//   H = exp(i dz (sqrt(km^2 - kappa^2) - km)) = exp(-i dz kappa^2 / (km + sqrt(km^2 - kappa^2))),
+//   km = 2 pi / lam_eff, kappa^2 = 4 pi^2 (fx^2 + fy^2); kappa > km (evanescent) -> 0.
+// Evaluated in double: the phase reaches hundreds of radians.
+// Layout: tile-major [N/C][N (ky)][C] with C the column-tile width of the kernel that reads it, so that a
+// column tile's multipliers are one contiguous 8 N C-byte block (coalesced, L2-resident).
+__global__ void __launch_bounds__(256) k_h2d_table(int N, int C, double dx, double lam_eff, double dz, int conj,
+                                                    float2 *__restrict__ out)
+{
+    const int kx = blockIdx.x * blockDim.x + threadIdx.x, ky = blockIdx.y;
+    if (kx >= N) return;
+    const double kPi = 3.14159265358979323846;
+    const double fx = (double)((kx < N / 2) ? kx : kx - N) / ((double)N * dx);
+    const double fy = (double)((ky < N / 2) ? ky : ky - N) / ((double)N * dx);
+    const double km = 2.0 * kPi / lam_eff, kap2 = 4.0 * kPi * kPi * (fx * fx + fy * fy);
+    float2 h = make_float2(0.f, 0.f);
+    if (kap2 <= km * km) {
+        double ang = -dz * kap2 / (km + sqrt(km * km - kap2));
+        if (conj) ang = -ang;
+        double s, c;
+        sincos(ang, &s, &c);
+        const double scale = 1.0 / ((double)N * (double)N);
+        h = make_float2((float)(scale * c), (float)(scale * s));
+    }
+    out[((size_t)(kx / C) * N + ky) * C + kx % C] = h;
+}
+
+int launch_h2d_table(ssp_ctx *ctx, int N, int C, double dx, double lam_eff, double dz, int conj, float2 *out)
+{
+    k_h2d_table<<<dim3((N + 255) / 256, N), 256, 0, ctx->stream>>>(N, C, dx, lam_eff, dz, conj, out);
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
 int launch_phase_mul(ssp_ctx *ctx, int N, int B, const float *theta, float sign, const float2 *in, float2 *out)
 {
     const size_t px = (size_t)N * N;

@@ -93,11 +93,11 @@ int launch_row(ssp_ctx *ctx, int N, bool first, bool second, const RowArgs &a)
 }
 
 // TMA-fed persistent column kernel (ssp_col_tma.cuh)
-template <int N>
-static int launch_col_tma_n(ssp_ctx *ctx, const ColArgs &a)
+template <int N, bool H2D>
+static int launch_col_tma_x(ssp_ctx *ctx, const ColArgs &a)
 {
     using CFG = ColTmaCfg<N>;
-    auto kern = k_col_tma<N>;
+    auto kern = k_col_tma<N, H2D>;
     CUtensorMap tm_in, tm_out;
     if (int rc = make_tmap_c64(ctx, a.in, N, (size_t)a.B * N, CFG::C, CFG::BOX_ROWS, &tm_in)) return rc;
     if (int rc = make_tmap_c64(ctx, a.out, N, (size_t)a.B * N, CFG::C, CFG::BOX_ROWS, &tm_out)) return rc;
@@ -106,7 +106,7 @@ static int launch_col_tma_n(ssp_ctx *ctx, const ColArgs &a)
     const int resident = ctx->num_sms * CFG::MIN_BLOCKS;
     // two buffers: persistent CTAs walk the tiles; one buffer: one tile per CTA
     const int grid = (CFG::NBUF == 2 && ntiles > resident) ? resident : ntiles;
-    ColTmaArgs ta{a.hy, a.tw, ntiles};
+    ColTmaArgs ta{a.hy, a.h2d, a.tw, ntiles};
     ctx->prof_begin("col_fft_h_ifft", 16.0 * (double)a.B * N * N);
     kern<<<grid, CFG::THREADS, CFG::SMEM, ctx->stream>>>(tm_in, tm_out, ta);
     ctx->prof_end();
@@ -115,9 +115,35 @@ static int launch_col_tma_n(ssp_ctx *ctx, const ColArgs &a)
     return SSP_OK;
 }
 
+template <int N>
+static int launch_col_tma_n(ssp_ctx *ctx, const ColArgs &a)
+{
+    return a.h2d ? launch_col_tma_x<N, true>(ctx, a) : launch_col_tma_x<N, false>(ctx, a);
+}
+
+template <int N>
+static constexpr int col_tile_width_n() { return ColTmaTune<N>::ENABLED ? ColTmaCfg<N>::C : ColCfg<N>::C; }
+
+int col_tile_width(int N)
+{
+    switch (N) {
+    case 8: return col_tile_width_n<8>();
+    case 16: return col_tile_width_n<16>();
+    case 32: return col_tile_width_n<32>();
+    case 64: return col_tile_width_n<64>();
+    case 128: return col_tile_width_n<128>();
+    case 256: return col_tile_width_n<256>();
+    case 512: return col_tile_width_n<512>();
+    case 1024: return col_tile_width_n<1024>();
+    case 2048: return col_tile_width_n<2048>();
+    case 4096: return col_tile_width_n<4096>();
+    default: return 1;
+    }
+}
+
 int launch_col_prop(ssp_ctx *ctx, int N, const ColArgs &a)
 {
-    if (a.hy) {
+    if (a.hy || a.h2d) {
         if (N == 512) return launch_col_tma_n<512>(ctx, a);
         if (N == 1024) return launch_col_tma_n<1024>(ctx, a);
         if (N == 2048) return launch_col_tma_n<2048>(ctx, a);

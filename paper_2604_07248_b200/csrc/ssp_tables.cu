@@ -106,6 +106,29 @@ int get_htable(ssp_ctx *ctx, const HKey &key, const float2 **out)
     return SSP_OK;
 }
 
+int get_h2d_table(ssp_ctx *ctx, const HKey &key, const float2 **out)
+{
+    auto it = ctx->h2d_tables.find(key);
+    if (it != ctx->h2d_tables.end()) { *out = it->second; return SSP_OK; }
+    const size_t bytes = sizeof(float2) * (size_t)key.N * key.N;
+    if (ctx->h2d_bytes + bytes > ((size_t)1 << 30)) { // long dz lists on big grids: drop the cache rather than grow
+        SSP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        for (auto &kv : ctx->h2d_tables) cudaFree(kv.second);
+        ctx->h2d_tables.clear();
+        ctx->h2d_bytes = 0;
+    }
+    float2 *d = nullptr;
+    SSP_CUDA(ctx, cudaMalloc(&d, bytes));
+    if (int rc = launch_h2d_table(ctx, key.N, col_tile_width(key.N), key.dx, key.lam_eff, key.dz, key.conj, d)) {
+        cudaFree(d);
+        return rc;
+    }
+    ctx->h2d_tables[key] = d;
+    ctx->h2d_bytes += bytes;
+    *out = d;
+    return SSP_OK;
+}
+
 // s[k] = (-1)^k: the centred DFT is (-1)^k FFT((-1)^n x) / sqrt(N) per axis (N % 4 == 0).
 int get_sign_table(ssp_ctx *ctx, int N, const float2 **out)
 {
