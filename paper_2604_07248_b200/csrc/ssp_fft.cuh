@@ -54,53 +54,28 @@ __host__ __device__ constexpr float cos32(int k)
 }
 __host__ __device__ constexpr float sin32(int k) { return cos32(k - 8); }
 
-// b *= W_R^K with W_R = exp(-/+ i 2 pi / R) (forward / inverse); K, R compile-time.
-template <int R, int K, bool INV>
-__device__ __forceinline__ void mul_w(float2 &b)
+// ---- radix-R butterflies in registers: decimation in time, FMA form ----------------------------------
+// One DIT butterfly (a, b) -> (a + w b, a - w b) with w = W_L^J = exp(-/+ i 2 pi J / L) (forward / inverse),
+// L, J compile-time.  Trivial w (1, -/+i) cost 4 additions.  Any other w costs 6 FMAs instead of the 8
+// operations of "multiply, then add and subtract":  X = a + w b as two chained FMAs per component with w's
+// components as immediates, and Y = a - w b = 2 a - X as one more FMA per component.
+template <int L, int J, bool INV>
+__device__ __forceinline__ void bfly_dit(float2 &a, float2 &b)
 {
-    constexpr int k32 = (K * (32 / R)) & 31;
+    constexpr int k32 = (J * (32 / L)) & 31;                      // w = W_32^k32, k32 < 16 since J < L/2
     if constexpr (k32 == 0) {
-    } else if constexpr (k32 == 8) { // -i (fwd) / +i (inv)
-        float2 t = b;
-        b = INV ? make_float2(-t.y, t.x) : make_float2(t.y, -t.x);
-    } else if constexpr (k32 == 16) {
-        b = make_float2(-b.x, -b.y);
-    } else if constexpr (k32 == 24) {
-        float2 t = b;
-        b = INV ? make_float2(t.y, -t.x) : make_float2(-t.y, t.x);
+        const float2 x = make_float2(a.x + b.x, a.y + b.y), y = make_float2(a.x - b.x, a.y - b.y);
+        a = x; b = y;
+    } else if constexpr (k32 == 8) {                              // w = -i (forward), +i (inverse)
+        const float2 wb = INV ? make_float2(-b.y, b.x) : make_float2(b.y, -b.x);
+        const float2 x = make_float2(a.x + wb.x, a.y + wb.y), y = make_float2(a.x - wb.x, a.y - wb.y);
+        a = x; b = y;
     } else {
-        constexpr float c = cos32(k32);
-        constexpr float s = INV ? sin32(k32) : -sin32(k32);
-        float2 t = b;
-        b = make_float2(fmaf(t.x, c, -t.y * s), fmaf(t.x, s, t.y * c));
-    }
-}
-
-// butterfly (a, b) -> (a + b, (a - b) W_R^K) on v[OFF+K], v[OFF+K+R/2]
-template <int R, int OFF, int K, bool INV>
-__device__ __forceinline__ void bfly(float2 *v)
-{
-    float2 a = v[OFF + K], b = v[OFF + K + R / 2];
-    v[OFF + K] = make_float2(a.x + b.x, a.y + b.y);
-    float2 d = make_float2(a.x - b.x, a.y - b.y);
-    mul_w<R, K, INV>(d);
-    v[OFF + K + R / 2] = d;
-}
-
-template <int R, int OFF, bool INV, int... K>
-__device__ __forceinline__ void dif_level(float2 *v, std::integer_sequence<int, K...>)
-{
-    (bfly<R, OFF, K, INV>(v), ...);
-}
-
-// In-place radix-2 DIF recursion on v[OFF .. OFF+R): leaves X[bitrev(i)] in v[OFF+i].
-template <int R, int OFF, bool INV>
-__device__ __forceinline__ void dif_rec(float2 *v)
-{
-    if constexpr (R >= 2) {
-        dif_level<R, OFF, INV>(v, std::make_integer_sequence<int, R / 2>{});
-        dif_rec<R / 2, OFF, INV>(v);
-        dif_rec<R / 2, OFF + R / 2, INV>(v);
+        constexpr float wr = cos32(k32);
+        constexpr float wi = INV ? sin32(k32) : -sin32(k32);
+        const float2 x = make_float2(fmaf(wr, b.x, fmaf(-wi, b.y, a.x)), fmaf(wr, b.y, fmaf(wi, b.x, a.y)));
+        const float2 y = make_float2(fmaf(2.f, a.x, -x.x), fmaf(2.f, a.y, -x.y));
+        a = x; b = y;
     }
 }
 
@@ -115,11 +90,28 @@ __host__ __device__ constexpr int bitrev(int i, int R)
 }
 
 template <int R, int... I>
-__device__ __forceinline__ void unscramble(float2 *v, std::integer_sequence<int, I...>)
+__device__ __forceinline__ void scramble(float2 *v, std::integer_sequence<int, I...>)
 {
     float2 t[R];
     ((t[I] = v[bitrev(I, R)]), ...);
     ((v[I] = t[I]), ...);
+}
+
+// all butterflies of the level that merges transforms of length L/2 into length L
+template <int R, int L, bool INV, int... B>
+__device__ __forceinline__ void dit_level(float2 *v, std::integer_sequence<int, B...>)
+{
+    // butterfly index B in [0, R/2): group B / (L/2), position J = B % (L/2)
+    (bfly_dit<L, B % (L / 2), INV>(v[(B / (L / 2)) * L + B % (L / 2)], v[(B / (L / 2)) * L + B % (L / 2) + L / 2]), ...);
+}
+
+template <int R, int L, bool INV>
+__device__ __forceinline__ void dit_levels(float2 *v)
+{
+    if constexpr (L <= R) {
+        dit_level<R, L, INV>(v, std::make_integer_sequence<int, R / 2>{});
+        dit_levels<R, 2 * L, INV>(v);
+    }
 }
 
 // Radix-R DFT of v[0..R) in registers, natural order in and out.  R in {1,2,4,8,16,32}.
@@ -127,8 +119,8 @@ template <int R, bool INV>
 __device__ __forceinline__ void radix(float2 *v)
 {
     if constexpr (R > 1) {
-        dif_rec<R, 0, INV>(v);
-        unscramble<R>(v, std::make_integer_sequence<int, R>{});
+        scramble<R>(v, std::make_integer_sequence<int, R>{});    // bit reversal: register renaming
+        dit_levels<R, 2, INV>(v);
     }
 }
 
@@ -170,10 +162,12 @@ struct PlanInfo {
     static constexpr int RL = (NSTAGE == 1) ? R1 : (NSTAGE == 2 ? R2 : R3); // last radix
     static constexpr int PADQ = N / R1;                    // one pad element per PADQ positions
     static constexpr int PADQ_REV = N / RL;
-    static constexpr int LINE_ELEMS = N + (R1 > RL ? R1 : RL); // padded line length (either direction)
+    static constexpr int LINE_ELEMS = N + (R1 > RL ? R1 : RL); // padded line length (either direction), pad 1
+    static constexpr int LINE_ELEMS2 = N + 2 * (R1 > RL ? R1 : RL); // the same with pad 2 (16-byte aligned rows)
     // twiddle tables (forward sign), built on the host in double:
-    //   tw1 [R1][N/R1]:  W_N^(m k1)            tw2 [R2][R3]: W_N^(R1 n3 k2)
-    //   tw1r[RL][N/RL] and tw2r[R2][R1] for the reversed plan (R3|R2, R2, R1)
+    //   tw1 [R1/2][N/R1][2]: W_N^(m k1), the twiddles of k1 = 2p, 2p+1 adjacent (one 16-byte load)
+    //   tw2 [R2][R3]: W_N^(R1 n3 k2)
+    //   tw1r[RL/2][N/RL][2] and tw2r[R2][R1] for the reversed plan (R3|R2, R2, R1)
     static constexpr int TW1 = 0;
     static constexpr int TW2 = TW1 + N;
     static constexpr int TW1R = TW2 + R2 * R3;
@@ -184,7 +178,9 @@ struct PlanInfo {
 // One complete transform of a line held in registers.
 //   DIR_REV = false: plan (R1,R2,R3): input strided by R1, output strided by RL.
 //   DIR_REV = true : plan (RL,..,R1): input strided by RL, output strided by R1.
-// SM: exchange accessor with  st(pos, val), ld(pos), sync()  on padded positions of this line.
+// SM: exchange accessor with  st(pos, val), ld(pos), sync()  on padded positions of this line, and
+// SM::PAD = pad elements per PADQ positions (1, or 2 with ld2(pos, a, b) reading two adjacent elements
+// as one 16-byte access: two-stage plans only).
 // TAIL_SYNC: synchronise right after the last exchange has been read, so that the caller may reuse
 // the buffer at once.  A barrier placed there is cheap (the threads have just left the previous one);
 // the same barrier after the last butterflies would re-align threads that have drifted apart.
@@ -201,7 +197,8 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 
     const float2 *tw2 = tw + (DIR_REV ? PI::TW2R : PI::TW2);
     // padded position of line index k1 * PADQ + r, r < PADQ: one pad element per PADQ positions.  Written
     // with k1 explicit so that no division of a run-time index is left in the address arithmetic.
-    constexpr int PITCH = PADQ + 1;
+    constexpr int PITCH = PADQ + SM::PAD;
+    static_assert(SM::PAD == 1 || NS <= 2, "16-byte exchange reads are laid out for two-stage plans");
 
     // ---- stage 1
     constexpr int M1 = N / Ra;
@@ -210,11 +207,15 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 
         radix<Ra, INV>(v + i * Ra);
         if constexpr (NS >= 2) {
             const int m = t + T * i;
+            const float4 *tw4 = reinterpret_cast<const float4 *>(tw1) + m;
 #pragma unroll
-            for (int k = 0; k < Ra; ++k) {
-                float2 x = v[i * Ra + k];
-                if (k > 0) x = cmul_c<INV>(x, __ldg(tw1 + k * M1 + m));
-                sm.st(k * PITCH + m, x);
+            for (int k = 0; k < Ra; k += 2) {
+                const float4 w = __ldg(tw4 + (k / 2) * M1);       // twiddles of k and k + 1
+                float2 x0 = v[i * Ra + k], x1 = v[i * Ra + k + 1];
+                if (k > 0) x0 = cmul_c<INV>(x0, make_float2(w.x, w.y));
+                x1 = cmul_c<INV>(x1, make_float2(w.z, w.w));
+                sm.st(k * PITCH + m, x0);
+                sm.st((k + 1) * PITCH + m, x1);
             }
         }
     }
@@ -226,8 +227,13 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 
 #pragma unroll
         for (int i = 0; i < E / Rb; ++i) {
             const int j = t + T * i;
+            if constexpr (SM::PAD == 2) {
 #pragma unroll
-            for (int n = 0; n < Rb; ++n) v[i * Rb + n] = sm.ld(j * PITCH + n);
+                for (int n = 0; n < Rb; n += 2) sm.ld2(j * PITCH + n, v[i * Rb + n], v[i * Rb + n + 1]);
+            } else {
+#pragma unroll
+                for (int n = 0; n < Rb; ++n) v[i * Rb + n] = sm.ld(j * PITCH + n);
+            }
         }
         if constexpr (TAIL_SYNC) sm.sync();
 #pragma unroll

@@ -81,7 +81,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
     const int lib = tid / T, t = tid % T;
     const long long line = (long long)blockIdx.x * CFG::LPB + lib;
     const int b = (int)(line / N), iy = (int)(line % N);
-    RowSmem<T> sm{smem + (size_t)lib * PI::LINE_ELEMS, 1 + lib};
+    RowSmem<T, CFG::WIDE> sm{smem + (size_t)lib * CFG::LINE_ELEMS, 1 + lib};
 
     // the screen row is streamed from HBM: fetch it asynchronously now, use it after the first transform
     float *phis = reinterpret_cast<float *>(smem_raw + CFG::SMEM_X) + (size_t)lib * N;

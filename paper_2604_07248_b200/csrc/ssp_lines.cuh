@@ -7,6 +7,11 @@
 namespace ssp {
 
 // ---- CTA shapes --------------------------------------------------------------------
+// WIDE: pad 2 per row of the exchange matrix (16-byte aligned rows) and 16-byte reads; taken where a warp's
+// accesses stay conflict-free with it: the two-stage plans of N = 512 and 1024.
+template <int N>
+struct RowWide { static constexpr bool value = (N == 512 || N == 1024); };
+
 // Row-kernel CTA size and resident CTAs per SM the register budget is sized for.  Default: 256
 // threads, 512 resident threads at E = 32 and 1024 at E = 16.  N = 1024 (one warp per row, 32 points
 // per thread) measured best on B200 with 168 registers: 3 CTAs of 4 rows.
@@ -32,8 +37,10 @@ struct RowCfg {
     static constexpr int THREADS = (T * N < RowTune<N>::MAX_THREADS) ? T * N : RowTune<N>::MAX_THREADS;
     static constexpr int LPB = THREADS / T;                        // lines (rows) per CTA
     static constexpr bool WARP_LOCAL = (T <= 32);                  // a line never spans two warps
+    static constexpr bool WIDE = RowWide<N>::value;
+    static constexpr int LINE_ELEMS = WIDE ? PlanInfo<N, 0>::LINE_ELEMS2 : PlanInfo<N, 0>::LINE_ELEMS;
     static constexpr size_t SMEM_X = (PlanInfo<N, 0>::NSTAGE == 1) ? 0
-        : sizeof(float2) * (size_t)LPB * PlanInfo<N, 0>::LINE_ELEMS;       // exchange buffers
+        : sizeof(float2) * (size_t)LPB * LINE_ELEMS;                       // exchange buffers
     static constexpr size_t SMEM_PHI = sizeof(float) * (size_t)LPB * N; // prefetched screen rows
     static constexpr size_t SMEM = SMEM_X + SMEM_PHI;
     static constexpr int MIN_BLOCKS = (THREADS < RowTune<N>::MAX_THREADS) ? 1 : RowTune<N>::MIN_BLOCKS;
@@ -55,10 +62,17 @@ struct ColCfg {
 // ---- shared-memory exchange accessors -------------------------------------------------
 // T = threads per line.  A line inside one warp synchronises with __syncwarp; a line spanning
 // several warps uses its own named barrier (id 1 + line-in-CTA), so lines never wait on each other.
-template <int T>
+template <int T, bool WIDE = false>
 struct RowSmem {
+    static constexpr int PAD = WIDE ? 2 : 1;
     float2 *base; // this line's padded buffer
     int bar_id;
+    __device__ __forceinline__ void ld2(int p, float2 &a, float2 &b) const
+    {
+        const float4 w = *reinterpret_cast<const float4 *>(base + p);
+        a = make_float2(w.x, w.y);
+        b = make_float2(w.z, w.w);
+    }
     __device__ __forceinline__ void st(int p, float2 x) { base[p] = x; }
     __device__ __forceinline__ float2 ld(int p) const { return base[p]; }
     __device__ __forceinline__ void sync()
@@ -70,6 +84,7 @@ struct RowSmem {
 
 template <int C>
 struct ColSmem {
+    static constexpr int PAD = 1;
     float2 *base; // tile base + this thread's column
     __device__ __forceinline__ void st(int p, float2 x) { base[p * C] = x; }
     __device__ __forceinline__ float2 ld(int p) const { return base[p * C]; }

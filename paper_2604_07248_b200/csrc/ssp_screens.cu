@@ -199,7 +199,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_s
     const int lib = tid / T, t = tid % T;
     const long long line = (long long)blockIdx.x * CFG::LPB + lib;
     const int scr = (int)(line / N), iy = (int)(line % N);
-    RowSmem<T> sm{smem + (size_t)lib * PI::LINE_ELEMS, 1 + lib};
+    RowSmem<T, CFG::WIDE> sm{smem + (size_t)lib * CFG::LINE_ELEMS, 1 + lib};
 
     float2 v[E];
     const float2 *src = a.in + line * N;

@@ -39,13 +39,16 @@ static void fill_twiddles(std::vector<float2> &h)
     using PI = PlanInfo<N, V>;
     h.assign(PI::TW_TOTAL, make_float2(1.f, 0.f));
     // forward plan (R1, R2, R3)
+    // first-stage tables: [k / 2][m][k % 2], so that one 16-byte load brings the twiddles of k and k + 1
     for (int k = 0; k < PI::R1; ++k)
-        for (int m = 0; m < N / PI::R1; ++m) h[PI::TW1 + k * (N / PI::R1) + m] = wn((long long)m * k, N);
+        for (int m = 0; m < N / PI::R1; ++m)
+            h[PI::TW1 + ((k / 2) * (N / PI::R1) + m) * 2 + (k & 1)] = wn((long long)m * k, N);
     for (int k = 0; k < PI::R2; ++k)
         for (int n3 = 0; n3 < PI::R3; ++n3) h[PI::TW2 + k * PI::R3 + n3] = wn((long long)PI::R1 * n3 * k, N);
     // reversed plan (RL, .., R1): first radix RL, third radix R1
     for (int k = 0; k < PI::RL; ++k)
-        for (int m = 0; m < N / PI::RL; ++m) h[PI::TW1R + k * (N / PI::RL) + m] = wn((long long)m * k, N);
+        for (int m = 0; m < N / PI::RL; ++m)
+            h[PI::TW1R + ((k / 2) * (N / PI::RL) + m) * 2 + (k & 1)] = wn((long long)m * k, N);
     for (int k = 0; k < PI::R2; ++k)
         for (int n3 = 0; n3 < PI::R1; ++n3) h[PI::TW2R + k * PI::R1 + n3] = wn((long long)PI::RL * n3 * k, N);
 }
