@@ -332,7 +332,8 @@ def run_ours(args):
     # ---- the oracle on the host cores, bounded sample (rank 0, N=1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        S_s = 2 if N >= 1024 else min(S, 5)
+        probe, _ = oracle_frame(wl, 1)                    # one screen: sizes a sample of about 15 s
+        S_s = int(max(1, min(S, 15.0 / max(probe, 1e-9))))
         dt, units = oracle_frame(wl, S_s)
         cpu = {"value": units / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"1 realisation x {S_s} of {S} screens, one frame (evolve + propagate + stats + adjoint), {dt:.1f} s"}
