@@ -183,7 +183,9 @@ int ssp_beam_stats(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_field, dou
 /* End-to-end form of ssp_propagate with HOST buffers: copies field and screens to the
  * device buffers given (d_field [B][N][N] c64, d_screens as above), propagates, copies
  * the output field and statistics back, and synchronises the stream.  h_* pointers are
- * host memory (pinned for full copy speed). */
+ * host memory (pinned for full copy speed and overlap).  The batch is processed in chunks of
+ * max(1, B/8) fields on two internal copy streams, so that the copies of neighbouring chunks
+ * overlap the propagation; results equal ssp_propagate's. */
 int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind,
                        int B, int n_steps, const double *dz,
                        const float *h_screens, long long screen_batch_stride, int S,

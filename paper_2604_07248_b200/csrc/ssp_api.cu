@@ -43,6 +43,9 @@ int ssp_destroy(ssp_ctx *ctx)
     for (auto &kv : ctx->sign_tables) cudaFree(kv.second);
     for (void *p : ctx->owned) cudaFree(p);
     for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
+    for (cudaEvent_t e : ctx->pipe_events) cudaEventDestroy(e);
+    if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
+    if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
     if (ctx->scratch) cudaFree(ctx->scratch);
     delete ctx;
     return SSP_OK;
@@ -301,18 +304,52 @@ int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, in
     if (h_stats && !d_stats) return ctx->fail(SSP_EINVAL, "d_stats is required with h_stats");
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));
     const size_t px = (size_t)grid.N * grid.N;
-    SSP_CUDA(ctx, cudaMemcpyAsync(d_field, h_field_in, sizeof(float) * 2 * px * B, cudaMemcpyHostToDevice, ctx->stream));
-    if (S > 0) {
-        const size_t n_scr = (screen_batch_stride == 0) ? (size_t)S * px
-                                                        : (size_t)(B - 1) * (size_t)screen_batch_stride + (size_t)S * px;
-        SSP_CUDA(ctx, cudaMemcpyAsync(d_screens, h_screens, sizeof(float) * n_scr, cudaMemcpyHostToDevice, ctx->stream));
+    // Chunked pipeline over the batch: the host->device copy of chunk c+1 (copy_in stream) overlaps the
+    // propagation of chunk c (context stream) and the device->host copy of chunk c-1 (copy_out stream).
+    if (!ctx->copy_in) {
+        SSP_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_in, cudaStreamNonBlocking));
+        SSP_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_out, cudaStreamNonBlocking));
     }
-    if (int rc = ssp_propagate(ctx, grid, lambda, n0, h_kind, B, n_steps, dz, d_screens, screen_batch_stride, S, win,
-                               d_field, d_field, nullptr, h_stats ? d_stats : nullptr, roi_frac, d_ws, ws_bytes))
-        return rc;
-    SSP_CUDA(ctx, cudaMemcpyAsync(h_field_out, d_field, sizeof(float) * 2 * px * B, cudaMemcpyDeviceToHost, ctx->stream));
-    if (h_stats)
-        SSP_CUDA(ctx, cudaMemcpyAsync(h_stats, d_stats, sizeof(ssp_stats) * B, cudaMemcpyDeviceToHost, ctx->stream));
+    const int Bc = (B >= 8) ? B / 8 : 1;                        // fields per chunk
+    const int n_chunks = (B + Bc - 1) / Bc;
+    while ((int)ctx->pipe_events.size() < 2 * n_chunks + 2) {
+        cudaEvent_t e;
+        SSP_CUDA(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        ctx->pipe_events.push_back(e);
+    }
+    cudaEvent_t ev_start = ctx->pipe_events[2 * n_chunks], ev_end = ctx->pipe_events[2 * n_chunks + 1];
+    // earlier work on the context's stream may still use the device buffers
+    SSP_CUDA(ctx, cudaEventRecord(ev_start, ctx->stream));
+    SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_in, ev_start, 0));
+    SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_out, ev_start, 0));
+    const bool shared = (screen_batch_stride == 0);
+    if (S > 0 && shared)
+        SSP_CUDA(ctx, cudaMemcpyAsync(d_screens, h_screens, sizeof(float) * (size_t)S * px, cudaMemcpyHostToDevice, ctx->copy_in));
+    for (int c = 0; c < n_chunks; ++c) {
+        const int b0 = c * Bc, nb = (B - b0 < Bc) ? B - b0 : Bc;
+        cudaEvent_t ev_in = ctx->pipe_events[2 * c], ev_done = ctx->pipe_events[2 * c + 1];
+        float *df = d_field + 2 * px * (size_t)b0;
+        SSP_CUDA(ctx, cudaMemcpyAsync(df, h_field_in + 2 * px * (size_t)b0, sizeof(float) * 2 * px * nb, cudaMemcpyHostToDevice, ctx->copy_in));
+        float *ds = d_screens;
+        if (S > 0 && !shared) {
+            ds = d_screens + (size_t)b0 * (size_t)screen_batch_stride;
+            const size_t n_scr = (size_t)(nb - 1) * (size_t)screen_batch_stride + (size_t)S * px;
+            SSP_CUDA(ctx, cudaMemcpyAsync(ds, h_screens + (size_t)b0 * (size_t)screen_batch_stride, sizeof(float) * n_scr,
+                                          cudaMemcpyHostToDevice, ctx->copy_in));
+        }
+        SSP_CUDA(ctx, cudaEventRecord(ev_in, ctx->copy_in));
+        SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ev_in, 0));
+        if (int rc = ssp_propagate(ctx, grid, lambda, n0, h_kind, nb, n_steps, dz, ds, screen_batch_stride, S, win,
+                                   df, df, nullptr, h_stats ? d_stats + b0 : nullptr, roi_frac, d_ws, ws_bytes))
+            return rc;
+        SSP_CUDA(ctx, cudaEventRecord(ev_done, ctx->stream));
+        SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_out, ev_done, 0));
+        SSP_CUDA(ctx, cudaMemcpyAsync(h_field_out + 2 * px * (size_t)b0, df, sizeof(float) * 2 * px * nb, cudaMemcpyDeviceToHost, ctx->copy_out));
+        if (h_stats)
+            SSP_CUDA(ctx, cudaMemcpyAsync(h_stats + b0, d_stats + b0, sizeof(ssp_stats) * nb, cudaMemcpyDeviceToHost, ctx->copy_out));
+    }
+    SSP_CUDA(ctx, cudaEventRecord(ev_end, ctx->copy_out));
+    SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ev_end, 0));
     SSP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return SSP_OK;
 }

@@ -45,6 +45,9 @@ struct ssp_ctx {
     size_t scratch_bytes = 0;
     std::vector<void *> owned;                   // misc device allocations freed at destroy
     void *encode_tiled = nullptr;                // cuTensorMapEncodeTiled, resolved through the runtime
+    // ssp_propagate_host: copy streams and events of the chunked host <-> device pipeline (created on first use)
+    cudaStream_t copy_in = nullptr, copy_out = nullptr;
+    std::vector<cudaEvent_t> pipe_events;
 
     // ---- optional per-launch timing with CUDA events on the context's stream (bench.py's roofline)
     struct ProfRec { const char *name; double bytes; int ev; };

@@ -239,3 +239,33 @@ def test_error_codes(ssp):
     with pytest.raises(TypeError):
         ssp.propagate(N, dx, lam, [1.0], u.cpu())                # no CPU fallback
     assert ssp.launch_count() >= 0
+
+
+@pytest.mark.parametrize("B,shared", [(1, False), (11, False), (16, True)])
+def test_propagate_host_matches_device_path(ssp, orc, B, shared):
+    """ssp_propagate_host (host buffers, chunked copy/compute pipeline) returns exactly what ssp_propagate returns on
+    the same inputs, and one field is checked against the oracle."""
+    import torch
+    from paper_2604_07248_b200 import api
+    N, n_steps, S = 128, 3, 3
+    dx, lam, dz, u0, scr = _case(N, B, n_steps, S, 100 + B)
+    if shared:
+        scr = scr[0]
+    kw = dict(win_order=16, win_sigma_frac=0.47)
+    stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+    ref_dev = ssp.propagate(N, dx, lam, list(dz), cu(u0), cu(scr), shared_screens=shared, stats=stats, roi_frac=0.5, **kw)
+    h_in = torch.from_numpy(u0).pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    h_scr = torch.from_numpy(np.ascontiguousarray(scr)).pin_memory()
+    h_st = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8).pin_memory()
+    d_field = torch.empty((B, N, N), dtype=torch.complex64, device="cuda")
+    d_scr = torch.empty(scr.shape, dtype=torch.float32, device="cuda")
+    d_st = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+    ssp.propagate_host(N, dx, lam, list(dz), h_in, h_out, h_scr, shared, S, 16, 0.47, h_st, 0.5, d_field, d_scr, d_st)
+    assert torch.equal(h_out, ref_dev.cpu())
+    for a, b in zip(api.stats_to_dicts(h_st), api.stats_to_dicts(stats)):   # fp64 atomics: order-dependent last bits
+        for k in ("power", "w2", "sxx", "syy", "roi_sumI", "roi_sumI2", "I_axis"):
+            assert abs(a[k] / b[k] - 1) < 1e-12, (k, a[k], b[k])
+        assert a["roi_n"] == b["roi_n"]
+    ref = orc.propagate(N, dx, lam, dz, u0[-1:], scr if shared else scr[-1:], shared_screens=shared, **kw)
+    assert rel_l2(h_out[-1:].numpy(), ref).max() < tol(N, S)
