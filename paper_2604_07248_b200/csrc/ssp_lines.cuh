@@ -26,7 +26,10 @@ struct RowTune<1024> {
     static constexpr int MIN_BLOCKS = 3;
 };
 template <>
-struct RowTune<2048> : RowTune<1024> {};
+struct RowTune<2048> {
+    static constexpr int MAX_THREADS = 64;
+    static constexpr int MIN_BLOCKS = 6;
+};
 template <>
 struct RowTune<4096> : RowTune<1024> {};
 
