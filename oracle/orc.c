@@ -167,6 +167,24 @@ double orc_psd_f(const orc_psd_t *psd, double lambda, double cn2, double dz, dou
         double twopi = 2.0 * M_PI;
         return twopi * twopi * twopi * k * k * dz * nikishov_phi_n(psd, twopi * f);
     }
+    if (psd->kind == ORC_PSD_POWER_LAW) {
+        /* General power-law medium (PAPER.md:331 S12, Table S1): Phi_n(kappa) = A kappa^-alpha, with the
+         * same optional outer / inner scale roll-offs as S17:
+         *   Phi_n = A (kappa^2 + kappa0^2)^(-alpha/2) exp(-kappa^2/kappam^2),
+         * kappa0 = 2 pi/L0 (L0 <= 0: none), kappam = km_coeff/l0 (l0 <= 0: none); projected like the ocean
+         * spectrum: Phi^f(f) = (2 pi)^3 k^2 dz Phi_n(2 pi f) (PAPER.md:346 S14).  cn2 is not used. */
+        double k = 2.0 * M_PI / lambda;
+        double twopi = 2.0 * M_PI;
+        double kap = twopi * f;
+        double kap0 = (psd->L0 > 0.0) ? twopi / psd->L0 : 0.0;
+        double phin = psd->A * pow(kap * kap + kap0 * kap0, -0.5 * psd->alpha);
+        if (psd->l0 > 0.0) {
+            double kmc = (psd->km_coeff > 0.0) ? psd->km_coeff : 2.0 * M_PI;
+            double kapm = kmc / psd->l0;
+            phin *= exp(-(kap * kap) / (kapm * kapm));
+        }
+        return twopi * twopi * twopi * k * k * dz * phin;
+    }
     return 0.0;
 }
 
@@ -633,6 +651,20 @@ int orc_dft2_centered(int N, int B, int inverse, const double *in, double *out)
 }
 
 /* grad = Im(g conj(u)) per pixel, summed over nothing (one map per batch entry). */
+int orc_aperture(int N, int B, long long r2max_px, const double *in, double *out)
+{
+    for (int b = 0; b < B; ++b)
+        for (int iy = 0; iy < N; ++iy)
+            for (int ix = 0; ix < N; ++ix) {
+                long long x = ix - N / 2, y = iy - N / 2;
+                size_t i = ((size_t)b * N + iy) * N + ix;
+                int inside = (x * x + y * y <= r2max_px);
+                out[2 * i] = inside ? in[2 * i] : 0.0;
+                out[2 * i + 1] = inside ? in[2 * i + 1] : 0.0;
+            }
+    return 0;
+}
+
 int orc_phase_grad(int N, int B, const double *g, const double *u, double *grad)
 {
     size_t n = (size_t)B * N * N;

@@ -34,7 +34,7 @@
 extern "C" {
 #endif
 
-enum { ORC_PSD_KOLMOGOROV = 0, ORC_PSD_VON_KARMAN = 1, ORC_PSD_OCEAN_NIKISHOV = 2 };
+enum { ORC_PSD_KOLMOGOROV = 0, ORC_PSD_VON_KARMAN = 1, ORC_PSD_OCEAN_NIKISHOV = 2, ORC_PSD_POWER_LAW = 3 };
 enum { ORC_H_FRESNEL = 0, ORC_H_ANGULAR_SPECTRUM = 1 };
 
 typedef struct {
@@ -42,6 +42,7 @@ typedef struct {
     double L0, l0;       /* outer / inner scale [m]; von Karman only */
     double km_coeff;     /* kappa_m = km_coeff / l0 ; <=0 -> 2 pi */
     double chi_T, eps, w, eta; /* ocean: eta<=0 -> (nu^3/eps)^(1/4), nu = 1e-6 */
+    double alpha, A;     /* power law (PAPER.md:331 S12, Table S1): Phi_n = A kappa^-alpha */
 } orc_psd_t;
 
 typedef struct {
@@ -95,6 +96,9 @@ int orc_welford(int N, int B, const double *field, double *mean, double *M2, lon
 int orc_phase_mul(int N, int B, const double *theta, double sign, const double *in, double *out);
 int orc_dft2_centered(int N, int B, int inverse, const double *in, double *out);
 int orc_phase_grad(int N, int B, const double *g, const double *u, double *grad);
+/* Circular receiver aperture: out = in where (ix-N/2)^2 + (iy-N/2)^2 <= r2max_px, else 0.
+ * r2max_px = floor((radius/dx)^2) is decided by the caller in double (an integer decision). */
+int orc_aperture(int N, int B, long long r2max_px, const double *in, double *out);
 
 #ifdef __cplusplus
 }

@@ -20,14 +20,14 @@ _SO = os.path.join(_HERE, "liborc.so")
 _SRC = os.path.join(_HERE, "orc.c")
 _HDR = os.path.join(_HERE, "orc.h")
 
-PSD_KOLMOGOROV, PSD_VON_KARMAN, PSD_OCEAN_NIKISHOV = 0, 1, 2
+PSD_KOLMOGOROV, PSD_VON_KARMAN, PSD_OCEAN_NIKISHOV, PSD_POWER_LAW = 0, 1, 2, 3
 H_FRESNEL, H_ANGULAR_SPECTRUM = 0, 1
 
 
 class _Psd(C.Structure):
     _fields_ = [("kind", C.c_int), ("L0", C.c_double), ("l0", C.c_double),
                 ("km_coeff", C.c_double), ("chi_T", C.c_double), ("eps", C.c_double),
-                ("w", C.c_double), ("eta", C.c_double)]
+                ("w", C.c_double), ("eta", C.c_double), ("alpha", C.c_double), ("A", C.c_double)]
 
 
 class _Stats(C.Structure):
@@ -46,9 +46,12 @@ class Psd:
     eps: float = 0.0
     w: float = 0.0
     eta: float = 0.0
+    alpha: float = 0.0
+    A: float = 0.0
 
     def c(self) -> _Psd:
-        return _Psd(self.kind, self.L0, self.l0, self.km_coeff, self.chi_T, self.eps, self.w, self.eta)
+        return _Psd(self.kind, self.L0, self.l0, self.km_coeff, self.chi_T, self.eps, self.w, self.eta,
+                    self.alpha, self.A)
 
 
 def build(force: bool = False) -> str:
@@ -265,6 +268,15 @@ def dft2_centered(N, field, inverse=False):
     out = np.empty_like(field)
     _chk(lib().orc_dft2_centered(C.c_int(N), C.c_int(field.shape[0]), C.c_int(int(inverse)),
                                  _p(field), _p(out)), "dft2_centered")
+    return out
+
+
+def aperture(N, dx, radius, field):
+    """Circular aperture of `radius` metres; the integer threshold floor((radius/dx)^2) is taken here in double."""
+    field = _c128(field)
+    out = np.empty_like(field)
+    r2 = int(np.floor((radius / dx) ** 2))
+    _chk(lib().orc_aperture(C.c_int(N), C.c_int(field.shape[0]), C.c_longlong(r2), _p(field), _p(out)), "aperture")
     return out
 
 

@@ -18,7 +18,7 @@ from typing import Optional
 
 import numpy as np
 
-PSD_KOLMOGOROV, PSD_VON_KARMAN, PSD_OCEAN_NIKISHOV = 0, 1, 2
+PSD_KOLMOGOROV, PSD_VON_KARMAN, PSD_OCEAN_NIKISHOV, PSD_POWER_LAW = 0, 1, 2, 3
 
 
 @dataclass(frozen=True)

@@ -242,3 +242,20 @@ def test_centered_dft_and_mask_helpers(orc):
     np.testing.assert_allclose(orc.phase_mul(N, th, u, sign=-1.0), u * np.exp(-1j * th), atol=1e-13)
     v = synth.random_field(N, 2, 12).astype(np.complex128)
     np.testing.assert_allclose(orc.phase_grad(N, u, v), np.imag(u * np.conj(v)), atol=1e-13)
+
+
+def test_circular_aperture(orc):
+    """the receiver aperture.  Pixel count -> disc area, Gaussian energy fraction 1 - exp(-2 R^2/w^2),
+    idempotent, nothing but 0 or the input."""
+    N, dx, w0, R = 256, 1e-3, 3e-2, 4.05e-2
+    u = synth.gaussian_beam(N, dx, w0, 2).astype(np.complex128) * (1 + 0.5j)
+    out = orc.aperture(N, dx, R, u)
+    inside = np.abs(out[0]) > 0
+    assert abs(inside.sum() * dx * dx / (np.pi * R * R) - 1) < 2 * dx / R          # perimeter-cell bound
+    frac = np.sum(np.abs(out[0]) ** 2) / np.sum(np.abs(u[0]) ** 2)
+    assert abs(frac - (1 - np.exp(-2 * R * R / (w0 * w0)))) < 2e-3
+    np.testing.assert_array_equal(orc.aperture(N, dx, R, out), out)
+    np.testing.assert_array_equal(out[inside[None].repeat(2, 0)], u[inside[None].repeat(2, 0)])
+    x = synth.coords(N, dx)
+    r2 = x[None, :] ** 2 + x[:, None] ** 2
+    assert inside[r2 < (R - dx) ** 2].all() and not inside[r2 > (R + dx) ** 2].any()

@@ -142,3 +142,60 @@ def test_single_frequency_noise_returns_one_sinusoid(orc):
     noise[0, 0, 0, 0] = (3.0, 4.0)
     scr, _, _ = orc.make_screens(N, dx, psd, LAM, [CN2], [DZ], 0, noise, None)
     assert np.all(scr == 0.0)
+
+
+# ---- general power-law media (PAPER.md:331 S12, Table S1) -------------------------------------------------
+def _closed_form_D(K, alpha, r):
+    """D(r) of Phi^f(f) = K f^-alpha (2 < alpha < 4): 4 pi K (2 pi r)^(alpha-2) int_0^inf x^(1-alpha) (1 - J0(x)) dx,
+    with int_0^inf x^-p (1 - J0(x)) dx = pi / (2^p Gamma((p+1)/2)^2 sin(pi (p-1)/2)), p = alpha - 1."""
+    p = alpha - 1.0
+    integral = np.pi / (2.0 ** p * special.gamma((p + 1) / 2) ** 2 * np.sin(np.pi * (p - 1) / 2))
+    return 4 * np.pi * K * (2 * np.pi * r) ** (alpha - 2) * integral
+
+
+def test_closed_form_reproduces_688_law():
+    """The closed form used below, fed the Kolmogorov constants, is the 6.88 law (an independent check of it)."""
+    c = paper_constants()
+    r0 = 0.1
+    D = _closed_form_D(c["psd_const"] * r0 ** (-5 / 3), 11 / 3, 0.05)
+    assert abs(D / (c["structure_const"] * (0.05 / r0) ** (5 / 3)) - 1) < 0.01
+
+
+@pytest.mark.parametrize("alpha", [3.5, 11 / 3, 3.9])
+def test_power_law_psd_structure_function(orc, alpha):
+    """kind = POWER_LAW: Phi^f(f) = (2 pi)^3 k^2 dz A (2 pi f)^-alpha; its structure function by direct Hankel
+    integration equals the closed form C r^(alpha-2) (Table S1: beta + 1 = alpha - 2)."""
+    A = 3.3e-16
+    psd = orc.Psd(kind=orc.PSD_POWER_LAW, alpha=alpha, A=A)
+    k = 2 * np.pi / LAM
+    K = (2 * np.pi) ** (3 - alpha) * k * k * DZ * A
+    f = np.array([0.7, 13.0])
+    np.testing.assert_allclose(orc.psd_f(psd, LAM, 0.0, DZ, f), K * f ** (-alpha), rtol=1e-13)
+    r = 0.05
+
+    def g(x):                                                  # x = 2 pi f r
+        ff = x / (2 * np.pi * r)
+        return 4 * np.pi * orc.psd_f(psd, LAM, 0.0, DZ, ff)[0] * (1.0 - special.j0(x)) * ff / (2 * np.pi * r)
+    # head x < 1e-2 from the series 1 - J0(x) = x^2/4 - x^4/64 (the integrand ~ x^(3-alpha) converges slowly at 0)
+    x0 = 1e-2
+    total = 4 * np.pi * K * (2 * np.pi * r) ** (alpha - 2) * (x0 ** (4 - alpha) / (4 * (4 - alpha)) - x0 ** (6 - alpha) / (64 * (6 - alpha)))
+    edges = np.concatenate([[x0], np.arange(0.5, 400.5, 1.0) * np.pi])
+    for a, b in zip(edges[:-1], edges[1:]):
+        total += integrate.quad(g, a, b, limit=200)[0]
+    X = edges[-1]                                              # tail: the J0 term averages out
+    total += 4 * np.pi * K * (2 * np.pi * r) ** (alpha - 2) * X ** (2 - alpha) / (alpha - 2)
+    assert abs(total / _closed_form_D(K, alpha, r) - 1) < 5e-3
+
+
+def test_power_law_reduces_to_the_atmospheric_kinds(orc):
+    """alpha = 11/3, A = 0.033 Cn2 is Kolmogorov / von Karman up to the printed constants: 0.033 (2 pi)^(-2/3) against
+    0.023 x 0.423 (0.4 % apart, Q24), with the same outer / inner scale roll-offs."""
+    f = np.array([0.05, 0.5, 5.0, 50.0, 400.0])
+    ratio = 0.033 * (2 * np.pi) ** (-2 / 3) / (0.023 * 0.423)
+    assert abs(ratio - 1) < 5e-3
+    pl = orc.Psd(kind=orc.PSD_POWER_LAW, alpha=11 / 3, A=0.033 * CN2)
+    np.testing.assert_allclose(orc.psd_f(pl, LAM, 0.0, DZ, f) / orc.psd_f(orc.Psd(kind=orc.PSD_KOLMOGOROV), LAM, CN2, DZ, f),
+                               ratio, rtol=1e-12)
+    pl = orc.Psd(kind=orc.PSD_POWER_LAW, alpha=11 / 3, A=0.033 * CN2, L0=10.0, l0=5e-3)
+    vk = orc.Psd(kind=orc.PSD_VON_KARMAN, L0=10.0, l0=5e-3)
+    np.testing.assert_allclose(orc.psd_f(pl, LAM, 0.0, DZ, f) / orc.psd_f(vk, LAM, CN2, DZ, f), ratio, rtol=1e-12)
