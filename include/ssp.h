@@ -49,7 +49,8 @@ typedef struct { int N; double dx; } ssp_grid;
 typedef enum {
     SSP_PSD_KOLMOGOROV = 0,     /* Table S1: S17 with L0 -> inf, l0 -> 0 (Q23) */
     SSP_PSD_VON_KARMAN = 1,     /* modified von Karman, PAPER.md:370 (S17) */
-    SSP_PSD_OCEAN_NIKISHOV = 2  /* Nikishov oceanic spectrum, open literature (Q20) */
+    SSP_PSD_OCEAN_NIKISHOV = 2, /* Nikishov oceanic spectrum, open literature (Q20) */
+    SSP_PSD_POWER_LAW = 3       /* general power-law medium, PAPER.md:331 (S12), Table S1 */
 } ssp_psd_kind;
 
 /* Phase PSD parameters.  Atmospheric kinds evaluate S17 with f in cycles/m:
@@ -57,11 +58,15 @@ typedef enum {
  *   f0 = 1/L0, fm = km_coeff/(2 pi l0) (km_coeff <= 0 -> 2 pi; Q4, Q5),
  *   r0 = (0.423 k^2 Cn2 dz)^(-3/5), k = 2 pi/lambda (PAPER.md:375 S18; Q16).
  * Ocean: Phi^f(f) = (2 pi)^3 k^2 dz Phi_n(2 pi f) with Nikishov's Phi_n; cn2 is ignored;
- *   eta <= 0 -> (nu^3/eps)^(1/4), nu = 1e-6 m^2/s. */
+ *   eta <= 0 -> (nu^3/eps)^(1/4), nu = 1e-6 m^2/s.
+ * Power law: Phi_n(kappa) = A (kappa^2 + kappa0^2)^(-alpha/2) exp(-kappa^2/kappam^2), 3 <= alpha < 5,
+ *   kappa0 = 2 pi/L0 (L0 <= 0: none), kappam = km_coeff/l0 (l0 <= 0: none), projected like the ocean
+ *   spectrum; cn2 is ignored.  alpha = 11/3, A = 0.033 Cn2 is the atmospheric case. */
 typedef struct {
     int kind;                  /* ssp_psd_kind */
-    double L0, l0, km_coeff;   /* von Karman */
+    double L0, l0, km_coeff;   /* von Karman, power law */
     double chi_T, eps, w, eta; /* ocean */
+    double alpha, A;           /* power law */
 } ssp_psd;
 
 /* Super-Gaussian absorbing window applied after every split step (north_star; Q12):
@@ -204,6 +209,10 @@ int ssp_phase_mul(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_theta, doub
 int ssp_dft2_centered(ssp_ctx *ctx, ssp_grid grid, int B, int inverse,
                       const float *d_in, float *d_out, void *d_ws, size_t ws_bytes);
 /* grad[b] = Im(g[b] conj(u[b])), dev fp32 [B][N][N]. */
+/* Circular aperture of `radius` metres about the grid centre: out = in where
+ * (ix-N/2)^2 + (iy-N/2)^2 <= floor((radius/dx)^2) (the threshold is an integer taken on the host in
+ * double), else 0.  d_in / d_out: dev complex64 [B][N][N]; may alias. */
+int ssp_aperture(ssp_ctx *ctx, ssp_grid grid, int B, double radius, const float *d_in, float *d_out);
 int ssp_phase_grad(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_g, const float *d_u,
                    float *d_grad);
 /* Per field b: d_out[b] = { Re <a,b>, Im <a,b>, sum |a|^2, sum |b|^2 } (doubles),

@@ -18,7 +18,7 @@ import torch
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libssp.so")
 
-PSD_KOLMOGOROV, PSD_VON_KARMAN, PSD_OCEAN_NIKISHOV = 0, 1, 2
+PSD_KOLMOGOROV, PSD_VON_KARMAN, PSD_OCEAN_NIKISHOV, PSD_POWER_LAW = 0, 1, 2, 3
 H_FRESNEL, H_ANGULAR_SPECTRUM = 0, 1
 OK, EINVAL, EUNSUPPORTED, EWORKSPACE, ECUDA = 0, -1, -2, -3, -4
 
@@ -27,7 +27,7 @@ SYMBOLS = (
     "ssp_create", "ssp_destroy", "ssp_last_error", "ssp_version", "ssp_launch_count",
     "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_propagate",
     "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_propagate_host", "ssp_phase_mul",
-    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb",
+    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture",
     "ssp_profile_enable", "ssp_profile_report",
 )
 
@@ -44,7 +44,8 @@ class Grid(C.Structure):
 
 class Psd(C.Structure):
     _fields_ = [("kind", C.c_int), ("L0", C.c_double), ("l0", C.c_double), ("km_coeff", C.c_double),
-                ("chi_T", C.c_double), ("eps", C.c_double), ("w", C.c_double), ("eta", C.c_double)]
+                ("chi_T", C.c_double), ("eps", C.c_double), ("w", C.c_double), ("eta", C.c_double),
+                ("alpha", C.c_double), ("A", C.c_double)]
 
 
 class Window(C.Structure):
@@ -92,6 +93,7 @@ def load():
     lib.ssp_phase_mul.argtypes = [P, Grid, I, P, D, P, P]
     lib.ssp_dft2_centered.argtypes = [P, Grid, I, I, P, P, P, C.c_size_t]
     lib.ssp_phase_grad.argtypes = [P, Grid, I, P, P, P]
+    lib.ssp_aperture.argtypes = [P, Grid, I, D, P, P]
     lib.ssp_inner_products.argtypes = [P, Grid, I, P, P, P]
     lib.ssp_lincomb.argtypes = [P, Grid, I, P, P, P, P, P]
     lib.ssp_profile_enable.argtypes = [P, I]
@@ -136,9 +138,12 @@ class PsdParams:
     eps: float = 0.0
     w: float = 0.0
     eta: float = 0.0
+    alpha: float = 0.0
+    A: float = 0.0
 
     def c(self) -> Psd:
-        return Psd(self.kind, self.L0, self.l0, self.km_coeff, self.chi_T, self.eps, self.w, self.eta)
+        return Psd(self.kind, self.L0, self.l0, self.km_coeff, self.chi_T, self.eps, self.w, self.eta,
+                   self.alpha, self.A)
 
 
 class Context:
@@ -301,6 +306,12 @@ class Context:
         out = torch.empty_like(field) if out is None else out
         self._chk(self._lib.ssp_dft2_centered(self._h, Grid(N, dx), field.shape[0], int(inverse),
                                               _dev(field, torch.complex64), _dev(out, torch.complex64), None, 0))
+        return out
+
+    def aperture(self, N, dx, radius, field, out=None):
+        out = torch.empty_like(field) if out is None else out
+        self._chk(self._lib.ssp_aperture(self._h, Grid(N, dx), field.shape[0], float(radius),
+                                         _dev(field, torch.complex64), _dev(out, torch.complex64)))
         return out
 
     def phase_grad(self, N, dx, g, u, out=None):

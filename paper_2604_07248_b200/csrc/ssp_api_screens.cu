@@ -58,6 +58,10 @@ double psd_scalar_sqrt(const ssp_psd *psd, double lambda, double cn2, double dz)
         const double tp = 2.0 * kPi;
         return sqrt(tp * tp * tp * k * k * dz * 0.388e-8 * pow(psd->eps, -1.0 / 3.0) * psd->chi_T / (psd->w * psd->w));
     }
+    if (psd->kind == SSP_PSD_POWER_LAW) { // (2 pi)^3 k^2 dz A (2 pi f)^-alpha: scalar part (PAPER.md:331 S12, :346 S14)
+        const double tp = 2.0 * kPi;
+        return sqrt(pow(tp, 3.0 - psd->alpha) * k * k * dz * psd->A);
+    }
     const double r0 = pow(0.423 * k * k * cn2 * dz, -3.0 / 5.0); // PAPER.md:375 (S18)
     return sqrt(0.023) * pow(r0, -5.0 / 6.0);                     // PAPER.md:370 (S17)
 }
@@ -75,13 +79,16 @@ double psd_shape_sqrt_host(const ssp_psd *psd, double f)
         return sqrt(pow(kap, -11.0 / 3.0) * (1.0 + 2.35 * pow(ke, 2.0 / 3.0)) * (br > 0 ? br : 0));
     }
     double f0 = 0, inv_fm2 = 0;
-    if (psd->kind == SSP_PSD_VON_KARMAN) {
-        f0 = 1.0 / psd->L0;
-        const double kmc = psd->km_coeff > 0 ? psd->km_coeff : 2.0 * kPi;
-        const double fm = kmc / (2.0 * kPi * psd->l0);
-        inv_fm2 = 1.0 / (fm * fm);
+    const bool pl = (psd->kind == SSP_PSD_POWER_LAW);
+    if (psd->kind == SSP_PSD_VON_KARMAN || pl) {
+        if (psd->L0 > 0) f0 = 1.0 / psd->L0;
+        if (psd->l0 > 0) {
+            const double kmc = psd->km_coeff > 0 ? psd->km_coeff : 2.0 * kPi;
+            const double fm = kmc / (2.0 * kPi * psd->l0);
+            inv_fm2 = 1.0 / (fm * fm);
+        }
     }
-    return exp(-0.5 * f * f * inv_fm2) * pow(f * f + f0 * f0, -11.0 / 12.0);
+    return exp(-0.5 * f * f * inv_fm2) * pow(f * f + f0 * f0, pl ? -0.25 * psd->alpha : -11.0 / 12.0);
 }
 
 int check_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, int B, int S,
@@ -93,14 +100,16 @@ int check_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda
     if (!(grid.dx > 0) || !(lambda > 0)) return ctx->fail(SSP_EINVAL, "dx and lambda must be > 0");
     if (!psd || B < 1 || S < 1 || !cn2 || !dz) return ctx->fail(SSP_EINVAL, "psd, B >= 1, S >= 1, cn2, dz are required");
     if (n_sh < 0 || n_sh > kMaxSh) return ctx->fail(SSP_EINVAL, "n_sh must be in [0, %d]", kMaxSh);
-    if (psd->kind < 0 || psd->kind > SSP_PSD_OCEAN_NIKISHOV) return ctx->fail(SSP_EINVAL, "unknown PSD kind %d", psd->kind);
+    if (psd->kind < 0 || psd->kind > SSP_PSD_POWER_LAW) return ctx->fail(SSP_EINVAL, "unknown PSD kind %d", psd->kind);
+    if (psd->kind == SSP_PSD_POWER_LAW && (!(psd->alpha >= 3.0 && psd->alpha < 5.0) || !(psd->A >= 0)))
+        return ctx->fail(SSP_EINVAL, "power-law PSD needs 3 <= alpha < 5 and A >= 0");
     if (psd->kind == SSP_PSD_VON_KARMAN && (!(psd->L0 > 0) || !(psd->l0 > 0)))
         return ctx->fail(SSP_EINVAL, "von Karman needs L0 > 0 and l0 > 0");
     if (psd->kind == SSP_PSD_OCEAN_NIKISHOV && (!(psd->eps > 0) || !(psd->chi_T > 0) || psd->w == 0))
         return ctx->fail(SSP_EINVAL, "ocean PSD needs eps > 0, chi_T > 0, w != 0");
     for (int s = 0; s < S; ++s) {
         if (!(dz[s] > 0)) return ctx->fail(SSP_EINVAL, "dz[%d] must be > 0", s);
-        if (psd->kind != SSP_PSD_OCEAN_NIKISHOV && !(cn2[s] >= 0)) return ctx->fail(SSP_EINVAL, "cn2[%d] must be >= 0", s);
+        if (psd->kind <= SSP_PSD_VON_KARMAN && !(cn2[s] >= 0)) return ctx->fail(SSP_EINVAL, "cn2[%d] must be >= 0", s);
     }
     if (!noise || !screens) return ctx->fail(SSP_EINVAL, "noise and screens pointers are required");
     if (n_sh > 0 && !noise_sh) return ctx->fail(SSP_EINVAL, "noise_sh is required when n_sh > 0");
@@ -207,11 +216,14 @@ int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
     flt.kind = psd->kind;
     flt.df = (float)df;
     flt.two_pi = (float)(2.0 * kPi);
-    if (psd->kind == SSP_PSD_VON_KARMAN) {
-        const double kmc = psd->km_coeff > 0 ? psd->km_coeff : 2.0 * kPi;
-        const double fm = kmc / (2.0 * kPi * psd->l0);
-        flt.f0sq = (float)(1.0 / (psd->L0 * psd->L0));
-        flt.inv_fm2_log2e = (float)(1.4426950408889634 / (2.0 * fm * fm));
+    flt.pexp = (psd->kind == SSP_PSD_POWER_LAW) ? (float)(0.25 * psd->alpha) : (float)(11.0 / 12.0);
+    if (psd->kind == SSP_PSD_VON_KARMAN || psd->kind == SSP_PSD_POWER_LAW) {
+        if (psd->L0 > 0) flt.f0sq = (float)(1.0 / (psd->L0 * psd->L0));
+        if (psd->l0 > 0) {
+            const double kmc = psd->km_coeff > 0 ? psd->km_coeff : 2.0 * kPi;
+            const double fm = kmc / (2.0 * kPi * psd->l0);
+            flt.inv_fm2_log2e = (float)(1.4426950408889634 / (2.0 * fm * fm));
+        }
     } else if (psd->kind == SSP_PSD_OCEAN_NIKISHOV) {
         flt.eta = (float)(psd->eta > 0 ? psd->eta : pow(1e-18 / psd->eps, 0.25));
         flt.w = (float)psd->w;
@@ -319,6 +331,17 @@ int ssp_dft2_centered(ssp_ctx *ctx, ssp_grid grid, int B, int inverse,
     ColArgs c{};
     c.in = r.out; c.out = r.out; c.B = B; c.hy = sg + N; c.tw = twc;
     return launch_col_single(ctx, N, inverse != 0, c);
+}
+
+int ssp_aperture(ssp_ctx *ctx, ssp_grid grid, int B, double radius, const float *d_in, float *d_out)
+{
+    if (!ctx) return SSP_EINVAL;
+    if (!valid_N(grid.N) || !(grid.dx > 0) || B < 1 || !(radius >= 0) || !d_in || !d_out)
+        return ctx->fail(SSP_EINVAL, "bad arguments");
+    SSP_CUDA(ctx, cudaSetDevice(ctx->device));
+    const double q = radius / grid.dx;
+    return launch_aperture(ctx, grid.N, B, (long long)floor(q * q), reinterpret_cast<const float2 *>(d_in),
+                           reinterpret_cast<float2 *>(d_out));
 }
 
 int ssp_phase_grad(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_g, const float *d_u, float *d_grad)

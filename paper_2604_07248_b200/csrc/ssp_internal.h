@@ -155,6 +155,7 @@ int launch_col_single(ssp_ctx *ctx, int N, bool inverse, const ColArgs &a);
 // ---- screens (ssp_screens.cu) ------------------------------------------------------
 struct ScreenFilter {
     int kind;
+    float pexp;          // (f^2 + f0^2)^(-pexp): 11/12 atmospheric, alpha/4 power law
     float f0sq;          // von Karman: 1/L0^2 (0 for Kolmogorov)
     float inv_fm2_log2e; // von Karman: log2(e) / (2 fm^2)   (0 when l0 == 0)
     float df;            // 1/(N dx)
@@ -200,6 +201,7 @@ int launch_welford(ssp_ctx *ctx, int N, int B, const float2 *field, float *mean,
                    long long count0);
 int launch_h2d_table(ssp_ctx *ctx, int N, int C, double dx, double lam_eff, double dz, int conj, float2 *out);
 int col_tile_width(int N);     // columns per tile of the kernel launch_col_prop picks for N (layout of the H map)
+int launch_aperture(ssp_ctx *ctx, int N, int B, long long r2max_px, const float2 *in, float2 *out);
 int launch_phase_mul(ssp_ctx *ctx, int N, int B, const float *theta, float sign,
                      const float2 *in, float2 *out);
 int launch_phase_grad(ssp_ctx *ctx, long long n, const float2 *g, const float2 *u, float *grad);

@@ -188,6 +188,24 @@ int launch_h2d_table(ssp_ctx *ctx, int N, int C, double dx, double lam_eff, doub
     return SSP_OK;
 }
 
+// circular aperture: integer test against a host-decided threshold
+__global__ void __launch_bounds__(256) k_aperture(int N, long long r2max, const float2 *__restrict__ in, float2 *__restrict__ out)
+{
+    const int ix = blockIdx.x * blockDim.x + threadIdx.x, iy = blockIdx.y, b = blockIdx.z;
+    if (ix >= N) return;
+    const long long x = ix - N / 2, y = iy - N / 2;
+    const size_t i = ((size_t)b * N + iy) * N + ix;
+    out[i] = (x * x + y * y <= r2max) ? in[i] : make_float2(0.f, 0.f);
+}
+
+int launch_aperture(ssp_ctx *ctx, int N, int B, long long r2max_px, const float2 *in, float2 *out)
+{
+    k_aperture<<<dim3((N + 255) / 256, N, B), 256, 0, ctx->stream>>>(N, r2max_px, in, out);
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
 int launch_phase_mul(ssp_ctx *ctx, int N, int B, const float *theta, float sign, const float2 *in, float2 *out)
 {
     const size_t px = (size_t)N * N;

@@ -24,8 +24,8 @@ __device__ __forceinline__ float psd_shape_sqrt_k(const ScreenFilter &f, float f
                          - 2.f * f.w * __expf(-9.41e-3f * delta);
         return exp2f(-1.8333334f * __log2f(kap)) * sqrtf(fmaxf((1.f + 2.35f * ke23) * br, 0.f));
     }
-    // von Karman / Kolmogorov: exp(-f2/(2 fm^2)) (f2 + f0^2)^(-11/12)
-    return exp2f(fmaf(-0.91666667f, __log2f(f2 + f.f0sq), -f2 * f.inv_fm2_log2e));
+    // von Karman / Kolmogorov / power law: exp(-f2/(2 fm^2)) (f2 + f0^2)^(-pexp), pexp = 11/12 or alpha/4
+    return exp2f(fmaf(-f.pexp, __log2f(f2 + f.f0sq), -f2 * f.inv_fm2_log2e));
 }
 __device__ __forceinline__ float psd_shape_sqrt(const ScreenFilter &f, float f2)
 {

@@ -269,3 +269,17 @@ def test_propagate_host_matches_device_path(ssp, orc, B, shared):
         assert a["roi_n"] == b["roi_n"]
     ref = orc.propagate(N, dx, lam, dz, u0[-1:], scr if shared else scr[-1:], shared_screens=shared, **kw)
     assert rel_l2(h_out[-1:].numpy(), ref).max() < tol(N, S)
+
+
+@pytest.mark.parametrize("N", [64, 1024])
+def test_aperture_bit_exact(ssp, orc, N):
+    """Circular aperture: an integer decision, so the mask is compared exactly."""
+    dx, B = 0.34e-3, 2
+    u = synth.random_field(N, B, 70 + N)
+    for R in (0.0, 0.3048 / 2 * N / 1024, 0.37 * N * dx, 10.0):
+        ref = orc.aperture(N, dx, R, u)
+        d = cu(u)
+        out = ssp.aperture(N, dx, R, d)
+        np.testing.assert_array_equal(out.cpu().numpy(), ref.astype(np.complex64))
+        ssp.aperture(N, dx, R, d, out=d)                      # in place
+        np.testing.assert_array_equal(d.cpu().numpy(), ref.astype(np.complex64))

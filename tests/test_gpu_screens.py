@@ -45,10 +45,14 @@ def _psds(orc):
         "von_karman_592": (orc.Psd(kind=1, L0=3.0, l0=1e-2, km_coeff=5.92),
                            api.PsdParams(kind=1, L0=3.0, l0=1e-2, km_coeff=5.92)),
         "ocean": (orc.Psd(kind=2, chi_T=1e-7, eps=1e-5, w=-2.0), api.PsdParams(kind=2, chi_T=1e-7, eps=1e-5, w=-2.0)),
+        # Table S1: biological-tissue exponent, pure power law; and an atmospheric one with both roll-offs
+        "power_law": (orc.Psd(kind=3, alpha=4.3, A=2e-16), api.PsdParams(kind=3, alpha=4.3, A=2e-16)),
+        "power_law_scales": (orc.Psd(kind=3, alpha=3.5, A=4e-16, L0=5.0, l0=8e-3),
+                             api.PsdParams(kind=3, alpha=3.5, A=4e-16, L0=5.0, l0=8e-3)),
     }
 
 
-@pytest.mark.parametrize("kind", ["kolmogorov", "von_karman", "von_karman_592", "ocean"])
+@pytest.mark.parametrize("kind", ["kolmogorov", "von_karman", "von_karman_592", "ocean", "power_law", "power_law_scales"])
 @pytest.mark.parametrize("N,n_sh", [(32, 3), (128, 3), (256, 0), (1024, 4)])
 def test_make_screens_parity(ssp, orc, kind, N, n_sh):
     import torch
