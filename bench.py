@@ -297,8 +297,8 @@ def run_ours(args):
     kernels = {k: {"launches": v["launches"], "ms": round(v["ms"], 4),
                    "GBps": round(v["bytes"] / (v["ms"] * 1e-3) / 1e9, 1)} for k, v in prof.items()}
     # split-step alone: col + row kernels of propagate and adjoint, 36 B/px per screen-step
-    ss_ms = sum(v["ms"] for k, v in prof.items() if k.startswith(("col_fft", "row_")))
-    ss_bytes = sum(v["bytes"] for k, v in prof.items() if k.startswith(("col_fft", "row_")))
+    ss_ms = sum(v["ms"] for k, v in prof.items() if k.startswith(("col_fft", "row_", "small_")))
+    ss_bytes = sum(v["bytes"] for k, v in prof.items() if k.startswith(("col_fft", "row_", "small_")))
     split_step = {"screen_steps_per_s": 2 * B * S * args.steps / (ss_ms * 1e-3) if ss_ms else None,
                   "GBps": ss_bytes / (ss_ms * 1e-3) / 1e9 if ss_ms else None,
                   "frac_of_peak": ss_bytes / (ss_ms * 1e-3) / 1e9 / peak if ss_ms else None}

@@ -47,6 +47,7 @@ int ssp_destroy(ssp_ctx *ctx)
     if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
     if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
     if (ctx->scratch) cudaFree(ctx->scratch);
+    if (ctx->small_steps) cudaFree(ctx->small_steps);
     delete ctx;
     return SSP_OK;
 }
@@ -124,6 +125,32 @@ void fill_window(RowArgs &r, ssp_window win, int N)
     }
 }
 
+// On-chip path (ssp_small.cu): upload the step list and launch one kernel for the whole stack.
+const size_t kSmallStepBytes = 16384;
+
+int run_small(ssp_ctx *ctx, int N, int B, const std::vector<SmallStep> &steps, int n_screens, const RowArgs &win,
+              const float2 *in, float2 *out, const float2 *tw, const float2 *twc)
+{
+    if (!ctx->small_steps) SSP_CUDA(ctx, cudaMalloc(&ctx->small_steps, kSmallStepBytes));
+    // pageable source: staged before cudaMemcpyAsync returns, so the vector may die afterwards
+    SSP_CUDA(ctx, cudaMemcpyAsync(ctx->small_steps, steps.data(), sizeof(SmallStep) * steps.size(), cudaMemcpyHostToDevice,
+                                  ctx->stream));
+    SmallArgs a{};
+    a.in = in; a.out = out;
+    a.n_steps = (int)steps.size() - 1;
+    a.n_screens = n_screens;
+    a.steps = reinterpret_cast<const SmallStep *>(ctx->small_steps);
+    a.win_on = win.win_on; a.win_qs = win.win_qs; a.win_half_order = win.win_half_order;
+    a.tw_row = tw; a.tw_col = twc;
+    return launch_small(ctx, N, B, a);
+}
+
+bool small_ok(int N, int h_kind, int n_steps, const void *planes)
+{
+    return small_path_available(N) && h_kind == SSP_H_FRESNEL && !planes &&
+           sizeof(SmallStep) * (size_t)(n_steps + 1) <= kSmallStepBytes;
+}
+
 } // namespace
 
 extern "C" {
@@ -149,6 +176,23 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
     if (int rc = get_twiddles(ctx, N, 1, &twc)) return rc;
     float2 *u = reinterpret_cast<float2 *>(d_field_out);
 
+    if (small_ok(N, h_kind, n_steps, d_planes)) { // whole stack in one kernel, field resident in shared memory
+        std::vector<SmallStep> ops(n_steps + 1);
+        RowArgs w{};
+        fill_window(w, win, N);
+        for (int j = 0; j <= n_steps; ++j) {
+            SmallStep &o = ops[j];
+            o = SmallStep{};
+            o.first = (j > 0); o.second = (j < n_steps); o.win = (j > 0);
+            if (j >= 1 && j <= S) { o.phi = d_screens + (size_t)(j - 1) * px; o.phi_batch_stride = screen_batch_stride; o.phase_sign = 1.f; }
+            if (j < n_steps) if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j], 0, 0}, &o.hx)) return rc;
+            if (j >= 1) if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j - 1], 0, 1}, &o.hy)) return rc;
+        }
+        if (int rc = run_small(ctx, N, B, ops, S, w, reinterpret_cast<const float2 *>(d_field_in), u, tw, twc)) return rc;
+        if (d_stats)
+            if (int rc = launch_stats(ctx, N, grid.dx, B, u, roi_frac, d_stats)) return rc;
+        return SSP_OK;
+    }
     // Fresnel: H = hx[kx] hy[ky], hx applied by the row kernels, hy by the column kernel.
     // Angular spectrum: H(ky,kx) is not separable; the column kernel applies the whole map, the rows none.
     const bool as = (h_kind == SSP_H_ANGULAR_SPECTRUM);
@@ -220,6 +264,21 @@ int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0,
     if (int rc = get_twiddles(ctx, N, 1, &twc)) return rc;
     float2 *g = reinterpret_cast<float2 *>(d_g_in);
 
+    if (small_ok(N, h_kind, n_steps, d_planes)) { // on-chip: op 0 = plane n_steps, then (column pass, plane j-1) for j = n_steps..1
+        std::vector<SmallStep> ops(n_steps + 1);
+        RowArgs w{};
+        fill_window(w, win, N);
+        for (int i = 0; i <= n_steps; ++i) {
+            const int plane = n_steps - i;                       // the plane whose pointwise stage this row pass applies
+            SmallStep &o = ops[i];
+            o = SmallStep{};
+            o.first = (i > 0); o.second = (plane >= 1); o.win = (plane >= 1);
+            if (plane >= 1 && plane <= S) { o.phi = d_screens + (size_t)(plane - 1) * px; o.phi_batch_stride = screen_batch_stride; o.phase_sign = -1.f; }
+            if (plane >= 1) if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[plane - 1], 1, 0}, &o.hx)) return rc;
+            if (i >= 1) if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[plane], 1, 1}, &o.hy)) return rc;
+        }
+        return run_small(ctx, N, B, ops, S, w, reinterpret_cast<const float2 *>(d_g_out), g, tw, twc);
+    }
     // pointwise stage of plane j: [grad_j] ; g <- W exp(-i phi_j) g
     auto plane_stage = [&](RowArgs &r, int j) {
         if (j <= S) {

@@ -45,6 +45,7 @@ struct ssp_ctx {
     size_t scratch_bytes = 0;
     std::vector<void *> owned;                   // misc device allocations freed at destroy
     void *encode_tiled = nullptr;                // cuTensorMapEncodeTiled, resolved through the runtime
+    void *small_steps = nullptr;                 // device list of step descriptors of the on-chip path (16 KB)
     // ssp_propagate_host: copy streams and events of the chunked host <-> device pipeline (created on first use)
     cudaStream_t copy_in = nullptr, copy_out = nullptr;
     std::vector<cudaEvent_t> pipe_events;
@@ -151,6 +152,29 @@ int launch_row(ssp_ctx *ctx, int N, bool first, bool second, const RowArgs &a);
 int launch_col_prop(ssp_ctx *ctx, int N, const ColArgs &a);
 // single column transform (inverse != 0: unnormalised inverse) followed by * hy.
 int launch_col_single(ssp_ctx *ctx, int N, bool inverse, const ColArgs &a);
+
+// ---- on-chip path for small grids (ssp_small.cu) -----------------------------------------
+struct SmallStep {               // one row pass, preceded (except op 0) by the column pass with hy
+    const float *phi;            // screen of field 0 for this row pass, or null
+    long long phi_batch_stride;
+    float phase_sign;
+    int first, second;           // inverse transform before / forward transform after the pointwise stage
+    int win;                     // apply the window in this row pass
+    const float2 *hx;            // multiplier after the forward transform, or null
+    const float2 *hy;            // multiplier of the column pass before this row pass (op > 0)
+};
+struct SmallArgs {
+    const float2 *in;
+    float2 *out;
+    int n_steps;                 // column passes; row passes = n_steps + 1
+    int n_screens;               // bookkeeping (algorithmic bytes)
+    const SmallStep *steps;      // device [n_steps + 1]
+    int win_on;
+    float win_qs, win_half_order;
+    const float2 *tw_row, *tw_col;
+};
+bool small_path_available(int N);
+int launch_small(ssp_ctx *ctx, int N, int B, const SmallArgs &a);
 
 // ---- screens (ssp_screens.cu) ------------------------------------------------------
 struct ScreenFilter {

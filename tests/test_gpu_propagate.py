@@ -283,3 +283,27 @@ def test_aperture_bit_exact(ssp, orc, N):
         np.testing.assert_array_equal(out.cpu().numpy(), ref.astype(np.complex64))
         ssp.aperture(N, dx, R, d, out=d)                      # in place
         np.testing.assert_array_equal(d.cpu().numpy(), ref.astype(np.complex64))
+
+
+@pytest.mark.parametrize("N", [64, 128])
+def test_on_chip_path_matches_multi_kernel_path(ssp, orc, N):
+    """N <= 128 without saved planes runs the whole stack in one CTA per field (ssp_small.cu); with planes the
+    row / column kernels run.  Same transforms, same tables: the two agree to fp32 rounding, and one launch
+    replaces 2 n_steps + 1."""
+    import torch
+    B, n_steps, S = 5, 6, 5
+    dx, lam, dz, u0, scr = _case(N, B, n_steps, S, 200 + N)
+    kw = dict(win_order=16, win_sigma_frac=0.47)
+    l0 = ssp.launch_count()
+    out = ssp.propagate(N, dx, lam, list(dz), cu(u0), cu(scr), **kw)
+    assert ssp.launch_count() - l0 == 1
+    planes = torch.empty((B, n_steps, N, N), dtype=torch.complex64, device="cuda")
+    out_mk = ssp.propagate(N, dx, lam, list(dz), cu(u0), cu(scr), planes=planes, **kw)
+    assert ssp.launch_count() - l0 == 1 + 2 * n_steps + 1
+    assert rel_l2(out.cpu().numpy(), out_mk.cpu().numpy().astype(np.complex128)).max() < 1e-6
+    ref = orc.propagate(N, dx, lam, dz, u0, scr, **kw)
+    assert rel_l2(out.cpu().numpy(), ref).max() < tol(N, S)
+    g = synth.random_field(N, B, 300 + N)
+    gin = ssp.propagate_adjoint(N, dx, lam, list(dz), cu(g), cu(scr), **kw)
+    gref = orc.propagate_adjoint(N, dx, lam, dz, g, scr, **kw)
+    assert rel_l2(gin.cpu().numpy(), gref).max() < tol(N, S)
