@@ -40,6 +40,7 @@ def parse_args():
                     help="transfer function: north_star's Fresnel form (default) or the paper's angular spectrum")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cufft-compare", action="store_true")
     return ap.parse_args()
 
 
@@ -329,6 +330,37 @@ def run_ours(args):
                "h2d_bytes_per_step": int(h_in.numel() * 8 + h_scr.numel() * 4),
                "d2h_bytes_per_step": int(h_out.numel() * 8 + h_st.numel()), "ms_per_step": dt * 1e3}
 
+    # ---- comparison only: the same forward split steps with cuFFT through torch.fft plus
+    # elementwise torch kernels -- the paper's own design -- never on the product path
+    cufft = None
+    if rank == 0 and world == 1 and not args.no_cufft_compare:
+        import math
+        fx = torch.fft.fftfreq(N, d=wl.dx, device=dev, dtype=torch.float64)
+        H = torch.exp(-1j * math.pi * wl.lam * dz[0] * (fx[None, :] ** 2 + fx[:, None] ** 2)).to(torch.complex64)
+        xc = (torch.arange(N, device=dev, dtype=torch.float64) - N // 2) * wl.dx
+        sig = wl.win_sigma_frac * N * wl.dx
+        W = torch.exp(-(((xc[None, :] ** 2 + xc[:, None] ** 2) / sig ** 2) ** (wl.win_order / 2))).to(torch.float32)
+        def torch_forward():
+            u = u0
+            for j in range(S):
+                u = torch.fft.ifft2(torch.fft.fft2(u) * H)
+                u = u * torch.polar(W.expand(B, N, N), screens[:, j])
+            return u
+        torch_forward()
+        torch.cuda.synchronize()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n_rep = 3
+        c0.record()
+        for _ in range(n_rep):
+            torch_forward()
+        c1.record()
+        torch.cuda.synchronize()
+        ms = c0.elapsed_time(c1) / n_rep
+        ours_fwd = sum(v["ms"] for k, v in prof.items() if k.startswith(("col_fft", "row_", "small_"))) / args.steps / 2
+        cufft = {"what": "forward split steps with torch.fft (cuFFT) + elementwise torch kernels, same batch; comparison only",
+                 "screen_steps_per_s": B * S / (ms * 1e-3), "ms_per_forward": ms,
+                 "ours_ms_per_forward": ours_fwd, "speedup": ms / ours_fwd if ours_fwd else None}
+
     # ---- the oracle on the host cores, bounded sample (rank 0, N=1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -348,7 +380,7 @@ def run_ours(args):
                        "units_per_step": units_step,
                        "l2": "inputs larger than L2 (no flush): each step streams > 10 GB"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches) * world, "roofline": roof,
-            "cpu_baseline": cpu, "kernels": kernels, "split_step": split_step,
+            "cpu_baseline": cpu, "kernels": kernels, "split_step": split_step, "cufft_comparison": cufft,
         }
         print(json.dumps(line))
     ctx.close()
