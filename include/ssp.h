@@ -209,6 +209,12 @@ int ssp_phase_mul(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_theta, doub
 int ssp_dft2_centered(ssp_ctx *ctx, ssp_grid grid, int B, int inverse,
                       const float *d_in, float *d_out, void *d_ws, size_t ws_bytes);
 /* grad[b] = Im(g[b] conj(u[b])), dev fp32 [B][N][N]. */
+/* One Adam step on a phase mask shared by B fields (D2NN training):
+ *   g = (1/B) sum_b d_grad[b];  m <- b1 m + (1-b1) g;  v <- b2 v + (1-b2) g^2;
+ *   theta <- theta - lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps),   t >= 1 the step count.
+ * d_grad: dev fp32 [B][N][N]; d_m, d_v, d_theta: dev fp32 [N][N], updated in place. */
+int ssp_adam_update(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_grad, double lr, double beta1,
+                    double beta2, double eps, int t, float *d_m, float *d_v, float *d_theta);
 /* Circular aperture of `radius` metres about the grid centre: out = in where
  * (ix-N/2)^2 + (iy-N/2)^2 <= floor((radius/dx)^2) (the threshold is an integer taken on the host in
  * double), else 0.  d_in / d_out: dev complex64 [B][N][N]; may alias. */

@@ -285,3 +285,14 @@ def phase_grad(N, g, u):
     out = np.empty(g.shape, dtype=np.float64)
     _chk(lib().orc_phase_grad(C.c_int(N), C.c_int(g.shape[0]), _p(g), _p(u), _p(out)), "phase_grad")
     return out
+
+
+def adam_step(grad, lr, t, m, v, theta, beta1=0.9, beta2=0.999, eps=1e-8):
+    """Adam (Kingma & Ba), the optimiser of PAPER.md:115, on a mask shared by the batch: g = mean_b grad[b].
+    Returns new (m, v, theta) in float64."""
+    g = np.mean(np.asarray(grad, dtype=np.float64), axis=0)
+    m = beta1 * np.asarray(m, dtype=np.float64) + (1.0 - beta1) * g
+    v = beta2 * np.asarray(v, dtype=np.float64) + (1.0 - beta2) * g * g
+    mhat = m / (1.0 - beta1 ** t)
+    vhat = v / (1.0 - beta2 ** t)
+    return m, v, np.asarray(theta, dtype=np.float64) - lr * mhat / (np.sqrt(vhat) + eps)

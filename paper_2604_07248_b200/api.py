@@ -27,7 +27,7 @@ SYMBOLS = (
     "ssp_create", "ssp_destroy", "ssp_last_error", "ssp_version", "ssp_launch_count",
     "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_propagate",
     "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_propagate_host", "ssp_phase_mul",
-    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture",
+    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update",
     "ssp_profile_enable", "ssp_profile_report",
 )
 
@@ -94,6 +94,7 @@ def load():
     lib.ssp_dft2_centered.argtypes = [P, Grid, I, I, P, P, P, C.c_size_t]
     lib.ssp_phase_grad.argtypes = [P, Grid, I, P, P, P]
     lib.ssp_aperture.argtypes = [P, Grid, I, D, P, P]
+    lib.ssp_adam_update.argtypes = [P, Grid, I, P, D, D, D, D, I, P, P, P]
     lib.ssp_inner_products.argtypes = [P, Grid, I, P, P, P]
     lib.ssp_lincomb.argtypes = [P, Grid, I, P, P, P, P, P]
     lib.ssp_profile_enable.argtypes = [P, I]
@@ -307,6 +308,12 @@ class Context:
         self._chk(self._lib.ssp_dft2_centered(self._h, Grid(N, dx), field.shape[0], int(inverse),
                                               _dev(field, torch.complex64), _dev(out, torch.complex64), None, 0))
         return out
+
+    def adam_update(self, N, dx, grad, lr, t, m, v, theta, beta1=0.9, beta2=0.999, eps=1e-8):
+        """One Adam step (in place on m, v, theta) with the gradient averaged over the batch axis of `grad`."""
+        self._chk(self._lib.ssp_adam_update(self._h, Grid(N, dx), grad.shape[0], _dev(grad, torch.float32), float(lr),
+                                            float(beta1), float(beta2), float(eps), int(t), _dev(m, torch.float32),
+                                            _dev(v, torch.float32), _dev(theta, torch.float32)))
 
     def aperture(self, N, dx, radius, field, out=None):
         out = torch.empty_like(field) if out is None else out

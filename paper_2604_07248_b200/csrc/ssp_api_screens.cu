@@ -333,6 +333,19 @@ int ssp_dft2_centered(ssp_ctx *ctx, ssp_grid grid, int B, int inverse,
     return launch_col_single(ctx, N, inverse != 0, c);
 }
 
+int ssp_adam_update(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_grad, double lr, double beta1,
+                    double beta2, double eps, int t, float *d_m, float *d_v, float *d_theta)
+{
+    if (!ctx) return SSP_EINVAL;
+    if (!valid_N(grid.N) || B < 1 || t < 1 || !d_grad || !d_m || !d_v || !d_theta || !(beta1 >= 0 && beta1 < 1) ||
+        !(beta2 >= 0 && beta2 < 1) || !(eps > 0))
+        return ctx->fail(SSP_EINVAL, "bad arguments");
+    SSP_CUDA(ctx, cudaSetDevice(ctx->device));
+    const double c1 = 1.0 / (1.0 - pow(beta1, (double)t)), c2 = 1.0 / (1.0 - pow(beta2, (double)t));
+    return launch_adam(ctx, (long long)grid.N * grid.N, B, d_grad, (float)lr, (float)beta1, (float)beta2, (float)eps,
+                       (float)c1, (float)c2, (float)(1.0 - beta1), (float)(1.0 - beta2), d_m, d_v, d_theta);
+}
+
 int ssp_aperture(ssp_ctx *ctx, ssp_grid grid, int B, double radius, const float *d_in, float *d_out)
 {
     if (!ctx) return SSP_EINVAL;

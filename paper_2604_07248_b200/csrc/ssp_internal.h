@@ -225,6 +225,8 @@ int launch_welford(ssp_ctx *ctx, int N, int B, const float2 *field, float *mean,
                    long long count0);
 int launch_h2d_table(ssp_ctx *ctx, int N, int C, double dx, double lam_eff, double dz, int conj, float2 *out);
 int col_tile_width(int N);     // columns per tile of the kernel launch_col_prop picks for N (layout of the H map)
+int launch_adam(ssp_ctx *ctx, long long n, int B, const float *grad, float lr, float b1, float b2, float eps,
+                float c1, float c2, float o1, float o2, float *m, float *v, float *theta);
 int launch_aperture(ssp_ctx *ctx, int N, int B, long long r2max_px, const float2 *in, float2 *out);
 int launch_phase_mul(ssp_ctx *ctx, int N, int B, const float *theta, float sign,
                      const float2 *in, float2 *out);

@@ -188,6 +188,33 @@ int launch_h2d_table(ssp_ctx *ctx, int N, int C, double dx, double lam_eff, doub
     return SSP_OK;
 }
 
+// Adam step on a mask shared by B fields; c1 = 1/(1-b1^t), c2 = 1/(1-b2^t), o1 = 1-b1, o2 = 1-b2
+// from the host in double (1 - 0.999f in fp32 is 6e-5 off)
+__global__ void __launch_bounds__(256) k_adam(size_t n, int B, const float *__restrict__ grad, float lr, float b1, float b2,
+                                               float eps, float c1, float c2, float o1, float o2, float *__restrict__ m,
+                                               float *__restrict__ v, float *__restrict__ theta)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float g = 0.f;
+    for (int b = 0; b < B; ++b) g += grad[(size_t)b * n + i];
+    g /= (float)B;
+    const float mi = fmaf(b1, m[i], o1 * g);
+    const float vi = fmaf(b2, v[i], o2 * g * g);
+    m[i] = mi;
+    v[i] = vi;
+    theta[i] -= lr * (mi * c1) / (sqrtf(vi * c2) + eps);
+}
+
+int launch_adam(ssp_ctx *ctx, long long n, int B, const float *grad, float lr, float b1, float b2, float eps,
+                float c1, float c2, float o1, float o2, float *m, float *v, float *theta)
+{
+    k_adam<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>((size_t)n, B, grad, lr, b1, b2, eps, c1, c2, o1, o2, m, v, theta);
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
 // circular aperture: integer test against a host-decided threshold
 __global__ void __launch_bounds__(256) k_aperture(int N, long long r2max, const float2 *__restrict__ in, float2 *__restrict__ out)
 {

@@ -11,10 +11,14 @@ Test infrastructure only; holds no kernel code.
 import numpy as np
 
 
-def oracle_chain(orc, N, dx, lam, dz, u0, scr32, th1, th2, kw):
-    """All quantities for ONE batch of fields on the oracle.  Returns a dict of float64 / complex128 arrays."""
+def oracle_chain(orc, N, dx, lam, dz, u0, scr32, th1, th2, kw, aperture_radius=None):
+    """All quantities for ONE batch of fields on the oracle.  Returns a dict of float64 / complex128 arrays.
+    aperture_radius: optional circular aperture applied to A(U0) and to the target; a real 0/1
+    mask, so the adjoint applies it again."""
+    ap = (lambda x: x) if aperture_radius is None else (lambda x: orc.aperture(N, dx, aperture_radius, x))
     V1, planes = orc.propagate(N, dx, lam, dz, u0, scr32, return_planes=True, **kw)
-    T = orc.propagate(N, dx, lam, dz, u0, None, **kw)
+    V1 = ap(V1)
+    T = ap(orc.propagate(N, dx, lam, dz, u0, None, **kw))
     V2 = orc.phase_mul(N, th1, V1)
     V3 = orc.dft2_centered(N, V2)
     V4 = orc.phase_mul(N, th2, V3)
@@ -31,7 +35,7 @@ def oracle_chain(orc, N, dx, lam, dz, u0, scr32, th1, th2, kw):
     g_th2 = orc.phase_grad(N, G4, V4)
     G2 = orc.dft2_centered(N, orc.phase_mul(N, th2, G4, sign=-1.0), inverse=True)
     g_th1 = orc.phase_grad(N, G2, V2)
-    G1 = orc.phase_mul(N, th1, G2, sign=-1.0)
+    G1 = ap(orc.phase_mul(N, th1, G2, sign=-1.0))
     G0, g_phi = orc.propagate_adjoint(N, dx, lam, dz, G1, scr32, planes=planes, **kw)
     return dict(loss=loss, V5=V5, g_th1=g_th1, g_th2=g_th2, g_phi=g_phi, G0=G0, planes=planes)
 
