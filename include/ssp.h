@@ -148,6 +148,21 @@ int ssp_evolve_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double l
                        float *d_spectrum, float *d_sh_coef, float *d_screens,
                        void *d_ws, size_t ws_bytes);
 
+/* ---- path description (host only) ------------------------------------------------ */
+
+/* Hufnagel-Valley 5/7 profile (PAPER.md:393 S21):
+ *   Cn2(h) = 0.00594 (V/27)^2 (1e-5 h)^10 exp(-h/1000) + 2.7e-16 exp(-h/1500) + A exp(-h/ground_scale),
+ * h in metres above ground, V the wind speed, A the ground-level constant.  ground_scale <= 0 takes the 1000 m
+ * the paper prints; the textbook profile has 100 m. */
+typedef struct { double A, V, ground_scale; } ssp_hv57;
+double ssp_hv57_cn2(const ssp_hv57 *p, double h);
+/* Vertical path h0 .. h0 + L cut into n equal slabs: cn2[j] = slab mean of Cn2 (cn2[j] dz[j] is the S18 integral
+ * of slab j), dz[j] = L/n; host double [n] each, ready for ssp_make_screens.  Optional outputs: the
+ * path's Rytov variance 3.27 k^(7/6) L^(5/6) int Cn2(z) (1 - z/L)^(5/3) dz (PAPER.md:380 S19, z from the source at
+ * h0) and its Fried parameter (S18). */
+int ssp_hv57_path(const ssp_hv57 *p, double h0, double L, int n, double lambda, double *cn2, double *dz,
+                  double *rytov, double *r0);
+
 /* ---- propagation --------------------------------------------------------------- */
 
 /* Split-step propagation (Eq.1; step order Q11):

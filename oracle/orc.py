@@ -296,3 +296,32 @@ def adam_step(grad, lr, t, m, v, theta, beta1=0.9, beta2=0.999, eps=1e-8):
     mhat = m / (1.0 - beta1 ** t)
     vhat = v / (1.0 - beta2 ** t)
     return m, v, np.asarray(theta, dtype=np.float64) - lr * mhat / (np.sqrt(vhat) + eps)
+
+
+# ---- path description (PAPER.md:393 S21, :375 S18, :380 S19) ------------------------------------------------
+def hv57_cn2(h, A, V=21.0, ground_scale=1000.0):
+    """Hufnagel-Valley 5/7 as printed in S21 (third scale height 1000 m there; the textbook value is 100 m)."""
+    h = np.asarray(h, dtype=np.float64)
+    return (0.00594 * (V / 27.0) ** 2 * (1e-5 * h) ** 10 * np.exp(-h / 1000.0) + 2.7e-16 * np.exp(-h / 1500.0)
+            + A * np.exp(-h / ground_scale))
+
+
+def hv57_slab_integral(a, b, A, V=21.0, ground_scale=1000.0):
+    """int_a^b Cn2(h) dh in closed form: exponentials, and the h^10 exp(-h/1000) term through the regularised
+    incomplete gamma function."""
+    from scipy import special
+    e = lambda s: s * (np.exp(-a / s) - np.exp(-b / s))
+    g11 = special.gamma(11.0) * (special.gammainc(11.0, b / 1000.0) - special.gammainc(11.0, a / 1000.0))
+    return 0.00594 * (V / 27.0) ** 2 * 1e-50 * 1000.0 ** 11 * g11 + 2.7e-16 * e(1500.0) + A * e(ground_scale)
+
+
+def hv57_path(h0, L, n, lam, A, V=21.0, ground_scale=1000.0):
+    """Equal slabs: (cn2[n] slab means, dz[n], Rytov variance by S19 with adaptive quadrature, r0 by S18)."""
+    from scipy import integrate
+    k = 2.0 * np.pi / lam
+    edges = h0 + L * np.arange(n + 1) / n
+    ints = np.array([hv57_slab_integral(edges[j], edges[j + 1], A, V, ground_scale) for j in range(n)])
+    w = integrate.quad(lambda z: float(hv57_cn2(h0 + z, A, V, ground_scale)) * (1.0 - z / L) ** (5.0 / 3.0), 0.0, L,
+                       epsabs=0, epsrel=1e-12, limit=400)[0]
+    rytov = 3.27 * k ** (7.0 / 6.0) * L ** (5.0 / 6.0) * w
+    return ints / (L / n), np.full(n, L / n), rytov, (0.423 * k * k * ints.sum()) ** (-3.0 / 5.0)

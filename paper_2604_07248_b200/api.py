@@ -27,7 +27,7 @@ SYMBOLS = (
     "ssp_create", "ssp_destroy", "ssp_last_error", "ssp_version", "ssp_launch_count",
     "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_propagate",
     "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_propagate_host", "ssp_phase_mul",
-    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update",
+    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path",
     "ssp_profile_enable", "ssp_profile_report",
 )
 
@@ -46,6 +46,10 @@ class Psd(C.Structure):
     _fields_ = [("kind", C.c_int), ("L0", C.c_double), ("l0", C.c_double), ("km_coeff", C.c_double),
                 ("chi_T", C.c_double), ("eps", C.c_double), ("w", C.c_double), ("eta", C.c_double),
                 ("alpha", C.c_double), ("A", C.c_double)]
+
+
+class Hv57(C.Structure):
+    _fields_ = [("A", C.c_double), ("V", C.c_double), ("ground_scale", C.c_double)]
 
 
 class Window(C.Structure):
@@ -94,6 +98,9 @@ def load():
     lib.ssp_dft2_centered.argtypes = [P, Grid, I, I, P, P, P, C.c_size_t]
     lib.ssp_phase_grad.argtypes = [P, Grid, I, P, P, P]
     lib.ssp_aperture.argtypes = [P, Grid, I, D, P, P]
+    lib.ssp_hv57_cn2.argtypes = [C.POINTER(Hv57), D]
+    lib.ssp_hv57_cn2.restype = D
+    lib.ssp_hv57_path.argtypes = [C.POINTER(Hv57), D, D, I, D, P, P, P, P]
     lib.ssp_adam_update.argtypes = [P, Grid, I, P, D, D, D, D, I, P, P, P]
     lib.ssp_inner_products.argtypes = [P, Grid, I, P, P, P]
     lib.ssp_lincomb.argtypes = [P, Grid, I, P, P, P, P, P]
@@ -145,6 +152,23 @@ class PsdParams:
     def c(self) -> Psd:
         return Psd(self.kind, self.L0, self.l0, self.km_coeff, self.chi_T, self.eps, self.w, self.eta,
                    self.alpha, self.A)
+
+
+def hv57_cn2(h, A, V=21.0, ground_scale=0.0):
+    """Hufnagel-Valley 5/7 Cn2 at height h [m] (host call, no context needed)."""
+    return load().ssp_hv57_cn2(C.byref(Hv57(A, V, ground_scale)), float(h))
+
+
+def hv57_path(h0, L, n, lam, A, V=21.0, ground_scale=0.0):
+    """Equal slabs of a vertical HV5/7 path: (cn2[n], dz[n], rytov variance, r0) as numpy / floats."""
+    import numpy as np
+    cn2, dz = np.empty(n), np.empty(n)
+    ry, r0 = C.c_double(), C.c_double()
+    rc = load().ssp_hv57_path(C.byref(Hv57(A, V, ground_scale)), float(h0), float(L), int(n), float(lam),
+                              cn2.ctypes.data_as(C.c_void_p), dz.ctypes.data_as(C.c_void_p), C.byref(ry), C.byref(r0))
+    if rc != OK:
+        raise SspError(rc, "ssp_hv57_path: bad arguments")
+    return cn2, dz, ry.value, r0.value
 
 
 class Context:
