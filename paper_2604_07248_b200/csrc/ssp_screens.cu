@@ -188,7 +188,7 @@ k_screen_col_tma(const __grid_constant__ CUtensorMap tm_noise, const __grid_cons
 }
 
 template <int N>
-__global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_screen_row(const ScreenRowArgs a)
+__global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS + (N == 1024 ? 1 : 0)) k_screen_row(const ScreenRowArgs a)
 {
     using PI = PlanInfo<N, 0>;
     using CFG = RowCfg<N>;
@@ -332,10 +332,13 @@ static int launch_screen_row_n(ssp_ctx *ctx, const ScreenRowArgs &a)
 {
     using CFG = RowCfg<N>;
     auto kern = k_screen_row<N>;
-    if (CFG::SMEM > 48 * 1024)
-        SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::SMEM));
+    // only the exchange buffers: no screen-row staging here, and what shared memory does not take stays L1
+    // (the phasor and twiddle tables are read through it)
+    constexpr size_t smem = CFG::SMEM_X;
+    if (smem > 48 * 1024)
+        SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ctx->prof_begin("screen_row", 12.0 * (double)a.nscr * N * N);
-    kern<<<(unsigned)((long long)a.nscr * N / CFG::LPB), CFG::THREADS, CFG::SMEM, ctx->stream>>>(a);
+    kern<<<(unsigned)((long long)a.nscr * N / CFG::LPB), CFG::THREADS, smem, ctx->stream>>>(a);
     ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
