@@ -207,3 +207,38 @@ def test_bench_launch_configuration_full_size(ssp, orc):
     # distinct noise per realisation gives distinct fields; all finite
     assert torch.isfinite(torch.view_as_real(out)).all()
     assert not torch.equal(out[0], out[1])
+
+
+@pytest.mark.parametrize("cid", [2, 4, 5])
+def test_full_size_configs_properties(ssp, cid):
+    """configs[1], [3], [4] at their FULL sizes (512^2 x 64 x 10, 2048^2 x 8 x 30, 4096^2 x 2 x 20): too large for the
+    fp64 oracle, so what is checked are properties that hold at any size -- finite output, power never grows
+    (|H| = 1, |W| <= 1, |exp(i phi)| = 1), <A x, A x> = <A^H A x, x> per realisation, piston-free screens -- on
+    screens generated on the device from seeded noise."""
+    import torch
+    from paper_2604_07248_b200 import api
+    wl = synth.CONFIGS[cid]
+    N, S, B = wl.N, wl.S, wl.B
+    pg = api.PsdParams(**wl.psd_dict())
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(100 + cid)
+    noise = torch.view_as_complex(torch.randn(B, S, N, N, 2, device="cuda", generator=gen))
+    nsh = torch.view_as_complex(torch.randn(B, S, max(wl.n_sh, 1), 3, 3, 2, device="cuda", generator=gen))
+    cn2 = list(wl.cn2_list) if cid != 2 else [wl.cn2_sweep[1]] * S
+    scr = ssp.make_screens(N, wl.dx, pg, wl.lam, cn2, list(wl.dz), wl.n_sh, noise, nsh if wl.n_sh else None)
+    del noise
+    assert torch.isfinite(scr).all()
+    m = scr.mean(dim=(-2, -1)).abs().max()
+    assert float(m) < 1e-3 * float(scr.abs().max())
+    u0 = cu(synth.input_field(wl, B))
+    kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
+    out = ssp.propagate(N, wl.dx, wl.lam, list(wl.dz), u0, scr, **kw)
+    gin = ssp.propagate_adjoint(N, wl.dx, wl.lam, list(wl.dz), out, scr, **kw)
+    assert torch.isfinite(torch.view_as_real(out)).all()
+    ip1 = ssp.inner_products(N, wl.dx, out, out).cpu().numpy()
+    ip2 = ssp.inner_products(N, wl.dx, gin, u0).cpu().numpy()
+    p0 = ssp.inner_products(N, wl.dx, u0, u0).cpu().numpy()[:, 2]
+    for b in range(B):
+        assert abs(ip1[b, 0] - ip2[b, 0]) < 2e-6 * S * ip1[b, 0], (b, ip1[b], ip2[b])
+        assert abs(ip2[b, 1]) < 2e-6 * S * ip1[b, 0]
+        assert ip1[b, 2] <= p0[b] * (1 + 1e-5)
