@@ -199,13 +199,15 @@ double orc_psd_f(const orc_psd_t *psd, double lambda, double cn2, double dz, dou
  * phi_hi = Re sum_k C[ky,kx] exp(+i 2 pi (kx ix + ky iy)/N)   (PAPER.md:359 S16; Q3, Q6)
  * phi_lo = sum_p sum_{m,n} Re{ c exp(i 2 pi (n df_p x + m df_p y)) }  (Eq.2; Q7)
  * phi = phi_hi + (phi_lo - mean phi_lo)                          (PAPER.md:63 Eq.3, :362) */
-static int synth_one(int N, double dx, int n_sh, const double *C, const double *shc,
-                     double *phi, double *work)
+/* part = 0: the real part of the synthesis (the screen, Q3); part = 1: its imaginary part, a second screen
+ * with the same statistics drawn from the same noise (the part Q3 discards). */
+static int synth_part(int N, double dx, int n_sh, const double *C, const double *shc,
+                      double *phi, double *work, int part)
 {
     size_t px = (size_t)N * N;
     memcpy(work, C, sizeof(double) * 2 * px);
     if (orc_fft2d(work, N, +1)) return -1;
-    for (size_t i = 0; i < px; ++i) phi[i] = work[2 * i];
+    for (size_t i = 0; i < px; ++i) phi[i] = work[2 * i + part];
     if (n_sh > 0) {
         double df = 1.0 / ((double)N * dx);
         double *lo = (double *)calloc(px, sizeof(double));
@@ -223,7 +225,8 @@ static int synth_one(int N, double dx, int n_sh, const double *C, const double *
                         for (int ix = 0; ix < N; ++ix) {
                             double x = (ix - N / 2) * dx;
                             double ang = 2.0 * M_PI * (fx * x + fy * y);
-                            lo[(size_t)iy * N + ix] += cr * cos(ang) - ci * sin(ang);
+                            lo[(size_t)iy * N + ix] += part ? cr * sin(ang) + ci * cos(ang)
+                                                            : cr * cos(ang) - ci * sin(ang);
                         }
                     }
                 }
@@ -234,6 +237,27 @@ static int synth_one(int N, double dx, int n_sh, const double *C, const double *
         for (size_t i = 0; i < px; ++i) phi[i] += lo[i] - mean;
         free(lo);
     }
+    return 0;
+}
+
+static int synth_one(int N, double dx, int n_sh, const double *C, const double *shc,
+                     double *phi, double *work)
+{
+    return synth_part(N, dx, n_sh, C, shc, phi, work, 0);
+}
+
+int orc_synthesize_im(int N, double dx, int B, int S, int n_sh,
+                      const double *spectrum, const double *sh_coef, double *screens)
+{
+    size_t px = (size_t)N * N;
+    double *work = (double *)malloc(sizeof(double) * 2 * px);
+    if (!work) return -1;
+    for (int bs = 0; bs < B * S; ++bs) {
+        const double *shc = (n_sh > 0) ? sh_coef + 2 * (size_t)bs * n_sh * 9 : NULL;
+        if (synth_part(N, dx, n_sh, spectrum + 2 * (size_t)bs * px, shc,
+                       screens + (size_t)bs * px, work, 1)) { free(work); return -1; }
+    }
+    free(work);
     return 0;
 }
 

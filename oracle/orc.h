@@ -68,6 +68,9 @@ int orc_make_screens(int N, double dx, const orc_psd_t *psd, double lambda, int 
 /* synthesis only: spectrum [B][S][N][N] c128 + sh_coef [B][S][n_sh][3][3] c128 -> screens */
 int orc_synthesize(int N, double dx, int B, int S, int n_sh,
                    const double *spectrum, const double *sh_coef, double *screens);
+/* The imaginary part of the same synthesis: a second, statistically independent screen from the same spectrum. */
+int orc_synthesize_im(int N, double dx, int B, int S, int n_sh,
+                      const double *spectrum, const double *sh_coef, double *screens);
 /* O5 (PAPER.md:74 Eq.4, :80 Eq.5). spectrum / sh_coef are in-out. */
 int orc_evolve_screens(int N, double dx, const orc_psd_t *psd, double lambda, int B, int S,
                        const double *cn2, const double *dz, int n_sh,

@@ -151,13 +151,16 @@ def make_screens(N, dx, psd: Psd, lam, cn2, dz, n_sh, noise, noise_sh, keep_spec
     return screens, spectrum, sh
 
 
-def synthesize(N, dx, n_sh, spectrum, sh_coef):
+def synthesize(N, dx, n_sh, spectrum, sh_coef, part="re"):
+    """Screens from stored spectra / subharmonic coefficients: the real part of the synthesis (the paper's screen,
+    Q3) or, with part="im", its imaginary part -- a second screen of the same statistics from the same noise."""
     spectrum = _c128(spectrum)
     B, S = spectrum.shape[0], spectrum.shape[1]
     sh = _c128(sh_coef) if n_sh > 0 else None
     screens = np.empty((B, S, N, N), dtype=np.float64)
-    _chk(lib().orc_synthesize(C.c_int(N), C.c_double(dx), C.c_int(B), C.c_int(S), C.c_int(n_sh),
-                              _p(spectrum), _p(sh), _p(screens)), "synthesize")
+    fn = lib().orc_synthesize_im if part == "im" else lib().orc_synthesize
+    _chk(fn(C.c_int(N), C.c_double(dx), C.c_int(B), C.c_int(S), C.c_int(n_sh),
+            _p(spectrum), _p(sh), _p(screens)), "synthesize")
     return screens
 
 

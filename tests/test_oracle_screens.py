@@ -195,3 +195,25 @@ def test_ar_decorrelation_follows_a_power_n(orc):
             corr = np.mean([np.corrcoef(scr0[b, 0].ravel(), scr[b, 0].ravel())[0, 1] for b in range(B)])
             assert abs(corr - a ** n) < 0.06, (n, corr, a ** n)
     assert abs(scr.var() / var0 - 1) < 0.15
+
+
+def test_imaginary_part_is_a_second_screen(orc):
+    """orc.synthesize(part="im") (the part of the synthesis that Q3 discards).  Exact link to the pinned
+    real-part path: Im(z) = Re(-i z), so the imaginary-part screens of noise n are the real-part screens of noise
+    -i n = (b, -a), subharmonics and mean removal included.  Ensemble: same variance as the real part, and
+    uncorrelated with it (a circular complex Gaussian spectrum)."""
+    N, dx, n_sh, B, S = 32, 2e-3, 3, 200, 1
+    psd = orc.Psd(kind=orc.PSD_VON_KARMAN, L0=10.0, l0=5e-3)
+    rng = np.random.default_rng(11)
+    hi = rng.standard_normal((B, S, N, N, 2), dtype=np.float32)
+    sh = rng.standard_normal((B, S, n_sh, 3, 3, 2), dtype=np.float32)
+    re, spec, shc = orc.make_screens(N, dx, psd, 1e-6, [1e-14], [100.0], n_sh, hi, sh)
+    im = orc.synthesize(N, dx, n_sh, spec, shc, part="im")
+    rot = lambda a: np.stack([a[..., 1], -a[..., 0]], axis=-1).astype(np.float32)      # n -> -i n
+    re_rot, _, _ = orc.make_screens(N, dx, psd, 1e-6, [1e-14], [100.0], n_sh, rot(hi), rot(sh))
+    np.testing.assert_allclose(im, re_rot, rtol=0, atol=1e-12 * np.abs(re).max())
+    np.testing.assert_allclose(orc.synthesize(N, dx, n_sh, spec, shc), re, rtol=0, atol=1e-12 * np.abs(re).max())
+    assert abs(im.var() / re.var() - 1) < 0.25
+    corr = np.mean(re * im) / np.sqrt(re.var() * im.var())
+    assert abs(corr) < 0.2, corr           # a few low-frequency modes dominate: ~1/sqrt(200 x few) sampling noise
+    assert np.abs(im.mean(axis=(-2, -1))).max() < 1e-10 * np.abs(im).max() + 1e-9    # piston removed here too
