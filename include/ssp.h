@@ -148,6 +148,23 @@ int ssp_evolve_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double l
                        float *d_spectrum, float *d_sh_coef, float *d_screens,
                        void *d_ws, size_t ws_bytes);
 
+/* The same two calls with a second output: d_screens_im (dev fp32 [B][S][N][N]) receives the IMAGINARY part of
+ * each synthesis, phi_im = Im(sum C exp(..)) + Im-part subharmonics - its mean: a second screen of the same
+ * statistics, uncorrelated with the first, from the same noise and the same transforms (the part that the
+ * paper's real-part screen discards, Q3).  One spectrum then yields two screens; under evolution both follow the
+ * stored spectrum. */
+int ssp_make_screens_pair(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
+                          int B, int S, const double *cn2, const double *dz, int n_sh,
+                          const float *d_noise, const float *d_noise_sh,
+                          float *d_spectrum, float *d_sh_coef, float *d_screens, float *d_screens_im,
+                          void *d_ws, size_t ws_bytes);
+int ssp_evolve_screens_pair(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
+                            int B, int S, const double *cn2, const double *dz, int n_sh,
+                            double a, double vx, double vy, double T,
+                            const float *d_fresh_noise, const float *d_fresh_noise_sh,
+                            float *d_spectrum, float *d_sh_coef, float *d_screens, float *d_screens_im,
+                            void *d_ws, size_t ws_bytes);
+
 /* ---- path description (host only) ------------------------------------------------ */
 
 /* Hufnagel-Valley 5/7 profile (PAPER.md:393 S21):

@@ -25,7 +25,7 @@ OK, EINVAL, EUNSUPPORTED, EWORKSPACE, ECUDA = 0, -1, -2, -3, -4
 # every symbol include/ssp.h declares (tests/test_abi.py checks the header against this list)
 SYMBOLS = (
     "ssp_create", "ssp_destroy", "ssp_last_error", "ssp_version", "ssp_launch_count",
-    "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_propagate",
+    "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_make_screens_pair", "ssp_evolve_screens_pair", "ssp_propagate",
     "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_propagate_host", "ssp_phase_mul",
     "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path",
     "ssp_profile_enable", "ssp_profile_report",
@@ -87,6 +87,9 @@ def load():
     lib.ssp_destroy.argtypes = [C.c_void_p]
     P, D, I, L = C.c_void_p, C.c_double, C.c_int, C.c_longlong
     lib.ssp_make_screens.argtypes = [P, Grid, C.POINTER(Psd), D, I, I, P, P, I, P, P, P, P, P, P, C.c_size_t]
+    lib.ssp_make_screens_pair.argtypes = [P, Grid, C.POINTER(Psd), D, I, I, P, P, I, P, P, P, P, P, P, P, C.c_size_t]
+    lib.ssp_evolve_screens_pair.argtypes = [P, Grid, C.POINTER(Psd), D, I, I, P, P, I, D, D, D, D, P, P, P, P, P, P, P,
+                                            C.c_size_t]
     lib.ssp_evolve_screens.argtypes = [P, Grid, C.POINTER(Psd), D, I, I, P, P, I, D, D, D, D, P, P, P, P, P, P,
                                        C.c_size_t]
     lib.ssp_propagate.argtypes = [P, Grid, D, D, I, I, I, P, P, L, I, Window, P, P, P, P, D, P, C.c_size_t]
@@ -227,13 +230,21 @@ class Context:
 
     # ---- screens ---------------------------------------------------------------------------
     def make_screens(self, N, dx, psd: PsdParams, lam, cn2, dz, n_sh, noise, noise_sh=None,
-                     spectrum=None, sh_coef=None, screens=None, ws=None):
-        """noise: complex64 [B][S][N][N]; noise_sh: complex64 [B][S][n_sh][3][3]; returns screens fp32."""
+                     spectrum=None, sh_coef=None, screens=None, ws=None, screens_im=None):
+        """noise: complex64 [B][S][N][N]; noise_sh: complex64 [B][S][n_sh][3][3]; returns screens fp32.
+        screens_im (fp32 [B][S][N][N]): also write the imaginary part of each synthesis as a second screen."""
         B, S = noise.shape[0], noise.shape[1]
         if screens is None:
             screens = torch.empty((B, S, N, N), dtype=torch.float32, device=noise.device)
         ws = self.workspace(N, dx, B, S) if ws is None else ws
         pc = psd.c()
+        if screens_im is not None:
+            self._chk(self._lib.ssp_make_screens_pair(
+                self._h, Grid(N, dx), C.byref(pc), lam, B, S, _host_doubles(cn2), _host_doubles(dz), n_sh,
+                _dev(noise, torch.complex64), _dev(noise_sh, torch.complex64) if n_sh > 0 else None,
+                _dev(spectrum, torch.complex64), _dev(sh_coef, torch.complex64), _dev(screens, torch.float32),
+                _dev(screens_im, torch.float32), _dev(ws), ws.numel()))
+            return screens
         self._chk(self._lib.ssp_make_screens(
             self._h, Grid(N, dx), C.byref(pc), lam, B, S, _host_doubles(cn2), _host_doubles(dz), n_sh,
             _dev(noise, torch.complex64), _dev(noise_sh, torch.complex64) if n_sh > 0 else None,
@@ -242,12 +253,19 @@ class Context:
         return screens
 
     def evolve_screens(self, N, dx, psd: PsdParams, lam, cn2, dz, n_sh, a, vx, vy, T, fresh, fresh_sh,
-                       spectrum, sh_coef, screens=None, ws=None):
+                       spectrum, sh_coef, screens=None, ws=None, screens_im=None):
         B, S = fresh.shape[0], fresh.shape[1]
         if screens is None:
             screens = torch.empty((B, S, N, N), dtype=torch.float32, device=fresh.device)
         ws = self.workspace(N, dx, B, S) if ws is None else ws
         pc = psd.c()
+        if screens_im is not None:
+            self._chk(self._lib.ssp_evolve_screens_pair(
+                self._h, Grid(N, dx), C.byref(pc), lam, B, S, _host_doubles(cn2), _host_doubles(dz), n_sh,
+                a, vx, vy, T, _dev(fresh, torch.complex64), _dev(fresh_sh, torch.complex64) if n_sh > 0 else None,
+                _dev(spectrum, torch.complex64), _dev(sh_coef, torch.complex64) if n_sh > 0 else None,
+                _dev(screens, torch.float32), _dev(screens_im, torch.float32), _dev(ws), ws.numel()))
+            return screens
         self._chk(self._lib.ssp_evolve_screens(
             self._h, Grid(N, dx), C.byref(pc), lam, B, S, _host_doubles(cn2), _host_doubles(dz), n_sh,
             a, vx, vy, T, _dev(fresh, torch.complex64), _dev(fresh_sh, torch.complex64) if n_sh > 0 else None,

@@ -38,7 +38,7 @@ WsLayout ws_layout(int N, int B, int S)
     L.tab_tauy = take(sizeof(float2) * N);
     L.tab_coef2 = take(sizeof(float2) * 2 * (size_t)B);   // ssp_lincomb scalars
     L.sh_coef = take(sizeof(float2) * nscr * kMaxSh * 9);
-    L.sh_mean = take(sizeof(float) * nscr);
+    L.sh_mean = take(sizeof(float) * 2 * nscr);
     const size_t per = sizeof(float2) * (size_t)N * N;
     size_t chunk = kChunkBytes / per;
     if (chunk < 1) chunk = 1;
@@ -124,7 +124,7 @@ int check_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda
 int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, int B, int S,
                  const double *cn2, const double *dz, int n_sh, bool ar, double a, double vx, double vy, double T,
                  const float *d_noise, const float *d_noise_sh, float *d_spectrum, float *d_sh_coef,
-                 float *d_screens, void *d_ws)
+                 float *d_screens, void *d_ws, float *d_screens_im = nullptr)
 {
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));
     const int N = grid.N;
@@ -249,7 +249,8 @@ int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
         r.screens = d_screens + (size_t)g0 * px;
         r.nscr = n; r.n_sh = n_sh;
         r.sh_coef = coef + (size_t)g0 * n_sh * 9;
-        r.sh_mean = mean + g0;
+        r.sh_mean = mean + 2 * (size_t)g0;
+        r.screens_im = d_screens_im ? d_screens_im + (size_t)g0 * px : nullptr;
         r.ex = d_ex;
         r.tw = tw;
         if (int rc = launch_screen_row(ctx, N, r)) return rc;
@@ -294,6 +295,37 @@ int ssp_evolve_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double l
     if (n_sh > 0 && !d_sh_coef) return ctx->fail(SSP_EINVAL, "d_sh_coef (in-out) is required when n_sh > 0");
     return screens_impl(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, true, a, vx, vy, T,
                         d_fresh_noise, d_fresh_noise_sh, d_spectrum, d_sh_coef, d_screens, d_ws);
+}
+
+int ssp_make_screens_pair(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
+                          int B, int S, const double *cn2, const double *dz, int n_sh,
+                          const float *d_noise, const float *d_noise_sh,
+                          float *d_spectrum, float *d_sh_coef, float *d_screens, float *d_screens_im,
+                          void *d_ws, size_t ws_bytes)
+{
+    if (int rc = check_screens(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, d_noise, d_noise_sh, d_screens, d_ws, ws_bytes))
+        return rc;
+    if (!d_screens_im || !aligned16(d_screens_im)) return ctx->fail(SSP_EINVAL, "d_screens_im is required (16-byte aligned)");
+    return screens_impl(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, false, 0.0, 0.0, 0.0, 0.0,
+                        d_noise, d_noise_sh, d_spectrum, d_sh_coef, d_screens, d_ws, d_screens_im);
+}
+
+int ssp_evolve_screens_pair(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
+                            int B, int S, const double *cn2, const double *dz, int n_sh,
+                            double a, double vx, double vy, double T,
+                            const float *d_fresh_noise, const float *d_fresh_noise_sh,
+                            float *d_spectrum, float *d_sh_coef, float *d_screens, float *d_screens_im,
+                            void *d_ws, size_t ws_bytes)
+{
+    if (int rc = check_screens(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, d_fresh_noise, d_fresh_noise_sh,
+                               d_screens, d_ws, ws_bytes))
+        return rc;
+    if (!(a >= 0.0 && a <= 1.0)) return ctx->fail(SSP_EINVAL, "a must be in [0, 1]");
+    if (!d_spectrum || !aligned16(d_spectrum)) return ctx->fail(SSP_EINVAL, "d_spectrum (in-out) is required");
+    if (n_sh > 0 && !d_sh_coef) return ctx->fail(SSP_EINVAL, "d_sh_coef (in-out) is required when n_sh > 0");
+    if (!d_screens_im || !aligned16(d_screens_im)) return ctx->fail(SSP_EINVAL, "d_screens_im is required (16-byte aligned)");
+    return screens_impl(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, true, a, vx, vy, T,
+                        d_fresh_noise, d_fresh_noise_sh, d_spectrum, d_sh_coef, d_screens, d_ws, d_screens_im);
 }
 
 // ---- mask-system helpers -----------------------------------------------------------------

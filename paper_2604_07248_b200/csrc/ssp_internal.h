@@ -205,7 +205,8 @@ struct ScreenRowArgs {
     int nscr;
     int n_sh;
     const float2 *sh_coef;    // [nscr][n_sh][3][3]
-    const float *sh_mean;     // [nscr]
+    float *screens_im;        // optional [nscr][N][N]: the imaginary part of the synthesis as a second screen
+    const float *sh_mean;     // [nscr][2]: analytic mean of phi_lo of the real-part and imaginary-part screens
     const float2 *ex;         // [n_sh][N] exp(i 2 pi df_p x)
     const float2 *tw;
 };

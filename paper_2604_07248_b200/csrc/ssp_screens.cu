@@ -187,7 +187,8 @@ k_screen_col_tma(const __grid_constant__ CUtensorMap tm_noise, const __grid_cons
     }
 }
 
-template <int N>
+// PAIR: also write the imaginary part of the synthesis as a second screen (a.screens_im).
+template <int N, bool PAIR>
 __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS + (N == 1024 ? 1 : 0)) k_screen_row(const ScreenRowArgs a)
 {
     using PI = PlanInfo<N, 0>;
@@ -212,9 +213,11 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS + (N
     // phi_lo(ix,iy) = sum_p Re( d_p0 conj(ex) + d_p1 + d_p2 ex ),  d_pb = c_p0b conj(ey) + c_p1b + c_p2b ey
     //              = sum_p [ (Re d_p0 + Re d_p2) cos_p(ix) + (Im d_p0 - Im d_p2) sin_p(ix) + Re d_p1 ]:
     // two FMAs per level and pixel; the ix-independent terms and the analytic mean go into one constant.
-    float cst = 0.f;
+    // The imaginary part: Im( d_p0 conj(ex) + d_p1 + d_p2 ex ) = (Im d_p0 + Im d_p2) cos_p + (Re d_p2 - Re d_p0) sin_p + Im d_p1.
+    float cst = 0.f, cst_im = 0.f;
     if (a.n_sh > 0) {
-        cst = -__ldg(a.sh_mean + scr);
+        cst = -__ldg(a.sh_mean + 2 * scr);
+        if constexpr (PAIR) cst_im = -__ldg(a.sh_mean + 2 * scr + 1);
         for (int p = 0; p < a.n_sh; ++p) {
             const float2 *cf = a.sh_coef + ((size_t)scr * a.n_sh + p) * 9;
             const float2 ey = __ldg(a.ex + (size_t)p * N + iy);
@@ -226,7 +229,9 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS + (N
                 d[bb] = make_float2(lo.x + c1.x + hi.x, lo.y + c1.y + hi.y);
             }
             const float ca = d[0].x + d[2].x, sa = d[0].y - d[2].y;
+            const float ci = d[0].y + d[2].y, si = d[2].x - d[0].x;
             cst += d[1].x;
+            if constexpr (PAIR) cst_im += d[1].y;
             const float2 *exp_ = a.ex + (size_t)p * N + t;
 #pragma unroll
             for (int i = 0; i < E / RL; ++i)
@@ -234,6 +239,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS + (N
                 for (int q = 0; q < RL; ++q) {
                     const float2 ex = __ldg(exp_ + (line_index<N, 0, RL>(t, i, q) - t));
                     v[i * RL + q].x = fmaf(ca, ex.x, fmaf(sa, ex.y, v[i * RL + q].x));
+                    if constexpr (PAIR) v[i * RL + q].y = fmaf(ci, ex.x, fmaf(si, ex.y, v[i * RL + q].y));
                 }
         }
     }
@@ -242,6 +248,13 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS + (N
     for (int i = 0; i < E / RL; ++i)
 #pragma unroll
         for (int q = 0; q < RL; ++q) dst[line_index<N, 0, RL>(t, i, q)] = v[i * RL + q].x + cst;
+    if constexpr (PAIR) {
+        float *dst_im = a.screens_im + line * N;
+#pragma unroll
+        for (int i = 0; i < E / RL; ++i)
+#pragma unroll
+            for (int q = 0; q < RL; ++q) dst_im[line_index<N, 0, RL>(t, i, q)] = v[i * RL + q].y + cst_im;
+    }
 }
 
 // one block per screen, one thread per (p, a, b)
@@ -250,9 +263,9 @@ __global__ void __launch_bounds__(96) k_sh_prep(int S, int n_sh, const float2 *_
                                                  float ar_a, float ar_g, const float2 *old_coef, float2 *coef_out,
                                                  const float2 *__restrict__ mfac, float *__restrict__ mean_out)
 {
-    __shared__ float red[96];
+    __shared__ float red[96], red_im[96];
     const int scr = blockIdx.x, i = threadIdx.x, s = scr % S;
-    float contrib = 0.f;
+    float contrib = 0.f, contrib_im = 0.f;
     if (i < 9 * n_sh) {
         const size_t idx = (size_t)scr * n_sh * 9 + i;
         const float amp = __ldg(amp_sh + (size_t)s * n_sh * 9 + i); // 0 at the centre
@@ -265,14 +278,17 @@ __global__ void __launch_bounds__(96) k_sh_prep(int S, int n_sh, const float2 *_
         }
         coef_out[idx] = cv;
         const float2 m = __ldg(mfac + i);
-        contrib = cv.x * m.x - cv.y * m.y;
+        contrib = cv.x * m.x - cv.y * m.y;                      // Re(c M): mean of the real-part screen's phi_lo
+        contrib_im = cv.x * m.y + cv.y * m.x;                   // Im(c M): of the imaginary-part screen's
     }
     red[i] = contrib;
+    red_im[i] = contrib_im;
     __syncthreads();
     if (i == 0) {
-        float sum = 0.f;
-        for (int k = 0; k < 9 * n_sh; ++k) sum += red[k];
-        mean_out[scr] = sum;
+        float sum = 0.f, sum_im = 0.f;
+        for (int k = 0; k < 9 * n_sh; ++k) { sum += red[k]; sum_im += red_im[k]; }
+        mean_out[2 * scr] = sum;
+        mean_out[2 * scr + 1] = sum_im;
     }
 }
 
@@ -331,13 +347,13 @@ template <int N>
 static int launch_screen_row_n(ssp_ctx *ctx, const ScreenRowArgs &a)
 {
     using CFG = RowCfg<N>;
-    auto kern = k_screen_row<N>;
+    auto kern = a.screens_im ? k_screen_row<N, true> : k_screen_row<N, false>;
     // only the exchange buffers: no screen-row staging here, and what shared memory does not take stays L1
     // (the phasor and twiddle tables are read through it)
     constexpr size_t smem = CFG::SMEM_X;
     if (smem > 48 * 1024)
         SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    ctx->prof_begin("screen_row", 12.0 * (double)a.nscr * N * N);
+    ctx->prof_begin("screen_row", (a.screens_im ? 16.0 : 12.0) * (double)a.nscr * N * N);
     kern<<<(unsigned)((long long)a.nscr * N / CFG::LPB), CFG::THREADS, smem, ctx->stream>>>(a);
     ctx->prof_end();
     ctx->launches++;

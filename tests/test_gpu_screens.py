@@ -178,3 +178,35 @@ def test_mask_system_helpers(ssp, orc):
     lc = ssp.lincomb(N, dx, al, cu(u), be, cu(v)).cpu().numpy()
     ref = np.stack([al[b] * u[b].astype(np.complex128) + be[b] * v[b].astype(np.complex128) for b in range(B)])
     assert rel_l2(lc, ref).max() < 1e-6
+
+
+@pytest.mark.parametrize("N,n_sh", [(64, 3), (1024, 3), (2048, 0)])
+def test_paired_screens_parity(ssp, orc, N, n_sh):
+    """ssp_make_screens_pair / ssp_evolve_screens_pair: the imaginary part of each synthesis as a second screen
+    (oracle: orc.synthesize(part="im"), pinned to the real-part path on the CPU)."""
+    import torch
+    from paper_2604_07248_b200 import api
+    dx, B, S = 2e-3, 1, 2
+    po, pg = orc.Psd(kind=1, L0=10.0, l0=5e-3), api.PsdParams(kind=1, L0=10.0, l0=5e-3)
+    cn2, dz = [1e-14, 3e-14], [100.0, 40.0]
+    hi, sh = synth.noise_batch(60 + N, 0, B, S, N, n_sh)
+    ref, spec_ref, shc_ref = orc.make_screens(N, dx, po, LAM, cn2, dz, n_sh, hi, sh if n_sh else None)
+    ref_im = orc.synthesize(N, dx, n_sh, spec_ref, shc_ref, part="im")
+    spec = torch.empty((B, S, N, N), dtype=torch.complex64, device="cuda")
+    shc = torch.zeros((B, S, max(n_sh, 1), 3, 3), dtype=torch.complex64, device="cuda")
+    im = torch.empty((B, S, N, N), dtype=torch.float32, device="cuda")
+    scr = ssp.make_screens(N, dx, pg, LAM, cn2, dz, n_sh, cu(c64(hi)), cu(c64(sh)) if n_sh else None,
+                           spectrum=spec, sh_coef=shc if n_sh else None, screens_im=im)
+    bound = 2e-5 * math.log2(N)
+    assert rel_l2(scr.cpu().numpy(), ref).max() < bound
+    assert rel_l2(im.cpu().numpy(), ref_im).max() < bound
+    # one AR step with wind: both screens follow the stored spectrum
+    hin, shn = synth.noise_batch(60 + N, 0, B, S, N, n_sh, frame=1)
+    a, T = 0.97, 0.01
+    vx, vy = 2.3 * dx / T, -0.7 * dx / T
+    ref2 = orc.evolve_screens(N, dx, po, LAM, cn2, dz, n_sh, a, vx, vy, T, hin, shn if n_sh else None, spec_ref, shc_ref)
+    ref2_im = orc.synthesize(N, dx, n_sh, spec_ref, shc_ref, part="im")      # spec_ref / shc_ref were advanced in place
+    scr2 = ssp.evolve_screens(N, dx, pg, LAM, cn2, dz, n_sh, a, vx, vy, T, cu(c64(hin)), cu(c64(shn)) if n_sh else None,
+                              spec, shc if n_sh else None, screens_im=im)
+    assert rel_l2(scr2.cpu().numpy(), ref2).max() < 2 * bound
+    assert rel_l2(im.cpu().numpy(), ref2_im).max() < 2 * bound
