@@ -50,10 +50,21 @@ __global__ void __launch_bounds__(256) k_stats_accum(const float2 *__restrict__ 
             if (iy == half && ix + e == half) a[ACC_AXIS] += I;
         }
     }
+    // warp shuffles, then one partial per warp through shared memory, then ONE fp64 atomic per block and moment:
+    // all blocks of a field add into the same nine addresses, so the atomics are the contended resource
+    __shared__ double part[8][ACC_N];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 #pragma unroll
     for (int i = 0; i < ACC_N; ++i) {
         const double s = warp_sum(a[i]);
-        if ((threadIdx.x & 31) == 0 && s != 0.0) atomicAdd(acc + (size_t)b * ACC_N + i, s);
+        if (lane == 0) part[warp][i] = s;
+    }
+    __syncthreads();
+    if (threadIdx.x < ACC_N) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) s += part[w][threadIdx.x];
+        if (s != 0.0) atomicAdd(acc + (size_t)b * ACC_N + threadIdx.x, s);
     }
 }
 
@@ -101,7 +112,7 @@ int launch_stats(ssp_ctx *ctx, int N, double dx, int B, const float2 *field, dou
     if (hi > N) hi = N;
     const long long roi_n = (long long)(hi - lo) * (hi - lo);
     const size_t pairs = (size_t)N * N / 2;
-    int bpf = (int)((pairs + 256 * 8 - 1) / (256 * 8)); // ~16 pixels per thread
+    int bpf = (int)((pairs + 256 * 32 - 1) / (256 * 32)); // ~64 pixels per thread
     if (bpf < 1) bpf = 1;
     ctx->prof_begin("stats", 8.0 * (double)B * N * N);
     k_stats_accum<<<dim3(bpf, B), 256, 0, ctx->stream>>>(field, N, lo, hi, acc);
