@@ -307,3 +307,17 @@ def test_on_chip_path_matches_multi_kernel_path(ssp, orc, N):
     gin = ssp.propagate_adjoint(N, dx, lam, list(dz), cu(g), cu(scr), **kw)
     gref = orc.propagate_adjoint(N, dx, lam, dz, g, scr, **kw)
     assert rel_l2(gin.cpu().numpy(), gref).max() < tol(N, S)
+
+
+def test_odd_batch_and_vacuum_paths_at_1024(ssp, orc):
+    """Edge cases of the TMA column kernel's persistent tile loop and of the fast / generic row instantiations:
+    a batch that does not fill the last wave evenly (B = 3), vacuum only (S = 0), window off, one step."""
+    N, dx, lam = 1024, 1e-3, 1e-6
+    u0 = synth.random_field(N, 3, 77)
+    scr = synth.random_screens(N, 3, 1, 78, rms=2.0)
+    dz = np.array([N * dx * dx / lam * 0.2])
+    for kw, s in ((dict(win_order=16, win_sigma_frac=0.47), scr), (dict(), scr), (dict(), None),
+                  (dict(win_order=4, win_sigma_frac=0.4), None)):
+        ref = orc.propagate(N, dx, lam, dz, u0, s, **kw)
+        out = ssp.propagate(N, dx, lam, list(dz), cu(u0), cu(s) if s is not None else None, **kw)
+        assert rel_l2(out.cpu().numpy(), ref).max() < tol(N, 1), kw

@@ -156,7 +156,7 @@ def test_mask_system_helpers(ssp, orc):
     u = synth.random_field(N, B, 61)
     v = synth.random_field(N, B, 62)
     th = synth.phase_masks(0, N, 1)[0]
-    for N2 in (8, 64, 256):
+    for N2 in (8, 64, 256, 512, 1024, 4096):
         w = synth.random_field(N2, B, 63)
         F = ssp.dft2_centered(N2, dx, cu(w))
         assert rel_l2(F.cpu().numpy(), orc.dft2_centered(N2, w)).max() < 2e-5 * math.log2(N2)
