@@ -180,6 +180,11 @@ double ssp_hv57_cn2(const ssp_hv57 *p, double h);
 int ssp_hv57_path(const ssp_hv57 *p, double h0, double L, int n, double lambda, double *cn2, double *dz,
                   double *rytov, double *r0);
 
+/* Workspace.  d_ws / ws_bytes: a caller-allocated device buffer of at least ssp_workspace_bytes(grid, B, S)
+ * bytes, 16-byte aligned.  The screen calls need it (tables, subharmonic coefficients, the column-transformed
+ * intermediate of a chunk of screens); the propagation calls, ssp_dft2_centered and ssp_propagate_host accept it
+ * for symmetry and do not use it today (NULL / 0 is fine there). */
+
 /* ---- propagation --------------------------------------------------------------- */
 
 /* Split-step propagation (Eq.1; step order Q11):

@@ -93,6 +93,22 @@ struct ssp_ctx {
                                cudaGetErrorString(e_), __FILE__, __LINE__);                  \
     } while (0)
 
+// Run EXPR with `NN` bound to the compile-time grid size matching the run-time N_.
+#define SSP_DISPATCH_N(N_, EXPR)                                   \
+    switch (N_) {                                                  \
+    case 8: { constexpr int NN = 8; return EXPR; }                 \
+    case 16: { constexpr int NN = 16; return EXPR; }               \
+    case 32: { constexpr int NN = 32; return EXPR; }               \
+    case 64: { constexpr int NN = 64; return EXPR; }               \
+    case 128: { constexpr int NN = 128; return EXPR; }             \
+    case 256: { constexpr int NN = 256; return EXPR; }             \
+    case 512: { constexpr int NN = 512; return EXPR; }             \
+    case 1024: { constexpr int NN = 1024; return EXPR; }           \
+    case 2048: { constexpr int NN = 2048; return EXPR; }           \
+    case 4096: { constexpr int NN = 4096; return EXPR; }           \
+    default: return ctx->fail(SSP_EINVAL, "unsupported N=%d", N_); \
+    }
+
 namespace ssp {
 
 // ---- tables (ssp_tables.cu) ------------------------------------------------------

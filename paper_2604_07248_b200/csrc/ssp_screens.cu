@@ -361,20 +361,6 @@ static int launch_screen_row_n(ssp_ctx *ctx, const ScreenRowArgs &a)
     return SSP_OK;
 }
 
-#define SSP_DISPATCH_N(N_, EXPR)                                   \
-    switch (N_) {                                                  \
-    case 8: { constexpr int NN = 8; return EXPR; }                 \
-    case 16: { constexpr int NN = 16; return EXPR; }               \
-    case 32: { constexpr int NN = 32; return EXPR; }               \
-    case 64: { constexpr int NN = 64; return EXPR; }               \
-    case 128: { constexpr int NN = 128; return EXPR; }             \
-    case 256: { constexpr int NN = 256; return EXPR; }             \
-    case 512: { constexpr int NN = 512; return EXPR; }             \
-    case 1024: { constexpr int NN = 1024; return EXPR; }           \
-    case 2048: { constexpr int NN = 2048; return EXPR; }           \
-    case 4096: { constexpr int NN = 4096; return EXPR; }           \
-    default: return ctx->fail(SSP_EINVAL, "unsupported N=%d", N_); \
-    }
 
 // the TMA generator runs the column plan (V = 1), the register-load one its own (V = 2); they differ at N >= 2048
 int screen_col_plan_variant(int N) { return (N == 512 || N == 1024) ? 1 : 2; }
