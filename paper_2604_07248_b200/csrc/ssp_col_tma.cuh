@@ -112,7 +112,7 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *sbuf = reinterpret_cast<float2 *>(smem_raw);
     unsigned long long *full = reinterpret_cast<unsigned long long *>(smem_raw + CFG::NBUF * sizeof(float2) * CFG::BUF_ELEMS);
-    const int tid = threadIdx.x, c = tid % C, t = tid / C;
+    const int tid = threadIdx.x, c = tid % C, t = fft_logical_t<N, 1, C>(tid / C);
 
     auto issue_load = [&](int tile, int buf) {
         const int b = tile / GROUPS, col0 = (tile % GROUPS) * C;

@@ -175,6 +175,30 @@ struct PlanInfo {
     static constexpr int TW_TOTAL = TW2R + R2 * R1;
 };
 
+// ---- three-stage plans (R, 2, R) with the middle stage done by warp shuffles -----------------------------
+// The radix-2 middle stage of N = 2048 pairs the elements m and m + N/(2R) of the first-stage output
+// (m = n2 (N/2R) + n3).  The thread that owns m is chosen so that the two partners sit 16 lanes apart in one warp:
+// with LS lanes per thread step (1 for rows, C for column tiles) and G = 16/LS,
+//     n2 = (t_phys / G) & 1,   n3 = (t_phys / 2G) G + t_phys % G.
+// The stage is then one __shfl_xor(.., 16) per value instead of a trip through shared memory -- one exchange and
+// one barrier per transform disappear -- and each half-warp still owns consecutive m, so global, tile and
+// exchange accesses stay contiguous.  All index arithmetic of the kernels runs on the LOGICAL thread index m
+// (fft_logical_t); input and output layouts stay "strided by R" in m.
+template <int N, int V>
+struct MidShuffle {
+    using P = Plan<N, V>;
+    static constexpr bool value = (P::R3 > 1) && (P::R2 == 2) && (P::R1 == P::R3) && (P::E == P::R1);
+};
+template <int N, int V, int LS>
+__device__ __forceinline__ int fft_logical_t(int t_phys)
+{
+    if constexpr (MidShuffle<N, V>::value) {
+        constexpr int G = 16 / LS;
+        static_assert(LS >= 1 && LS <= 8 && (N / Plan<N, V>::E) % (2 * G) == 0, "both partners inside one warp");
+        return ((t_phys / G) & 1) * Plan<N, V>::R3 + (t_phys / (2 * G)) * G + t_phys % G;
+    } else return t_phys;
+}
+
 // One complete transform of a line held in registers.
 //   DIR_REV = false: plan (R1,R2,R3): input strided by R1, output strided by RL.
 //   DIR_REV = true : plan (RL,..,R1): input strided by RL, output strided by R1.
@@ -199,6 +223,41 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 
     // with k1 explicit so that no division of a run-time index is left in the address arithmetic.
     constexpr int PITCH = PADQ + SM::PAD;
     static_assert(SM::PAD == 1 || NS <= 2, "16-byte exchange reads are laid out for two-stage plans");
+
+    if constexpr (MidShuffle<N, V>::value) {
+        // t is the logical index m = n2 Rc + n3; its partner (other n2) sits 16 lanes away
+        static_assert(E == Ra && Ra == Rc && Rb == 2, "(R, 2, R) plans with one first-stage butterfly per thread");
+        const int n2 = t / Rc, n3 = t % Rc;
+        radix<Ra, INV>(v);
+        const float4 *tw4 = reinterpret_cast<const float4 *>(tw1) + t;
+        const float2 w2 = __ldg(tw2 + Rc + n3);                    // W_N^(Ra n3) for the k2 = 1 output
+        // exchange pitches of k1 and k2: a half-warp owns one k2 and consecutive n3 (writes) / consecutive k1 (reads),
+        // and 2 Rc + 1 = 1 mod 16 spreads the reads over 16 bank pairs for rows and for C-column tiles alike
+        constexpr int P2 = Rc, P1 = 2 * Rc + 1;
+#pragma unroll
+        for (int k = 0; k < Ra; k += 2) {
+            const float4 w = __ldg(tw4 + (k / 2) * (N / Ra));
+            float2 x[2] = {v[k], v[k + 1]};
+            if (k > 0) x[0] = cmul_c<INV>(x[0], make_float2(w.x, w.y));
+            x[1] = cmul_c<INV>(x[1], make_float2(w.z, w.w));
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const float px = __shfl_xor_sync(0xffffffffu, x[e].x, 16);
+                const float py = __shfl_xor_sync(0xffffffffu, x[e].y, 16);
+                // k2 = n2: own + partner for k2 = 0, (partner - own) W_N^(Ra n3) for k2 = 1
+                float2 y = n2 ? make_float2(px - x[e].x, py - x[e].y) : make_float2(x[e].x + px, x[e].y + py);
+                if (n2) y = cmul_c<INV>(y, w2);
+                sm.st((k + e) * P1 + n2 * P2 + n3, y);
+            }
+        }
+        sm.sync();
+        const int k1 = t % Ra, k2 = t / Ra;                        // output X[k1 + Ra k2 + 2 Ra k3] = X[t + 2 Ra k3]
+#pragma unroll
+        for (int n = 0; n < Rc; ++n) v[n] = sm.ld(k1 * P1 + k2 * P2 + n);
+        if constexpr (TAIL_SYNC) sm.sync();
+        radix<Rc, INV>(v);
+        return;
+    }
 
     // ---- stage 1
     constexpr int M1 = N / Ra;

@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
     float2 *smem = reinterpret_cast<float2 *>(smem_raw);
 
     const int tid = threadIdx.x;
-    const int lib = tid / T, t = tid % T;
+    const int lib = tid / T, t = fft_logical_t<N, 0, 1>(tid % T);
     const long long line = (long long)blockIdx.x * CFG::LPB + lib;
     const int b = (int)(line / N), iy = (int)(line % N);
     RowSmem<T, CFG::WIDE> sm{smem + (size_t)lib * CFG::LINE_ELEMS, 1 + lib};
@@ -183,7 +183,7 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_c
     float2 *smem = reinterpret_cast<float2 *>(smem_raw);
 
     const int tid = threadIdx.x;
-    const int c = tid % C, t = tid / C;
+    const int c = tid % C, t = fft_logical_t<N, 1, C>(tid / C);
     constexpr int GROUPS = N / C;
     const int b = blockIdx.x / GROUPS, col = (blockIdx.x % GROUPS) * C + c;
     ColSmem<C> sm{smem + c};

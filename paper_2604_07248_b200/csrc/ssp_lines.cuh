@@ -68,6 +68,7 @@ struct ColCfg {
 template <int T, bool WIDE = false>
 struct RowSmem {
     static constexpr int PAD = WIDE ? 2 : 1;
+    static constexpr int LANE_STRIDE = 1;       // lanes per thread step of a line (ssp_fft.cuh: fft_logical_t)
     float2 *base; // this line's padded buffer
     int bar_id;
     __device__ __forceinline__ void ld2(int p, float2 &a, float2 &b) const
@@ -88,6 +89,7 @@ struct RowSmem {
 template <int C>
 struct ColSmem {
     static constexpr int PAD = 1;
+    static constexpr int LANE_STRIDE = C;       // lanes per thread step of a line (ssp_fft.cuh: fft_logical_t)
     float2 *base; // tile base + this thread's column
     __device__ __forceinline__ void st(int p, float2 x) { base[p * C] = x; }
     __device__ __forceinline__ float2 ld(int p) const { return base[p * C]; }

@@ -197,7 +197,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS + (N
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *smem = reinterpret_cast<float2 *>(smem_raw);
     const int tid = threadIdx.x;
-    const int lib = tid / T, t = tid % T;
+    const int lib = tid / T, t = fft_logical_t<N, 0, 1>(tid % T);
     const long long line = (long long)blockIdx.x * CFG::LPB + lib;
     const int scr = (int)(line / N), iy = (int)(line % N);
     RowSmem<T, CFG::WIDE> sm{smem + (size_t)lib * CFG::LINE_ELEMS, 1 + lib};
