@@ -145,12 +145,13 @@ SSP_PLAN(1024, 0, 32, 32, 1, 32);   SSP_PLAN(1024, 1, 32, 32, 1, 32);
 SSP_PLAN(2048, 0, 32, 2, 32, 32);   SSP_PLAN(2048, 1, 32, 2, 32, 32);
 SSP_PLAN(4096, 0, 32, 4, 32, 32);  SSP_PLAN(4096, 1, 32, 4, 32, 32);
 // V = 2 ("screen column" variant): what the register-load screen generator k_screen_col runs.  Equal to V = 1
-//   except at N >= 2048, where the single inverse transform measured faster with short last radices
-//   (4022 vs 3278 GB/s at 2048); the TMA generator (N <= 1024) uses V = 1.
+//   except at N = 4096, where the single inverse transform measured faster with short last radices than with
+//   (32,4,32); at 2048 it is the shuffle plan (32,2,32) like V = 1 (4216 vs 3430 GB/s with (32,8,8)).  The TMA
+//   generator (N = 512, 1024) uses V = 1.
 SSP_PLAN(8, 2, 8, 1, 1, 8);        SSP_PLAN(16, 2, 16, 1, 1, 16);     SSP_PLAN(32, 2, 32, 1, 1, 32);
 SSP_PLAN(64, 2, 8, 8, 1, 8);       SSP_PLAN(128, 2, 16, 8, 1, 16);    SSP_PLAN(256, 2, 16, 16, 1, 16);
 SSP_PLAN(512, 2, 32, 16, 1, 32);   SSP_PLAN(1024, 2, 32, 32, 1, 32);
-SSP_PLAN(2048, 2, 32, 8, 8, 32);   SSP_PLAN(4096, 2, 32, 16, 8, 32);
+SSP_PLAN(2048, 2, 32, 2, 32, 32);   SSP_PLAN(4096, 2, 32, 16, 8, 32);
 #undef SSP_PLAN
 
 template <int N, int V>

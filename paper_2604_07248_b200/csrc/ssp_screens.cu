@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(ColCfg<N, 2>::THREADS, ColCfg<N, 2>::MIN_BLOCK
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *smem = reinterpret_cast<float2 *>(smem_raw);
     const int tid = threadIdx.x;
-    const int c = tid % C, t = tid / C;
+    const int c = tid % C, t = fft_logical_t<N, 2, C>(tid / C);
     constexpr int GROUPS = N / C;
     const int scr = blockIdx.x / GROUPS, kx = (blockIdx.x % GROUPS) * C + c;
     ColSmem<C> sm{smem + c};
