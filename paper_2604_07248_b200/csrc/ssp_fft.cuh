@@ -140,7 +140,7 @@ SSP_PLAN(32, 0, 32, 1, 1, 32);     SSP_PLAN(32, 1, 32, 1, 1, 32);
 SSP_PLAN(64, 0, 8, 8, 1, 8);       SSP_PLAN(64, 1, 8, 8, 1, 8);
 SSP_PLAN(128, 0, 16, 8, 1, 16);    SSP_PLAN(128, 1, 16, 8, 1, 16);
 SSP_PLAN(256, 0, 16, 16, 1, 16);   SSP_PLAN(256, 1, 16, 16, 1, 16);
-SSP_PLAN(512, 0, 32, 16, 1, 32);   SSP_PLAN(512, 1, 32, 16, 1, 32);
+SSP_PLAN(512, 0, 16, 2, 16, 16);   SSP_PLAN(512, 1, 32, 16, 1, 32);
 SSP_PLAN(1024, 0, 32, 32, 1, 32);   SSP_PLAN(1024, 1, 32, 32, 1, 32);
 SSP_PLAN(2048, 0, 32, 2, 32, 32);   SSP_PLAN(2048, 1, 32, 2, 32, 32);
 SSP_PLAN(4096, 0, 32, 4, 32, 32);  SSP_PLAN(4096, 1, 32, 4, 32, 32);
@@ -195,7 +195,7 @@ __device__ __forceinline__ int fft_logical_t(int t_phys)
 {
     if constexpr (MidShuffle<N, V>::value) {
         constexpr int G = 16 / LS;
-        static_assert(LS >= 1 && LS <= 8 && (N / Plan<N, V>::E) % (2 * G) == 0, "both partners inside one warp");
+        static_assert(LS >= 1 && LS <= 16 && (N / Plan<N, V>::E) % (2 * G) == 0, "both partners inside one warp");
         return ((t_phys / G) & 1) * Plan<N, V>::R3 + (t_phys / (2 * G)) * G + t_phys % G;
     } else return t_phys;
 }

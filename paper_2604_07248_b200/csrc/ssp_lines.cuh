@@ -10,7 +10,7 @@ namespace ssp {
 // WIDE: pad 2 per row of the exchange matrix (16-byte aligned rows) and 16-byte reads; taken where a warp's
 // accesses stay conflict-free with it: the two-stage plans of N = 512 and 1024.
 template <int N>
-struct RowWide { static constexpr bool value = (N == 512 || N == 1024); };
+struct RowWide { static constexpr bool value = (N == 1024); };
 
 // Row-kernel CTA size and resident CTAs per SM the register budget is sized for.  Default: 256
 // threads, 512 resident threads at E = 32 and 1024 at E = 16.  N = 1024 (one warp per row, 32 points

@@ -117,7 +117,7 @@ k_screen_col_tma(const __grid_constant__ CUtensorMap tm_noise, const __grid_cons
     unsigned long long *full = reinterpret_cast<unsigned long long *>(smem_raw);
     float2 *buf_x = reinterpret_cast<float2 *>(smem_raw + CFG::HEAD);     // noise -> exchange -> result
     float2 *buf_s = buf_x + CFG::BUF_ELEMS;                               // old -> new spectrum (present iff used)
-    const int tid = threadIdx.x, c = tid % C, t = tid / C;
+    const int tid = threadIdx.x, c = tid % C, t = fft_logical_t<N, 1, C>(tid / C);
     const int scr = blockIdx.x / GROUPS, col0 = (blockIdx.x % GROUPS) * C, kx = col0 + c;
     constexpr bool ar = AR;
 

@@ -53,7 +53,7 @@ def _psds(orc):
 
 
 @pytest.mark.parametrize("kind", ["kolmogorov", "von_karman", "von_karman_592", "ocean", "power_law", "power_law_scales"])
-@pytest.mark.parametrize("N,n_sh", [(32, 3), (128, 3), (256, 0), (1024, 4)])
+@pytest.mark.parametrize("N,n_sh", [(32, 3), (128, 3), (256, 0), (512, 2), (1024, 4), (2048, 1)])
 def test_make_screens_parity(ssp, orc, kind, N, n_sh):
     import torch
     po, pg = _psds(orc)[kind]
