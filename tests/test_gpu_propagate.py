@@ -236,6 +236,12 @@ def test_error_codes(ssp):
     with pytest.raises(api.SspError) as e:
         ssp.propagate(N, dx, -1.0, [1.0], u)
     assert e.value.code == api.EINVAL
+    with pytest.raises(api.SspError) as e:                        # empty batch
+        ssp.propagate(N, dx, lam, [1.0], torch.zeros((0, N, N), dtype=torch.complex64, device="cuda"))
+    assert e.value.code == api.EINVAL
+    with pytest.raises(api.SspError) as e:                        # no steps
+        ssp.propagate(N, dx, lam, [], u)
+    assert e.value.code == api.EINVAL
     with pytest.raises(TypeError):
         ssp.propagate(N, dx, lam, [1.0], u.cpu())                # no CPU fallback
     assert ssp.launch_count() >= 0
