@@ -180,6 +180,26 @@ double ssp_hv57_cn2(const ssp_hv57 *p, double h);
 int ssp_hv57_path(const ssp_hv57 *p, double h0, double L, int n, double lambda, double *cn2, double *dz,
                   double *rytov, double *r0);
 
+/* Screen placement (Sec. 2.4).  Host-only, double precision.
+ * ssp_dz_max: the largest step the angular-spectrum transfer function (Eq. 6) supports before its phase
+ * aliases on the grid: |d psi / d kappa| dkappa <= pi at kappa0 = pi/dx, dkappa = 2 pi/(N dx), i.e.
+ * dz_max = (N dx / 2) sqrt(n0^2 k0^2 - kappa0^2) / kappa0 (Eq. 7 with the ratio and kappa0 corrected, Q17;
+ * paraxial limit N dx^2 n0 / lambda).  0 when the arguments are invalid or n0 k0 <= kappa0.
+ * ssp_place_screens: the routine of PAPER.md:109 on a piecewise-linear Cn2 profile (z_prof ascending, cn2_prof >= 0,
+ * host [n_prof]; constant beyond its ends) and the caller's desired interval edges (host [n_edges], ascending):
+ *   1. an interval whose Rytov variance (S19, z from the interval's start) exceeds rytov_limit is halved
+ *      until every piece is within it;  2. neighbours whose union stays within the limit are merged, left to right;
+ *   3. marching from the start, each end is moved to where the straight line through (last old edge within the
+ *      limit, its variance) and (next old edge, its variance) meets the limit, the move halved while the result
+ *      exceeds the limit (Q28);  4. an interval longer than dz_max is halved until it is not (dz_max <= 0: skip).
+ * Outputs, host [max_out] each: dz[j], the slab mean cn2[j] (ready for ssp_make_screens), optionally rytov[j]; *n_out =
+ * the number of intervals.  SSP_EWORKSPACE when more than max_out intervals are needed (*n_out = a lower bound on
+ * the count), SSP_EUNSUPPORTED when the limit cannot be met within 2^40 halvings, SSP_EINVAL on bad arguments. */
+double ssp_dz_max(ssp_grid grid, double lambda, double n0);
+int ssp_place_screens(const double *z_prof, const double *cn2_prof, int n_prof, const double *edges, int n_edges,
+                      double lambda, double rytov_limit, double dz_max, int max_out, double *dz, double *cn2,
+                      double *rytov, int *n_out);
+
 /* Workspace.  d_ws / ws_bytes: a caller-allocated device buffer of at least ssp_workspace_bytes(grid, B, S)
  * bytes, 16-byte aligned.  The screen calls need it (tables, subharmonic coefficients, the column-transformed
  * intermediate of a chunk of screens); the propagation calls, ssp_dft2_centered and ssp_propagate_host accept it

@@ -328,3 +328,100 @@ def hv57_path(h0, L, n, lam, A, V=21.0, ground_scale=1000.0):
                        epsabs=0, epsrel=1e-12, limit=400)[0]
     rytov = 3.27 * k ** (7.0 / 6.0) * L ** (5.0 / 6.0) * w
     return ints / (L / n), np.full(n, L / n), rytov, (0.423 * k * k * ints.sum()) ** (-3.0 / 5.0)
+
+
+# ---- screen placement (Sec 2.4; Eq. 7 with reading Q17; steps of :109 with reading Q28) -------
+def dz_max_angular_spectrum(N, dx, lam, n0=1.0):
+    """Largest step the angular-spectrum H (Eq. 6) supports before its phase aliases on the grid.
+    Phase psi = dz sqrt(n0^2 k0^2 - kappa^2); |d psi / d kappa| dkappa <= pi at the largest axis frequency
+    kappa0 = pi / dx with dkappa = 2 pi / (N dx) gives dz <= (N dx / 2) sqrt(n0^2 k0^2 - kappa0^2) / kappa0 (Q17:
+    Eq. 7 as printed has the ratio inverted and kappa0 = 2 pi / dx).  Paraxial limit: N dx^2 n0 / lam."""
+    k0 = 2.0 * np.pi / lam
+    kap = np.pi / dx
+    if n0 * k0 <= kap:
+        return 0.0
+    return 0.5 * N * dx * np.sqrt(n0 * n0 * k0 * k0 - kap * kap) / kap
+
+
+def interval_rytov(cn2_of_z, a, b, lam, kinks=()):
+    """S19 over the interval [a, b], z measured from a; adaptive quadrature, piece by piece between
+    the profile's kinks."""
+    from scipy import integrate
+    k = 2.0 * np.pi / lam
+    d = b - a
+    if d <= 0:
+        return 0.0
+    cuts = [a] + [float(p) for p in kinks if a < p < b] + [b]
+    w = sum(integrate.quad(lambda z: float(cn2_of_z(z)) * (1.0 - (z - a) / d) ** (5.0 / 3.0), lo, hi,
+                           epsabs=0, epsrel=1e-13)[0] for lo, hi in zip(cuts[:-1], cuts[1:]))
+    return 3.27 * k ** (7.0 / 6.0) * d ** (5.0 / 6.0) * w
+
+
+def place_screens(z_prof, cn2_prof, edges, lam, rytov_limit, dz_max=0.0, return_stages=False):
+    """The placement routine of PAPER.md:109, sentence by sentence, on a piecewise-linear Cn2(z) profile:
+      1. an interval whose Rytov variance exceeds the limit is halved until every piece is within it;
+      2. neighbours whose union stays within the limit are merged (left to right);
+      3. "linear fit": marching from the start, each interval's end is moved to where the straight line through
+         (last old edge within the limit, its variance) and (next old edge, its variance) meets the limit (Q28);
+         if the profile is not convex enough for that point to be within the limit, the move is halved until it is;
+      4. an interval longer than dz_max (Eq. 7) is halved until it is not.
+    Returns dz[n], the slab-mean cn2[n] and the interval Rytov variances."""
+    from scipy import integrate
+    z_prof = np.asarray(z_prof, dtype=np.float64)
+    cn2_prof = np.asarray(cn2_prof, dtype=np.float64)
+    f = lambda z: np.interp(z, z_prof, cn2_prof)
+    ry = lambda a, b: interval_rytov(f, a, b, lam, z_prof)
+    e = [float(x) for x in edges]
+    # 1
+    out = [e[0]]
+    for a, b in zip(e[:-1], e[1:]):
+        parts = 1
+        while max(ry(a + (b - a) * i / parts, a + (b - a) * (i + 1) / parts) for i in range(parts)) > rytov_limit:
+            parts *= 2
+        out += [a + (b - a) * (i + 1) / parts for i in range(parts)]
+    s1_edges = list(out)
+    # 2
+    i = 0
+    while i + 2 < len(out):
+        if ry(out[i], out[i + 2]) <= rytov_limit:
+            del out[i + 1]
+        else:
+            i += 1
+    s2_edges = list(out)
+    # 3
+    new, a, j, end = [out[0]], out[0], 1, out[-1]
+    while True:
+        b1, v1 = a, 0.0
+        while j < len(out) and (out[j] <= a or ry(a, out[j]) <= rytov_limit):
+            if out[j] > a:
+                b1, v1 = out[j], ry(a, out[j])
+            j += 1
+        if j >= len(out):
+            if end > a:
+                new.append(end)
+            break
+        b2, v2 = out[j], ry(a, out[j])
+        step = (rytov_limit - v1) / (v2 - v1) * (b2 - b1)
+        while ry(a, b1 + step) > rytov_limit:
+            step *= 0.5
+        new.append(b1 + step)
+        a = b1 + step
+    s3_edges = list(new)
+    # 4
+    fin = [new[0]]
+    for a, b in zip(new[:-1], new[1:]):
+        parts = 1
+        while dz_max > 0 and (b - a) / parts > dz_max:
+            parts *= 2
+        fin += [a + (b - a) * (i + 1) / parts for i in range(parts)]
+    fin = np.array(fin)
+    dz = np.diff(fin)
+    def seg(a, b):
+        cuts = [a] + [float(p) for p in z_prof if a < p < b] + [b]
+        return sum(integrate.quad(lambda z: float(f(z)), lo, hi, epsabs=0, epsrel=1e-13)[0]
+                   for lo, hi in zip(cuts[:-1], cuts[1:]))
+    cn2 = np.array([seg(a, b) for a, b in zip(fin[:-1], fin[1:])]) / dz
+    rys = np.array([ry(a, b) for a, b in zip(fin[:-1], fin[1:])])
+    if return_stages:
+        return dz, cn2, rys, dict(split=np.array(s1_edges), merged=np.array(s2_edges), fitted=np.array(s3_edges))
+    return dz, cn2, rys

@@ -27,7 +27,7 @@ SYMBOLS = (
     "ssp_create", "ssp_destroy", "ssp_last_error", "ssp_version", "ssp_launch_count",
     "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_make_screens_pair", "ssp_evolve_screens_pair", "ssp_propagate",
     "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_propagate_host", "ssp_phase_mul",
-    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path",
+    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path", "ssp_dz_max", "ssp_place_screens",
     "ssp_profile_enable", "ssp_profile_report",
 )
 
@@ -104,6 +104,9 @@ def load():
     lib.ssp_hv57_cn2.argtypes = [C.POINTER(Hv57), D]
     lib.ssp_hv57_cn2.restype = D
     lib.ssp_hv57_path.argtypes = [C.POINTER(Hv57), D, D, I, D, P, P, P, P]
+    lib.ssp_dz_max.argtypes = [Grid, D, D]
+    lib.ssp_dz_max.restype = D
+    lib.ssp_place_screens.argtypes = [P, P, I, P, I, D, D, D, I, P, P, P, P]
     lib.ssp_adam_update.argtypes = [P, Grid, I, P, D, D, D, D, I, P, P, P]
     lib.ssp_inner_products.argtypes = [P, Grid, I, P, P, P]
     lib.ssp_lincomb.argtypes = [P, Grid, I, P, P, P, P, P]
@@ -172,6 +175,29 @@ def hv57_path(h0, L, n, lam, A, V=21.0, ground_scale=0.0):
     if rc != OK:
         raise SspError(rc, "ssp_hv57_path: bad arguments")
     return cn2, dz, ry.value, r0.value
+
+
+def dz_max(N, dx, lam, n0=1.0):
+    """Largest alias-free angular-spectrum step on the grid (host call)."""
+    return load().ssp_dz_max(Grid(N, dx), float(lam), float(n0))
+
+
+def place_screens(z_prof, cn2_prof, edges, lam, rytov_limit, dz_max=0.0, max_out=4096):
+    """Screen placement on a piecewise-linear Cn2 profile: (dz[n], cn2[n], rytov[n]) as numpy (host call)."""
+    import numpy as np
+    zp = np.ascontiguousarray(z_prof, dtype=np.float64)
+    cp = np.ascontiguousarray(cn2_prof, dtype=np.float64)
+    ed = np.ascontiguousarray(edges, dtype=np.float64)
+    if zp.shape != cp.shape or zp.ndim != 1 or ed.ndim != 1:
+        raise SspError(EINVAL, "place_screens: z_prof / cn2_prof / edges must be 1-D, profile arrays of equal length")
+    dz, cn2, ry = np.empty(max_out), np.empty(max_out), np.empty(max_out)
+    n = C.c_int()
+    vp = lambda a: a.ctypes.data_as(C.c_void_p)
+    rc = load().ssp_place_screens(vp(zp), vp(cp), zp.size, vp(ed), ed.size, float(lam), float(rytov_limit),
+                                  float(dz_max), int(max_out), vp(dz), vp(cn2), vp(ry), C.byref(n))
+    if rc != OK:
+        raise SspError(rc, "ssp_place_screens failed (needs at least %d intervals)" % n.value)
+    return dz[:n.value].copy(), cn2[:n.value].copy(), ry[:n.value].copy()
 
 
 class Context:
