@@ -16,9 +16,13 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
-// grid: (blocks_per_field, B).  Each thread walks float4 pairs (2 pixels) grid-stride.
-__global__ void __launch_bounds__(256) k_stats_accum(const float2 *__restrict__ field, int N, int lo, int hi,
-                                                      double *__restrict__ acc)
+// grid: (blocks_per_field, B).  A block walks rows grid-stride; lanes = min(64, N/2) threads share a row
+// (lane_shift = log2(lanes)), each owning float4 pairs (2 pixels) at fixed columns.  Within one row a thread sums
+// I, x I, x^2 I and the ROI terms over its <= 64 pixels in fp32 (x is an exact small integer; the partial sums carry a
+// relative rounding of a few 1e-7 that averages out over the >= 10^4 partials of a field), then promotes the partials
+// to double once per row, where y enters.  Per-pixel fp64 accumulation ran at half the bandwidth: the fp64 pipe is narrow.
+__global__ void __launch_bounds__(256) k_stats_accum(const float2 *__restrict__ field, int N, int lane_shift, int lo,
+                                                      int hi, double *__restrict__ acc)
 {
     const int b = blockIdx.y;
     const size_t px = (size_t)N * N;
@@ -26,32 +30,49 @@ __global__ void __launch_bounds__(256) k_stats_accum(const float2 *__restrict__ 
     double a[ACC_N];
 #pragma unroll
     for (int i = 0; i < ACC_N; ++i) a[i] = 0.0;
-    const int half = N / 2;
-    for (size_t p2 = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p2 < px / 2;
-         p2 += (size_t)gridDim.x * blockDim.x) {
-        const float4 u = __ldg(f4 + p2);
-        const size_t p = 2 * p2;
-        const int iy = (int)(p / N), ix = (int)(p % N);
-        const float I2[2] = {fmaf(u.x, u.x, u.y * u.y), fmaf(u.z, u.z, u.w * u.w)};
+    const int half = N / 2, lanes = 1 << lane_shift, rows_per_pass = 256 >> lane_shift;
+    const int col0 = threadIdx.x & (lanes - 1);
+    for (int iy = blockIdx.x * rows_per_pass + (threadIdx.x >> lane_shift); iy < N; iy += gridDim.x * rows_per_pass) {
+        const float4 *row = f4 + (size_t)iy * half;
+        const bool roi_row = iy >= lo && iy < hi;
+        float s0 = 0.f, s1 = 0.f, s2 = 0.f, r1 = 0.f, r2 = 0.f, ax = 0.f;
+        for (int c = col0; c < half; c += 4 * lanes) {
+            float4 u[4];                                                 // four independent loads in flight;
 #pragma unroll
-        for (int e = 0; e < 2; ++e) {
-            const double I = (double)I2[e];
-            const double x = (double)(ix + e - half), y = (double)(iy - half);
-            a[ACC_I] += I;
-            a[ACC_X] += x * I;
-            a[ACC_Y] += y * I;
-            a[ACC_XX] += x * x * I;
-            a[ACC_YY] += y * y * I;
-            a[ACC_XY] += x * y * I;
-            if (iy >= lo && iy < hi && ix + e >= lo && ix + e < hi) {
-                a[ACC_RI] += I;
-                a[ACC_RI2] += I * I;
+            for (int j = 0; j < 4; ++j) {                                // a column past the end reads as zeros: adds nothing
+                const int cc = c + j * lanes;
+                u[j] = cc < half ? __ldg(row + cc) : make_float4(0.f, 0.f, 0.f, 0.f);
             }
-            if (iy == half && ix + e == half) a[ACC_AXIS] += I;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const float I2[2] = {fmaf(u[j].x, u[j].x, u[j].y * u[j].y), fmaf(u[j].z, u[j].z, u[j].w * u[j].w)};
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int ix = 2 * (c + j * lanes) + e;
+                    const float I = I2[e], x = (float)(ix - half), xI = x * I;
+                    s0 += I;
+                    s1 += xI;
+                    s2 = fmaf(x, xI, s2);
+                    const float Ir = (roi_row && ix >= lo && ix < hi) ? I : 0.f;
+                    r1 += Ir;
+                    r2 = fmaf(Ir, Ir, r2);
+                    ax += (iy == half && ix == half) ? I : 0.f;
+                }
+            }
         }
+        const double y = (double)(iy - half), d0 = (double)s0, d1 = (double)s1;
+        a[ACC_I] += d0;
+        a[ACC_X] += d1;
+        a[ACC_XX] += (double)s2;
+        a[ACC_Y] = fma(y, d0, a[ACC_Y]);
+        a[ACC_YY] = fma(y * y, d0, a[ACC_YY]);
+        a[ACC_XY] = fma(y, d1, a[ACC_XY]);
+        a[ACC_RI] += (double)r1;
+        a[ACC_RI2] += (double)r2;
+        a[ACC_AXIS] += (double)ax;
     }
-    // warp shuffles, then one partial per warp through shared memory, then ONE fp64 atomic per block and moment:
-    // all blocks of a field add into the same nine addresses, so the atomics are the contended resource
+    // warp shuffles, then one partial per warp through shared memory, then one partial per block and moment in
+    // acc[b][block][moment]; k_stats_final adds them in block order (no atomics: the result is reproducible bit by bit)
     __shared__ double part[8][ACC_N];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 #pragma unroll
@@ -64,16 +85,23 @@ __global__ void __launch_bounds__(256) k_stats_accum(const float2 *__restrict__ 
         double s = 0.0;
 #pragma unroll
         for (int w = 0; w < 8; ++w) s += part[w][threadIdx.x];
-        if (s != 0.0) atomicAdd(acc + (size_t)b * ACC_N + threadIdx.x, s);
+        acc[((size_t)b * gridDim.x + blockIdx.x) * ACC_N + threadIdx.x] = s;
     }
 }
 
-__global__ void k_stats_final(const double *__restrict__ acc, int B, double dx, long long roi_n,
-                              ssp_stats *__restrict__ out)
+// one warp per field: lane i < ACC_N adds moment i over the field's blocks, lane 0 finishes
+__global__ void __launch_bounds__(32) k_stats_final(const double *__restrict__ acc, int bpf, double dx, long long roi_n,
+                                                     ssp_stats *__restrict__ out)
 {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= B) return;
-    const double *a = acc + (size_t)b * ACC_N;
+    const int b = blockIdx.x;
+    __shared__ double a[ACC_N];
+    if (threadIdx.x < ACC_N) {
+        double s = 0.0;
+        for (int k = 0; k < bpf; ++k) s += acc[((size_t)b * bpf + k) * ACC_N + threadIdx.x];
+        a[threadIdx.x] = s;
+    }
+    __syncwarp();
+    if (threadIdx.x != 0) return;
     ssp_stats s;
     const double sI = a[ACC_I];
     s.power = sI * dx * dx;
@@ -102,21 +130,27 @@ __global__ void k_stats_final(const double *__restrict__ acc, int B, double dx, 
 int launch_stats(ssp_ctx *ctx, int N, double dx, int B, const float2 *field, double roi_frac,
                  ssp_stats *d_stats)
 {
-    if (int rc = ensure_scratch(ctx, sizeof(double) * ACC_N * (size_t)B)) return rc;
-    double *acc = reinterpret_cast<double *>(ctx->scratch);
-    SSP_CUDA(ctx, cudaMemsetAsync(acc, 0, sizeof(double) * ACC_N * (size_t)B, ctx->stream));
     int h = (int)floor(roi_frac * N / 2.0);
     int lo = N / 2 - h, hi = N / 2 + h;
     if (h <= 0) { lo = N / 2; hi = N / 2 + 1; }
     if (lo < 0) lo = 0;
     if (hi > N) hi = N;
     const long long roi_n = (long long)(hi - lo) * (hi - lo);
-    const size_t pairs = (size_t)N * N / 2;
-    int bpf = (int)((pairs + 256 * 32 - 1) / (256 * 32)); // ~64 pixels per thread
-    if (bpf < 1) bpf = 1;
+    int lane_shift = 0;
+    while ((2 << lane_shift) <= N / 2 && lane_shift < 6) ++lane_shift;       // lanes = min(64, N/2)
+    const int rows_per_pass = 256 >> lane_shift;
+    // blocks per field: all B * bpf blocks resident at once (8 per SM) when the batch allows, every block the same
+    // number of row passes (to within one)
+    const int passes = N / rows_per_pass;
+    int target = (ctx->num_sms * 8) / B;
+    if (target < 1) target = 1;
+    const int per = (passes + target - 1) / target;
+    const int bpf = (passes + per - 1) / per;
+    if (int rc = ensure_scratch(ctx, sizeof(double) * ACC_N * (size_t)B * bpf)) return rc;
+    double *acc = reinterpret_cast<double *>(ctx->scratch);
     ctx->prof_begin("stats", 8.0 * (double)B * N * N);
-    k_stats_accum<<<dim3(bpf, B), 256, 0, ctx->stream>>>(field, N, lo, hi, acc);
-    k_stats_final<<<(B + 127) / 128, 128, 0, ctx->stream>>>(acc, B, dx, roi_n, d_stats);
+    k_stats_accum<<<dim3(bpf, B), 256, 0, ctx->stream>>>(field, N, lane_shift, lo, hi, acc);
+    k_stats_final<<<B, 32, 0, ctx->stream>>>(acc, bpf, dx, roi_n, d_stats);
     ctx->prof_end();
     ctx->launches += 2;
     SSP_CUDA(ctx, cudaGetLastError());
