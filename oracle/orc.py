@@ -425,3 +425,42 @@ def place_screens(z_prof, cn2_prof, edges, lam, rytov_limit, dz_max=0.0, return_
     if return_stages:
         return dz, cn2, rys, dict(split=np.array(s1_edges), merged=np.array(s2_edges), fitted=np.array(s3_edges))
     return dz, cn2, rys
+
+
+# ---- counter-based noise (the "unit-variance complex Gaussian" draws of S16; reading Q29) -------------
+def philox4x32_10(counter, key):
+    """Philox-4x32 with 10 rounds (Salmon et al., SC'11), vectorised over counters.
+    counter: uint32 [n][4], key: (k0, k1).  Returns uint32 [n][4].
+    One round:  (c0, c1, c2, c3) <- (hi(M1 c2) ^ c1 ^ k0, lo(M1 c2), hi(M0 c0) ^ c3 ^ k1, lo(M0 c0)),
+    then the key is bumped by the Weyl constants."""
+    M0, M1, W0, W1 = 0xD2511F53, 0xCD9E8D57, 0x9E3779B9, 0xBB67AE85
+    c = [np.asarray(counter)[:, i].astype(np.uint64) for i in range(4)]
+    k0, k1 = int(key[0]) & 0xFFFFFFFF, int(key[1]) & 0xFFFFFFFF
+    mask = np.uint64(0xFFFFFFFF)
+    for _ in range(10):
+        p0 = np.uint64(M0) * c[0]
+        p1 = np.uint64(M1) * c[2]
+        c = [(p1 >> np.uint64(32)) ^ c[1] ^ np.uint64(k0), p1 & mask,
+             (p0 >> np.uint64(32)) ^ c[3] ^ np.uint64(k1), p0 & mask]
+        k0 = (k0 + W0) & 0xFFFFFFFF
+        k1 = (k1 + W1) & 0xFFFFFFFF
+    return np.stack(c, axis=1).astype(np.uint32)
+
+
+def noise(seed, stream, n, first=0):
+    """n complex draws, Re and Im each N(0, 1) (Q3), numbered first .. first+n-1 within (seed, stream).
+    Draws 2i and 2i+1 come from the Philox block with counter (i mod 2^32, i >> 32, stream mod 2^32, stream >> 32) and
+    key (seed mod 2^32, seed >> 32): words (x0, x1) make draw 2i, (x2, x3) draw 2i+1, by Box-Muller on 24-bit
+    uniforms (exact in fp32 and fp64):  u = ((x_even >> 8) + 1/2) 2^-24,  f = ((x_odd >> 8) + 1/2) 2^-24,
+    z = sqrt(-2 ln u) (cos 2 pi f + i sin 2 pi f)."""
+    i0, i1 = first // 2, (first + n + 1) // 2
+    idx = np.arange(i0, i1, dtype=np.uint64)
+    ctr = np.stack([idx & np.uint64(0xFFFFFFFF), idx >> np.uint64(32),
+                    np.full(idx.shape, int(stream) & 0xFFFFFFFF, dtype=np.uint64),
+                    np.full(idx.shape, (int(stream) >> 32) & 0xFFFFFFFF, dtype=np.uint64)], axis=1)
+    x = philox4x32_10(ctr, (int(seed) & 0xFFFFFFFF, (int(seed) >> 32) & 0xFFFFFFFF)).astype(np.float64)
+    x = x.reshape(-1, 2)                                                   # one (radius word, angle word) pair per draw
+    u = (np.floor(x[:, 0] / 256.0) + 0.5) / 16777216.0
+    f = (np.floor(x[:, 1] / 256.0) + 0.5) / 16777216.0
+    z = np.sqrt(-2.0 * np.log(u)) * np.exp(2j * np.pi * f)
+    return z[first - 2 * i0: first - 2 * i0 + n]
