@@ -180,6 +180,14 @@ double ssp_hv57_cn2(const ssp_hv57 *p, double h);
 int ssp_hv57_path(const ssp_hv57 *p, double h0, double L, int n, double lambda, double *cn2, double *dz,
                   double *rytov, double *r0);
 
+/* Device-side noise draws (PAPER.md:359 S16 "unit-variance complex Gaussian"; Q3, Q29).  Fills d_out (dev
+ * complex64 [n], 16-byte aligned) with draws first .. first+n-1 of the stream (seed, stream); Re and Im each N(0, 1).
+ * Philox-4x32-10 block i = counter (i, stream), key seed; words (x0,x1) -> draw 2i, (x2,x3) -> draw 2i+1 by Box-Muller
+ * on 23-bit uniforms.  first must be even.  The result is a plain noise array for ssp_make_screens / ssp_evolve_screens
+ * (their noise arguments stay inputs: any generator may fill them).  Enqueued on the context's stream. */
+int ssp_fill_noise(ssp_ctx *ctx, unsigned long long seed, unsigned long long stream, unsigned long long first,
+                   unsigned long long n, float *d_out);
+
 /* Screen placement (Sec. 2.4).  Host-only, double precision.
  * ssp_dz_max: the largest step the angular-spectrum transfer function (Eq. 6) supports before its phase
  * aliases on the grid: |d psi / d kappa| dkappa <= pi at kappa0 = pi/dx, dkappa = 2 pi/(N dx), i.e.

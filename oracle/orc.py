@@ -450,8 +450,8 @@ def philox4x32_10(counter, key):
 def noise(seed, stream, n, first=0):
     """n complex draws, Re and Im each N(0, 1) (Q3), numbered first .. first+n-1 within (seed, stream).
     Draws 2i and 2i+1 come from the Philox block with counter (i mod 2^32, i >> 32, stream mod 2^32, stream >> 32) and
-    key (seed mod 2^32, seed >> 32): words (x0, x1) make draw 2i, (x2, x3) draw 2i+1, by Box-Muller on 24-bit
-    uniforms (exact in fp32 and fp64):  u = ((x_even >> 8) + 1/2) 2^-24,  f = ((x_odd >> 8) + 1/2) 2^-24,
+    key (seed mod 2^32, seed >> 32): words (x0, x1) make draw 2i, (x2, x3) draw 2i+1, by Box-Muller on 23-bit
+    uniforms (k + 1/2 with k < 2^23 is exact in fp32 and fp64):  u = ((x_even >> 9) + 1/2) 2^-23,  f = ((x_odd >> 9) + 1/2) 2^-23,
     z = sqrt(-2 ln u) (cos 2 pi f + i sin 2 pi f)."""
     i0, i1 = first // 2, (first + n + 1) // 2
     idx = np.arange(i0, i1, dtype=np.uint64)
@@ -460,7 +460,7 @@ def noise(seed, stream, n, first=0):
                     np.full(idx.shape, (int(stream) >> 32) & 0xFFFFFFFF, dtype=np.uint64)], axis=1)
     x = philox4x32_10(ctr, (int(seed) & 0xFFFFFFFF, (int(seed) >> 32) & 0xFFFFFFFF)).astype(np.float64)
     x = x.reshape(-1, 2)                                                   # one (radius word, angle word) pair per draw
-    u = (np.floor(x[:, 0] / 256.0) + 0.5) / 16777216.0
-    f = (np.floor(x[:, 1] / 256.0) + 0.5) / 16777216.0
+    u = (np.floor(x[:, 0] / 512.0) + 0.5) / 8388608.0
+    f = (np.floor(x[:, 1] / 512.0) + 0.5) / 8388608.0
     z = np.sqrt(-2.0 * np.log(u)) * np.exp(2j * np.pi * f)
     return z[first - 2 * i0: first - 2 * i0 + n]

@@ -27,7 +27,7 @@ SYMBOLS = (
     "ssp_create", "ssp_destroy", "ssp_last_error", "ssp_version", "ssp_launch_count",
     "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_make_screens_pair", "ssp_evolve_screens_pair", "ssp_propagate",
     "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_propagate_host", "ssp_phase_mul",
-    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path", "ssp_dz_max", "ssp_place_screens",
+    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path", "ssp_dz_max", "ssp_place_screens", "ssp_fill_noise",
     "ssp_profile_enable", "ssp_profile_report",
 )
 
@@ -104,6 +104,7 @@ def load():
     lib.ssp_hv57_cn2.argtypes = [C.POINTER(Hv57), D]
     lib.ssp_hv57_cn2.restype = D
     lib.ssp_hv57_path.argtypes = [C.POINTER(Hv57), D, D, I, D, P, P, P, P]
+    lib.ssp_fill_noise.argtypes = [P, C.c_ulonglong, C.c_ulonglong, C.c_ulonglong, C.c_ulonglong, P]
     lib.ssp_dz_max.argtypes = [Grid, D, D]
     lib.ssp_dz_max.restype = D
     lib.ssp_place_screens.argtypes = [P, P, I, P, I, D, D, D, I, P, P, P, P]
@@ -382,6 +383,12 @@ class Context:
         self._chk(self._lib.ssp_adam_update(self._h, Grid(N, dx), grad.shape[0], _dev(grad, torch.float32), float(lr),
                                             float(beta1), float(beta2), float(eps), int(t), _dev(m, torch.float32),
                                             _dev(v, torch.float32), _dev(theta, torch.float32)))
+
+    def fill_noise(self, seed, stream, out, first=0):
+        """Fill the complex64 CUDA tensor `out` (any shape, contiguous) with draws first.. of the stream (seed, stream)."""
+        self._chk(self._lib.ssp_fill_noise(self._h, int(seed), int(stream), int(first), out.numel(),
+                                           _dev(out, torch.complex64)))
+        return out
 
     def aperture(self, N, dx, radius, field, out=None):
         out = torch.empty_like(field) if out is None else out

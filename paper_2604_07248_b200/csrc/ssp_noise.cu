@@ -1,0 +1,81 @@
+// ssp_noise.cu -- device-side draws of the "unit-variance complex Gaussian" noise of the screen synthesis
+// (PAPER.md:359 S16; Q3, Q29).  The paper draws it with its framework's generator on the GPU; here the noise
+// arrays stay plain inputs of the screen calls and this kernel optionally fills them from (seed, stream).
+//
+// Generator: Philox-4x32 with 10 rounds (Salmon, Moraes, Dror, Shaw, SC'11).  Block i of a stream has counter
+// (i mod 2^32, i >> 32, stream mod 2^32, stream >> 32) and key (seed mod 2^32, seed >> 32); its words (x0, x1) make
+// draw 2i and (x2, x3) draw 2i+1 by Box-Muller on 23-bit uniforms (k + 1/2, k < 2^23, is exact in fp32):
+//   u = ((x_even >> 9) + 1/2) 2^-23,  f = ((x_odd >> 9) + 1/2) 2^-23,  z = sqrt(-2 ln u) (cos 2 pi f + i sin 2 pi f).
+// One thread makes one block = two complex64 draws = one 16-byte store; pure ALU + write stream (8 B per draw).
+#include "ssp_internal.h"
+
+namespace ssp {
+
+__device__ __forceinline__ void philox_round(uint32_t (&c)[4], uint32_t k0, uint32_t k1)
+{
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+    const uint32_t h0 = __umulhi(M0, c[0]), l0 = M0 * c[0];
+    const uint32_t h1 = __umulhi(M1, c[2]), l1 = M1 * c[2];
+    c[0] = h1 ^ c[1] ^ k0;
+    c[1] = l1;
+    c[2] = h0 ^ c[3] ^ k1;
+    c[3] = l0;
+}
+
+__device__ __forceinline__ float2 box_muller(uint32_t xr, uint32_t xa)
+{
+    const float u = ((float)(xr >> 9) + 0.5f) * 1.1920928955078125e-7f;          // 2^-23; k + 1/2 needs 24 bits: exact
+    const float f2 = ((float)(xa >> 9) + 0.5f) * 2.384185791015625e-7f;          // 2 f, so that sincospi sees the angle 2 pi f
+    const float r = sqrtf(-2.0f * logf(u));
+    float s, c;
+    sincospif(f2, &s, &c);
+    return make_float2(r * c, r * s);
+}
+
+__global__ void __launch_bounds__(256) k_fill_noise(uint32_t k0, uint32_t k1, uint32_t s0, uint32_t s1,
+                                                     unsigned long long first_block, unsigned long long n_draws,
+                                                     float2 *__restrict__ out)
+{
+    const unsigned long long j = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;   // block within this call
+    if (2 * j >= n_draws) return;
+    const unsigned long long i = first_block + j;
+    uint32_t c[4] = {(uint32_t)i, (uint32_t)(i >> 32), s0, s1};
+    uint32_t a = k0, b = k1;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        philox_round(c, a, b);
+        a += 0x9E3779B9u;
+        b += 0xBB67AE85u;
+    }
+    const float2 z0 = box_muller(c[0], c[1]), z1 = box_muller(c[2], c[3]);
+    if (2 * j + 1 < n_draws) reinterpret_cast<float4 *>(out)[j] = make_float4(z0.x, z0.y, z1.x, z1.y);
+    else out[2 * j] = z0;
+}
+
+int launch_fill_noise(ssp_ctx *ctx, unsigned long long seed, unsigned long long stream, unsigned long long first,
+                      unsigned long long n, float2 *out)
+{
+    const unsigned long long blocks = (n + 1) / 2;
+    const unsigned long long grid = (blocks + 255) / 256;
+    if (grid > 0x7FFFFFFFull) return ctx->fail(SSP_EINVAL, "ssp_fill_noise: more than 2^40 draws in one call");
+    ctx->prof_begin("fill_noise", 8.0 * (double)n);
+    k_fill_noise<<<(unsigned)grid, 256, 0, ctx->stream>>>((uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)stream,
+                                                          (uint32_t)(stream >> 32), first / 2, n, out);
+    ctx->prof_end();
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
+} // namespace ssp
+
+extern "C" int ssp_fill_noise(ssp_ctx *ctx, unsigned long long seed, unsigned long long stream,
+                              unsigned long long first, unsigned long long n, float *d_out)
+{
+    if (!ctx) return SSP_EINVAL;
+    if (n == 0) return SSP_OK;
+    if (!d_out || (first & 1ull) || (reinterpret_cast<uintptr_t>(d_out) & 15u))
+        return ctx->fail(SSP_EINVAL, "ssp_fill_noise: null or misaligned output, or odd first draw");
+    SSP_CUDA(ctx, cudaSetDevice(ctx->device));
+    return ssp::launch_fill_noise(ctx, seed, stream, first, n, reinterpret_cast<float2 *>(d_out));
+}

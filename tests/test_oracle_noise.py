@@ -18,8 +18,8 @@ def test_noise_law(orc):
     assert abs(np.mean(np.abs(z) ** 2) - 2) < 4 * 2 / np.sqrt(NS)                # E|z|^2 = 2 (Q3)
     assert stats.kstest(np.abs(z) ** 2, "expon", args=(0, 2)).pvalue > 1e-3      # |z|^2 ~ Exp(mean 2)
     assert stats.kstest(np.angle(z), "uniform", args=(-np.pi, 2 * np.pi)).pvalue > 1e-3
-    # 24-bit uniforms: the radius is finite and at most sqrt(-2 ln 2^-25)
-    assert np.all(np.isfinite(z.view(np.float64))) and np.abs(z).max() <= np.sqrt(50 * np.log(2)) + 1e-12
+    # 23-bit uniforms: the radius is finite and at most sqrt(-2 ln 2^-24)
+    assert np.all(np.isfinite(z.view(np.float64))) and np.abs(z).max() <= np.sqrt(48 * np.log(2)) + 1e-12
 
 
 def test_noise_independence(orc):
