@@ -253,7 +253,9 @@ int ssp_beam_stats(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_field, dou
 /* End-to-end form of ssp_propagate with HOST buffers: copies field and screens to the
  * device buffers given (d_field [B][N][N] c64, d_screens as above), propagates, copies
  * the output field and statistics back, and synchronises the stream.  h_* pointers are
- * host memory (pinned for full copy speed and overlap).  The batch is processed in chunks of
+ * host memory (pinned for full copy speed and overlap).  h_screens == NULL with S > 0: the
+ * screens are already in d_screens (made there by ssp_make_screens / ssp_evolve_screens, e.g.
+ * from ssp_fill_noise draws) and only the fields travel.  The batch is processed in chunks of
  * max(1, B/8) fields on two internal copy streams, so that the copies of neighbouring chunks
  * overlap the propagation; results equal ssp_propagate's. */
 int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind,
@@ -263,6 +265,30 @@ int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, in
                        ssp_stats *h_stats, double roi_frac,
                        float *d_field, float *d_screens, ssp_stats *d_stats,
                        void *d_ws, size_t ws_bytes);
+
+/* One temporal frame end to end from HOST fields (the workload of PAPER.md:76-84: every frame the screens evolve
+ * by the autoregression of Eq. 5 and a batch of fields propagates through them).  Per chunk of ssp_frame_chunk(B)
+ * fields: fresh noise is drawn on the device (ssp_fill_noise: stream 2*frame for the grid noise of the whole batch,
+ * draw index = element index in [B][S][N][N]; stream 2*frame+1 for the subharmonic noise [B][S][n_sh][3][3]), the
+ * chunk's screen stacks evolve (ssp_evolve_screens), its fields propagate through them (ssp_propagate with
+ * n_steps = S, step dz[j] = slab dz[j], per-field stacks; launched per group of n/2, n/4, .., 1, 1 chunks), and output
+ * fields and statistics return to the host; the uploads run under the first chunks' draws and evolution, the
+ * downloads under the next chunks' work.  The result
+ * equals those three calls on the whole batch.  Device buffers: d_field c64 [B][N][N]; d_spectrum c64
+ * [B][S][N][N] and d_sh_coef c64 [B][S][n_sh][3][3], in-out (the AR state, from ssp_make_screens); d_screens fp32
+ * [B][S][N][N] (out: this frame's screens); d_noise c64 [ssp_frame_chunk(B)][S][N][N] scratch; d_noise_sh c64
+ * [B][S][n_sh][3][3] scratch; d_stats [B]; d_ws >= ssp_workspace_bytes(grid, ssp_frame_chunk(B), S).
+ * Synchronises the stream. */
+typedef struct {
+    double a, vx, vy, T;            /* blending factor, wind [m/s], frame interval [s] (Eq. 4, 5) */
+    unsigned long long seed, frame; /* noise streams 2*frame and 2*frame+1 of this seed */
+} ssp_ar;
+int ssp_frame_chunk(int B);
+int ssp_frame_host(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, double n0, int h_kind,
+                   int B, int S, const double *cn2, const double *dz, int n_sh, const ssp_ar *ar,
+                   ssp_window win, const float *h_field_in, float *h_field_out, ssp_stats *h_stats, double roi_frac,
+                   float *d_field, float *d_spectrum, float *d_sh_coef, float *d_screens,
+                   float *d_noise, float *d_noise_sh, ssp_stats *d_stats, void *d_ws, size_t ws_bytes);
 
 /* ---- helpers for mask systems (config 4; O9) ----------------- */
 

@@ -27,7 +27,7 @@ SYMBOLS = (
     "ssp_create", "ssp_destroy", "ssp_last_error", "ssp_version", "ssp_launch_count",
     "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_make_screens_pair", "ssp_evolve_screens_pair", "ssp_propagate",
     "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_propagate_host", "ssp_phase_mul",
-    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path", "ssp_dz_max", "ssp_place_screens", "ssp_fill_noise",
+    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path", "ssp_dz_max", "ssp_place_screens", "ssp_fill_noise", "ssp_frame_chunk", "ssp_frame_host",
     "ssp_profile_enable", "ssp_profile_report",
 )
 
@@ -54,6 +54,11 @@ class Hv57(C.Structure):
 
 class Window(C.Structure):
     _fields_ = [("order", C.c_int), ("sigma_frac", C.c_double)]
+
+
+class Ar(C.Structure):
+    _fields_ = [("a", C.c_double), ("vx", C.c_double), ("vy", C.c_double), ("T", C.c_double),
+                ("seed", C.c_ulonglong), ("frame", C.c_ulonglong)]
 
 
 class Stats(C.Structure):
@@ -97,6 +102,9 @@ def load():
     lib.ssp_beam_stats.argtypes = [P, Grid, I, P, D, P, P, P, C.POINTER(L)]
     lib.ssp_propagate_host.argtypes = [P, Grid, D, D, I, I, I, P, P, L, I, Window, P, P, P, D, P, P, P, P,
                                        C.c_size_t]
+    lib.ssp_frame_chunk.argtypes = [I]
+    lib.ssp_frame_host.argtypes = [P, Grid, P, D, D, I, I, I, P, P, I, P, Window, P, P, P, D, P, P, P, P, P, P, P, P,
+                                   C.c_size_t]
     lib.ssp_phase_mul.argtypes = [P, Grid, I, P, D, P, P]
     lib.ssp_dft2_centered.argtypes = [P, Grid, I, I, P, P, P, C.c_size_t]
     lib.ssp_phase_grad.argtypes = [P, Grid, I, P, P, P]
@@ -176,6 +184,11 @@ def hv57_path(h0, L, n, lam, A, V=21.0, ground_scale=0.0):
     if rc != OK:
         raise SspError(rc, "ssp_hv57_path: bad arguments")
     return cn2, dz, ry.value, r0.value
+
+
+def frame_chunk(B):
+    """Fields per pipeline chunk of frame_host / propagate_host."""
+    return int(load().ssp_frame_chunk(int(B)))
 
 
 def dz_max(N, dx, lam, n0=1.0):
@@ -364,6 +377,22 @@ class Context:
             hp(h_screens), stride, S, Window(win_order, win_sigma_frac), hp(h_field_in), hp(h_field_out),
             hp(h_stats), roi_frac, _dev(d_field, torch.complex64), _dev(d_screens, torch.float32),
             _dev(d_stats), None, 0))
+
+    def frame_host(self, N, dx, psd: PsdParams, lam, cn2, dz, n_sh, a, vx, vy, T, seed, frame, h_field_in, h_field_out,
+                   h_stats, roi_frac, d_field, spectrum, sh_coef, screens, d_noise, d_noise_sh, d_stats, ws,
+                   win_order=0, win_sigma_frac=0.0, n0=1.0, h_kind=H_FRESNEL):
+        """One temporal frame from pinned host fields: device-side noise draws, AR screen evolution, propagation,
+        results back on the host.  d_noise: complex64 [frame_chunk(B)][S][N][N] scratch.  Synchronises the stream."""
+        B, S = d_field.shape[0], screens.shape[1]
+        pc, ar = psd.c(), Ar(a, vx, vy, T, int(seed), int(frame))
+        hp = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+        self._chk(self._lib.ssp_frame_host(
+            self._h, Grid(N, dx), C.byref(pc), lam, n0, h_kind, B, S, _host_doubles(cn2), _host_doubles(dz), n_sh,
+            C.byref(ar), Window(win_order, win_sigma_frac), hp(h_field_in), hp(h_field_out), hp(h_stats), roi_frac,
+            _dev(d_field, torch.complex64), _dev(spectrum, torch.complex64),
+            _dev(sh_coef, torch.complex64) if n_sh > 0 else None, _dev(screens, torch.float32),
+            _dev(d_noise, torch.complex64), _dev(d_noise_sh, torch.complex64) if n_sh > 0 else None,
+            _dev(d_stats), _dev(ws), ws.numel()))
 
     # ---- helpers ---------------------------------------------------------------------------
     def phase_mul(self, N, dx, theta, field, sign=1.0, out=None):

@@ -359,7 +359,7 @@ int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, in
     if (!ctx) return SSP_EINVAL;
     if (!valid_N(grid.N) || B < 1 || S < 0) return ctx->fail(SSP_EINVAL, "bad grid, batch or S");
     if (!h_field_in || !h_field_out || !d_field) return ctx->fail(SSP_EINVAL, "field buffers are required");
-    if (S > 0 && (!h_screens || !d_screens)) return ctx->fail(SSP_EINVAL, "screen buffers are required");
+    if (S > 0 && !d_screens) return ctx->fail(SSP_EINVAL, "d_screens is required");
     if (h_stats && !d_stats) return ctx->fail(SSP_EINVAL, "d_stats is required with h_stats");
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));
     const size_t px = (size_t)grid.N * grid.N;
@@ -382,7 +382,8 @@ int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, in
     SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_in, ev_start, 0));
     SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_out, ev_start, 0));
     const bool shared = (screen_batch_stride == 0);
-    if (S > 0 && shared)
+    const bool copy_screens = S > 0 && h_screens;               // NULL: the screens are already in d_screens
+    if (copy_screens && shared)
         SSP_CUDA(ctx, cudaMemcpyAsync(d_screens, h_screens, sizeof(float) * (size_t)S * px, cudaMemcpyHostToDevice, ctx->copy_in));
     for (int c = 0; c < n_chunks; ++c) {
         const int b0 = c * Bc, nb = (B - b0 < Bc) ? B - b0 : Bc;
@@ -390,8 +391,8 @@ int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, in
         float *df = d_field + 2 * px * (size_t)b0;
         SSP_CUDA(ctx, cudaMemcpyAsync(df, h_field_in + 2 * px * (size_t)b0, sizeof(float) * 2 * px * nb, cudaMemcpyHostToDevice, ctx->copy_in));
         float *ds = d_screens;
-        if (S > 0 && !shared) {
-            ds = d_screens + (size_t)b0 * (size_t)screen_batch_stride;
+        if (S > 0 && !shared) ds = d_screens + (size_t)b0 * (size_t)screen_batch_stride;
+        if (copy_screens && !shared) {
             const size_t n_scr = (size_t)(nb - 1) * (size_t)screen_batch_stride + (size_t)S * px;
             SSP_CUDA(ctx, cudaMemcpyAsync(ds, h_screens + (size_t)b0 * (size_t)screen_batch_stride, sizeof(float) * n_scr,
                                           cudaMemcpyHostToDevice, ctx->copy_in));
@@ -406,6 +407,85 @@ int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, in
         SSP_CUDA(ctx, cudaMemcpyAsync(h_field_out + 2 * px * (size_t)b0, df, sizeof(float) * 2 * px * nb, cudaMemcpyDeviceToHost, ctx->copy_out));
         if (h_stats)
             SSP_CUDA(ctx, cudaMemcpyAsync(h_stats + b0, d_stats + b0, sizeof(ssp_stats) * nb, cudaMemcpyDeviceToHost, ctx->copy_out));
+    }
+    SSP_CUDA(ctx, cudaEventRecord(ev_end, ctx->copy_out));
+    SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ev_end, 0));
+    SSP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SSP_OK;
+}
+
+int ssp_frame_chunk(int B) { return B >= 8 ? B / 8 : 1; }
+
+int ssp_frame_host(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, double n0, int h_kind,
+                   int B, int S, const double *cn2, const double *dz, int n_sh, const ssp_ar *ar,
+                   ssp_window win, const float *h_field_in, float *h_field_out, ssp_stats *h_stats, double roi_frac,
+                   float *d_field, float *d_spectrum, float *d_sh_coef, float *d_screens,
+                   float *d_noise, float *d_noise_sh, ssp_stats *d_stats, void *d_ws, size_t ws_bytes)
+{
+    if (!ctx) return SSP_EINVAL;
+    if (!valid_N(grid.N) || B < 1 || S < 1 || !ar || !psd) return ctx->fail(SSP_EINVAL, "bad grid, batch, S or parameters");
+    if (!h_field_in || !h_field_out || !d_field || !d_spectrum || !d_screens || !d_noise)
+        return ctx->fail(SSP_EINVAL, "field, spectrum, screen and noise buffers are required");
+    if (n_sh > 0 && (!d_sh_coef || !d_noise_sh)) return ctx->fail(SSP_EINVAL, "subharmonic buffers are required");
+    if (h_stats && !d_stats) return ctx->fail(SSP_EINVAL, "d_stats is required with h_stats");
+    SSP_CUDA(ctx, cudaSetDevice(ctx->device));
+    const size_t px = (size_t)grid.N * grid.N;
+    if (!ctx->copy_in) {
+        SSP_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_in, cudaStreamNonBlocking));
+        SSP_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_out, cudaStreamNonBlocking));
+    }
+    const int Bc = ssp_frame_chunk(B);
+    const int n_chunks = (B + Bc - 1) / Bc;
+    while ((int)ctx->pipe_events.size() < 2 * n_chunks + 2) {
+        cudaEvent_t e;
+        SSP_CUDA(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        ctx->pipe_events.push_back(e);
+    }
+    cudaEvent_t ev_start = ctx->pipe_events[2 * n_chunks], ev_end = ctx->pipe_events[2 * n_chunks + 1];
+    SSP_CUDA(ctx, cudaEventRecord(ev_start, ctx->stream));       // earlier work may still use the device buffers
+    SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_in, ev_start, 0));
+    SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_out, ev_start, 0));
+    // every field's upload is queued at once: it runs under the noise draws and the screen evolution of the first chunks
+    for (int c = 0; c < n_chunks; ++c) {
+        const int b0 = c * Bc, nb = (B - b0 < Bc) ? B - b0 : Bc;
+        SSP_CUDA(ctx, cudaMemcpyAsync(d_field + 2 * px * (size_t)b0, h_field_in + 2 * px * (size_t)b0,
+                                      sizeof(float) * 2 * px * nb, cudaMemcpyHostToDevice, ctx->copy_in));
+        SSP_CUDA(ctx, cudaEventRecord(ctx->pipe_events[2 * c], ctx->copy_in));
+    }
+    const size_t sh_per_field = (size_t)S * (size_t)(n_sh > 0 ? n_sh : 0) * 9;
+    if (n_sh > 0)
+        if (int rc = ssp_fill_noise(ctx, ar->seed, 2 * ar->frame + 1, 0, (unsigned long long)B * sh_per_field, d_noise_sh)) return rc;
+    // Screens evolve in uniform chunks (the noise scratch holds one chunk); the fields propagate in groups of chunks
+    // that halve towards the end -- n/2, n/4, .., 1, 1 chunks -- so that the big groups run at full-batch efficiency
+    // and only a small group's download is left uncovered at the end.
+    int group_end = (n_chunks + 1) / 2, group_begin = 0;
+    for (int c = 0; c < n_chunks; ++c) {
+        const int b0 = c * Bc, nb = (B - b0 < Bc) ? B - b0 : Bc;
+        const size_t off = (size_t)b0 * S * px;                   // in screens; complex arrays: 2 floats per element
+        if (int rc = ssp_fill_noise(ctx, ar->seed, 2 * ar->frame, off, (unsigned long long)nb * S * px, d_noise)) return rc;
+        if (int rc = ssp_evolve_screens(ctx, grid, psd, lambda, nb, S, cn2, dz, n_sh, ar->a, ar->vx, ar->vy, ar->T, d_noise,
+                                        n_sh > 0 ? d_noise_sh + 2 * (size_t)b0 * sh_per_field : nullptr, d_spectrum + 2 * off,
+                                        n_sh > 0 ? d_sh_coef + 2 * (size_t)b0 * sh_per_field : nullptr, d_screens + off,
+                                        d_ws, ws_bytes))
+            return rc;
+        if (c + 1 < group_end) continue;
+        // fields of chunks group_begin .. c
+        const int g0 = group_begin * Bc, gn = (b0 + nb) - g0;
+        float *df = d_field + 2 * px * (size_t)g0;
+        SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->pipe_events[2 * c], 0));   // copy_in is in order: chunk c done => all earlier done
+        if (int rc = ssp_propagate(ctx, grid, lambda, n0, h_kind, gn, S, dz, d_screens + (size_t)g0 * S * px,
+                                   (long long)S * (long long)px, S, win, df, df, nullptr, h_stats ? d_stats + g0 : nullptr,
+                                   roi_frac, d_ws, ws_bytes))
+            return rc;
+        cudaEvent_t ev_done = ctx->pipe_events[2 * c + 1];
+        SSP_CUDA(ctx, cudaEventRecord(ev_done, ctx->stream));
+        SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_out, ev_done, 0));
+        SSP_CUDA(ctx, cudaMemcpyAsync(h_field_out + 2 * px * (size_t)g0, df, sizeof(float) * 2 * px * gn, cudaMemcpyDeviceToHost, ctx->copy_out));
+        if (h_stats)
+            SSP_CUDA(ctx, cudaMemcpyAsync(h_stats + g0, d_stats + g0, sizeof(ssp_stats) * gn, cudaMemcpyDeviceToHost, ctx->copy_out));
+        group_begin = c + 1;
+        const int left = n_chunks - group_begin;
+        group_end = group_begin + (left + 1) / 2;
     }
     SSP_CUDA(ctx, cudaEventRecord(ev_end, ctx->copy_out));
     SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ev_end, 0));

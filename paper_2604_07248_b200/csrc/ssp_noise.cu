@@ -22,17 +22,23 @@ __device__ __forceinline__ void philox_round(uint32_t (&c)[4], uint32_t k0, uint
     c[3] = l0;
 }
 
+// sin / cos through the special-function unit (absolute error about 2^-21 on [-pi, pi]; the draw's error is that times
+// r <= 5.8, below the fp32 rounding the screen generator adds afterwards); the logarithm stays the accurate one, because
+// for u -> 1 the radius is sqrt of a small difference and an absolute error in ln u would be divided by r.
 __device__ __forceinline__ float2 box_muller(uint32_t xr, uint32_t xa)
 {
     const float u = ((float)(xr >> 9) + 0.5f) * 1.1920928955078125e-7f;          // 2^-23; k + 1/2 needs 24 bits: exact
-    const float f2 = ((float)(xa >> 9) + 0.5f) * 2.384185791015625e-7f;          // 2 f, so that sincospi sees the angle 2 pi f
-    const float r = sqrtf(-2.0f * logf(u));
-    float s, c;
-    sincospif(f2, &s, &c);
-    return make_float2(r * c, r * s);
+    const float g = ((float)(xa >> 9) + 0.5f) * 2.384185791015625e-7f - 1.0f;    // 2 f - 1 in (-1, 1), exact
+    float r;
+    asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(-2.0f * logf(u)));
+    // angle 2 pi f = pi g + pi:  cos(2 pi f) = -cos(pi g),  sin(2 pi f) = -sin(pi g)
+    const float th = 3.14159265358979f * g;
+    return make_float2(-r * __cosf(th), -r * __sinf(th));
 }
 
-__global__ void __launch_bounds__(256) k_fill_noise(uint32_t k0, uint32_t k1, uint32_t s0, uint32_t s1,
+struct RoundKeys { uint32_t k[10][2]; };   // the key schedule (key + r * Weyl constants), computed once on the host
+
+__global__ void __launch_bounds__(256) k_fill_noise(const RoundKeys keys, uint32_t s0, uint32_t s1,
                                                      unsigned long long first_block, unsigned long long n_draws,
                                                      float2 *__restrict__ out)
 {
@@ -40,13 +46,8 @@ __global__ void __launch_bounds__(256) k_fill_noise(uint32_t k0, uint32_t k1, ui
     if (2 * j >= n_draws) return;
     const unsigned long long i = first_block + j;
     uint32_t c[4] = {(uint32_t)i, (uint32_t)(i >> 32), s0, s1};
-    uint32_t a = k0, b = k1;
 #pragma unroll
-    for (int r = 0; r < 10; ++r) {
-        philox_round(c, a, b);
-        a += 0x9E3779B9u;
-        b += 0xBB67AE85u;
-    }
+    for (int r = 0; r < 10; ++r) philox_round(c, keys.k[r][0], keys.k[r][1]);
     const float2 z0 = box_muller(c[0], c[1]), z1 = box_muller(c[2], c[3]);
     if (2 * j + 1 < n_draws) reinterpret_cast<float4 *>(out)[j] = make_float4(z0.x, z0.y, z1.x, z1.y);
     else out[2 * j] = z0;
@@ -58,9 +59,13 @@ int launch_fill_noise(ssp_ctx *ctx, unsigned long long seed, unsigned long long 
     const unsigned long long blocks = (n + 1) / 2;
     const unsigned long long grid = (blocks + 255) / 256;
     if (grid > 0x7FFFFFFFull) return ctx->fail(SSP_EINVAL, "ssp_fill_noise: more than 2^40 draws in one call");
+    RoundKeys keys;
+    for (int r = 0; r < 10; ++r) {
+        keys.k[r][0] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u;
+        keys.k[r][1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+    }
     ctx->prof_begin("fill_noise", 8.0 * (double)n);
-    k_fill_noise<<<(unsigned)grid, 256, 0, ctx->stream>>>((uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)stream,
-                                                          (uint32_t)(stream >> 32), first / 2, n, out);
+    k_fill_noise<<<(unsigned)grid, 256, 0, ctx->stream>>>(keys, (uint32_t)stream, (uint32_t)(stream >> 32), first / 2, n, out);
     ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
