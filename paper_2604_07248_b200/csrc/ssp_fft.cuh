@@ -169,11 +169,15 @@ struct PlanInfo {
     //   tw1 [R1/2][N/R1][2]: W_N^(m k1), the twiddles of k1 = 2p, 2p+1 adjacent (one 16-byte load)
     //   tw2 [R2][R3]: W_N^(R1 n3 k2)
     //   tw1r[RL/2][N/RL][2] and tw2r[R2][R1] for the reversed plan (R3|R2, R2, R1)
+    // A plan that reads the same forwards and backwards (R1 == RL) has identical tables in both directions: they are
+    // stored once, which halves the table's L1 footprint (at N = 4096: 33 KB instead of 66 KB beside the 32 KB h table).
+    static constexpr bool SYM = (R1 == RL);
     static constexpr int TW1 = 0;
     static constexpr int TW2 = TW1 + N;
-    static constexpr int TW1R = TW2 + R2 * R3;
-    static constexpr int TW2R = TW1R + N;
-    static constexpr int TW_TOTAL = TW2R + R2 * R1;
+    static constexpr int TW1R = SYM ? TW1 : TW2 + R2 * R3;
+    static constexpr int TW2R = SYM ? TW2 : TW1R + N;
+    // (two-stage plans never read tw2 / tw2r; the builder still writes R2 * R1 entries there)
+    static constexpr int TW_TOTAL = SYM ? TW2 + R2 * (R3 > R1 ? R3 : R1) : TW2R + R2 * R1;
 };
 
 // ---- three-stage plans (R, 2, R) with the middle stage done by warp shuffles -----------------------------
