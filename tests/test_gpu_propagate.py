@@ -337,8 +337,8 @@ def test_odd_batch_and_vacuum_paths_at_1024(ssp, orc):
 def test_bitwise_determinism(ssp, N):
     """Race check by other means (compute-sanitizer is closed on this pool): the shared-memory exchanges, mbarrier /
     TMA pipelines and named barriers have no data race if repeated runs on the same inputs are bitwise identical.
-    Fields, adjoint fields and evolved screens are compared over five runs (statistics use fp64 atomics and are
-    excluded)."""
+    Fields, adjoint fields, evolved screens and the statistics records (per-block partials added in a fixed order, no
+    atomics) are compared over five runs."""
     import torch
     from paper_2604_07248_b200 import api
     B, S = (6, 3) if N <= 1024 else (2, 2)
@@ -352,14 +352,15 @@ def test_bitwise_determinism(ssp, N):
     nsh = [torch.view_as_complex(torch.randn(B, S, 3, 3, 3, 2, device="cuda", generator=gen)) for _ in range(2)]
     first = None
     for run in range(5):
-        out = ssp.propagate(N, dx, lam, list(dz), d_u0, d_scr, **kw)
+        st = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+        out = ssp.propagate(N, dx, lam, list(dz), d_u0, d_scr, stats=st, roi_frac=0.5, **kw)
         gin = ssp.propagate_adjoint(N, dx, lam, list(dz), out, d_scr, **kw)
         out_as = ssp.propagate(N, dx, lam, list(dz), d_u0, d_scr, h_kind=api.H_ANGULAR_SPECTRUM, **kw)
         spec = torch.empty((B, S, N, N), dtype=torch.complex64, device="cuda")
         shc = torch.zeros((B, S, 3, 3, 3), dtype=torch.complex64, device="cuda")
         ssp.make_screens(N, dx, psd, lam, [1e-14] * S, [100.0] * S, 3, noise[0], nsh[0], spectrum=spec, sh_coef=shc)
         ev = ssp.evolve_screens(N, dx, psd, lam, [1e-14] * S, [100.0] * S, 3, 0.99, 0.3, -0.2, 0.01, noise[1], nsh[1], spec, shc)
-        got = [out.clone(), gin.clone(), out_as.clone(), ev.clone(), spec.clone()]
+        got = [out.clone(), gin.clone(), out_as.clone(), ev.clone(), spec.clone(), st.clone()]
         if first is None:
             first = got
         else:
