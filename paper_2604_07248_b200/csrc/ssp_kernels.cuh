@@ -29,13 +29,51 @@ __device__ __forceinline__ float2 swap_if(float2 x) { return SWAP ? make_float2(
 // result is in plain form either way.  GENERIC = false is the common split step (screen and window
 // both present, nothing saved): no per-element flag tests in the unrolled body.  GENERIC = true reads
 // the run-time flags: optional screen / window, saved planes, phase gradient.
-template <int N, int RL, int E, int T, bool GENERIC, bool SWAPPED>
+template <int N, int RL, int E, int T, bool GENERIC, bool SWAPPED, bool PK = false>
 __device__ __forceinline__ void row_pointwise(float2 *v, const RowArgs &a, const float *phis, int t, int b, int iy)
 {
     const long long pix0 = (long long)iy * N;
     const float yc = (float)(iy - N / 2);
     const float y2 = yc * yc * a.win_qs;
     const float xf = (float)(t - N / 2);
+    if constexpr (PK) {
+    // Two pixels at a time: the phase reduction, the window argument and the amplitude products are packed
+    // fp32 pairs ACROSS the two pixels (FMUL2 / FFMA2), only the SFU calls stay scalar; the complex multiply then
+    // takes cos and sin of each pixel as broadcast scalars and the field value as the packed operand.
+#pragma unroll
+    for (int j = 0; j < E; j += 2) {
+        const int off0 = (j % RL) * (N / RL) + T * (j / RL);      // ix = t + off, off compile-time
+        const int off1 = ((j + 1) % RL) * (N / RL) + T * ((j + 1) / RL);
+        float2 mr = make_float2(1.f, 1.f), mi = make_float2(0.f, 0.f);
+        if (!GENERIC || a.phi) {
+            sincos_reduced2(make_float2(phis[t + off0], phis[t + off1]), &mi, &mr);
+            mi = f2mul(mi, make_float2(a.phase_sign, a.phase_sign));
+        }
+        if (!GENERIC || a.win_on) {
+            const float2 xc = f2add(make_float2(xf, xf), make_float2((float)off0, (float)off1));
+            const float2 amp = window_amp2(f2fma(f2mul(xc, xc), make_float2(a.win_qs, a.win_qs), make_float2(y2, y2)),
+                                           a.win_half_order);
+            mr = f2mul(mr, amp);
+            mi = f2mul(mi, amp);
+        }
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int off = e ? off1 : off0;
+            const float2 u = swap_if<SWAPPED>(v[j + e]);
+            if constexpr (GENERIC) {
+                if (a.grad) {
+                    const float2 U = a.plane_in[b * a.plane_stride + pix0 + t + off];
+                    a.grad[b * a.grad_stride + pix0 + t + off] = u.y * U.x - u.x * U.y; // Im(G conj(U))
+                }
+            }
+            const float2 r = cmul(e ? make_float2(mr.y, mi.y) : make_float2(mr.x, mi.x), u);
+            if constexpr (GENERIC) {
+                if (a.plane_out) a.plane_out[b * a.plane_stride + pix0 + t + off] = r;
+            }
+            v[j + e] = r;
+        }
+    }
+    } else {
 #pragma unroll
     for (int i = 0; i < E / RL; ++i)
 #pragma unroll
@@ -65,6 +103,7 @@ __device__ __forceinline__ void row_pointwise(float2 *v, const RowArgs &a, const
             }
             v[i * RL + q] = r;
         }
+    }
 }
 
 template <int N, bool FIRST, bool SECOND, bool GENERIC>
@@ -74,6 +113,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
     using CFG = RowCfg<N>;
     constexpr int E = PI::E, T = PI::T, R1 = PI::R1, RL = PI::RL;
     constexpr bool SYM = (R1 == RL);                              // output layout == input layout
+    constexpr bool PK = RowCfg<N>::PACKED;                        // packed fp32 pairs (ssp_fft.cuh), where measured faster
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *smem = reinterpret_cast<float2 *>(smem_raw);
 
@@ -128,31 +168,31 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
                 // the exchange buffer is reused by the next pass: a row spanning several warps synchronises
                 // right after its last exchange read (TAIL), a warp-local row after the pointwise stage
                 constexpr bool TAIL = (T > 32);
-                fft_line<N, 0, false, false, TAIL>(v, t, sm, a.tw);
+                fft_line<N, 0, false, false, TAIL, PK>(v, t, sm, a.tw);
                 if (pass == 0) {
                     wait_phi();
-                    row_pointwise<N, RL, E, T, GENERIC, true>(v, a, phis, t, b, iy);
+                    row_pointwise<N, RL, E, T, GENERIC, true, PK>(v, a, phis, t, b, iy);
                     if constexpr (!TAIL) sm.sync();
                 }
             }
         } else if constexpr (FIRST) {
-            fft_line<N, 0, false, false>(v, t, sm, a.tw);
+            fft_line<N, 0, false, false, false, PK>(v, t, sm, a.tw);
             wait_phi();
-            row_pointwise<N, RL, E, T, GENERIC, true>(v, a, phis, t, b, iy);
+            row_pointwise<N, RL, E, T, GENERIC, true, PK>(v, a, phis, t, b, iy);
         } else {
             if (pointwise) {
                 wait_phi();
-                row_pointwise<N, RL, E, T, GENERIC, false>(v, a, phis, t, b, iy);
+                row_pointwise<N, RL, E, T, GENERIC, false, PK>(v, a, phis, t, b, iy);
             }
-            fft_line<N, 0, false, false>(v, t, sm, a.tw);
+            fft_line<N, 0, false, false, false, PK>(v, t, sm, a.tw);
         }
     } else {
-        if constexpr (FIRST) fft_line<N, 0, false, true, SECOND>(v, t, sm, a.tw); // inverse; now strided by RL
+        if constexpr (FIRST) fft_line<N, 0, false, true, SECOND, PK>(v, t, sm, a.tw); // inverse; now strided by RL
         if (pointwise) {
             wait_phi();
-            row_pointwise<N, RL, E, T, GENERIC, false>(v, a, phis, t, b, iy);
+            row_pointwise<N, RL, E, T, GENERIC, false, PK>(v, a, phis, t, b, iy);
         }
-        if constexpr (SECOND) fft_line<N, 0, true, false>(v, t, sm, a.tw); // forward, reversed plan; strided by R1
+        if constexpr (SECOND) fft_line<N, 0, true, false, false, PK>(v, t, sm, a.tw); // forward, reversed plan; strided by R1
     }
 
     float2 *dst = a.out + line * N;
@@ -162,7 +202,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
 #pragma unroll
             for (int q = 0; q < ROUT; ++q) {
                 const int k = line_index<N, 0, ROUT>(t, i, q);
-                dst[k] = cmul(v[i * ROUT + q], __ldg(a.hx + k));
+                dst[k] = cmul_c<false, PK>(v[i * ROUT + q], __ldg(a.hx + k));
             }
     } else {
 #pragma unroll

@@ -47,6 +47,8 @@ struct RowCfg {
     static constexpr size_t SMEM_PHI = sizeof(float) * (size_t)LPB * N; // prefetched screen rows
     static constexpr size_t SMEM = SMEM_X + SMEM_PHI;
     static constexpr int MIN_BLOCKS = (THREADS < RowTune<N>::MAX_THREADS) ? 1 : RowTune<N>::MIN_BLOCKS;
+    // packed fp32 pairs in the split-step row kernel: measured 1024 +4 %, 2048 +1.4 %, 4096 +4.6 %, 512 -23 %
+    static constexpr bool PACKED = (N >= 1024);
 };
 
 template <int N, int V_ = 1>
@@ -116,6 +118,17 @@ __device__ __forceinline__ void sincos_reduced(float x, float *s, float *c)
     *c = __cosf(r);
 }
 
+// the same reduction on two arguments at once (packed fp32 pairs; the SFU calls stay scalar)
+__device__ __forceinline__ void sincos_reduced2(float2 x, float2 *s, float2 *c)
+{
+    const float2 kk = f2mul(x, make_float2(0.15915494309189535f, 0.15915494309189535f));
+    const float2 nk = make_float2(-rintf(kk.x), -rintf(kk.y));
+    float2 r = f2fma(nk, make_float2(6.2831854820251465f, 6.2831854820251465f), x);
+    r = f2fma(nk, make_float2(-1.7484555e-7f, -1.7484555e-7f), r);
+    *s = make_float2(__sinf(r.x), __sinf(r.y));
+    *c = make_float2(__cosf(r.x), __cosf(r.y));
+}
+
 __device__ __forceinline__ float ex2_approx(float x)
 {
     float y;
@@ -134,6 +147,13 @@ __device__ __forceinline__ float lg2_approx(float x)
 __device__ __forceinline__ float window_amp(float q, float h)
 {
     return ex2_approx(-1.4426950408889634f * ex2_approx(h * lg2_approx(q)));
+}
+
+__device__ __forceinline__ float2 window_amp2(float2 q, float h)
+{
+    const float2 e = f2mul(make_float2(lg2_approx(q.x), lg2_approx(q.y)), make_float2(h, h));
+    const float2 f = f2mul(make_float2(ex2_approx(e.x), ex2_approx(e.y)), make_float2(-1.4426950408889634f, -1.4426950408889634f));
+    return make_float2(ex2_approx(f.x), ex2_approx(f.y));
 }
 
 } // namespace ssp
