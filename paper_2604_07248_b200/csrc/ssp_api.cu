@@ -219,6 +219,7 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
         // K6: IFFT_x -> * exp(i phi_j) W -> [FFT_x -> * hx_{j+1}]
         RowArgs r{};
         r.in = u; r.out = u; r.n_lines = B * N; r.tw = tw;
+        r.in_swapped = mid_swapped(N);
         if (j <= S) {
             r.phi = d_screens + (size_t)(j - 1) * px;
             r.phi_batch_stride = screen_batch_stride;
@@ -314,6 +315,7 @@ int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0,
         if (int rc = launch_col_prop(ctx, N, c)) return rc;
         RowArgs r{};
         r.in = g; r.out = g; r.n_lines = B * N; r.tw = tw;
+        r.in_swapped = mid_swapped(N);
         const bool last = (j == 1);
         if (!last) {
             plane_stage(r, j - 1);

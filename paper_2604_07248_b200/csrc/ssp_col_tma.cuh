@@ -110,6 +110,7 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
     using CFG = ColTmaCfg<N>;
     constexpr int E = PI::E, C = CFG::C, R1 = PI::R1, RL = PI::RL;
     constexpr bool SYM = (R1 == RL), PK = CFG::PACKED;
+    static_assert(SYM || !MidSwapped<N>::value, "the swapped hand-over needs the forward-only body");
     constexpr int GROUPS = N / C;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *sbuf = reinterpret_cast<float2 *>(smem_raw);
@@ -171,7 +172,7 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
 #pragma unroll
                 for (int q = 0; q < R1; ++q) {
                     const float2 x = v[i * R1 + q];
-                    tile_s[line_index<N, 1, R1>(t, i, q) * C + c] = make_float2(x.y, x.x);
+                    tile_s[line_index<N, 1, R1>(t, i, q) * C + c] = MidSwapped<N>::value ? x : make_float2(x.y, x.x);
                 }
         } else {
             fft_line<N, 1, false, false, true, PK>(v, t, sm, a.tw);   // strided by RL

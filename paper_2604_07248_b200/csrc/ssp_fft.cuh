@@ -20,6 +20,7 @@
 #pragma once
 
 #include <cuda_runtime.h>
+#include <type_traits>
 #include <utility>
 
 namespace ssp {

@@ -149,6 +149,7 @@ struct RowArgs {
     // generic pre-multiply on the input line index (centred DFT): [N] or null
     const float2 *pre;
     const float2 *pre_line;      // per-line factor pre_line[iy] multiplying the whole line, or null
+    int in_swapped;              // the input holds (im, re) pairs: written by launch_col_prop when mid_swapped(N)
     const float2 *tw;
 };
 
@@ -166,6 +167,8 @@ struct ColArgs {
 int launch_row(ssp_ctx *ctx, int N, bool first, bool second, const RowArgs &a);
 // column pass of the propagator: FFT_y -> * hy -> IFFT_y, in place allowed.
 int launch_col_prop(ssp_ctx *ctx, int N, const ColArgs &a);
+// true when launch_col_prop leaves its output re/im-swapped for the row kernel that follows (RowArgs::in_swapped)
+bool mid_swapped(int N);
 // single column transform (inverse != 0: unnormalised inverse) followed by * hy.
 int launch_col_single(ssp_ctx *ctx, int N, bool inverse, const ColArgs &a);
 

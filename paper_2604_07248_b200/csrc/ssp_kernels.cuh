@@ -136,8 +136,10 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
     float2 v[E];
     // FIRST (an inverse transform comes first) loads re/im-swapped when the forward code runs it
     constexpr bool SWAP_IN = FIRST && SYM;
+    constexpr bool MID = MidSwapped<N>::value;                    // the column kernel left the field swapped already
     constexpr int RIN = (FIRST || SYM) ? R1 : RL;
-    {
+    auto load_line = [&](auto swap_tag) {
+        constexpr bool SW = decltype(swap_tag)::value;
         const float2 *src = a.in + line * N;
 #pragma unroll
         for (int i = 0; i < E / RIN; ++i)
@@ -150,9 +152,14 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
                         x = cmul(x, cmul(pl, __ldg(a.pre + line_index<N, 0, RIN>(t, i, q))));
                     }
                 }
-                v[i * RIN + q] = swap_if<SWAP_IN>(x);
+                v[i * RIN + q] = swap_if<SW>(x);
             }
-    }
+    };
+    if constexpr (SWAP_IN && MID) {
+        // the column kernel has left the field swapped (always so on the common path; a run-time flag otherwise)
+        if (!GENERIC || a.in_swapped) load_line(std::false_type{});
+        else load_line(std::true_type{});
+    } else load_line(std::integral_constant<bool, SWAP_IN>{});
     auto wait_phi = [&]() {
         if (!GENERIC || a.phi) {
             cp_async_wait_all();

@@ -51,6 +51,15 @@ struct RowCfg {
     static constexpr bool PACKED = (N >= 1024);
 };
 
+// Between the column kernel and the row kernel of a split step the field may stay re/im-swapped: the column
+// kernel's inverse transform runs as forward code on swapped data and the row kernel's inverse transform wants
+// exactly that, so neither swaps.  With scalar arithmetic the swap is register renaming and nothing is gained; with
+// packed pairs it would cost two MOVs per element on each side.  Only the TMA column kernel writes this form.
+template <int N>
+struct MidSwapped {
+    static constexpr bool value = RowCfg<N>::PACKED && PlanInfo<N, 0>::SYM && PlanInfo<N, 1>::SYM;
+};
+
 template <int N, int V_ = 1>
 struct ColCfg {
     static constexpr int V = V_;                                  // plan variant

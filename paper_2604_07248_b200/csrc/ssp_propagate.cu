@@ -44,7 +44,10 @@ static int launch_row_x(ssp_ctx *ctx, const RowArgs &a)
 template <int N, bool FIRST, bool SECOND>
 static int launch_row_n(ssp_ctx *ctx, const RowArgs &a)
 {
-    const bool common = a.phi && a.win_on && !a.grad && !a.plane_out && !a.pre;
+    constexpr bool MID = FIRST && MidSwapped<N>::value;
+    if (a.in_swapped && !MID) return ctx->fail(SSP_EINVAL, "swapped row input for a kernel that does not take it");
+    if (a.in_swapped && a.pre) return ctx->fail(SSP_EINVAL, "pre-multiply on a swapped row input");
+    const bool common = a.phi && a.win_on && !a.grad && !a.plane_out && !a.pre && (!MID || a.in_swapped);
     if (common) return launch_row_x<N, FIRST, SECOND, false>(ctx, a);
     return launch_row_x<N, FIRST, SECOND, true>(ctx, a);
 }
@@ -127,8 +130,26 @@ int col_tile_width(int N)
     }
 }
 
+template <int N>
+static constexpr bool mid_swapped_n() { return ColTmaTune<N>::ENABLED && MidSwapped<N>::value; }
+static_assert(!MidSwapped<8>::value && !MidSwapped<16>::value && !MidSwapped<32>::value && !MidSwapped<64>::value &&
+              !MidSwapped<128>::value && !MidSwapped<256>::value && !MidSwapped<512>::value,
+              "only the TMA column kernel hands the field over swapped");
+static_assert(ColTmaTune<1024>::ENABLED && ColTmaTune<2048>::ENABLED && ColTmaTune<4096>::ENABLED, "see MidSwapped");
+
+bool mid_swapped(int N)
+{
+    switch (N) {
+    case 1024: return mid_swapped_n<1024>();
+    case 2048: return mid_swapped_n<2048>();
+    case 4096: return mid_swapped_n<4096>();
+    default: return false;
+    }
+}
+
 int launch_col_prop(ssp_ctx *ctx, int N, const ColArgs &a)
 {
+    if (!(a.hy || a.h2d) && mid_swapped(N)) return ctx->fail(SSP_EINVAL, "column pass without a multiplier");
     if (a.hy || a.h2d) {
         if (N == 512) return launch_col_tma_n<512>(ctx, a);
         if (N == 1024) return launch_col_tma_n<1024>(ctx, a);
