@@ -69,7 +69,7 @@ struct ColTmaCfg {
     static constexpr int BUF_ELEMS = C * PlanInfo<N, 1>::LINE_ELEMS;  // float2 per buffer (padded exchange)
     static constexpr size_t SMEM = NBUF * sizeof(float2) * BUF_ELEMS + 16;
     static constexpr unsigned TILE_BYTES = (unsigned)(sizeof(float2) * C * N);
-    // packed fp32 pairs: measured 2048 +3.6 %, 4096 +1.3 %, 1024 -2.6 %, 512 -1.3 %
+    // packed fp32 pairs: measured 2048 +3.6 %, 4096 +1.3 %; 1024 -1 % and 512 +1 % (within noise) stay scalar
     static constexpr bool PACKED = (N >= 2048);
 };
 

@@ -47,7 +47,7 @@ struct RowCfg {
     static constexpr size_t SMEM_PHI = sizeof(float) * (size_t)LPB * N; // prefetched screen rows
     static constexpr size_t SMEM = SMEM_X + SMEM_PHI;
     static constexpr int MIN_BLOCKS = (THREADS < RowTune<N>::MAX_THREADS) ? 1 : RowTune<N>::MIN_BLOCKS;
-    // packed fp32 pairs in the split-step row kernel: measured 1024 +4 %, 2048 +1.4 %, 4096 +4.6 %, 512 -23 %
+    // packed fp32 pairs in the split-step row kernel: measured 1024 +4 %, 2048 +2 %, 4096 +4 %; 512 (shuffle plan, one warp per row at 16 points per thread) -20 %
     static constexpr bool PACKED = (N >= 1024);
 };
 
