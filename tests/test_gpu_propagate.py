@@ -333,6 +333,28 @@ def test_odd_batch_and_vacuum_paths_at_1024(ssp, orc):
         assert rel_l2(out.cpu().numpy(), ref).max() < tol(N, 1), kw
 
 
+@pytest.mark.parametrize("N", [1024, 2048])
+def test_swapped_handover_common_vs_generic(ssp, N):
+    """For N >= 1024 the TMA column kernel hands the field to the row kernel re/im-swapped (DESIGN.md section 6,
+    packed pairs).  The common row instantiation assumes that form, the generic one (saved planes, phase gradient)
+    reads a run-time flag: both must produce the same bits, forward and adjoint."""
+    import torch
+    B, n_steps, S = 2, 3, 3
+    dx, lam, dz, u0, scr = _case(N, B, n_steps, S, 4000 + N)
+    kw = dict(win_order=16, win_sigma_frac=0.47)
+    out = ssp.propagate(N, dx, lam, list(dz), cu(u0), cu(scr), **kw)
+    planes = torch.empty((B, n_steps, N, N), dtype=torch.complex64, device="cuda")
+    out_g = ssp.propagate(N, dx, lam, list(dz), cu(u0), cu(scr), planes=planes, **kw)
+    assert torch.equal(out, out_g)
+    assert torch.equal(planes[:, -1], out)
+    g = cu(synth.random_field(N, B, 4100 + N))
+    gin = ssp.propagate_adjoint(N, dx, lam, list(dz), g, cu(scr), **kw)
+    grad = torch.empty((B, S, N, N), dtype=torch.float32, device="cuda")
+    gin_g = ssp.propagate_adjoint(N, dx, lam, list(dz), g, cu(scr), planes=planes, phase_grad=grad, **kw)
+    assert torch.equal(gin, gin_g)
+    assert torch.isfinite(grad).all()
+
+
 @pytest.mark.parametrize("N", [128, 512, 1024, 2048])
 def test_bitwise_determinism(ssp, N):
     """Race check by other means (compute-sanitizer is closed on this pool): the shared-memory exchanges, mbarrier /
