@@ -226,6 +226,7 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
             r.phase_sign = 1.f;
         }
         fill_window(r, win, N);
+        r.win_map = window_map(ctx, N, r);
         if (d_planes) {
             r.plane_out = reinterpret_cast<float2 *>(d_planes) + (size_t)(j - 1) * px;
             r.plane_stride = (long long)n_steps * (long long)px;
@@ -294,6 +295,7 @@ int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0,
             }
         }
         fill_window(r, win, N);
+        r.win_map = window_map(ctx, N, r);
     };
 
     const bool as = (h_kind == SSP_H_ANGULAR_SPECTRUM);

@@ -41,6 +41,7 @@ struct ssp_ctx {
     std::map<ssp::HKey, float2 *> h2d_tables;    // 2-D transfer functions [N][N] (angular spectrum), device
     size_t h2d_bytes = 0;
     std::map<int, float2 *> sign_tables;         // (-1)^k tables for the centred DFT
+    std::map<std::tuple<int, float, float>, float *> win_maps; // window amplitude maps per (N, 1/sigma^2, order/2)
     void *scratch = nullptr;                     // small device scratch (stat accumulators, tables)
     size_t scratch_bytes = 0;
     std::vector<void *> owned;                   // misc device allocations freed at destroy
@@ -139,6 +140,7 @@ struct RowArgs {
     int win_on;
     float win_qs;                // 1 / (sigma_frac N)^2
     float win_half_order;        // order / 2
+    const float *win_map;        // [N][N] window amplitudes from the context cache (window_map()), or null: per pixel
     float2 *plane_out;           // optional: field after the pointwise stage, field b at + b*plane_stride
     long long plane_stride;      // elements (float2) between fields
     const float2 *plane_in;      // optional (adjoint gradient): forward plane
@@ -169,6 +171,10 @@ int launch_row(ssp_ctx *ctx, int N, bool first, bool second, const RowArgs &a);
 int launch_col_prop(ssp_ctx *ctx, int N, const ColArgs &a);
 // true when launch_col_prop leaves its output re/im-swapped for the row kernel that follows (RowArgs::in_swapped)
 bool mid_swapped(int N);
+// The window amplitudes W(ix,iy) of r's window as an fp32 [N][N] map cached in the context (built once by a kernel that
+// evaluates the same expression as the row kernel: identical bits), for the grids whose common row kernel reads it
+// (N = 1024); null otherwise or when it cannot be allocated -- the row kernel then evaluates W per pixel.
+const float *window_map(ssp_ctx *ctx, int N, const RowArgs &r);
 // single column transform (inverse != 0: unnormalised inverse) followed by * hy.
 int launch_col_single(ssp_ctx *ctx, int N, bool inverse, const ColArgs &a);
 

@@ -50,9 +50,15 @@ __device__ __forceinline__ void row_pointwise(float2 *v, const RowArgs &a, const
             mi = f2mul(mi, make_float2(a.phase_sign, a.phase_sign));
         }
         if (!GENERIC || a.win_on) {
-            const float2 xc = f2add(make_float2(xf, xf), make_float2((float)off0, (float)off1));
-            const float2 amp = window_amp2(f2fma(f2mul(xc, xc), make_float2(a.win_qs, a.win_qs), make_float2(y2, y2)),
-                                           a.win_half_order);
+            float2 amp;
+            if (GENERIC ? (a.win_map != nullptr) : WinMap<N>::value) {
+                // cached map: the lanes of a warp read 32 consecutive floats per element (one 128-byte line)
+                amp = make_float2(__ldg(a.win_map + pix0 + t + off0), __ldg(a.win_map + pix0 + t + off1));
+            } else {
+                const float2 xc = f2add(make_float2(xf, xf), make_float2((float)off0, (float)off1));
+                amp = window_amp2(f2fma(f2mul(xc, xc), make_float2(a.win_qs, a.win_qs), make_float2(y2, y2)),
+                                  a.win_half_order);
+            }
             mr = f2mul(mr, amp);
             mi = f2mul(mi, amp);
         }
@@ -93,7 +99,8 @@ __device__ __forceinline__ void row_pointwise(float2 *v, const RowArgs &a, const
             }
             if (!GENERIC || a.win_on) {
                 const float xc = xf + (float)off;
-                const float amp = window_amp(fmaf(xc * xc, a.win_qs, y2), a.win_half_order);
+                const float amp = (GENERIC && a.win_map) ? __ldg(a.win_map + pix0 + t + off)
+                                                         : window_amp(fmaf(xc * xc, a.win_qs, y2), a.win_half_order);
                 mr *= amp;
                 mi *= amp;
             }

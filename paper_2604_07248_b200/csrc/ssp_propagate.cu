@@ -47,7 +47,8 @@ static int launch_row_n(ssp_ctx *ctx, const RowArgs &a)
     constexpr bool MID = FIRST && MidSwapped<N>::value;
     if (a.in_swapped && !MID) return ctx->fail(SSP_EINVAL, "swapped row input for a kernel that does not take it");
     if (a.in_swapped && a.pre) return ctx->fail(SSP_EINVAL, "pre-multiply on a swapped row input");
-    const bool common = a.phi && a.win_on && !a.grad && !a.plane_out && !a.pre && (!MID || a.in_swapped);
+    const bool common = a.phi && a.win_on && !a.grad && !a.plane_out && !a.pre && (!MID || a.in_swapped) &&
+                        ((a.win_map != nullptr) == WinMap<N>::value);
     if (common) return launch_row_x<N, FIRST, SECOND, false>(ctx, a);
     return launch_row_x<N, FIRST, SECOND, true>(ctx, a);
 }
@@ -128,6 +129,43 @@ int col_tile_width(int N)
     case 4096: return col_tile_width_n<4096>();
     default: return 1;
     }
+}
+
+// ---- cached window map (RowArgs::win_map) ------------------------------------------------------
+__global__ void __launch_bounds__(256) k_window_map(int N, float qs, float half_order, float *__restrict__ out)
+{
+    const int iy = blockIdx.x;
+    const float yc = (float)(iy - N / 2);
+    const float y2 = yc * yc * qs;                                // the expressions of row_pointwise, term for term
+    for (int ix = threadIdx.x; ix < N; ix += blockDim.x) {
+        const float xc = (float)(ix - N / 2);
+        out[(size_t)iy * N + ix] = window_amp(fmaf(xc * xc, qs, y2), half_order);
+    }
+}
+
+template <int N>
+static constexpr bool win_map_n() { return WinMap<N>::value; }
+
+const float *window_map(ssp_ctx *ctx, int N, const RowArgs &r)
+{
+    bool use = false;
+    switch (N) {
+    case 1024: use = win_map_n<1024>(); break;
+    default: break;
+    }
+    if (!use || !r.win_on) return nullptr;
+    const auto key = std::make_tuple(N, r.win_qs, r.win_half_order);
+    auto it = ctx->win_maps.find(key);
+    if (it != ctx->win_maps.end()) return it->second;
+    if (ctx->win_maps.size() >= 8) return nullptr;                // a caller cycling through windows: evaluate per pixel
+    float *d = nullptr;
+    if (cudaMalloc(&d, sizeof(float) * (size_t)N * N) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    k_window_map<<<N, 256, 0, ctx->stream>>>(N, r.win_qs, r.win_half_order, d);
+    ctx->launches++;
+    if (cudaGetLastError() != cudaSuccess) { cudaFree(d); return nullptr; }
+    ctx->owned.push_back(d);
+    ctx->win_maps[key] = d;
+    return d;
 }
 
 template <int N>
