@@ -15,8 +15,9 @@
  *   - Forward DFT X[k] = sum_n x[n] exp(-i 2 pi k n / N), unnormalised.
  *   - "dev" pointers are device memory of the context's device, 16-byte aligned, owned by
  *     the caller (allocate them with torch / cudaMalloc); "host" pointers are read during
- *     the call and not retained.  The library allocates only small tables inside the
- *     context and frees them in ssp_destroy.
+ *     the call and not retained.  The library allocates only tables inside the context
+ *     (twiddles, transfer-function tables, at N = 1024 up to 8 cached window maps of 4 MB)
+ *     and frees them in ssp_destroy.
  *   - Calls enqueue work on the context's stream and return without synchronising,
  *     except the *_host entry points, which synchronise the stream before returning.
  *   - Return value: 0 on success, a negative ssp_status otherwise; ssp_last_error gives
