@@ -21,11 +21,16 @@
  *
  * Pins (tests/test_oracle_*.py): P0 FFT vs naive DFT / numpy; P1 Gaussian beam
  * width; P1b power conservation; P2 structure function; P3 filter amplitude;
- * P4 analytic mean; P5 Rytov scintillation; P6 AR recursion; P7 adjoint
- * identity; P8 finite-difference gradients.
- * PARITY UNPINNED (defined by the survey, not by the paper): the Nikishov
- * oceanic constants (Q20), the super-Gaussian window form (Q12), the config-4
- * beam / loss (Q21).
+ * P4 analytic mean; P5 Rytov scintillation; P6 AR recursion (incl. the
+ * subharmonic coefficients under wind: the closed-form moved sinusoid); P7
+ * adjoint identity; P8 finite-difference gradients; the non-paraxial term of
+ * Eq. 6 on a tilted plane wave against 50-digit arithmetic; Philox-4x32-10
+ * against its authors' known-answer vectors.
+ * PARITY UNPINNED BY THE PAPER (defined by the survey / the open literature,
+ * not by PAPER.md): the Nikishov oceanic constants (Q20; re-typed with their
+ * source in tests/golden/nikishov_constants.txt and checked against that
+ * file, which catches a typo but is not a pin by the paper), the
+ * super-Gaussian window form (Q12), the config-4 beam (Q21).
  */
 #ifndef ORC_H
 #define ORC_H

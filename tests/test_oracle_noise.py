@@ -2,8 +2,12 @@
 only the law of the draws ("unit-variance complex Gaussian", PAPER.md:359 S16; Q3: Re and Im each N(0, 1), independent), so
 the pins are that law, independence across draws / streams / seeds, and the generator's structure (bijective rounds, full
 64-bit draw index, avalanche)."""
+import os
+
 import numpy as np
 from scipy import stats
+
+from tests.util import GOLDEN
 
 NS = 1 << 20
 
@@ -85,3 +89,42 @@ def test_philox_is_a_keyed_bijection_with_avalanche(orc):
     big = orc.philox4x32_10(np.stack([np.arange(1 << 16, dtype=np.uint32)] + [np.zeros(1 << 16, np.uint32)] * 3, axis=1), key)
     cnt = np.bincount(big.view(np.uint8).ravel(), minlength=256)
     assert stats.chisquare(cnt).pvalue > 1e-3
+
+
+def philox_kat_vectors():
+    """(counter[4], key[2], expected[4]) from tests/golden/philox_kat.txt (Salmon et al., SC'11; Random123)."""
+    out = []
+    with open(os.path.join(GOLDEN, "philox_kat.txt")) as fh:
+        for line in fh:
+            line = line.split("#")[0].replace("->", " ").split()
+            if line:
+                w = [int(x, 16) for x in line]
+                assert len(w) == 10
+                out.append((w[0:4], w[4:6], w[6:10]))
+    assert len(out) == 3
+    return out
+
+
+def test_philox_known_answer_vectors(orc):
+    """The name "Philox-4x32-10" is a claim the published algorithm fixes: the three known-answer vectors of its authors
+    (all-zero, all-ones, pi digits) must come out word for word."""
+    for ctr, key, want in philox_kat_vectors():
+        got = orc.philox4x32_10(np.array([ctr], dtype=np.uint32), key)[0]
+        assert [int(v) for v in got] == want, ([hex(int(v)) for v in got], [hex(v) for v in want])
+    # vectorised over counters: the same three in one call per key
+    for ctr, key, want in philox_kat_vectors():
+        many = np.array([ctr, [1, 2, 3, 4], ctr], dtype=np.uint32)
+        got = orc.philox4x32_10(many, key)
+        assert [int(v) for v in got[0]] == want and [int(v) for v in got[2]] == want
+    # and noise() addresses the blocks as DESIGN.md Q29 says: block i of (seed, stream) = counter (i lo, i hi, stream lo,
+    # stream hi), key (seed lo, seed hi); draw 2i from (x0, x1), draw 2i+1 from (x2, x3), 23-bit uniforms
+    ctr, key, want = philox_kat_vectors()[2]
+    i = ctr[0] | (ctr[1] << 32)
+    stream = ctr[2] | (ctr[3] << 32)
+    seed = key[0] | (key[1] << 32)
+    z = orc.noise(seed, stream, 2, first=2 * i)
+    for d in range(2):
+        u = ((want[2 * d] >> 9) + 0.5) / 2.0 ** 23
+        f = ((want[2 * d + 1] >> 9) + 0.5) / 2.0 ** 23
+        ref = np.sqrt(-2.0 * np.log(u)) * np.exp(2j * np.pi * f)
+        assert abs(z[d] - ref) < 1e-14 * abs(ref)

@@ -69,6 +69,36 @@ def test_angular_spectrum_reduces_to_fresnel_when_paraxial(orc):
     assert np.abs(m - v).max() < 1e-13
 
 
+@pytest.mark.parametrize("mx,my,n0", [(5, 3, 1.0), (-7, 2, 1.0), (4, -4, 1.33)])
+def test_angular_spectrum_non_paraxial_plane_wave(orc, mx, my, n0):
+    """The non-paraxial term of Eq.6: a tilted plane wave exp(i 2 pi (mx ix + my iy)/N), periodic on the
+    grid, with |kappa0| ~ 0.5 k is an eigenfunction of the step and must come out multiplied by
+    exp(i dz (sqrt(k^2 - kappa0^2) - k)), k = 2 pi n0 / lambda (carrier removed, Q2).  The phase is evaluated here from
+    Eq.6 itself with 50-digit arithmetic (mpmath); dz is chosen so that the Fresnel kernel is off by several radians,
+    i.e. the test fails if the oracle falls back to the paraxial form or drops the square root."""
+    import mpmath as mp
+    mp.mp.dps = 50
+    N, lam = 64, 1.0e-6
+    dx = lam / n0 * 11.5 / N                                  # |f| = hypot(mx, my)/(N dx) ~ 0.5 n0/lambda for hypot ~ 5.8
+    dz = 100.0 * lam
+    iy, ix = np.mgrid[0:N, 0:N]
+    u0 = np.exp(2j * np.pi * (mx * ix + my * iy) / N)[None]
+    u = orc.propagate(N, dx, lam, [dz], u0, n0=n0, h_kind=orc.H_ANGULAR_SPECTRUM)
+    k = 2 * mp.pi * mp.mpf(n0) / mp.mpf(lam)
+    kap2 = (2 * mp.pi) ** 2 * (mp.mpf(mx) ** 2 + mp.mpf(my) ** 2) / (mp.mpf(N) * mp.mpf(dx)) ** 2
+    assert 0.15 < float(kap2 / k ** 2) < 0.5                  # far from paraxial, still propagating
+    ang = mp.mpf(dz) * (mp.sqrt(k ** 2 - kap2) - k)
+    ang_fresnel = -mp.mpf(dz) * kap2 / (2 * k)
+    assert abs(float(ang - ang_fresnel)) > 1.0                # > 1 rad away from the Fresnel phase
+    factor = complex(mp.cos(ang), mp.sin(ang))
+    assert np.abs(u[0] - factor * u0[0]).max() < 1e-10
+    # two half steps compose (the phase is linear in dz), and the adjoint step undoes it (|H| = 1)
+    u2 = orc.propagate(N, dx, lam, [dz / 2, dz / 2], u0, n0=n0, h_kind=orc.H_ANGULAR_SPECTRUM)
+    assert np.abs(u2 - u).max() < 1e-10
+    back = orc.propagate_adjoint(N, dx, lam, [dz], u, n0=n0, h_kind=orc.H_ANGULAR_SPECTRUM)
+    assert np.abs(back - u0).max() < 1e-10
+
+
 def test_tilt_screen_steers_the_beam(orc):
     """Sign of exp(+i phi) (Eq.1) and axis order: a prism phi = 2 pi ft x placed
     after step 1 moves the centroid by +lambda ft dz2 in x only."""

@@ -120,6 +120,51 @@ def test_ocean_spectrum_low_kappa_limit_and_projection(orc):
     np.testing.assert_allclose(orc.psd_f(psd_eta, lam, 0.0, dz, ff), ph, rtol=1e-12)
 
 
+def _nikishov_constants():
+    import os
+    from tests.util import GOLDEN
+    out = {}
+    with open(os.path.join(GOLDEN, "nikishov_constants.txt")) as fh:
+        for line in fh:
+            line = line.split("#")[0].split()
+            if line:
+                out[line[0]] = float(line[1])
+    return out
+
+
+@pytest.mark.parametrize("w", [-2.0, -0.5, -4.0])
+def test_nikishov_against_retyped_constants(orc, w):
+    """Q20: the oceanic spectrum is not in PAPER.md; its seven literature constants are re-typed in
+    tests/golden/nikishov_constants.txt (with their source) and Phi_n is re-evaluated here from that file, term by
+    term, at kappa eta = 0.01, 0.3, 3 and 10 (inertial range, the bump, the dissipation range, and the salinity-only
+    tail where exp(-A_S delta) is all that is left), for three
+    temperature / salinity balances w.  Every constant moves at least one of these values by far more than the
+    tolerance: A_T / A_S / A_TS / D1 / D2 weigh in at kappa eta >= 0.3, C1 at 0.3, C0 everywhere."""
+    c = _nikishov_constants()
+    chi_T, eps = 1e-7, 1e-5
+    lam, dz = 0.532e-6, 2.5
+    k = 2 * np.pi / lam
+    eta = (c["nu"] ** 3 / eps) ** 0.25
+    psd = orc.Psd(kind=orc.PSD_OCEAN_NIKISHOV, chi_T=chi_T, eps=eps, w=w)
+    for ke in (0.01, 0.3, 3.0, 10.0):
+        kap = ke / eta
+        delta = c["D1"] * ke ** (4.0 / 3.0) + c["D2"] * ke ** 2
+        phin = (c["C0"] * eps ** (-1.0 / 3.0) * kap ** (-11.0 / 3.0) * (1.0 + c["C1"] * ke ** (2.0 / 3.0)) * chi_T / w ** 2
+                * (w ** 2 * np.exp(-c["A_T"] * delta) + np.exp(-c["A_S"] * delta) - 2.0 * w * np.exp(-c["A_TS"] * delta)))
+        want = (2 * np.pi) ** 3 * k * k * dz * phin                 # PAPER.md:346 (S14) projection, cycles/m
+        got = orc.psd_f(psd, lam, 0.0, dz, kap / (2 * np.pi))[0]
+        assert abs(got / want - 1) < 1e-12, (ke, got, want)
+    # sensitivity of the sample points: a 1 % change of any constant moves some value by > 1e-4 relative
+    def phi(cc, ke):
+        delta = cc["D1"] * ke ** (4.0 / 3.0) + cc["D2"] * ke ** 2
+        return (cc["C0"] * (1.0 + cc["C1"] * ke ** (2.0 / 3.0))
+                * (w ** 2 * np.exp(-cc["A_T"] * delta) + np.exp(-cc["A_S"] * delta) - 2.0 * w * np.exp(-cc["A_TS"] * delta)))
+    for name in ("C0", "C1", "A_T", "A_S", "A_TS", "D1", "D2"):
+        cc = dict(c)
+        cc[name] *= 1.01
+        assert max(abs(phi(cc, ke) / phi(c, ke) - 1) for ke in (0.01, 0.3, 3.0, 10.0)) > 1e-4, name
+
+
 def test_single_frequency_noise_returns_one_sinusoid(orc):
     """P3 (deterministic form): unit noise at one bin -> Re{ sqrt(Phi) df exp(+i 2 pi (kx ix + ky iy)/N) }
     (PAPER.md:359 S16: unnormalised inverse DFT, amplitude sqrt(Phi dfx dfy); Q3, Q6)."""

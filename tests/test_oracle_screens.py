@@ -176,6 +176,39 @@ def test_ar_wind_shift_is_circular_roll(orc):
     np.testing.assert_allclose(out[0, 0], expect, atol=1e-11 * np.abs(scr0).max())
 
 
+@pytest.mark.parametrize("p,a,b", [(1, 0, 2), (2, 2, 1), (3, 1, 0), (2, 0, 0)])
+def test_ar_wind_on_subharmonics_is_the_closed_form(orc, p, a, b):
+    """Q8 under wind (Eq.4 applied to the subharmonic coefficients of Eq.2): one subharmonic coefficient
+    c at (fx, fy) = ((b-1) df_p, (a-1) df_p), zero grid noise, AR factor 1, wind (vx, vy) over T.  The evolved screen
+    must be  Re{ c exp(-i 2 pi T (fx vx + fy vy)) exp(i 2 pi (fx x + fy y)) }  minus its mean -- the sinusoid moved by
+    +v T -- with vx != vy and (a, b) off the diagonal, so an x/y swap, a dropped level scaling of df_p or a sign error
+    in tau fails.  The expectation is written out here from the formula, not taken from the oracle."""
+    N, dx, n_sh = 32, 0.05, 3
+    psd = orc.Psd(kind=orc.PSD_VON_KARMAN, L0=10.0, l0=5e-3)
+    nsh = np.zeros((1, 1, n_sh, 3, 3, 2), np.float32)
+    nsh[0, 0, p - 1, a, b] = (0.75, -1.25)
+    zero = np.zeros((1, 1, N, N, 2), np.float32)
+    _, spec, shc = orc.make_screens(N, dx, psd, LAM, [CN2], [DZ], n_sh, zero, nsh)
+    c = shc[0, 0, p - 1, a, b]
+    assert abs(c) > 0
+    T, vx, vy = 0.37, 1.9, -0.8                              # v T = (0.70, -0.30) m: a fraction of the 43 m .. 14 m periods
+    fresh_sh = np.zeros_like(nsh)
+    fresh_sh[0, 0, :, :, :] = (3.0, -2.0)                    # a = 1: fresh draws must not enter
+    out = orc.evolve_screens(N, dx, psd, LAM, [CN2], [DZ], n_sh, 1.0, vx, vy, T, zero, fresh_sh, spec, shc)
+    dfp = 1.0 / (N * dx) / 3.0 ** p
+    fx, fy = (b - 1) * dfp, (a - 1) * dfp
+    x = synth.coords(N, dx)
+    X, Y = np.meshgrid(x, x)
+    tau = np.exp(-2j * np.pi * T * (fx * vx + fy * vy))
+    lo = np.real(c * tau * np.exp(2j * np.pi * (fx * X + fy * Y)))
+    np.testing.assert_allclose(out[0, 0], lo - lo.mean(), rtol=0, atol=1e-12 * abs(c))
+    # the same statement as a shift: phi_new(x, y) = phi_old(x - vx T, y - vy T) before mean removal
+    shifted = np.real(c * np.exp(2j * np.pi * (fx * (X - vx * T) + fy * (Y - vy * T))))
+    np.testing.assert_allclose(lo, shifted, rtol=0, atol=1e-12 * abs(c))
+    assert abs(shc[0, 0, p - 1, a, b] - c * tau) < 1e-14 * abs(c)           # the stored coefficient carries the tilt
+    assert abs(tau - 1) > 0.01                                # the wind does something at this level
+
+
 def test_ar_decorrelation_follows_a_power_n(orc):
     """P6 statistical: with v = 0, corr(phi_t, phi_{t+n}) -> a^n and the variance stays stationary
     (Pearson score, threshold 0.4; a = 0.99 crosses 0.4 at n ~ 91)."""
