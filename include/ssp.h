@@ -188,6 +188,12 @@ int ssp_hv57_path(const ssp_hv57 *p, double h0, double L, int n, double lambda, 
  * (their noise arguments stay inputs: any generator may fill them).  Enqueued on the context's stream. */
 int ssp_fill_noise(ssp_ctx *ctx, unsigned long long seed, unsigned long long stream, unsigned long long first,
                    unsigned long long n, float *d_out);
+/* The raw words of the same generator, for checking it against the published known-answer vectors of Philox-4x32-10
+ * (Salmon et al., SC'11): d_out[4 j .. 4 j + 3] = the four 32-bit output words of block first_block + j (index mod 2^64)
+ * of (seed, stream), i.e. counter (i mod 2^32, i >> 32, stream mod 2^32, stream >> 32), key (seed mod 2^32, seed >> 32).
+ * d_out: dev uint32 [n_blocks][4], 16-byte aligned.  Enqueued on the context's stream. */
+int ssp_philox_words(ssp_ctx *ctx, unsigned long long seed, unsigned long long stream, unsigned long long first_block,
+                     unsigned long long n_blocks, unsigned int *d_out);
 
 /* Screen placement (Sec. 2.4).  Host-only, double precision.
  * ssp_dz_max: the largest step the angular-spectrum transfer function (Eq. 6) supports before its phase
@@ -300,7 +306,6 @@ int ssp_phase_mul(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_theta, doub
  * (inverse != 0: its inverse).  in may alias out. */
 int ssp_dft2_centered(ssp_ctx *ctx, ssp_grid grid, int B, int inverse,
                       const float *d_in, float *d_out, void *d_ws, size_t ws_bytes);
-/* grad[b] = Im(g[b] conj(u[b])), dev fp32 [B][N][N]. */
 /* One Adam step on a phase mask shared by B fields (D2NN training):
  *   g = (1/B) sum_b d_grad[b];  m <- b1 m + (1-b1) g;  v <- b2 v + (1-b2) g^2;
  *   theta <- theta - lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps),   t >= 1 the step count.
@@ -311,6 +316,7 @@ int ssp_adam_update(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_grad, dou
  * (ix-N/2)^2 + (iy-N/2)^2 <= floor((radius/dx)^2) (the threshold is an integer taken on the host in
  * double), else 0.  d_in / d_out: dev complex64 [B][N][N]; may alias. */
 int ssp_aperture(ssp_ctx *ctx, ssp_grid grid, int B, double radius, const float *d_in, float *d_out);
+/* grad[b] = Im(g[b] conj(u[b])), dev fp32 [B][N][N]; d_g, d_u dev complex64 [B][N][N]. */
 int ssp_phase_grad(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_g, const float *d_u,
                    float *d_grad);
 /* Per field b: d_out[b] = { Re <a,b>, Im <a,b>, sum |a|^2, sum |b|^2 } (doubles),

@@ -27,7 +27,7 @@ SYMBOLS = (
     "ssp_create", "ssp_destroy", "ssp_last_error", "ssp_version", "ssp_launch_count",
     "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_make_screens_pair", "ssp_evolve_screens_pair", "ssp_propagate",
     "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_propagate_host", "ssp_phase_mul",
-    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path", "ssp_dz_max", "ssp_place_screens", "ssp_fill_noise", "ssp_frame_chunk", "ssp_frame_host",
+    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path", "ssp_dz_max", "ssp_place_screens", "ssp_fill_noise", "ssp_philox_words", "ssp_frame_chunk", "ssp_frame_host",
     "ssp_profile_enable", "ssp_profile_report",
 )
 
@@ -113,6 +113,7 @@ def load():
     lib.ssp_hv57_cn2.restype = D
     lib.ssp_hv57_path.argtypes = [C.POINTER(Hv57), D, D, I, D, P, P, P, P]
     lib.ssp_fill_noise.argtypes = [P, C.c_ulonglong, C.c_ulonglong, C.c_ulonglong, C.c_ulonglong, P]
+    lib.ssp_philox_words.argtypes = [P, C.c_ulonglong, C.c_ulonglong, C.c_ulonglong, C.c_ulonglong, P]
     lib.ssp_dz_max.argtypes = [Grid, D, D]
     lib.ssp_dz_max.restype = D
     lib.ssp_place_screens.argtypes = [P, P, I, P, I, D, D, D, I, P, P, P, P]
@@ -417,6 +418,13 @@ class Context:
         """Fill the complex64 CUDA tensor `out` (any shape, contiguous) with draws first.. of the stream (seed, stream)."""
         self._chk(self._lib.ssp_fill_noise(self._h, int(seed), int(stream), int(first), out.numel(),
                                            _dev(out, torch.complex64)))
+        return out
+
+    def philox_words(self, seed, stream, first_block, n_blocks):
+        """The generator's raw 32-bit words, int32 CUDA tensor [n_blocks][4] (bit patterns of the unsigned words)."""
+        out = torch.empty((int(n_blocks), 4), dtype=torch.int32, device=torch.device("cuda", self.device))
+        self._chk(self._lib.ssp_philox_words(self._h, int(seed), int(stream), int(first_block), int(n_blocks),
+                                             _dev(out, torch.int32)))
         return out
 
     def aperture(self, N, dx, radius, field, out=None):

@@ -3,6 +3,7 @@
 // runs in the kernels of ssp_propagate.cu / ssp_misc.cu.
 #include <cmath>
 #include <cstring>
+#include <string>
 
 #include "ssp_internal.h"
 
@@ -145,6 +146,19 @@ int run_small(ssp_ctx *ctx, int N, int B, const std::vector<SmallStep> &steps, i
     return launch_small(ctx, N, B, a);
 }
 
+// A *_host call that fails after copies have been queued must not return while DMA into the caller's host or
+// device buffers is still in flight: wait for both copy streams and the context's stream, keep the first error.
+int drain_pipeline(ssp_ctx *ctx, int rc)
+{
+    const std::string first = ctx->err;
+    if (ctx->copy_in) cudaStreamSynchronize(ctx->copy_in);
+    if (ctx->copy_out) cudaStreamSynchronize(ctx->copy_out);
+    cudaStreamSynchronize(ctx->stream);
+    cudaGetLastError();
+    ctx->err = first;
+    return rc;
+}
+
 bool small_ok(int N, int h_kind, int n_steps, const void *planes)
 {
     return small_path_available(N) && h_kind == SSP_H_FRESNEL && !planes &&
@@ -168,6 +182,7 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
     if (screen_batch_stride < 0 || (screen_batch_stride & 3))
         return ctx->fail(SSP_EINVAL, "screen_batch_stride must be >= 0 and a multiple of 4 elements");
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (int rc = trim_htables(ctx)) return rc;
     const int N = grid.N;
     const size_t px = (size_t)N * N;
     const double lam_eff = lambda / n0;
@@ -258,6 +273,7 @@ int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0,
     if ((d_planes == nullptr) != (d_phase_grad == nullptr))
         return ctx->fail(SSP_EINVAL, "d_planes and d_phase_grad must both be given or both be null");
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (int rc = trim_htables(ctx)) return rc;
     const int N = grid.N;
     const size_t px = (size_t)N * N;
     const double lam_eff = lambda / n0;
@@ -365,8 +381,13 @@ int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, in
     if (!h_field_in || !h_field_out || !d_field) return ctx->fail(SSP_EINVAL, "field buffers are required");
     if (S > 0 && !d_screens) return ctx->fail(SSP_EINVAL, "d_screens is required");
     if (h_stats && !d_stats) return ctx->fail(SSP_EINVAL, "d_stats is required with h_stats");
+    // everything the inner ssp_propagate calls would reject is rejected here, before the first copy is queued
+    if (int rc = check_prop(ctx, grid, lambda, n0, h_kind, B, n_steps, dz, d_screens, S, d_field, d_field)) return rc;
+    if (screen_batch_stride < 0 || (screen_batch_stride & 3))
+        return ctx->fail(SSP_EINVAL, "screen_batch_stride must be >= 0 and a multiple of 4 elements");
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));
     const size_t px = (size_t)grid.N * grid.N;
+    const int rc_pipe = [&]() -> int {
     // Chunked pipeline over the batch: the host->device copy of chunk c+1 (copy_in stream) overlaps the
     // propagation of chunk c (context stream) and the device->host copy of chunk c-1 (copy_out stream).
     if (!ctx->copy_in) {
@@ -416,6 +437,8 @@ int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, in
     SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ev_end, 0));
     SSP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return SSP_OK;
+    }();
+    return rc_pipe ? drain_pipeline(ctx, rc_pipe) : SSP_OK;
 }
 
 int ssp_frame_chunk(int B) { return B >= 8 ? B / 8 : 1; }
@@ -432,12 +455,21 @@ int ssp_frame_host(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambd
         return ctx->fail(SSP_EINVAL, "field, spectrum, screen and noise buffers are required");
     if (n_sh > 0 && (!d_sh_coef || !d_noise_sh)) return ctx->fail(SSP_EINVAL, "subharmonic buffers are required");
     if (h_stats && !d_stats) return ctx->fail(SSP_EINVAL, "d_stats is required with h_stats");
+    // everything the inner calls would reject is rejected here, before the first copy is queued
+    if (int rc = check_prop(ctx, grid, lambda, n0, h_kind, B, S, dz, d_screens, S, d_field, d_field)) return rc;
+    if (int rc = check_screen_args(ctx, grid, psd, lambda, ssp_frame_chunk(B), S, cn2, dz, n_sh, d_noise, d_noise_sh,
+                                   d_screens, d_ws, ws_bytes))
+        return rc;
+    if (!(ar->a >= 0.0 && ar->a <= 1.0)) return ctx->fail(SSP_EINVAL, "AR factor a must be in [0, 1]");
+    if (!aligned16(d_spectrum) || !aligned16(d_sh_coef) || !aligned16(d_noise_sh))
+        return ctx->fail(SSP_EINVAL, "device pointers must be 16-byte aligned");
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));
     const size_t px = (size_t)grid.N * grid.N;
     if (!ctx->copy_in) {
         SSP_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_in, cudaStreamNonBlocking));
         SSP_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_out, cudaStreamNonBlocking));
     }
+    const int rc_pipe = [&]() -> int {
     const int Bc = ssp_frame_chunk(B);
     const int n_chunks = (B + Bc - 1) / Bc;
     while ((int)ctx->pipe_events.size() < 2 * n_chunks + 2) {
@@ -495,6 +527,8 @@ int ssp_frame_host(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambd
     SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ev_end, 0));
     SSP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return SSP_OK;
+    }();
+    return rc_pipe ? drain_pipeline(ctx, rc_pipe) : SSP_OK;
 }
 
 } // extern "C"

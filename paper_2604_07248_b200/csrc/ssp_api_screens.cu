@@ -260,6 +260,13 @@ int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
 
 } // namespace
 
+int ssp::check_screen_args(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, int B, int S, const double *cn2,
+                           const double *dz, int n_sh, const void *noise, const void *noise_sh, const void *screens,
+                           const void *ws, size_t ws_bytes)
+{
+    return check_screens(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, noise, noise_sh, screens, ws, ws_bytes);
+}
+
 extern "C" {
 
 size_t ssp_workspace_bytes(ssp_grid grid, int B, int S)

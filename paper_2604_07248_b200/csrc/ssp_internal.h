@@ -116,6 +116,9 @@ namespace ssp {
 // V = 0: row-plan tables, V = 1: column-plan tables (ssp_fft.cuh)
 int get_twiddles(ssp_ctx *ctx, int N, int V, const float2 **out);
 int get_htable(ssp_ctx *ctx, const HKey &key, const float2 **out);
+// Drops the 1-D table cache when it has grown past 4096 entries.  Called once at the entry of ssp_propagate /
+// ssp_propagate_adjoint, never between the table look-ups of one call (their pointers stay valid until the launch).
+int trim_htables(ssp_ctx *ctx);
 // Angular-spectrum transfer function H(ky,kx)/N^2 as a complex64 map [N][N] (Eq.6, carrier removed,
 // evanescent bins 0), evaluated once per (grid, lambda/n0, dz, conj) in double on the device and cached
 // (8 N^2 bytes each, L2-resident at N <= 1024; the cache is dropped when it passes 1 GiB).
@@ -235,6 +238,11 @@ struct ScreenRowArgs {
     const float2 *ex;         // [n_sh][N] exp(i 2 pi df_p x)
     const float2 *tw;
 };
+// argument checks of ssp_make_screens / ssp_evolve_screens (ssp_api_screens.cu), for callers that must validate
+// before they queue anything (ssp_frame_host)
+int check_screen_args(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, int B, int S, const double *cn2,
+                      const double *dz, int n_sh, const void *noise, const void *noise_sh, const void *screens,
+                      const void *ws, size_t ws_bytes);
 int launch_screen_col(ssp_ctx *ctx, int N, const ScreenColArgs &a);
 int screen_col_plan_variant(int N);   // plan variant (ssp_fft.cuh) whose twiddles launch_screen_col expects in a.tw
 int launch_screen_row(ssp_ctx *ctx, int N, const ScreenRowArgs &a);

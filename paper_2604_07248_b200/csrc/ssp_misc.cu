@@ -1,8 +1,9 @@
 // ssp_misc.cu -- statistics reducer (K8) and the small element-wise helpers.
 //
 // K8 (PAPER.md:423 S25, :143; O8): per field, raw intensity moments about the grid
-// centre in pixel units, accumulated per thread in fp64, combined by warp shuffles and one
-// fp64 atomic per warp; a one-thread-per-field finaliser turns them into ssp_stats.
+// centre in pixel units: fp32 partial sums within a row, promoted to fp64 once per row, combined by
+// warp shuffles into one partial per block and moment (no atomics: bit-reproducible); a one-warp-per-field
+// finaliser adds the block partials in block order and turns them into ssp_stats.
 #include "ssp_internal.h"
 
 namespace ssp {
@@ -141,7 +142,7 @@ int launch_stats(ssp_ctx *ctx, int N, double dx, int B, const float2 *field, dou
     const int rows_per_pass = 256 >> lane_shift;
     // blocks per field: all B * bpf blocks resident at once (8 per SM) when the batch allows, every block the same
     // number of row passes (to within one)
-    const int passes = N / rows_per_pass;
+    const int passes = (N + rows_per_pass - 1) / rows_per_pass;               // >= 1 (N = 8, 16: one partial pass; the kernel guards iy < N)
     int target = (ctx->num_sms * 8) / B;
     if (target < 1) target = 1;
     const int per = (passes + target - 1) / target;

@@ -38,19 +38,48 @@ __device__ __forceinline__ float2 box_muller(uint32_t xr, uint32_t xa)
 
 struct RoundKeys { uint32_t k[10][2]; };   // the key schedule (key + r * Weyl constants), computed once on the host
 
+// the four output words of block i of stream (s0, s1)
+__device__ __forceinline__ void philox_block(const RoundKeys &keys, unsigned long long i, uint32_t s0, uint32_t s1,
+                                             uint32_t (&c)[4])
+{
+    c[0] = (uint32_t)i; c[1] = (uint32_t)(i >> 32); c[2] = s0; c[3] = s1;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) philox_round(c, keys.k[r][0], keys.k[r][1]);
+}
+
 __global__ void __launch_bounds__(256) k_fill_noise(const RoundKeys keys, uint32_t s0, uint32_t s1,
                                                      unsigned long long first_block, unsigned long long n_draws,
                                                      float2 *__restrict__ out)
 {
     const unsigned long long j = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;   // block within this call
     if (2 * j >= n_draws) return;
-    const unsigned long long i = first_block + j;
-    uint32_t c[4] = {(uint32_t)i, (uint32_t)(i >> 32), s0, s1};
-#pragma unroll
-    for (int r = 0; r < 10; ++r) philox_round(c, keys.k[r][0], keys.k[r][1]);
+    uint32_t c[4];
+    philox_block(keys, first_block + j, s0, s1, c);
     const float2 z0 = box_muller(c[0], c[1]), z1 = box_muller(c[2], c[3]);
     if (2 * j + 1 < n_draws) reinterpret_cast<float4 *>(out)[j] = make_float4(z0.x, z0.y, z1.x, z1.y);
     else out[2 * j] = z0;
+}
+
+// the generator's raw words (no Box-Muller): block first_block + j -> out[j] = (x0, x1, x2, x3); the block index wraps mod 2^64
+__global__ void __launch_bounds__(256) k_philox_words(const RoundKeys keys, uint32_t s0, uint32_t s1,
+                                                       unsigned long long first_block, unsigned long long n_blocks,
+                                                       uint4 *__restrict__ out)
+{
+    const unsigned long long j = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_blocks) return;
+    uint32_t c[4];
+    philox_block(keys, first_block + j, s0, s1, c);
+    out[j] = make_uint4(c[0], c[1], c[2], c[3]);
+}
+
+RoundKeys key_schedule(unsigned long long seed)
+{
+    RoundKeys keys;
+    for (int r = 0; r < 10; ++r) {
+        keys.k[r][0] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u;
+        keys.k[r][1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+    }
+    return keys;
 }
 
 int launch_fill_noise(ssp_ctx *ctx, unsigned long long seed, unsigned long long stream, unsigned long long first,
@@ -59,11 +88,7 @@ int launch_fill_noise(ssp_ctx *ctx, unsigned long long seed, unsigned long long 
     const unsigned long long blocks = (n + 1) / 2;
     const unsigned long long grid = (blocks + 255) / 256;
     if (grid > 0x7FFFFFFFull) return ctx->fail(SSP_EINVAL, "ssp_fill_noise: more than 2^40 draws in one call");
-    RoundKeys keys;
-    for (int r = 0; r < 10; ++r) {
-        keys.k[r][0] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u;
-        keys.k[r][1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
-    }
+    const RoundKeys keys = key_schedule(seed);
     ctx->prof_begin("fill_noise", 8.0 * (double)n);
     k_fill_noise<<<(unsigned)grid, 256, 0, ctx->stream>>>(keys, (uint32_t)stream, (uint32_t)(stream >> 32), first / 2, n, out);
     ctx->prof_end();
@@ -83,4 +108,20 @@ extern "C" int ssp_fill_noise(ssp_ctx *ctx, unsigned long long seed, unsigned lo
         return ctx->fail(SSP_EINVAL, "ssp_fill_noise: null or misaligned output, or odd first draw");
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));
     return ssp::launch_fill_noise(ctx, seed, stream, first, n, reinterpret_cast<float2 *>(d_out));
+}
+
+extern "C" int ssp_philox_words(ssp_ctx *ctx, unsigned long long seed, unsigned long long stream,
+                                unsigned long long first_block, unsigned long long n_blocks, unsigned int *d_out)
+{
+    if (!ctx) return SSP_EINVAL;
+    if (n_blocks == 0) return SSP_OK;
+    if (!d_out || (reinterpret_cast<uintptr_t>(d_out) & 15u) || n_blocks > (1ull << 38))
+        return ctx->fail(SSP_EINVAL, "ssp_philox_words: null or misaligned output, or more than 2^38 blocks");
+    SSP_CUDA(ctx, cudaSetDevice(ctx->device));
+    const ssp::RoundKeys keys = ssp::key_schedule(seed);
+    ssp::k_philox_words<<<(unsigned)((n_blocks + 255) / 256), 256, 0, ctx->stream>>>(
+        keys, (uint32_t)stream, (uint32_t)(stream >> 32), first_block, n_blocks, reinterpret_cast<uint4 *>(d_out));
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
 }

@@ -85,11 +85,6 @@ int get_htable(ssp_ctx *ctx, const HKey &key, const float2 **out)
 {
     auto it = ctx->htables.find(key);
     if (it != ctx->htables.end()) { *out = it->second; return SSP_OK; }
-    if (ctx->htables.size() > 4096) { // unbounded dz lists: drop the cache rather than grow
-        SSP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-        for (auto &kv : ctx->htables) cudaFree(kv.second);
-        ctx->htables.clear();
-    }
     const double kPi = 3.14159265358979323846;
     const int N = key.N;
     std::vector<float2> h(N);
@@ -106,6 +101,17 @@ int get_htable(ssp_ctx *ctx, const HKey &key, const float2 **out)
     if (int rc = upload(ctx, h, &d)) return rc;
     ctx->htables[key] = d;
     *out = d;
+    return SSP_OK;
+}
+
+// Callers may collect several table pointers before launching (the on-chip path gathers the tables of a whole
+// stack), so get_htable never frees: the cap is enforced here, once, at the entry of a propagation call.
+int trim_htables(ssp_ctx *ctx)
+{
+    if (ctx->htables.size() <= 4096) return SSP_OK;   // unbounded dz lists: drop the cache rather than grow
+    SSP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (auto &kv : ctx->htables) cudaFree(kv.second);
+    ctx->htables.clear();
     return SSP_OK;
 }
 

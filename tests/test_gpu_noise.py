@@ -108,3 +108,76 @@ def test_fill_noise_errors(ssp):
     with pytest.raises(api.SspError):
         ssp.fill_noise(1, 1, out[1:])                          # 8-byte aligned only
     ssp.fill_noise(1, 1, out[:0])                              # empty: no-op
+
+
+def test_philox_known_answer_vectors_on_device(ssp):
+    """The device generator word for word against the published Philox-4x32-10 vectors (tests/golden/philox_kat.txt,
+    Salmon et al. SC'11): counter (i lo, i hi, stream lo, stream hi), key (seed lo, seed hi) as DESIGN.md Q29 states."""
+    from tests.test_oracle_noise import philox_kat_vectors
+    for ctr, key, want in philox_kat_vectors():
+        i = ctr[0] | (ctr[1] << 32)
+        stream = ctr[2] | (ctr[3] << 32)
+        seed = key[0] | (key[1] << 32)
+        w = ssp.philox_words(seed, stream, i, 1).cpu().numpy().view(np.uint32)[0]
+        assert [int(v) for v in w] == want, ([hex(int(v)) for v in w], [hex(v) for v in want])
+
+
+def test_philox_words_are_what_fill_noise_draws_from(ssp, orc):
+    """ssp_philox_words and ssp_fill_noise share one device function: Box-Muller (in fp64, here) on the words equals the draws,
+    and the words equal the oracle's independent integer implementation bit for bit, ragged block counts included."""
+    seed, stream, first_block, nb = 0x0123456789ABCDEF, 0xFEDCBA9876543210, (1 << 32) - 3, 1029
+    w = ssp.philox_words(seed, stream, first_block, nb).cpu().numpy().view(np.uint32)
+    idx = np.arange(first_block, first_block + nb, dtype=np.uint64)
+    ctr = np.stack([idx & np.uint64(0xFFFFFFFF), idx >> np.uint64(32),
+                    np.full(nb, stream & 0xFFFFFFFF, dtype=np.uint64), np.full(nb, stream >> 32, dtype=np.uint64)], axis=1)
+    ref = orc.philox4x32_10(ctr.astype(np.uint32), (seed & 0xFFFFFFFF, seed >> 32))
+    assert np.array_equal(w, ref)
+    out = torch.zeros(2 * nb, dtype=torch.complex64, device="cuda")
+    ssp.fill_noise(seed, stream, out, first=2 * first_block)
+    x = w.astype(np.float64).reshape(-1, 2)
+    u = (np.floor(x[:, 0] / 512.0) + 0.5) / 8388608.0
+    f = (np.floor(x[:, 1] / 512.0) + 0.5) / 8388608.0
+    z = np.sqrt(-2.0 * np.log(u)) * np.exp(2j * np.pi * f)
+    assert np.all(np.abs(out.cpu().numpy() - z) < 1e-6 * (1 + np.abs(z)))
+
+
+def test_frame_host_rejects_bad_arguments_before_any_copy(ssp):
+    """A bad dz / a / S in ssp_frame_host is an SSP_EINVAL raised before anything is queued: the host output buffer is
+    untouched, and the same buffers then serve a valid call whose result equals a fresh run."""
+    from paper_2604_07248_b200 import api, synth
+    N, dx, lam, S, B, n_sh = 128, 2e-3, 1.55e-6, 3, 4, 2
+    cn2, dz = [1e-14, 3e-14, 2e-15], [100.0, 40.0, 250.0]
+    psd = api.PsdParams(kind=api.PSD_VON_KARMAN, L0=20.0, l0=4e-3)
+    kw = dict(win_order=16, win_sigma_frac=0.47)
+    c64 = lambda *sh: torch.empty(sh, dtype=torch.complex64, device="cuda")
+    noise, nsh = c64(B, S, N, N), c64(B, S, n_sh, 3, 3)
+    ssp.fill_noise(9, 100, noise)
+    ssp.fill_noise(9, 101, nsh)
+    spec, shc = c64(B, S, N, N), c64(B, S, n_sh, 3, 3)
+    ssp.make_screens(N, dx, psd, lam, cn2, dz, n_sh, noise, nsh, spectrum=spec, sh_coef=shc)
+    spec0, shc0 = spec.clone(), shc.clone()
+    u0 = torch.from_numpy(synth.gaussian_beam(N, dx, 3e-2, B))
+    h_in = u0.pin_memory()
+    h_out = torch.full_like(u0, 7.0 + 7.0j).pin_memory()
+    h_st = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8).pin_memory()
+    Bc = api.frame_chunk(B)
+    d_field, scr = c64(B, N, N), torch.empty((B, S, N, N), dtype=torch.float32, device="cuda")
+    d_noise, d_nsh = c64(Bc, S, N, N), c64(B, S, n_sh, 3, 3)
+    d_st = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+    ws = ssp.workspace(N, dx, B, S)
+    d_field.zero_()
+    run = lambda dz_, a_: ssp.frame_host(N, dx, psd, lam, cn2, dz_, n_sh, a_, 3.0, -2.0, 1e-3, 77, 0, h_in, h_out, h_st, 0.5,
+                                         d_field, spec, shc, scr, d_noise, d_nsh, d_st, ws, **kw)
+    for bad_dz, bad_a in (([100.0, -40.0, 250.0], 0.97), ([100.0, 40.0, float("nan")], 0.97), (dz, 1.5)):
+        with pytest.raises(api.SspError) as ei:
+            run(bad_dz, bad_a)
+        assert ei.value.code == api.EINVAL
+        torch.cuda.synchronize()
+        assert torch.all(h_out == 7.0 + 7.0j)                  # nothing was copied back
+        assert torch.all(d_field == 0)                         # nothing was uploaded
+        assert torch.equal(spec, spec0) and torch.equal(shc, shc0)   # the AR state did not advance
+    run(dz, 0.97)
+    got = h_out.clone()
+    spec.copy_(spec0); shc.copy_(shc0)
+    run(dz, 0.97)
+    assert torch.equal(got, h_out) and torch.all(torch.isfinite(torch.view_as_real(h_out)))

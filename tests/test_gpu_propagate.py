@@ -215,6 +215,55 @@ def test_beam_stats_and_welford(ssp, orc):
     np.testing.assert_allclose(M2.cpu().numpy(), M2_ref, rtol=2e-4, atol=1e-7)
 
 
+@pytest.mark.parametrize("N", [8, 16, 32, 64])
+def test_beam_stats_small_grids(ssp, orc, N):
+    """Grids with fewer rows than one pass of the reducer (N = 8, 16: a host-side division by zero in round 1), through
+    ssp_beam_stats and through ssp_propagate's statistics epilogue, B = 1, 4 and a batch beyond one wave."""
+    from paper_2604_07248_b200 import api
+    dx = 1e-3
+    for B in (1, 4, 300):
+        u = (synth.random_field(N, B, 100 + N) + synth.gaussian_beam(N, dx, 0.2 * N * dx, B)).astype(np.complex64)
+        for roi in (0.0, 0.5, 1.0):
+            st_ref = orc.beam_stats(N, dx, u, roi_frac=roi)
+            stats, _ = ssp.beam_stats(N, dx, cu(u), roi_frac=roi)
+            for a, r in zip(api.stats_to_dicts(stats), st_ref):
+                for k in ("power", "w2", "sxx", "syy", "I_axis", "roi_sumI", "roi_sumI2"):
+                    assert abs(a[k] / r[k] - 1) < 1e-6, (B, roi, k, a[k], r[k])
+                assert abs(a["cx"] - r["cx"]) < 1e-7 * dx * N and abs(a["cy"] - r["cy"]) < 1e-7 * dx * N
+                assert a["roi_n"] == r["roi_n"]
+    import torch
+    B = 3
+    dx, lam, dz, u0, scr = _case(N, B, 2, 2, 7 * N)
+    stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+    out = ssp.propagate(N, dx, lam, list(dz), cu(u0), cu(scr), win_order=16, win_sigma_frac=0.47, stats=stats, roi_frac=0.5)
+    ref = orc.propagate(N, dx, lam, dz, u0, scr, win_order=16, win_sigma_frac=0.47)
+    for a, r in zip(api.stats_to_dicts(stats), orc.beam_stats(N, dx, ref, roi_frac=0.5)):
+        for k in ("power", "w2", "I_axis", "roi_sumI", "roi_sumI2"):
+            assert abs(a[k] / r[k] - 1) < 1e-4, (k, a[k], r[k])
+
+
+def test_transfer_table_cache_overflow_keeps_pointers_valid(ssp, orc):
+    """The context caches one 1-D transfer-function table per distinct (N, dx, lambda, dz, conj, scaled) and drops the
+    cache beyond 4096 entries -- at the entry of a call only, never between the look-ups of one call (round 1 freed
+    tables the on-chip path had already collected).  Fill the cache past the cap with throw-away steps, then run an
+    N = 128 stack of distinct steps (on-chip path: all tables gathered before the one launch) against the oracle."""
+    N, B, n_steps = 128, 2, 6
+    dx, lam, dz, u0, scr = _case(N, B, n_steps, n_steps, 4242)
+    ref = orc.propagate(N, dx, lam, dz, u0, scr, win_order=16, win_sigma_frac=0.47)
+    d_u0, d_scr = cu(u0), cu(scr)
+    small = cu(synth.random_field(8, 1, 1))
+    for rep in range(3):
+        for chunk in range(9):                                     # 9 x 240 steps x 2 tables each > 4096 per repetition
+            dzs = [1.0 + 1e-3 * (rep * 10000 + chunk * 240 + j) for j in range(240)]
+            ssp.propagate(8, dx, lam, dzs, small, None)
+        out = ssp.propagate(N, dx, lam, list(dz), d_u0, d_scr, win_order=16, win_sigma_frac=0.47)
+        err = rel_l2(out.cpu().numpy(), ref)
+        assert err.max() < tol(N, n_steps), (rep, err)
+        g = ssp.propagate_adjoint(N, dx, lam, list(dz), out, d_scr, win_order=16, win_sigma_frac=0.47)
+        gref = orc.propagate_adjoint(N, dx, lam, dz, out.cpu().numpy(), scr, win_order=16, win_sigma_frac=0.47)
+        assert rel_l2(g.cpu().numpy(), gref).max() < tol(N, n_steps)
+
+
 def test_error_codes(ssp):
     import torch
     from paper_2604_07248_b200 import api
