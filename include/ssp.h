@@ -285,7 +285,12 @@ int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, in
  * [B][S][N][N] and d_sh_coef c64 [B][S][n_sh][3][3], in-out (the AR state, from ssp_make_screens); d_screens fp32
  * [B][S][N][N] (out: this frame's screens); d_noise c64 [ssp_frame_chunk(B)][S][N][N] scratch; d_noise_sh c64
  * [B][S][n_sh][3][3] scratch; d_stats [B]; d_ws >= ssp_workspace_bytes(grid, ssp_frame_chunk(B), S).
- * Synchronises the stream. */
+ * h_adjoint_out (host c64 [B][N][N], optional; with it d_adjoint, dev c64 [B][N][N] scratch): the frame also runs the
+ * adjoint split step on each group's received fields, h_adjoint_out = A^H U_out (ssp_propagate_adjoint with
+ * d_g_out = the received field: the gradient of the received power (1/2) sum |U_out|^2 w.r.t. the input field, i.e.
+ * the time-reversed return), and copies it back under the next group's work.  NULL: forward only.
+ * Every argument is validated before the first copy is queued; if an inner call still fails, both copy streams and
+ * the context's stream are drained before the error is returned.  Synchronises the stream. */
 typedef struct {
     double a, vx, vy, T;            /* blending factor, wind [m/s], frame interval [s] (Eq. 4, 5) */
     unsigned long long seed, frame; /* noise streams 2*frame and 2*frame+1 of this seed */
@@ -295,7 +300,8 @@ int ssp_frame_host(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambd
                    int B, int S, const double *cn2, const double *dz, int n_sh, const ssp_ar *ar,
                    ssp_window win, const float *h_field_in, float *h_field_out, ssp_stats *h_stats, double roi_frac,
                    float *d_field, float *d_spectrum, float *d_sh_coef, float *d_screens,
-                   float *d_noise, float *d_noise_sh, ssp_stats *d_stats, void *d_ws, size_t ws_bytes);
+                   float *d_noise, float *d_noise_sh, ssp_stats *d_stats, void *d_ws, size_t ws_bytes,
+                   float *h_adjoint_out, float *d_adjoint);
 
 /* ---- helpers for mask systems (config 4; O9) ----------------- */
 

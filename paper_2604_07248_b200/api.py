@@ -104,7 +104,7 @@ def load():
                                        C.c_size_t]
     lib.ssp_frame_chunk.argtypes = [I]
     lib.ssp_frame_host.argtypes = [P, Grid, P, D, D, I, I, I, P, P, I, P, Window, P, P, P, D, P, P, P, P, P, P, P, P,
-                                   C.c_size_t]
+                                   C.c_size_t, P, P]
     lib.ssp_phase_mul.argtypes = [P, Grid, I, P, D, P, P]
     lib.ssp_dft2_centered.argtypes = [P, Grid, I, I, P, P, P, C.c_size_t]
     lib.ssp_phase_grad.argtypes = [P, Grid, I, P, P, P]
@@ -381,9 +381,10 @@ class Context:
 
     def frame_host(self, N, dx, psd: PsdParams, lam, cn2, dz, n_sh, a, vx, vy, T, seed, frame, h_field_in, h_field_out,
                    h_stats, roi_frac, d_field, spectrum, sh_coef, screens, d_noise, d_noise_sh, d_stats, ws,
-                   win_order=0, win_sigma_frac=0.0, n0=1.0, h_kind=H_FRESNEL):
+                   win_order=0, win_sigma_frac=0.0, n0=1.0, h_kind=H_FRESNEL, h_adjoint_out=None, d_adjoint=None):
         """One temporal frame from pinned host fields: device-side noise draws, AR screen evolution, propagation,
-        results back on the host.  d_noise: complex64 [frame_chunk(B)][S][N][N] scratch.  Synchronises the stream."""
+        results back on the host.  d_noise: complex64 [frame_chunk(B)][S][N][N] scratch.  h_adjoint_out / d_adjoint:
+        also send the received fields back through the screens (A^H U_out) and return that.  Synchronises the stream."""
         B, S = d_field.shape[0], screens.shape[1]
         pc, ar = psd.c(), Ar(a, vx, vy, T, int(seed), int(frame))
         hp = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
@@ -393,7 +394,7 @@ class Context:
             _dev(d_field, torch.complex64), _dev(spectrum, torch.complex64),
             _dev(sh_coef, torch.complex64) if n_sh > 0 else None, _dev(screens, torch.float32),
             _dev(d_noise, torch.complex64), _dev(d_noise_sh, torch.complex64) if n_sh > 0 else None,
-            _dev(d_stats), _dev(ws), ws.numel()))
+            _dev(d_stats), _dev(ws), ws.numel(), hp(h_adjoint_out), _dev(d_adjoint, torch.complex64)))
 
     # ---- helpers ---------------------------------------------------------------------------
     def phase_mul(self, N, dx, theta, field, sign=1.0, out=None):

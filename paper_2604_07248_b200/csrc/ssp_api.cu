@@ -447,7 +447,8 @@ int ssp_frame_host(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambd
                    int B, int S, const double *cn2, const double *dz, int n_sh, const ssp_ar *ar,
                    ssp_window win, const float *h_field_in, float *h_field_out, ssp_stats *h_stats, double roi_frac,
                    float *d_field, float *d_spectrum, float *d_sh_coef, float *d_screens,
-                   float *d_noise, float *d_noise_sh, ssp_stats *d_stats, void *d_ws, size_t ws_bytes)
+                   float *d_noise, float *d_noise_sh, ssp_stats *d_stats, void *d_ws, size_t ws_bytes,
+                   float *h_adjoint_out, float *d_adjoint)
 {
     if (!ctx) return SSP_EINVAL;
     if (!valid_N(grid.N) || B < 1 || S < 1 || !ar || !psd) return ctx->fail(SSP_EINVAL, "bad grid, batch, S or parameters");
@@ -455,6 +456,8 @@ int ssp_frame_host(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambd
         return ctx->fail(SSP_EINVAL, "field, spectrum, screen and noise buffers are required");
     if (n_sh > 0 && (!d_sh_coef || !d_noise_sh)) return ctx->fail(SSP_EINVAL, "subharmonic buffers are required");
     if (h_stats && !d_stats) return ctx->fail(SSP_EINVAL, "d_stats is required with h_stats");
+    if (h_adjoint_out && (!d_adjoint || !aligned16(d_adjoint)))
+        return ctx->fail(SSP_EINVAL, "d_adjoint (16-byte aligned) is required with h_adjoint_out");
     // everything the inner calls would reject is rejected here, before the first copy is queued
     if (int rc = check_prop(ctx, grid, lambda, n0, h_kind, B, S, dz, d_screens, S, d_field, d_field)) return rc;
     if (int rc = check_screen_args(ctx, grid, psd, lambda, ssp_frame_chunk(B), S, cn2, dz, n_sh, d_noise, d_noise_sh,
@@ -519,6 +522,16 @@ int ssp_frame_host(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambd
         SSP_CUDA(ctx, cudaMemcpyAsync(h_field_out + 2 * px * (size_t)g0, df, sizeof(float) * 2 * px * gn, cudaMemcpyDeviceToHost, ctx->copy_out));
         if (h_stats)
             SSP_CUDA(ctx, cudaMemcpyAsync(h_stats + g0, d_stats + g0, sizeof(ssp_stats) * gn, cudaMemcpyDeviceToHost, ctx->copy_out));
+        if (h_adjoint_out) {
+            // the received fields sent back through the same screens: A^H U_out (reads df while it is being downloaded)
+            float *dg = d_adjoint + 2 * px * (size_t)g0;
+            if (int rc = ssp_propagate_adjoint(ctx, grid, lambda, n0, h_kind, gn, S, dz, d_screens + (size_t)g0 * S * px,
+                                               (long long)S * (long long)px, S, win, df, dg, nullptr, nullptr, d_ws, ws_bytes))
+                return rc;
+            SSP_CUDA(ctx, cudaEventRecord(ev_done, ctx->stream));   // re-recorded: the earlier wait has captured the first record
+            SSP_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_out, ev_done, 0));
+            SSP_CUDA(ctx, cudaMemcpyAsync(h_adjoint_out + 2 * px * (size_t)g0, dg, sizeof(float) * 2 * px * gn, cudaMemcpyDeviceToHost, ctx->copy_out));
+        }
         group_begin = c + 1;
         const int left = n_chunks - group_begin;
         group_end = group_begin + (left + 1) / 2;

@@ -11,14 +11,21 @@ Test infrastructure only; holds no kernel code.
 import numpy as np
 
 
-def oracle_chain(orc, N, dx, lam, dz, u0, scr32, th1, th2, kw, aperture_radius=None):
+def oracle_chain(orc, N, dx, lam, dz, u0, scr32, th1, th2, kw, aperture_radius=None, parallel=False):
     """All quantities for ONE batch of fields on the oracle.  Returns a dict of float64 / complex128 arrays.
     aperture_radius: optional circular aperture applied to A(U0) and to the target; a real 0/1
-    mask, so the adjoint applies it again."""
+    mask, so the adjoint applies it again.  parallel: issue the two independent propagations (through the screens,
+    and through vacuum for the target) side by side."""
     ap = (lambda x: x) if aperture_radius is None else (lambda x: orc.aperture(N, dx, aperture_radius, x))
-    V1, planes = orc.propagate(N, dx, lam, dz, u0, scr32, return_planes=True, **kw)
+    legs = [lambda: orc.propagate(N, dx, lam, dz, u0, scr32, return_planes=True, **kw),
+            lambda: orc.propagate(N, dx, lam, dz, u0, None, **kw)]
+    if parallel:
+        from tests.util import pmap
+        (V1, planes), T = pmap(lambda f: f(), legs)
+    else:
+        (V1, planes), T = legs[0](), legs[1]()
     V1 = ap(V1)
-    T = ap(orc.propagate(N, dx, lam, dz, u0, None, **kw))
+    T = ap(T)
     V2 = orc.phase_mul(N, th1, V1)
     V3 = orc.dft2_centered(N, V2)
     V4 = orc.phase_mul(N, th2, V3)

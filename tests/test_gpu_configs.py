@@ -1,8 +1,10 @@
-"""GPU parity on BASELINE.json configs 2-5 (slices the fp64 oracle finishes in tens of seconds; config 1
-runs in full in test_gpu_propagate.py) and on the bench launch configuration at full size.
+"""GPU parity on BASELINE.json configs 2-5 at the slices SURVEY.md 8(d) states (config 1 runs in full in
+test_gpu_propagate.py) and on the bench launch configuration at full size.
 
-Slices (stated per test): the grid, geometry, medium, beam and batch layout are the
-config's own; what is cut is the number of realisations and, for 2048^2 / 4096^2, the number of screens.
+Slices: the grid, geometry, medium, beam, batch layout AND the number of screens / split steps are the config's own;
+what is cut is the number of realisations (config 2: 4 of 64 per Cn2; config 3: 2 of 32 stacks and 3 of 100 AR frames;
+configs 4 and 5: B = 1) -- the fp64 oracle needs 2.8 s / 12 s per split step at 2048^2 / 4096^2.  Independent oracle
+calls (one per screen, forward / vacuum legs) are issued side by side from threads (tests/util.py: pmap).
 Bar: per-field relative L2 <= 2e-5 log2(N) screens (north_star); screens 2e-5 log2(N) each."""
 import math
 
@@ -10,7 +12,7 @@ import numpy as np
 import pytest
 
 from paper_2604_07248_b200 import synth
-from tests.util import rel_l2
+from tests.util import oracle_screens_parallel, pmap, record, rel_l2
 
 pytestmark = pytest.mark.gpu
 
@@ -53,111 +55,139 @@ def _check_stats(st, st_ref, wl):
 
 
 def test_config2_scintillation_sweep_slice(ssp, orc):
-    """configs[1]: 512^2 plane wave, 10 Kolmogorov screens, Cn2 in {1e-15, 1e-14, 1e-13}; slice = 2 of the 64
-    realisations per Cn2.  Screens, received field and the ROI sums behind the scintillation index."""
+    """configs[1]: 512^2 plane wave, 10 Kolmogorov screens, Cn2 in {1e-15, 1e-14, 1e-13}; slice = 4 of the 64
+    realisations per Cn2 (SURVEY.md 8(d)).  Screens, received field and the ROI sums behind the scintillation index."""
     import torch
     from paper_2604_07248_b200 import api
     wl = synth.CONFIGS[2]
-    N, S, B = wl.N, wl.S, 2
+    N, S, B = wl.N, wl.S, 4
     po, pg = _psd(wl, orc)
     u0 = synth.input_field(wl, B)
     for ic, cn2 in enumerate(wl.cn2_sweep):
         hi, sh = synth.noise_batch(2, ic, B, S, N, 0)
         cn2s = np.full(S, cn2)
-        scr_ref, _, _ = orc.make_screens(N, wl.dx, po, wl.lam, cn2s, wl.dz, 0, hi, sh, keep_spectrum=False)
+        scr_ref, _, _ = oracle_screens_parallel(orc, N, wl.dx, po, wl.lam, cn2s, wl.dz, 0, hi, sh)
         scr = ssp.make_screens(N, wl.dx, pg, wl.lam, list(cn2s), list(wl.dz), 0, cu(c64(hi)))
-        assert rel_l2(scr.cpu().numpy(), scr_ref).max() < tol(N, 1)
+        e_scr = rel_l2(scr.cpu().numpy(), scr_ref).max()
+        assert e_scr < tol(N, 1)
         scr32 = scr_ref.astype(np.float32)                    # identical fp32 screens feed both propagators
         kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
-        ref = orc.propagate(N, wl.dx, wl.lam, wl.dz, u0, scr32, **kw)
+        ref = np.concatenate(pmap(lambda b: orc.propagate(N, wl.dx, wl.lam, wl.dz, u0[b:b + 1], scr32[b:b + 1], **kw), range(B)))
         stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
         out = ssp.propagate(N, wl.dx, wl.lam, list(wl.dz), cu(u0), cu(scr32), stats=stats, roi_frac=0.5, **kw)
         err = rel_l2(out.cpu().numpy(), ref)
         assert err.max() < tol(N, S), (cn2, err)
+        record("config2", cn2=float(cn2), B=B, S=S, screens=float(e_scr), field=float(err.max()), bound=tol(N, S))
         _check_stats(api.stats_to_dicts(stats), orc.beam_stats(N, wl.dx, ref, roi_frac=0.5), wl)
 
 
 def test_config3_temporal_slice(ssp, orc):
-    """configs[2]: 1024^2, 20 von Karman screens + 3 subharmonic levels, AR a = 0.99, Gaussian beam; slice = 1 of
-    the 32 stacks, 2 of the 100 time steps.  Per frame: evolved screens, received field, beam width."""
+    """configs[2]: 1024^2, 20 von Karman screens + 3 subharmonic levels, AR a = 0.99, Gaussian beam; slice = 2 of
+    the 32 stacks x 3 of the 100 AR frames.  Per frame: every evolved screen, the received fields, the
+    beam statistics.  (The 100-step AR chain on one screen is test_gpu_screens.py::test_ar_chain_100_steps.)"""
     import torch
     from paper_2604_07248_b200 import api
     wl = synth.CONFIGS[3]
-    N, S, B = wl.N, wl.S, 1
+    N, S, B, T = wl.N, wl.S, 2, 3
     po, pg = _psd(wl, orc)
-    frames = synth.noise(3, 0, 0, S, N, wl.n_sh, frames=3)
-    hi0, sh0 = frames[0]
-    _, spec_ref, shc_ref = orc.make_screens(N, wl.dx, po, wl.lam, wl.cn2_list, wl.dz, wl.n_sh, hi0[None], sh0[None])
+    frames = [synth.noise(3, 0, b, S, N, wl.n_sh, frames=T + 1) for b in range(B)]          # [b][t] -> (hi, sh)
+    hi = lambda t: np.stack([frames[b][t][0] for b in range(B)])
+    sh = lambda t: np.stack([frames[b][t][1] for b in range(B)])
+    _, spec_ref, shc_ref = oracle_screens_parallel(orc, N, wl.dx, po, wl.lam, wl.cn2_list, wl.dz, wl.n_sh, hi(0), sh(0),
+                                                   keep_spectrum=True)
+    spec_ref, shc_ref = np.ascontiguousarray(spec_ref), np.ascontiguousarray(shc_ref)
     spec = torch.empty((B, S, N, N), dtype=torch.complex64, device="cuda")
     shc = torch.zeros((B, S, wl.n_sh, 3, 3), dtype=torch.complex64, device="cuda")
-    ssp.make_screens(N, wl.dx, pg, wl.lam, list(wl.cn2_list), list(wl.dz), wl.n_sh, cu(c64(hi0[None])), cu(c64(sh0[None])),
+    ssp.make_screens(N, wl.dx, pg, wl.lam, list(wl.cn2_list), list(wl.dz), wl.n_sh, cu(c64(hi(0))), cu(c64(sh(0))),
                      spectrum=spec, sh_coef=shc)
     u0 = synth.input_field(wl, B)
     kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
-    for t in (1, 2):
-        hi, sh = frames[t]
-        scr_ref = orc.evolve_screens(N, wl.dx, po, wl.lam, wl.cn2_list, wl.dz, wl.n_sh, wl.ar_a, 0, 0, 0, hi[None], sh[None],
-                                     spec_ref, shc_ref)
+    for t in range(1, T + 1):
+        h_t, s_t = hi(t), sh(t)
+
+        def evolve_one(bs):                                    # one (stack, screen) at a time: the AR state is per screen
+            b, j = divmod(bs, S)
+            sp, sc = np.ascontiguousarray(spec_ref[b:b + 1, j:j + 1]), np.ascontiguousarray(shc_ref[b:b + 1, j:j + 1])
+            out = orc.evolve_screens(N, wl.dx, po, wl.lam, [wl.cn2_list[j]], [wl.dz[j]], wl.n_sh, wl.ar_a, 0, 0, 0,
+                                     h_t[b:b + 1, j:j + 1], s_t[b:b + 1, j:j + 1], sp, sc)
+            return out[0, 0], sp[0, 0], sc[0, 0]
+        res = pmap(evolve_one, range(B * S))
+        scr_ref = np.stack([r[0] for r in res]).reshape(B, S, N, N)
+        spec_ref = np.stack([r[1] for r in res]).reshape(B, S, N, N)
+        shc_ref = np.stack([r[2] for r in res]).reshape(B, S, wl.n_sh, 3, 3)
         scr = ssp.evolve_screens(N, wl.dx, pg, wl.lam, list(wl.cn2_list), list(wl.dz), wl.n_sh, wl.ar_a, 0, 0, 0,
-                                 cu(c64(hi[None])), cu(c64(sh[None])), spec, shc)
-        err = rel_l2(scr.cpu().numpy(), scr_ref)
-        assert err.max() < tol(N, t + 1), (t, err)
-    scr32 = scr_ref.astype(np.float32)
-    ref = orc.propagate(N, wl.dx, wl.lam, wl.dz, u0, scr32, **kw)
-    stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
-    out = ssp.propagate(N, wl.dx, wl.lam, list(wl.dz), cu(u0), cu(scr32), stats=stats, roi_frac=0.25, **kw)
-    assert rel_l2(out.cpu().numpy(), ref).max() < tol(N, S)
-    _check_stats(api.stats_to_dicts(stats), orc.beam_stats(N, wl.dx, ref, roi_frac=0.25), wl)
+                                 cu(c64(h_t)), cu(c64(s_t)), spec, shc)
+        e_scr = rel_l2(scr.cpu().numpy(), scr_ref)
+        assert e_scr.max() < tol(N, t + 1), (t, e_scr)
+        scr32 = scr_ref.astype(np.float32)
+        ref = np.concatenate(pmap(lambda b: orc.propagate(N, wl.dx, wl.lam, wl.dz, u0[b:b + 1], scr32[b:b + 1], **kw), range(B)))
+        stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+        out = ssp.propagate(N, wl.dx, wl.lam, list(wl.dz), cu(u0), cu(scr32), stats=stats, roi_frac=0.25, **kw)
+        e_f = rel_l2(out.cpu().numpy(), ref)
+        assert e_f.max() < tol(N, S), (t, e_f)
+        record("config3", frame=t, B=B, S=S, screens=float(e_scr.max()), field=float(e_f.max()), bound=tol(N, S))
+        _check_stats(api.stats_to_dicts(stats), orc.beam_stats(N, wl.dx, ref, roi_frac=0.25), wl)
 
 
-def test_config4_forward_adjoint_masks_slice(ssp, orc):
-    """configs[3]: 2048^2, Kolmogorov Cn2 = 1e-13 screens at dz = L/30, Gaussian beam, two uniform-random phase
-    masks (receiver pupil, Fourier plane of a 2f system), Gaussian-overlap loss and its gradients w.r.t. both
-    masks and every screen via the adjoint split step.  Slice = 1 of 8 fields, the first 3 of the 30 screens."""
+def test_config4_forward_adjoint_masks_all_screens(ssp, orc):
+    """configs[3] at its own step count: 2048^2, all 30 Kolmogorov Cn2 = 1e-13 screens at dz = L/30, Gaussian beam, two
+    uniform-random phase masks (receiver pupil, Fourier plane of a 2f system), Gaussian-overlap loss and its gradients
+    w.r.t. both masks and every one of the 30 screens via the adjoint split step.  Slice = 1 of the 8 fields."""
     from tests import o9
     wl = synth.CONFIGS[4]
-    N, S, B = wl.N, 3, 1
+    N, S, B = wl.N, wl.S, 1
     po, pg = _psd(wl, orc)
-    dz, cn2 = wl.dz[:S], wl.cn2_list[:S]
+    dz, cn2 = wl.dz, wl.cn2_list
     hi, sh = synth.noise_batch(4, 0, B, S, N, 0)
-    scr_ref, _, _ = orc.make_screens(N, wl.dx, po, wl.lam, cn2, dz, 0, hi, sh, keep_spectrum=False)
+    scr_ref, _, _ = oracle_screens_parallel(orc, N, wl.dx, po, wl.lam, cn2, dz, 0, hi, sh)
     scr = ssp.make_screens(N, wl.dx, pg, wl.lam, list(cn2), list(dz), 0, cu(c64(hi)))
-    assert rel_l2(scr.cpu().numpy(), scr_ref).max() < tol(N, 1)
+    e_scr = rel_l2(scr.cpu().numpy(), scr_ref).max()
+    assert e_scr < tol(N, 1)
+    del hi, scr
     scr32 = scr_ref.astype(np.float32)
+    del scr_ref
     th = synth.phase_masks(0, N, 2)
     u0 = synth.input_field(wl, B)
     kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
-    ref = o9.oracle_chain(orc, N, wl.dx, wl.lam, dz, u0, scr32, th[0], th[1], kw)
+    ref = o9.oracle_chain(orc, N, wl.dx, wl.lam, dz, u0, scr32, th[0], th[1], kw, parallel=True)
     got = o9.gpu_chain(ssp, N, wl.dx, wl.lam, dz, u0, scr32, th[0], th[1], kw)
-    assert rel_l2(got["V5"].cpu().numpy(), ref["V5"]).max() < tol(N, S + 2)
+    e = dict(V5=rel_l2(got["V5"].cpu().numpy(), ref["V5"]).max(), G0=rel_l2(got["G0"].cpu().numpy(), ref["G0"]).max(),
+             g_th1=rel_l2(got["g_th1"].cpu().numpy(), ref["g_th1"]).max(),
+             g_th2=rel_l2(got["g_th2"].cpu().numpy(), ref["g_th2"]).max(),
+             g_phi=rel_l2(got["g_phi"].cpu().numpy(), ref["g_phi"]).max())
+    record("config4", B=B, S=S, screens=float(e_scr), loss_gpu=float(got["loss"][0]), loss_ref=float(ref["loss"][0]),
+           bound_fwd=tol(N, S + 2), bound_bwd=tol(N, 2 * S + 4), **{k: float(v) for k, v in e.items()})
+    assert e["V5"] < tol(N, S + 2), e
     assert abs(got["loss"][0] - ref["loss"][0]) < 1e-4 * max(ref["loss"][0], 1e-3), (got["loss"], ref["loss"])
-    assert rel_l2(got["G0"].cpu().numpy(), ref["G0"]).max() < tol(N, 2 * S + 4)
-    for k in ("g_th1", "g_th2"):
-        assert rel_l2(got[k].cpu().numpy(), ref[k]).max() < tol(N, 2 * S + 4), k
-    gerr = rel_l2(got["g_phi"].cpu().numpy(), ref["g_phi"])
-    assert gerr.max() < tol(N, 2 * S + 4), gerr
+    for k in ("G0", "g_th1", "g_th2", "g_phi"):
+        assert e[k] < tol(N, 2 * S + 4), (k, e)
 
 
-def test_config5_ocean_slice(ssp, orc):
-    """configs[4]: 4096^2, Nikishov oceanic spectrum with 4 subharmonic levels, Gaussian beam w0 = 5 mm,
-    dz = L/20; slice = 1 of 2 fields, the first 2 of the 20 screens.  Screens, received field, beam statistics."""
+def test_config5_ocean_all_screens(ssp, orc):
+    """configs[4] at its own step count: 4096^2, all 20 Nikishov oceanic screens with 4 subharmonic levels, Gaussian
+    beam w0 = 5 mm, dz = L/20.  Slice = 1 of the 2 fields.  Every screen, the received field, the beam statistics."""
     import torch
     from paper_2604_07248_b200 import api
     wl = synth.CONFIGS[5]
-    N, S, B = wl.N, 2, 1
+    N, S, B = wl.N, wl.S, 1
     po, pg = _psd(wl, orc)
-    dz, cn2 = wl.dz[:S], wl.cn2_list[:S]
+    dz, cn2 = wl.dz, wl.cn2_list
     hi, sh = synth.noise_batch(5, 0, B, S, N, wl.n_sh)
-    scr_ref, _, _ = orc.make_screens(N, wl.dx, po, wl.lam, cn2, dz, wl.n_sh, hi, sh, keep_spectrum=False)
-    scr = ssp.make_screens(N, wl.dx, pg, wl.lam, list(cn2), list(dz), wl.n_sh, cu(c64(hi)), cu(c64(sh)))
-    assert rel_l2(scr.cpu().numpy(), scr_ref).max() < tol(N, 1)
+    scr = ssp.make_screens(N, wl.dx, pg, wl.lam, list(cn2), list(dz), wl.n_sh, cu(c64(hi)), cu(c64(sh))).cpu().numpy()
+    scr_ref, _, _ = oracle_screens_parallel(orc, N, wl.dx, po, wl.lam, cn2, dz, wl.n_sh, hi, sh)
+    e_scr = rel_l2(scr, scr_ref)
+    assert e_scr.max() < tol(N, 1), e_scr
+    del hi, scr
     scr32 = scr_ref.astype(np.float32)
+    del scr_ref
     u0 = synth.input_field(wl, B)
     kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
-    ref = orc.propagate(N, wl.dx, wl.lam, dz, u0, scr32, **kw)
     stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
-    out = ssp.propagate(N, wl.dx, wl.lam, list(dz), cu(u0), cu(scr32), stats=stats, roi_frac=0.25, **kw)
-    assert rel_l2(out.cpu().numpy(), ref).max() < tol(N, S)
+    out = ssp.propagate(N, wl.dx, wl.lam, list(dz), cu(u0), cu(scr32), stats=stats, roi_frac=0.25, **kw).cpu().numpy()
+    ref = orc.propagate(N, wl.dx, wl.lam, dz, u0, scr32, **kw)
+    e_f = rel_l2(out, ref).max()
+    record("config5", B=B, S=S, screens=float(e_scr.max()), field=float(e_f), bound=tol(N, S))
+    assert e_f < tol(N, S)
     _check_stats(api.stats_to_dicts(stats), orc.beam_stats(N, wl.dx, ref, roi_frac=0.25), wl)
 
 

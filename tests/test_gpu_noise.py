@@ -83,9 +83,11 @@ def test_frame_host_equals_the_separate_calls(ssp, B, n_sh):
     d_noise, d_nsh = c64(Bc, S, N, N), c64(B, S, max(n_sh, 1), 3, 3)
     d_st = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device=dev)
     ws = ssp.workspace(N, dx, B, S)
+    h_adj, d_adj = torch.empty_like(u0).pin_memory(), c64(B, N, N)
     for frame in (0, 1):
+        adj = dict(h_adjoint_out=h_adj, d_adjoint=d_adj) if frame == 1 else {}      # frame 0: forward only
         ssp.frame_host(N, dx, psd, lam, cn2, dz, n_sh, 0.97, 3.0, -2.0, 1e-3, 77, frame, h_in, h_out, h_st, 0.5,
-                       d_field, spec, shc, scr, d_noise, d_nsh, d_st, ws, **kw)
+                       d_field, spec, shc, scr, d_noise, d_nsh, d_st, ws, **kw, **adj)
         ssp.fill_noise(77, 2 * frame, noise)
         if n_sh:
             ssp.fill_noise(77, 2 * frame + 1, nsh_c)
@@ -95,6 +97,9 @@ def test_frame_host_equals_the_separate_calls(ssp, B, n_sh):
         out_ref = ssp.propagate(N, dx, lam, dz, u0.cuda(), scr_ref, stats=st_ref, roi_frac=0.5, **kw)
         assert torch.equal(scr, scr_ref) and torch.equal(spec, spec2)
         assert torch.equal(h_out, out_ref.cpu())
+        if frame == 1:                                           # the adjoint leg: A^H of the received fields
+            g_ref = ssp.propagate_adjoint(N, dx, lam, dz, out_ref, scr_ref, **kw)
+            assert torch.equal(h_adj, g_ref.cpu())
         for a, b in zip(api.stats_to_dicts(h_st), api.stats_to_dicts(st_ref)):
             for k in ("power", "w2", "I_axis", "roi_sumI2"):
                 assert abs(a[k] / b[k] - 1) < 1e-12

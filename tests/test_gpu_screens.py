@@ -130,6 +130,43 @@ def test_evolve_screens_parity(ssp, orc):
     assert e.value.code == api.EWORKSPACE
 
 
+@pytest.mark.parametrize("N,n_sh,kind", [(512, 3, 1), (4096, 3, 1), (512, 2, 2)])
+def test_evolve_screens_wind_and_subharmonics_large_grids(ssp, orc, N, n_sh, kind):
+    """AR evolution with wind AND subharmonics against the oracle on the grids whose kernels round 1 never compared
+    under AR: 512 (k_screen_col_tma<512,.,AR,TILT>) and 4096 (register-load generator, (32,16,8) plan); fractional-pixel
+    wind with vx != vy; von Karman and (512) the oceanic filter.  One stack of one screen, two AR frames at 512, one at
+    4096 (the oracle needs about half a minute per 4096^2 screen)."""
+    import torch
+    from paper_2604_07248_b200 import api
+    from tests.util import record
+    dx, B, S = 1e-3, 1, 1
+    if kind == 1:
+        po, pg = orc.Psd(kind=1, L0=20.0, l0=4e-3), api.PsdParams(kind=1, L0=20.0, l0=4e-3)
+    else:
+        po = orc.Psd(kind=2, chi_T=1e-7, eps=1e-5, w=-2.0)
+        pg = api.PsdParams(kind=2, chi_T=1e-7, eps=1e-5, w=-2.0)
+    cn2, dz = [3e-14], [120.0]
+    frames = synth.noise(80 + N, kind, 0, S, N, n_sh, frames=3 if N <= 512 else 2)
+    hi0, sh0 = frames[0]
+    _, spec_ref, shc_ref = orc.make_screens(N, dx, po, LAM, cn2, dz, n_sh, hi0[None], sh0[None])
+    spec = torch.empty((B, S, N, N), dtype=torch.complex64, device="cuda")
+    shc = torch.zeros((B, S, n_sh, 3, 3), dtype=torch.complex64, device="cuda")
+    ssp.make_screens(N, dx, pg, LAM, cn2, dz, n_sh, cu(c64(hi0[None])), cu(c64(sh0[None])), spectrum=spec, sh_coef=shc)
+    a, T = 0.95, 0.02
+    vx, vy = 2.37 * dx / T, -0.61 * dx / T
+    for t in range(1, len(frames)):
+        hi, sh = frames[t]
+        ref = orc.evolve_screens(N, dx, po, LAM, cn2, dz, n_sh, a, vx, vy, T, hi[None], sh[None], spec_ref, shc_ref)
+        scr = ssp.evolve_screens(N, dx, pg, LAM, cn2, dz, n_sh, a, vx, vy, T, cu(c64(hi[None])), cu(c64(sh[None])), spec, shc)
+        err = rel_l2(scr.cpu().numpy(), ref).max()
+        record("evolve_wind_sh", N=N, kind=kind, frame=t, screens=float(err), bound=2e-5 * math.log2(N) * (t + 1))
+        assert err < 2e-5 * math.log2(N) * (t + 1), (t, err)
+        # the stored AR state too: spectrum and subharmonic coefficients
+        es = np.linalg.norm(spec.cpu().numpy() - spec_ref) / np.linalg.norm(spec_ref)
+        ec = np.linalg.norm(shc.cpu().numpy() - shc_ref) / np.linalg.norm(shc_ref)
+        assert es < 1e-6 * (t + 1) and ec < 1e-6 * (t + 1), (es, ec)
+
+
 def test_ar_chain_100_steps(ssp, orc):
     """Config-3 style AR chain on one screen: 100 steps at a = 0.99, GPU fp32 state vs oracle fp64 state."""
     import torch
