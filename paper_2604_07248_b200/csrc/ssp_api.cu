@@ -129,8 +129,10 @@ void fill_window(RowArgs &r, ssp_window win, int N)
 // On-chip path (ssp_small.cu): upload the step list and launch one kernel for the whole stack.
 const size_t kSmallStepBytes = 16384;
 
+struct SmallStats { ssp_stats *stats; int lo, hi; long long n; double dx; };
+
 int run_small(ssp_ctx *ctx, int N, int B, const std::vector<SmallStep> &steps, int n_screens, const RowArgs &win,
-              const float2 *in, float2 *out, const float2 *tw, const float2 *twc)
+              const float2 *in, float2 *out, const float2 *tw, const float2 *twc, const SmallStats *st = nullptr)
 {
     if (!ctx->small_steps) SSP_CUDA(ctx, cudaMalloc(&ctx->small_steps, kSmallStepBytes));
     // pageable source: staged before cudaMemcpyAsync returns, so the vector may die afterwards
@@ -143,6 +145,7 @@ int run_small(ssp_ctx *ctx, int N, int B, const std::vector<SmallStep> &steps, i
     a.steps = reinterpret_cast<const SmallStep *>(ctx->small_steps);
     a.win_on = win.win_on; a.win_qs = win.win_qs; a.win_half_order = win.win_half_order;
     a.tw_row = tw; a.tw_col = twc;
+    if (st && st->stats) { a.stats = st->stats; a.roi_lo = st->lo; a.roi_hi = st->hi; a.roi_n = st->n; a.dx = st->dx; }
     return launch_small(ctx, N, B, a);
 }
 
@@ -190,6 +193,10 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
     if (int rc = get_twiddles(ctx, N, 0, &tw)) return rc;
     if (int rc = get_twiddles(ctx, N, 1, &twc)) return rc;
     float2 *u = reinterpret_cast<float2 *>(d_field_out);
+    // K8 rides on the last row pass (the output pixels are in registers there): ROI bounds decided here, in double
+    int roi_lo = 0, roi_hi = 0;
+    long long roi_n = 0;
+    if (d_stats) stats_roi(N, roi_frac, &roi_lo, &roi_hi, &roi_n);
 
     if (small_ok(N, h_kind, n_steps, d_planes)) { // whole stack in one kernel, field resident in shared memory
         std::vector<SmallStep> ops(n_steps + 1);
@@ -203,11 +210,12 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
             if (j < n_steps) if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j], 0, 0}, &o.hx)) return rc;
             if (j >= 1) if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j - 1], 0, 1}, &o.hy)) return rc;
         }
-        if (int rc = run_small(ctx, N, B, ops, S, w, reinterpret_cast<const float2 *>(d_field_in), u, tw, twc)) return rc;
-        if (d_stats)
-            if (int rc = launch_stats(ctx, N, grid.dx, B, u, roi_frac, d_stats)) return rc;
-        return SSP_OK;
+        SmallStats st{d_stats, roi_lo, roi_hi, roi_n, grid.dx};
+        return run_small(ctx, N, B, ops, S, w, reinterpret_cast<const float2 *>(d_field_in), u, tw, twc, &st);
     }
+    const int bpf = row_stats_records(N);                     // records per field written by the last row kernel
+    if (d_stats)
+        if (int rc = ensure_scratch(ctx, sizeof(double) * 9 * (size_t)B * bpf)) return rc;
     // Fresnel: H = hx[kx] hy[ky], hx applied by the row kernels, hy by the column kernel.
     // Angular spectrum: H(ky,kx) is not separable; the column kernel applies the whole map, the rows none.
     const bool as = (h_kind == SSP_H_ANGULAR_SPECTRUM);
@@ -251,10 +259,14 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
             if (int rc = get_htable(ctx, HKey{N, grid.dx, lam_eff, dz[j], 0, 0}, &hx)) return rc;
             r.hx = hx;
         }
+        if (last && d_stats) {
+            r.stats_acc = reinterpret_cast<double *>(ctx->scratch);
+            r.roi_lo = roi_lo; r.roi_hi = roi_hi;
+        }
         if (int rc = launch_row(ctx, N, true, !last, r)) return rc;
     }
     if (d_stats)
-        if (int rc = launch_stats(ctx, N, grid.dx, B, u, roi_frac, d_stats)) return rc;
+        if (int rc = launch_stats_final(ctx, B, bpf, grid.dx, roi_n, reinterpret_cast<const double *>(ctx->scratch), d_stats)) return rc;
     return SSP_OK;
 }
 

@@ -54,8 +54,19 @@ template <int N>
 struct ColTmaTune { static constexpr int C = 4, NBUF = 2, MIN_BLOCKS = 3; static constexpr bool ENABLED = false; };
 template <> struct ColTmaTune<512> { static constexpr int C = 8, NBUF = 2, MIN_BLOCKS = 3; static constexpr bool ENABLED = true; };
 template <> struct ColTmaTune<1024> { static constexpr int C = 4, NBUF = 2, MIN_BLOCKS = 3; static constexpr bool ENABLED = true; };
-template <> struct ColTmaTune<2048> { static constexpr int C = 4, NBUF = 1, MIN_BLOCKS = 2; static constexpr bool ENABLED = true; };
-template <> struct ColTmaTune<4096> { static constexpr int C = 2, NBUF = 1, MIN_BLOCKS = 2; static constexpr bool ENABLED = true; };
+#ifndef SSP_T2048_C
+#define SSP_T2048_C 4
+#define SSP_T2048_NBUF 1
+#define SSP_T2048_MINB 2
+#endif
+#ifndef SSP_T4096_C
+#define SSP_T4096_C 2
+#define SSP_T4096_NBUF 1
+#define SSP_T4096_MINB 2
+#endif
+template <int C_, int NBUF_, int MINB_> struct ColTmaTuneV { static constexpr int C = C_, NBUF = NBUF_, MIN_BLOCKS = MINB_; static constexpr bool ENABLED = true; };
+template <> struct ColTmaTune<2048> : ColTmaTuneV<SSP_T2048_C, SSP_T2048_NBUF, SSP_T2048_MINB> {};
+template <> struct ColTmaTune<4096> : ColTmaTuneV<SSP_T4096_C, SSP_T4096_NBUF, SSP_T4096_MINB> {};
 
 template <int N>
 struct ColTmaCfg {

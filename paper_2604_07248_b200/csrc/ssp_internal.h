@@ -156,6 +156,10 @@ struct RowArgs {
     const float2 *pre_line;      // per-line factor pre_line[iy] multiplying the whole line, or null
     int in_swapped;              // the input holds (im, re) pairs: written by launch_col_prop when mid_swapped(N)
     const float2 *tw;
+    // statistics epilogue of the LAST row kernel (first && !second): partial sums of the nine accumulators of
+    // ssp_stats.cuh, stats_acc[field][row_stats_records(N)][ACC_N] (null: none); ROI = [roi_lo, roi_hi)^2
+    double *stats_acc;
+    int roi_lo, roi_hi;
 };
 
 struct ColArgs {
@@ -170,6 +174,8 @@ struct ColArgs {
 
 // first: inverse FFT_x before the pointwise stage; second: forward FFT_x after it.
 int launch_row(ssp_ctx *ctx, int N, bool first, bool second, const RowArgs &a);
+// records of the nine statistics accumulators that the last row kernel writes per field (RowArgs::stats_acc)
+int row_stats_records(int N);
 // column pass of the propagator: FFT_y -> * hy -> IFFT_y, in place allowed.
 int launch_col_prop(ssp_ctx *ctx, int N, const ColArgs &a);
 // true when launch_col_prop leaves its output re/im-swapped for the row kernel that follows (RowArgs::in_swapped)
@@ -194,6 +200,10 @@ struct SmallStep {               // one row pass, preceded (except op 0) by the 
 struct SmallArgs {
     const float2 *in;
     float2 *out;
+    ssp_stats *stats;            // optional: beam statistics of the output fields, finished inside the kernel
+    int roi_lo, roi_hi;
+    long long roi_n;
+    double dx;
     int n_steps;                 // column passes; row passes = n_steps + 1
     int n_screens;               // bookkeeping (algorithmic bytes)
     const SmallStep *steps;      // device [n_steps + 1]
@@ -255,6 +265,10 @@ int launch_sh_prep(ssp_ctx *ctx, int nscr, int S, int n_sh, const float2 *noise_
 // ---- misc (ssp_misc.cu) ------------------------------------------------------------
 int launch_stats(ssp_ctx *ctx, int N, double dx, int B, const float2 *field, double roi_frac,
                  ssp_stats *d_stats);
+// ROI bounds of the statistics: [lo, hi)^2 with h = floor(roi_frac N / 2) pixels each side of N/2 (h = 0: the pixel N/2)
+void stats_roi(int N, double roi_frac, int *lo, int *hi, long long *roi_n);
+// per-field finaliser over bpf per-CTA partial records acc[b][k][ACC_N] (ssp_stats.cuh)
+int launch_stats_final(ssp_ctx *ctx, int B, int bpf, double dx, long long roi_n, const double *acc, ssp_stats *d_stats);
 int launch_welford(ssp_ctx *ctx, int N, int B, const float2 *field, float *mean, float *M2,
                    long long count0);
 int launch_h2d_table(ssp_ctx *ctx, int N, int C, double dx, double lam_eff, double dz, int conj, float2 *out);

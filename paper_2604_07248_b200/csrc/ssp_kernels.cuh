@@ -18,6 +18,7 @@
 
 #include "ssp_internal.h"
 #include "ssp_lines.cuh"
+#include "ssp_stats.cuh"
 
 namespace ssp {
 
@@ -209,6 +210,21 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
         if constexpr (SECOND) fft_line<N, 0, true, false, false, PK>(v, t, sm, a.tw); // forward, reversed plan; strided by R1
     }
 
+    if constexpr (FIRST && !SECOND) {
+        // K8 fused into the last row kernel of a propagation (0 B/px): the output pixels are in registers.
+        // Row sums in fp32, promoted to double per row, reduced over the row's lanes by shuffles; every lane group (a row,
+        // or the part of a row inside one warp) writes ONE record of the nine accumulators, lanes 0..8 one moment each
+        // (a 72-byte store; no shared memory, no barrier).  k_stats_final adds a field's records in a fixed order.
+        if (a.stats_acc) {
+            constexpr int W = StatsGroup<N>::W;
+            double r[ROW_N];
+            row_point_sums<N, ROUT, E, T>(v, t, iy, a.roi_lo, a.roi_hi, r);
+            group_sum<W>(r);
+            const size_t rec = ((size_t)blockIdx.x * CFG::THREADS + tid) / W;
+            const double y = (double)(iy - N / 2);
+            for (int m = tid % W; m < ACC_N; m += W) a.stats_acc[rec * ACC_N + m] = row_to_acc(m, r, y);
+        }
+    }
     float2 *dst = a.out + line * N;
     if (a.hx) {
 #pragma unroll

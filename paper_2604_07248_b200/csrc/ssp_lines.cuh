@@ -66,6 +66,15 @@ struct MidSwapped {
 template <int N>
 struct WinMap { static constexpr bool value = RowCfg<N>::PACKED && N == 1024; };
 
+// Statistics epilogue of the last row kernel: lanes of one row inside a warp form a group that writes one record;
+// a field has N * T / W records.
+template <int N>
+struct StatsGroup {
+    static constexpr int T = PlanInfo<N, 0>::T;
+    static constexpr int W = T < 32 ? T : 32;
+    static constexpr int RECORDS_PER_FIELD = N * (T / W);
+};
+
 template <int N, int V_ = 1>
 struct ColCfg {
     static constexpr int V = V_;                                  // plan variant

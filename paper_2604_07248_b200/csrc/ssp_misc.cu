@@ -4,11 +4,9 @@
 // centre in pixel units: fp32 partial sums within a row, promoted to fp64 once per row, combined by
 // warp shuffles into one partial per block and moment (no atomics: bit-reproducible); a one-warp-per-field
 // finaliser adds the block partials in block order and turns them into ssp_stats.
-#include "ssp_internal.h"
+#include "ssp_stats.cuh"
 
 namespace ssp {
-
-enum { ACC_I = 0, ACC_X, ACC_Y, ACC_XX, ACC_YY, ACC_XY, ACC_RI, ACC_RI2, ACC_AXIS, ACC_N };
 
 __device__ __forceinline__ double warp_sum(double v)
 {
@@ -90,53 +88,63 @@ __global__ void __launch_bounds__(256) k_stats_accum(const float2 *__restrict__ 
     }
 }
 
-// one warp per field: lane i < ACC_N adds moment i over the field's blocks, lane 0 finishes
-__global__ void __launch_bounds__(32) k_stats_final(const double *__restrict__ acc, int bpf, double dx, long long roi_n,
-                                                     ssp_stats *__restrict__ out)
+// one CTA per field: the partial records acc[b][k][moment], k < bpf, are added in a fixed order (thread j takes the
+// records k = j mod 256 in ascending order, then a shuffle tree per warp, then the eight warp sums in order): no
+// atomics, bit-reproducible; thread 0 finishes
+__global__ void __launch_bounds__(256) k_stats_final(const double *__restrict__ acc, int bpf, double dx, long long roi_n,
+                                                      ssp_stats *__restrict__ out)
 {
-    const int b = blockIdx.x;
-    __shared__ double a[ACC_N];
-    if (threadIdx.x < ACC_N) {
-        double s = 0.0;
-        for (int k = 0; k < bpf; ++k) s += acc[((size_t)b * bpf + k) * ACC_N + threadIdx.x];
-        a[threadIdx.x] = s;
+    const int b = blockIdx.x, tid = threadIdx.x;
+    double a[ACC_N];
+#pragma unroll
+    for (int i = 0; i < ACC_N; ++i) a[i] = 0.0;
+    for (int k = tid; k < bpf; k += 256) {
+        const double *p = acc + ((size_t)b * bpf + k) * ACC_N;
+#pragma unroll
+        for (int i = 0; i < ACC_N; ++i) a[i] += p[i];
     }
-    __syncwarp();
-    if (threadIdx.x != 0) return;
-    ssp_stats s;
-    const double sI = a[ACC_I];
-    s.power = sI * dx * dx;
-    double cx = 0, cy = 0, sxx = 0, syy = 0, sxy = 0;
-    if (sI > 0) {
-        cx = a[ACC_X] / sI;
-        cy = a[ACC_Y] / sI;
-        sxx = a[ACC_XX] / sI - cx * cx;
-        syy = a[ACC_YY] / sI - cy * cy;
-        sxy = a[ACC_XY] / sI - cx * cy;
+    __shared__ double part[8][ACC_N];
+#pragma unroll
+    for (int i = 0; i < ACC_N; ++i) {
+        const double s = warp_sum(a[i]);
+        if ((tid & 31) == 0) part[tid >> 5][i] = s;
     }
-    s.cx = cx * dx;
-    s.cy = cy * dx;
-    s.sxx = sxx * dx * dx;
-    s.syy = syy * dx * dx;
-    s.sxy = sxy * dx * dx;
-    const double tr = s.sxx + s.syy;
-    s.w2 = sqrt(2.0 * (tr > 0 ? tr : 0.0));
-    s.I_axis = a[ACC_AXIS];
-    s.roi_sumI = a[ACC_RI];
-    s.roi_sumI2 = a[ACC_RI2];
-    s.roi_n = roi_n;
-    out[b] = s;
+    __syncthreads();
+    if (tid == 0) {
+        double t[ACC_N];
+        for (int i = 0; i < ACC_N; ++i) {
+            t[i] = 0.0;
+            for (int w = 0; w < 8; ++w) t[i] += part[w][i];
+        }
+        out[b] = finalize_stats(t, dx, roi_n);
+    }
 }
 
-int launch_stats(ssp_ctx *ctx, int N, double dx, int B, const float2 *field, double roi_frac,
-                 ssp_stats *d_stats)
+void stats_roi(int N, double roi_frac, int *lo_out, int *hi_out, long long *roi_n)
 {
     int h = (int)floor(roi_frac * N / 2.0);
     int lo = N / 2 - h, hi = N / 2 + h;
     if (h <= 0) { lo = N / 2; hi = N / 2 + 1; }
     if (lo < 0) lo = 0;
     if (hi > N) hi = N;
-    const long long roi_n = (long long)(hi - lo) * (hi - lo);
+    *lo_out = lo; *hi_out = hi;
+    *roi_n = (long long)(hi - lo) * (hi - lo);
+}
+
+int launch_stats_final(ssp_ctx *ctx, int B, int bpf, double dx, long long roi_n, const double *acc, ssp_stats *d_stats)
+{
+    k_stats_final<<<B, 256, 0, ctx->stream>>>(acc, bpf, dx, roi_n, d_stats);
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
+int launch_stats(ssp_ctx *ctx, int N, double dx, int B, const float2 *field, double roi_frac,
+                 ssp_stats *d_stats)
+{
+    int lo, hi;
+    long long roi_n;
+    stats_roi(N, roi_frac, &lo, &hi, &roi_n);
     int lane_shift = 0;
     while ((2 << lane_shift) <= N / 2 && lane_shift < 6) ++lane_shift;       // lanes = min(64, N/2)
     const int rows_per_pass = 256 >> lane_shift;
@@ -151,7 +159,7 @@ int launch_stats(ssp_ctx *ctx, int N, double dx, int B, const float2 *field, dou
     double *acc = reinterpret_cast<double *>(ctx->scratch);
     ctx->prof_begin("stats", 8.0 * (double)B * N * N);
     k_stats_accum<<<dim3(bpf, B), 256, 0, ctx->stream>>>(field, N, lane_shift, lo, hi, acc);
-    k_stats_final<<<B, 32, 0, ctx->stream>>>(acc, bpf, dx, roi_n, d_stats);
+    k_stats_final<<<B, 256, 0, ctx->stream>>>(acc, bpf, dx, roi_n, d_stats);
     ctx->prof_end();
     ctx->launches += 2;
     SSP_CUDA(ctx, cudaGetLastError());

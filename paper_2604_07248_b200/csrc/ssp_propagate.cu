@@ -47,6 +47,7 @@ static int launch_row_n(ssp_ctx *ctx, const RowArgs &a)
     constexpr bool MID = FIRST && MidSwapped<N>::value;
     if (a.in_swapped && !MID) return ctx->fail(SSP_EINVAL, "swapped row input for a kernel that does not take it");
     if (a.in_swapped && a.pre) return ctx->fail(SSP_EINVAL, "pre-multiply on a swapped row input");
+    if (a.stats_acc && !(FIRST && !SECOND)) return ctx->fail(SSP_EINVAL, "statistics epilogue on a row kernel that is not the last");
     const bool common = a.phi && a.win_on && !a.grad && !a.plane_out && !a.pre && (!MID || a.in_swapped) &&
                         ((a.win_map != nullptr) == WinMap<N>::value);
     if (common) return launch_row_x<N, FIRST, SECOND, false>(ctx, a);
@@ -76,6 +77,23 @@ static int launch_col_n(ssp_ctx *ctx, const ColArgs &a)
     return SSP_OK;
 }
 
+
+int row_stats_records(int N)
+{
+    switch (N) {
+    case 8: return StatsGroup<8>::RECORDS_PER_FIELD;
+    case 16: return StatsGroup<16>::RECORDS_PER_FIELD;
+    case 32: return StatsGroup<32>::RECORDS_PER_FIELD;
+    case 64: return StatsGroup<64>::RECORDS_PER_FIELD;
+    case 128: return StatsGroup<128>::RECORDS_PER_FIELD;
+    case 256: return StatsGroup<256>::RECORDS_PER_FIELD;
+    case 512: return StatsGroup<512>::RECORDS_PER_FIELD;
+    case 1024: return StatsGroup<1024>::RECORDS_PER_FIELD;
+    case 2048: return StatsGroup<2048>::RECORDS_PER_FIELD;
+    case 4096: return StatsGroup<4096>::RECORDS_PER_FIELD;
+    default: return 1;
+    }
+}
 
 int launch_row(ssp_ctx *ctx, int N, bool first, bool second, const RowArgs &a)
 {

@@ -11,6 +11,7 @@
 //   row(op 0);  for k = 1..n:  col(hy_k);  row(op k)
 //   row = [IFFT_x] -> * exp(+-i phi) W -> [FFT_x] -> * hx,   col = FFT_y -> * hy/N^2 -> IFFT_y.   (Eq.1)
 #include "ssp_kernels.cuh"
+#include "ssp_stats.cuh"
 
 namespace ssp {
 
@@ -126,6 +127,29 @@ __global__ void __launch_bounds__(SmallCfg<N>::THREADS, 1) k_small(const SmallAr
                 for (int i = 0; i < E / RL; ++i)
 #pragma unroll
                     for (int q = 0; q < RL; ++q) line[line_index<N, 0, RL>(t, i, q)] = v[i * RL + q];
+                if (a.stats && op == a.n_steps) {
+                    // K8 on the output pixels in registers (ssp_stats.cuh): row sums -> one record per row in shared
+                    // memory -> moment i summed over the rows in row order by thread i -> finished here, no extra launch
+                    static_assert(T <= 32, "a row's threads sit in one warp");
+                    __shared__ double part[N][ROW_N];
+                    __shared__ double accs[ACC_N];
+                    double rs[ROW_N];
+                    row_point_sums<N, RL, E, T>(v, t, row, a.roi_lo, a.roi_hi, rs);
+                    group_sum<T>(rs);
+                    if (t == 0) {
+#pragma unroll
+                        for (int i = 0; i < ROW_N; ++i) part[row][i] = rs[i];
+                    }
+                    __syncthreads();
+                    if (tid < ACC_N) {
+                        double sum = 0.0;
+#pragma unroll 1
+                        for (int r2 = 0; r2 < N; ++r2) sum += row_to_acc(tid, part[r2], (double)(r2 - N / 2));
+                        accs[tid] = sum;
+                    }
+                    __syncthreads();
+                    if (tid == 0) a.stats[b] = finalize_stats(accs, a.dx, a.roi_n);
+                }
             }
             __syncthreads();
         }

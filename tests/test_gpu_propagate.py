@@ -288,6 +288,43 @@ def test_beam_stats_small_grids(ssp, orc, N):
             assert abs(a[k] / r[k] - 1) < 1e-4, (k, a[k], r[k])
 
 
+@pytest.mark.parametrize("N", [8, 16, 32, 64, 128, 256, 512, 1024, 2048, 4096])
+def test_statistics_epilogue_of_the_last_row_kernel(ssp, orc, N):
+    """K8 rides on the last row pass (fused, 0 B/px): ssp_propagate(..., d_stats) launches no stand-alone
+    reducer -- one finaliser launch on top of the propagation (none on the on-chip path) -- and the records equal those
+    of ssp_beam_stats on the returned field (same pixels, different summation order: 1e-6) and the oracle's (1e-4).
+    Odd batch, per-field screens, trailing vacuum step, and the planes-saving generic kernel as well."""
+    import torch
+    from paper_2604_07248_b200 import api
+    B, n_steps, S = (3, 3, 2) if N <= 1024 else (1, 2, 2)
+    dx, lam, dz, u0, scr = _case(N, B, n_steps, S, 5000 + N)
+    u0 = (u0 + 3.0 * synth.gaussian_beam(N, dx, 0.15 * N * dx, B)).astype(np.complex64)   # a beam over noise: nontrivial moments
+    kw = dict(win_order=16, win_sigma_frac=0.47)
+    ref = orc.propagate(N, dx, lam, dz, u0, scr, **kw) if N <= 1024 else None
+    ssp.propagate(N, dx, lam, list(dz), cu(u0), cu(scr), **kw)          # first use builds cached tables (window map)
+    for roi, with_planes in ((0.25, False), (0.0, False), (1.0, True)):
+        stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+        planes = torch.empty((B, n_steps, N, N), dtype=torch.complex64, device="cuda") if with_planes else None
+        l0 = ssp.launch_count()
+        out = ssp.propagate(N, dx, lam, list(dz), cu(u0), cu(scr), stats=stats, roi_frac=roi, planes=planes, **kw)
+        n_launch = ssp.launch_count() - l0
+        on_chip = N in (64, 128) and not with_planes
+        assert n_launch == (1 if on_chip else 2 * n_steps + 1 + 1), n_launch
+        got = api.stats_to_dicts(stats)
+        alone, _ = ssp.beam_stats(N, dx, out, roi_frac=roi)
+        for a, r in zip(got, api.stats_to_dicts(alone)):
+            for k in ("power", "w2", "sxx", "syy", "I_axis", "roi_sumI", "roi_sumI2"):
+                assert abs(a[k] / r[k] - 1) < 1e-6, (roi, k, a[k], r[k])
+            assert abs(a["cx"] - r["cx"]) < 1e-7 * dx * N and abs(a["cy"] - r["cy"]) < 1e-7 * dx * N
+            assert abs(a["sxy"] - r["sxy"]) < 1e-6 * (r["sxx"] + r["syy"])
+            assert a["roi_n"] == r["roi_n"]
+        if ref is not None:
+            for a, r in zip(got, orc.beam_stats(N, dx, ref, roi_frac=roi)):
+                for k in ("power", "w2", "I_axis", "roi_sumI", "roi_sumI2"):
+                    assert abs(a[k] / r[k] - 1) < 1e-4, (roi, k, a[k], r[k])
+                assert a["roi_n"] == r["roi_n"]
+
+
 def test_transfer_table_cache_overflow_keeps_pointers_valid(ssp, orc):
     """The context caches one 1-D transfer-function table per distinct (N, dx, lambda, dz, conj, scaled) and drops the
     cache beyond 4096 entries -- at the entry of a call only, never between the look-ups of one call (round 1 freed
