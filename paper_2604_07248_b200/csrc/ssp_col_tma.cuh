@@ -78,10 +78,16 @@ struct ColTmaCfg {
     static constexpr int BOX_ROWS = (N < 256) ? N : 256;              // TMA box dimensions are <= 256
     static constexpr int BOXES = N / BOX_ROWS;
     static constexpr int BUF_ELEMS = C * PlanInfo<N, 1>::LINE_ELEMS;  // float2 per buffer (padded exchange)
-    static constexpr size_t SMEM = NBUF * sizeof(float2) * BUF_ELEMS + 16;
+    static constexpr size_t SMEM = NBUF * sizeof(float2) * BUF_ELEMS + 32;   // + two mbarriers + the TMEM address slot
     static constexpr unsigned TILE_BYTES = (unsigned)(sizeof(float2) * C * N);
     // packed fp32 pairs: measured 2048 +3.6 %, 4096 +1.3 %; 1024 -1 % and 512 +1 % (within noise) stay scalar
     static constexpr bool PACKED = (N >= 2048);
+    // first-stage twiddles and the hy table kept per thread in tensor memory (128 columns per CTA): persistent CTAs only
+#ifndef SSP_COL1024_TMEM
+#define SSP_COL1024_TMEM 1
+#endif
+    static constexpr bool TMEM = (N == 1024) && SSP_COL1024_TMEM && NBUF == 2 && PlanInfo<N, 1>::NSTAGE == 2 && PlanInfo<N, 1>::SYM;
+    static constexpr int TMEM_COLS = 128;                             // 64: twiddle pairs, 64: hy of this thread's 32 points
 };
 
 // Screen generator (K1+K2): one tile per CTA, one buffer (noise -> exchange -> result) plus a second one only
@@ -142,7 +148,30 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
         fence_mbar_init();
         if ((int)blockIdx.x < a.ntiles) issue_load(blockIdx.x, 0);
     }
+    // Tensor memory as a per-thread constant cache: this thread's 16 twiddle pairs W_N^(t k) and the 32 hy values of
+    // its points never change while the CTA walks its tiles, so they are read from the thread's own TMEM lane
+    // (tcgen05.ld) instead of through the LSU data pipe, which this kernel saturates first.
+    constexpr bool TM = CFG::TMEM && !H2D;
+    unsigned &tmem_slot = *reinterpret_cast<unsigned *>(full + 2);     // (a static __shared__ would shift the TMA buffers)
+    unsigned taddr = 0;
+    if constexpr (TM) {
+        if (tid < 32) tmem_alloc(&tmem_slot, CFG::TMEM_COLS);
+        tmem_fence_before_sync();
+    }
     __syncthreads();
+    if constexpr (TM) {
+        tmem_fence_after_sync();
+        taddr = tmem_slot + ((unsigned)(tid & ~31) << 16);            // lanes 32 w .. 32 w + 31 belong to warp w
+        const float4 *tw4 = reinterpret_cast<const float4 *>(a.tw + PI::TW1) + t;
+#pragma unroll
+        for (int p = 0; p < R1 / 2; ++p) tmem_st4(taddr + 4 * p, __ldg(tw4 + p * (N / R1)));
+#pragma unroll
+        for (int q = 0; q < RL; q += 2) {
+            const float2 h0 = __ldg(a.hy + line_index<N, 1, RL>(t, 0, q)), h1 = __ldg(a.hy + line_index<N, 1, RL>(t, 0, q + 1));
+            tmem_st4(taddr + 64 + 2 * q, make_float4(h0.x, h0.y, h1.x, h1.y));
+        }
+        tmem_wait_st();
+    }
 
     int it = 0;
     for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x, ++it) {
@@ -167,8 +196,23 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
             // pass 0: forward; * hy, leaving the product re/im-swapped; pass 1: forward on swapped data = inverse
 #pragma unroll 1
             for (int pass = 0; pass < 2; ++pass) {
-                fft_line<N, 1, false, false, true, PK>(v, t, sm, a.tw);
+                if constexpr (TM) fft_line<N, 1, false, false, true, PK>(v, t, sm, TwTmem{a.tw, taddr});
+                else fft_line<N, 1, false, false, true, PK>(v, t, sm, a.tw);
                 if (pass == 0) {
+                    if constexpr (TM) {
+#pragma unroll
+                        for (int q = 0; q < RL; q += 4) {
+                            float4 ha, hb;
+                            tmem_ld8(taddr + 64 + 2 * q, ha, hb);
+                            const float2 h[4] = {make_float2(ha.x, ha.y), make_float2(ha.z, ha.w), make_float2(hb.x, hb.y),
+                                                 make_float2(hb.z, hb.w)};
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) {
+                                const float2 x = v[q + e];
+                                v[q + e] = make_float2(fmaf(x.x, h[e].y, x.y * h[e].x), fmaf(x.x, h[e].x, -x.y * h[e].y));
+                            }
+                        }
+                    } else {
 #pragma unroll
                     for (int i = 0; i < E / RL; ++i)
 #pragma unroll
@@ -176,6 +220,7 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
                             const float2 h = __ldg(hcol + (size_t)line_index<N, 1, RL>(t, i, q) * HS), x = v[i * RL + q];
                             v[i * RL + q] = make_float2(fmaf(x.x, h.y, x.y * h.x), fmaf(x.x, h.x, -x.y * h.y));
                         }
+                    }
                 }
             }
 #pragma unroll
@@ -209,6 +254,11 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
         }
     }
     if (tid == 0) tma_store_wait_read();
+    if constexpr (TM) {
+        tmem_fence_before_sync();
+        __syncthreads();
+        if (tid < 32) tmem_dealloc(tmem_slot, CFG::TMEM_COLS);
+    }
 }
 
 } // namespace ssp

@@ -238,6 +238,43 @@ __device__ __forceinline__ int fft_logical_t(int t_phys)
     } else return t_phys;
 }
 
+// ---- where the first-stage twiddles come from ------------------------------------------------------------------
+// TwGlobal: the table in global memory (read-only path, L1-resident).  TwTmem: a per-thread copy in tensor memory
+// (tcgen05.ld from the thread's own TMEM lane): for persistent kernels whose twiddles depend on the thread only, it
+// takes 16 B per point and transform off the LSU data pipe, the unit these kernels saturate first.
+struct TwGlobal {
+    const float2 *tw;
+    __device__ __forceinline__ const float2 *table() const { return tw; }
+};
+__device__ __forceinline__ float4 tmem_ld4(unsigned taddr)
+{
+    unsigned a, b, c, d;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];\n\ttcgen05.wait::ld.sync.aligned;"
+                 : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"(taddr) : "memory");
+    return make_float4(__uint_as_float(a), __uint_as_float(b), __uint_as_float(c), __uint_as_float(d));
+}
+__device__ __forceinline__ void tmem_ld8(unsigned taddr, float4 &x, float4 &y)
+{
+    unsigned r[8];
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];\n\ttcgen05.wait::ld.sync.aligned;"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr) : "memory");
+    x = make_float4(__uint_as_float(r[0]), __uint_as_float(r[1]), __uint_as_float(r[2]), __uint_as_float(r[3]));
+    y = make_float4(__uint_as_float(r[4]), __uint_as_float(r[5]), __uint_as_float(r[6]), __uint_as_float(r[7]));
+}
+__device__ __forceinline__ void tmem_st4(unsigned taddr, float4 v)
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
+                 :: "r"(taddr), "r"(__float_as_uint(v.x)), "r"(__float_as_uint(v.y)), "r"(__float_as_uint(v.z)),
+                    "r"(__float_as_uint(v.w)) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+struct TwTmem {
+    const float2 *tw;      // the global table (for the parts a plan does not keep in TMEM)
+    unsigned taddr;        // this warp's TMEM address of column 0 of the twiddle block: columns 4 p .. 4 p + 3 = twiddles of k = 2p, 2p+1
+    __device__ __forceinline__ const float2 *table() const { return tw; }
+};
+
 // One complete transform of a line held in registers.
 //   DIR_REV = false: plan (R1,R2,R3): input strided by R1, output strided by RL.
 //   DIR_REV = true : plan (RL,..,R1): input strided by RL, output strided by R1.
@@ -250,6 +287,14 @@ __device__ __forceinline__ int fft_logical_t(int t_phys)
 template <int N, int V, bool DIR_REV, bool INV, bool TAIL_SYNC = false, bool PK = false, class SM>
 __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 *__restrict__ tw)
 {
+    fft_line<N, V, DIR_REV, INV, TAIL_SYNC, PK>(v, t, sm, TwGlobal{tw});
+}
+
+template <int N, int V, bool DIR_REV, bool INV, bool TAIL_SYNC = false, bool PK = false, class SM, class TWP>
+__device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const TWP twp)
+{
+    const float2 *__restrict__ tw = twp.table();
+    constexpr bool TW_TMEM = std::is_same<TWP, TwTmem>::value;
     using PI = PlanInfo<N, V>;
     constexpr int E = PI::E, T = PI::T, NS = PI::NSTAGE;
     constexpr int Ra = DIR_REV ? PI::RL : PI::R1;                        // first radix
@@ -308,7 +353,11 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 
             const float4 *tw4 = reinterpret_cast<const float4 *>(tw1) + m;
 #pragma unroll
             for (int k = 0; k < Ra; k += 2) {
-                const float4 w = __ldg(tw4 + (k / 2) * M1);       // twiddles of k and k + 1
+                float4 w;                                         // twiddles of k and k + 1
+                if constexpr (TW_TMEM) {
+                    static_assert(!TW_TMEM || (E == Ra && !DIR_REV), "TMEM twiddles: one first-stage butterfly per thread");
+                    w = tmem_ld4(twp.taddr + 2 * k);
+                } else w = __ldg(tw4 + (k / 2) * M1);
                 float2 x0 = v[i * Ra + k], x1 = v[i * Ra + k + 1];
                 if (k > 0) x0 = cmul_c<INV, PK>(x0, make_float2(w.x, w.y));
                 x1 = cmul_c<INV, PK>(x1, make_float2(w.z, w.w));

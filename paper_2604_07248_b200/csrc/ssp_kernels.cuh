@@ -25,6 +25,9 @@ namespace ssp {
 template <bool SWAP>
 __device__ __forceinline__ float2 swap_if(float2 x) { return SWAP ? make_float2(x.y, x.x) : x; }
 
+template <int N>
+struct SYM_PLAN { static constexpr bool value = PlanInfo<N, 0>::SYM && PlanInfo<N, 0>::NSTAGE == 2 && PlanInfo<N, 0>::E == PlanInfo<N, 0>::R1; };
+
 // Pointwise stage in real space on a line held in the layout strided by RL.  SWAPPED: the registers
 // hold the field re/im-swapped (it came out of an inverse transform run by the forward code); the
 // result is in plain form either way.  GENERIC = false is the common split step (screen and window
@@ -127,9 +130,35 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
 
     const int tid = threadIdx.x;
     const int lib = tid / T, t = fft_logical_t<N, 0, 1>(tid % T);
-    const long long line = (long long)blockIdx.x * CFG::LPB + lib;
-    const int b = (int)(line / N), iy = (int)(line % N);
     RowSmem<T, CFG::WIDE> sm{smem + (size_t)lib * CFG::LINE_ELEMS, 1 + lib};
+    // Persistent form (RowCfg<N>::TMEM): the CTA walks row blocks blk = blockIdx.x, + gridDim.x, ..; this thread's 16
+    // twiddle pairs W_N^(t k) and the 32 hx values of its output points do not change from row to row and are read
+    // from the thread's own tensor-memory lane (tcgen05.ld) instead of through the LSU data pipe.
+    constexpr bool TM = RowCfg<N>::TMEM && FIRST && SECOND && !GENERIC;
+    unsigned taddr = 0;
+    if constexpr (TM) {
+        static_assert(!TM || (CFG::THREADS == 128 && T == 32 && SYM_PLAN<N>::value), "one warp per row, four rows per CTA");
+        unsigned *slot = reinterpret_cast<unsigned *>(smem_raw + CFG::SMEM);
+        if (tid < 32) tmem_alloc(slot, 128);
+        tmem_fence_before_sync();
+        __syncthreads();
+        tmem_fence_after_sync();
+        taddr = *slot + ((unsigned)(tid & ~31) << 16);
+        const float4 *tw4 = reinterpret_cast<const float4 *>(a.tw + PI::TW1) + t;
+#pragma unroll
+        for (int p = 0; p < PI::R1 / 2; ++p) tmem_st4(taddr + 4 * p, __ldg(tw4 + p * (N / PI::R1)));
+#pragma unroll
+        for (int q = 0; q < PI::R1; q += 2) {
+            const float2 h0 = __ldg(a.hx + line_index<N, 0, PI::R1>(t, 0, q)), h1 = __ldg(a.hx + line_index<N, 0, PI::R1>(t, 0, q + 1));
+            tmem_st4(taddr + 64 + 2 * q, make_float4(h0.x, h0.y, h1.x, h1.y));
+        }
+        tmem_wait_st();
+    }
+    const long long nblk = TM ? (long long)(a.n_lines / CFG::LPB) : (long long)blockIdx.x + 1;
+    for (long long blk = blockIdx.x; blk < nblk; blk += gridDim.x) {
+    const long long line = blk * CFG::LPB + lib;
+    const int b = (int)(line / N), iy = (int)(line % N);
+    if constexpr (TM) sm.sync();                                  // the previous row's last reads of the exchange / screen buffers
 
     // the screen row is streamed from HBM: fetch it asynchronously now, use it after the first transform
     float *phis = reinterpret_cast<float *>(smem_raw + CFG::SMEM_X) + (size_t)lib * N;
@@ -183,7 +212,8 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
                 // the exchange buffer is reused by the next pass: a row spanning several warps synchronises
                 // right after its last exchange read (TAIL), a warp-local row after the pointwise stage
                 constexpr bool TAIL = (T > 32);
-                fft_line<N, 0, false, false, TAIL, PK>(v, t, sm, a.tw);
+                if constexpr (TM) fft_line<N, 0, false, false, TAIL, PK>(v, t, sm, TwTmem{a.tw, taddr});
+                else fft_line<N, 0, false, false, TAIL, PK>(v, t, sm, a.tw);
                 if (pass == 0) {
                     wait_phi();
                     row_pointwise<N, RL, E, T, GENERIC, true, PK>(v, a, phis, t, b, iy);
@@ -220,13 +250,22 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
             double r[ROW_N];
             row_point_sums<N, ROUT, E, T>(v, t, iy, a.roi_lo, a.roi_hi, r);
             group_sum<W>(r);
-            const size_t rec = ((size_t)blockIdx.x * CFG::THREADS + tid) / W;
+            const size_t rec = ((size_t)blk * CFG::THREADS + tid) / W;
             const double y = (double)(iy - N / 2);
             for (int m = tid % W; m < ACC_N; m += W) a.stats_acc[rec * ACC_N + m] = row_to_acc(m, r, y);
         }
     }
     float2 *dst = a.out + line * N;
-    if (a.hx) {
+    if constexpr (TM) {
+#pragma unroll
+        for (int q = 0; q < ROUT; q += 4) {
+            float4 ha, hb;
+            tmem_ld8(taddr + 64 + 2 * q, ha, hb);
+            const float2 h[4] = {make_float2(ha.x, ha.y), make_float2(ha.z, ha.w), make_float2(hb.x, hb.y), make_float2(hb.z, hb.w)};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) dst[line_index<N, 0, ROUT>(t, 0, q + e)] = cmul_c<false, PK>(v[q + e], h[e]);
+        }
+    } else if (a.hx) {
 #pragma unroll
         for (int i = 0; i < E / ROUT; ++i)
 #pragma unroll
@@ -239,6 +278,12 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
         for (int i = 0; i < E / ROUT; ++i)
 #pragma unroll
             for (int q = 0; q < ROUT; ++q) dst[line_index<N, 0, ROUT>(t, i, q)] = v[i * ROUT + q];
+    }
+    }   // row blocks
+    if constexpr (TM) {
+        tmem_fence_before_sync();
+        __syncthreads();
+        if (tid < 32) tmem_dealloc(*reinterpret_cast<unsigned *>(smem_raw + CFG::SMEM), 128);
     }
 }
 

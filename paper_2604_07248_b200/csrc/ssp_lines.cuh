@@ -49,6 +49,11 @@ struct RowCfg {
     static constexpr int MIN_BLOCKS = (THREADS < RowTune<N>::MAX_THREADS) ? 1 : RowTune<N>::MIN_BLOCKS;
     // packed fp32 pairs in the split-step row kernel: measured 1024 +4 %, 2048 +2 %, 4096 +4 %; 512 (shuffle plan, one warp per row at 16 points per thread) -20 %
     static constexpr bool PACKED = (N >= 1024);
+    // persistent common split-step kernel with the twiddles and hx per thread in tensor memory (+ 16 bytes for the TMEM slot)
+#ifndef SSP_ROW1024_TMEM
+#define SSP_ROW1024_TMEM 1
+#endif
+    static constexpr bool TMEM = (N == 1024) && SSP_ROW1024_TMEM;
 };
 
 // Between the column kernel and the row kernel of a split step the field may stay re/im-swapped: the column
@@ -121,6 +126,19 @@ struct ColSmem {
     __device__ __forceinline__ float2 ld(int p) const { return base[p * C]; }
     __device__ __forceinline__ void sync() { __syncthreads(); }
 };
+
+// ---- tensor-memory allocation (tcgen05.alloc / dealloc; one warp, address through shared memory) ----------------
+__device__ __forceinline__ void tmem_alloc(unsigned *smem_slot, int cols_pow2)
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(smem_slot)), "r"(cols_pow2) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(unsigned taddr, int cols_pow2)
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols_pow2) : "memory");
+}
+__device__ __forceinline__ void tmem_fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
 // ---- asynchronous global -> shared copies (LDGSTS), 16 bytes each
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gmem_src)

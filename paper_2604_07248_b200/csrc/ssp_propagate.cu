@@ -28,11 +28,18 @@ static int launch_row_x(ssp_ctx *ctx, const RowArgs &a)
     using CFG = RowCfg<N>;
     if (a.n_lines % CFG::LPB) return ctx->fail(SSP_EINVAL, "row launch: %d lines not a multiple of %d", a.n_lines, CFG::LPB);
     auto kern = k_row<N, FIRST, SECOND, GENERIC>;
-    if (int rc = set_smem(ctx, kern, CFG::SMEM)) return rc;
+    if (int rc = set_smem(ctx, kern, CFG::SMEM + 16)) return rc;
     // algorithmic bytes: field in + out, + the screen, + saved / read planes and the gradient
     const double bpp = 16.0 + (a.phi ? 4.0 : 0.0) + (a.plane_out ? 8.0 : 0.0) + (a.grad ? 12.0 : 0.0);
     ctx->prof_begin(FIRST ? (SECOND ? "row_ifft_pw_fft" : "row_ifft_pw") : "row_pw_fft", bpp * (double)a.n_lines * N);
-    kern<<<a.n_lines / CFG::LPB, CFG::THREADS, CFG::SMEM, ctx->stream>>>(a);
+    constexpr bool TM = CFG::TMEM && FIRST && SECOND && !GENERIC;           // persistent form (ssp_kernels.cuh)
+    int grid = a.n_lines / CFG::LPB;
+    if (TM) {
+        if (!a.hx) return ctx->fail(SSP_EINVAL, "persistent row kernel without hx");
+        const int resident = ctx->num_sms * CFG::MIN_BLOCKS;
+        if (grid > resident) grid = resident;
+    }
+    kern<<<grid, CFG::THREADS, CFG::SMEM + (TM ? 16 : 0), ctx->stream>>>(a);
     ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
@@ -48,8 +55,11 @@ static int launch_row_n(ssp_ctx *ctx, const RowArgs &a)
     if (a.in_swapped && !MID) return ctx->fail(SSP_EINVAL, "swapped row input for a kernel that does not take it");
     if (a.in_swapped && a.pre) return ctx->fail(SSP_EINVAL, "pre-multiply on a swapped row input");
     if (a.stats_acc && !(FIRST && !SECOND)) return ctx->fail(SSP_EINVAL, "statistics epilogue on a row kernel that is not the last");
+    // (the persistent tensor-memory form of the common kernel caches hx per thread: without hx -- angular spectrum --
+    // the generic kernel runs)
     const bool common = a.phi && a.win_on && !a.grad && !a.plane_out && !a.pre && (!MID || a.in_swapped) &&
-                        ((a.win_map != nullptr) == WinMap<N>::value);
+                        ((a.win_map != nullptr) == WinMap<N>::value) &&
+                        (!(RowCfg<N>::TMEM && FIRST && SECOND) || a.hx);
     if (common) return launch_row_x<N, FIRST, SECOND, false>(ctx, a);
     return launch_row_x<N, FIRST, SECOND, true>(ctx, a);
 }
