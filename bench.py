@@ -348,6 +348,37 @@ def run_ours(args):
                   "GBps": ss_gbps, "frac_of_peak": ss_gbps / peak if ss_ms else None,
                   "frac_of_nominal": ss_gbps / NOMINAL if ss_ms else None}
 
+    # ---- forward-only temporal frame (the screens are used once): ssp_evolve_screens + ssp_propagate against
+    # ssp_evolve_propagate, which synthesises each screen row inside the split step's row kernel (N = 1024)
+    fwd_frame = None
+    if N == 1024 and args.h_kind == "fresnel":
+        ycol = torch.empty((B, S, N, N), dtype=torch.complex64, device=dev)
+        def frame_unfused(i):
+            ctx.evolve_screens(N, wl.dx, psd, wl.lam, cn2, dz, n_sh, a, 0.0, 0.0, 0.0, noise[i & 1],
+                               noise_sh[i & 1] if n_sh else None, spectrum, sh_coef if n_sh else None, screens=screens, ws=ws)
+            ctx.propagate(N, wl.dx, wl.lam, dz, u0, screens, out=out, stats=stats, **kw)
+        def frame_fused(i):
+            ctx.evolve_propagate(N, wl.dx, psd, wl.lam, cn2, dz, n_sh, a, 0.0, 0.0, 0.0, noise[i & 1],
+                                 noise_sh[i & 1] if n_sh else None, spectrum, sh_coef if n_sh else None, u0, ycol,
+                                 win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac, out=out, stats=stats, ws=ws)
+        def time_frames(fn, n):
+            fn(0); fn(1)
+            sync_all()
+            f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            f0.record()
+            for i in range(n):
+                fn(i)
+            f1.record()
+            sync_all()
+            return f0.elapsed_time(f1) / n
+        n_ff = max(2, min(args.steps, 10))
+        ms_u, ms_f = time_frames(frame_unfused, n_ff), time_frames(frame_fused, n_ff)
+        fwd_frame = {"what": "forward-only frame, device resident: evolve_screens + propagate + stats (unfused) against "
+                             "ssp_evolve_propagate (screen row pass fused into the split step's row kernel)",
+                     "unfused_ms": ms_u, "fused_ms": ms_f, "fused_screen_steps_per_s": B * S * world / (ms_f * 1e-3),
+                     "unfused_screen_steps_per_s": B * S * world / (ms_u * 1e-3), "speedup": ms_u / ms_f}
+        del ycol
+
     # ---- e2e: through ssp_frame_host with pinned HOST buffers.  Per step: the input fields go host -> device, the
     # screen stacks are evolved ON the device from (seed, stream) noise draws (the paper's pipeline draws its noise on
     # the GPU too), the fields propagate, output fields and statistics come back; chunks of the batch overlap.
@@ -464,7 +495,7 @@ def run_ours(args):
                        "units_per_step": units_step,
                        "l2": "inputs larger than L2 (no flush): each step streams > 10 GB"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches) * world, "roofline": roof,
-            "cpu_baseline": cpu, "kernels": kernels, "split_step": split_step, "cufft_comparison": cufft,
+            "cpu_baseline": cpu, "kernels": kernels, "split_step": split_step, "forward_frame": fwd_frame, "cufft_comparison": cufft,
         }
         print(json.dumps(line))
     ctx.close()

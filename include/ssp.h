@@ -273,6 +273,23 @@ int ssp_propagate_host(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, in
                        float *d_field, float *d_screens, ssp_stats *d_stats,
                        void *d_ws, size_t ws_bytes);
 
+/* Forward-only temporal frame on the device with the screen synthesis fused into the propagation (
+ * the workload of PAPER.md:76-84 when the screens are used once).  Equivalent to ssp_evolve_screens followed by
+ * ssp_propagate with n_steps = S and step j = slab dz[j] -- the AR state d_spectrum / d_sh_coef advances the same way,
+ * d_field_out and d_stats are the same up to fp32 rounding -- but the evolved screens are never written: the generator
+ * stops after its column pass, keeps every screen's column-transformed spectrum in d_ycol (dev c64 [B][S][N][N],
+ * scratch), and the split step's row kernel synthesises row iy of screen j itself (IFFT_x, real part, subharmonics,
+ * analytic mean; PAPER.md:57 Eq.2, :63 Eq.3, :362) right before it applies it: 8 B/px read there instead of the
+ * 12 B/px row pass plus a 4 B/px read.  Built for N = 1024 (SSP_EUNSUPPORTED otherwise), Fresnel H, window on.
+ * d_ws >= ssp_workspace_bytes(grid, B, S).  Enqueued on the context's stream. */
+int ssp_evolve_propagate(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, double n0,
+                         int B, int S, const double *cn2, const double *dz, int n_sh,
+                         double a, double vx, double vy, double T,
+                         const float *d_fresh_noise, const float *d_fresh_noise_sh,
+                         float *d_spectrum, float *d_sh_coef,
+                         ssp_window win, const float *d_field_in, float *d_field_out,
+                         ssp_stats *d_stats, double roi_frac, float *d_ycol, void *d_ws, size_t ws_bytes);
+
 /* One temporal frame end to end from HOST fields (the workload of PAPER.md:76-84: every frame the screens evolve
  * by the autoregression of Eq. 5 and a batch of fields propagates through them).  Per chunk of ssp_frame_chunk(B)
  * fields: fresh noise is drawn on the device (ssp_fill_noise: stream 2*frame for the grid noise of the whole batch,

@@ -27,7 +27,7 @@ SYMBOLS = (
     "ssp_create", "ssp_destroy", "ssp_last_error", "ssp_version", "ssp_launch_count",
     "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_make_screens_pair", "ssp_evolve_screens_pair", "ssp_propagate",
     "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_propagate_host", "ssp_phase_mul",
-    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path", "ssp_dz_max", "ssp_place_screens", "ssp_fill_noise", "ssp_philox_words", "ssp_frame_chunk", "ssp_frame_host",
+    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path", "ssp_dz_max", "ssp_place_screens", "ssp_fill_noise", "ssp_philox_words", "ssp_evolve_propagate", "ssp_frame_chunk", "ssp_frame_host",
     "ssp_profile_enable", "ssp_profile_report",
 )
 
@@ -98,6 +98,8 @@ def load():
     lib.ssp_evolve_screens.argtypes = [P, Grid, C.POINTER(Psd), D, I, I, P, P, I, D, D, D, D, P, P, P, P, P, P,
                                        C.c_size_t]
     lib.ssp_propagate.argtypes = [P, Grid, D, D, I, I, I, P, P, L, I, Window, P, P, P, P, D, P, C.c_size_t]
+    lib.ssp_evolve_propagate.argtypes = [P, Grid, C.POINTER(Psd), D, D, I, I, P, P, I, D, D, D, D, P, P, P, P, Window, P, P,
+                                         P, D, P, P, C.c_size_t]
     lib.ssp_propagate_adjoint.argtypes = [P, Grid, D, D, I, I, I, P, P, L, I, Window, P, P, P, P, P, C.c_size_t]
     lib.ssp_beam_stats.argtypes = [P, Grid, I, P, D, P, P, P, C.POINTER(L)]
     lib.ssp_propagate_host.argtypes = [P, Grid, D, D, I, I, I, P, P, L, I, Window, P, P, P, D, P, P, P, P,
@@ -339,6 +341,24 @@ class Context:
             _dev(scr, torch.float32), stride, S, Window(win_order, win_sigma_frac),
             _dev(field, torch.complex64), _dev(out, torch.complex64), _dev(planes, torch.complex64),
             _dev(stats), roi_frac, None, 0))
+        return out
+
+    def evolve_propagate(self, N, dx, psd: PsdParams, lam, cn2, dz, n_sh, a, vx, vy, T, fresh_noise, fresh_noise_sh,
+                         spectrum, sh_coef, field, ycol, win_order=16, win_sigma_frac=0.47, n0=1.0, out=None, stats=None,
+                         roi_frac=0.5, ws=None):
+        """Forward-only temporal frame with the screen synthesis fused into the propagation (N = 1024): advances the AR
+        state in place and returns the received fields; ycol: complex64 [B][S][N][N] scratch."""
+        B, S = spectrum.shape[0], spectrum.shape[1]
+        ws = self.workspace(N, dx, B, S) if ws is None else ws
+        if out is None:
+            out = torch.empty_like(field)
+        pc = psd.c()
+        self._chk(self._lib.ssp_evolve_propagate(
+            self._h, Grid(N, dx), C.byref(pc), lam, n0, B, S, _host_doubles(cn2), _host_doubles(dz), n_sh, a, vx, vy, T,
+            _dev(fresh_noise, torch.complex64), _dev(fresh_noise_sh, torch.complex64) if n_sh > 0 else None,
+            _dev(spectrum, torch.complex64), _dev(sh_coef, torch.complex64) if n_sh > 0 else None,
+            Window(win_order, win_sigma_frac), _dev(field, torch.complex64), _dev(out, torch.complex64), _dev(stats),
+            roi_frac, _dev(ycol, torch.complex64), _dev(ws), ws.numel()))
         return out
 
     def propagate_adjoint(self, N, dx, lam, dz, g_out, screens=None, shared_screens=False, win_order=0,

@@ -172,18 +172,18 @@ bool small_ok(int N, int h_kind, int n_steps, const void *planes)
 
 extern "C" {
 
-int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind,
-                  int B, int n_steps, const double *dz,
-                  const float *d_screens, long long screen_batch_stride, int S,
-                  ssp_window win, const float *d_field_in, float *d_field_out,
-                  float *d_planes, ssp_stats *d_stats, double roi_frac,
-                  void *d_ws, size_t ws_bytes)
+} // extern "C"
+
+namespace {
+
+// ssp_propagate, and (fused != null) the propagation half of ssp_evolve_propagate, in which the screen of step j is
+// synthesised inside the row kernel from the column-transformed spectra instead of being read from d_screens.
+int propagate_core(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind,
+                   int B, int n_steps, const double *dz,
+                   const float *d_screens, long long screen_batch_stride, int S,
+                   ssp_window win, const float *d_field_in, float *d_field_out,
+                   float *d_planes, ssp_stats *d_stats, double roi_frac, const FusedScreens *fused)
 {
-    (void)d_ws; (void)ws_bytes;
-    if (int rc = check_prop(ctx, grid, lambda, n0, h_kind, B, n_steps, dz, d_screens, S, d_field_in, d_field_out))
-        return rc;
-    if (screen_batch_stride < 0 || (screen_batch_stride & 3))
-        return ctx->fail(SSP_EINVAL, "screen_batch_stride must be >= 0 and a multiple of 4 elements");
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));
     if (int rc = trim_htables(ctx)) return rc;
     const int N = grid.N;
@@ -198,7 +198,7 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
     long long roi_n = 0;
     if (d_stats) stats_roi(N, roi_frac, &roi_lo, &roi_hi, &roi_n);
 
-    if (small_ok(N, h_kind, n_steps, d_planes)) { // whole stack in one kernel, field resident in shared memory
+    if (!fused && small_ok(N, h_kind, n_steps, d_planes)) { // whole stack in one kernel, field resident in shared memory
         std::vector<SmallStep> ops(n_steps + 1);
         RowArgs w{};
         fill_window(w, win, N);
@@ -243,7 +243,11 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
         RowArgs r{};
         r.in = u; r.out = u; r.n_lines = B * N; r.tw = tw;
         r.in_swapped = mid_swapped(N);
-        if (j <= S) {
+        if (j <= S && fused) {
+            r.ycol = fused->ycol; r.scr0 = j - 1; r.scr_stride = S; r.n_sh = fused->n_sh;
+            r.sh_coef = fused->sh_coef; r.sh_mean = fused->sh_mean; r.ex = fused->ex;
+            r.phase_sign = 1.f;
+        } else if (j <= S) {
             r.phi = d_screens + (size_t)(j - 1) * px;
             r.phi_batch_stride = screen_batch_stride;
             r.phase_sign = 1.f;
@@ -268,6 +272,48 @@ int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_k
     if (d_stats)
         if (int rc = launch_stats_final(ctx, B, bpf, grid.dx, roi_n, reinterpret_cast<const double *>(ctx->scratch), d_stats)) return rc;
     return SSP_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int ssp_propagate(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind,
+                  int B, int n_steps, const double *dz,
+                  const float *d_screens, long long screen_batch_stride, int S,
+                  ssp_window win, const float *d_field_in, float *d_field_out,
+                  float *d_planes, ssp_stats *d_stats, double roi_frac,
+                  void *d_ws, size_t ws_bytes)
+{
+    (void)d_ws; (void)ws_bytes;
+    if (int rc = check_prop(ctx, grid, lambda, n0, h_kind, B, n_steps, dz, d_screens, S, d_field_in, d_field_out))
+        return rc;
+    if (screen_batch_stride < 0 || (screen_batch_stride & 3))
+        return ctx->fail(SSP_EINVAL, "screen_batch_stride must be >= 0 and a multiple of 4 elements");
+    return propagate_core(ctx, grid, lambda, n0, h_kind, B, n_steps, dz, d_screens, screen_batch_stride, S, win, d_field_in,
+                          d_field_out, d_planes, d_stats, roi_frac, nullptr);
+}
+
+int ssp_evolve_propagate(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, double n0,
+                         int B, int S, const double *cn2, const double *dz, int n_sh,
+                         double a, double vx, double vy, double T,
+                         const float *d_fresh_noise, const float *d_fresh_noise_sh,
+                         float *d_spectrum, float *d_sh_coef,
+                         ssp_window win, const float *d_field_in, float *d_field_out,
+                         ssp_stats *d_stats, double roi_frac, float *d_ycol, void *d_ws, size_t ws_bytes)
+{
+    if (!ctx) return SSP_EINVAL;
+    if (grid.N != 1024) return ctx->fail(SSP_EUNSUPPORTED, "ssp_evolve_propagate is built for N = 1024 (use ssp_evolve_screens + ssp_propagate)");
+    if (!(win.order > 0 && win.sigma_frac > 0)) return ctx->fail(SSP_EUNSUPPORTED, "ssp_evolve_propagate needs the absorbing window");
+    if (!d_ycol || !aligned16(d_ycol)) return ctx->fail(SSP_EINVAL, "d_ycol (16-byte aligned) is required");
+    // the propagation's argument checks first (d_ycol stands in for the screens: non-null, aligned), then the screens'
+    if (int rc = check_prop(ctx, grid, lambda, n0, SSP_H_FRESNEL, B, S, dz, d_ycol, S, d_field_in, d_field_out)) return rc;
+    FusedScreens fs{};
+    if (int rc = evolve_to_ycol(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, a, vx, vy, T, d_fresh_noise, d_fresh_noise_sh,
+                                d_spectrum, d_sh_coef, d_ycol, d_ws, ws_bytes, &fs))
+        return rc;
+    return propagate_core(ctx, grid, lambda, n0, SSP_H_FRESNEL, B, S, dz, nullptr, 0, S, win, d_field_in, d_field_out,
+                          nullptr, d_stats, roi_frac, &fs);
 }
 
 int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_kind,

@@ -124,7 +124,8 @@ int check_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda
 int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, int B, int S,
                  const double *cn2, const double *dz, int n_sh, bool ar, double a, double vx, double vy, double T,
                  const float *d_noise, const float *d_noise_sh, float *d_spectrum, float *d_sh_coef,
-                 float *d_screens, void *d_ws, float *d_screens_im = nullptr)
+                 float *d_screens, void *d_ws, float *d_screens_im = nullptr, float2 *ycol_out = nullptr,
+                 ssp::FusedScreens *fused = nullptr)
 {
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));
     const int N = grid.N;
@@ -236,7 +237,7 @@ int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
         c.noise = reinterpret_cast<const float2 *>(d_noise) + (size_t)g0 * px;
         c.old_spec = ar ? reinterpret_cast<const float2 *>(d_spectrum) + (size_t)g0 * px : nullptr;
         c.spec_out = d_spectrum ? reinterpret_cast<float2 *>(d_spectrum) + (size_t)g0 * px : nullptr;
-        c.out = inter;
+        c.out = ycol_out ? ycol_out + (size_t)g0 * px : inter;   // fused synthesis: every screen's column-transformed spectrum is kept
         c.nscr = n; c.g0 = g0; c.S = S;
         c.amp = d_amp;
         c.flt = flt;
@@ -244,6 +245,7 @@ int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
         c.taux = d_taux; c.tauy = d_tauy;
         c.tw = twc;
         if (int rc = launch_screen_col(ctx, N, c)) return rc;
+        if (ycol_out) continue;                                   // K3 runs inside the propagation's row kernels
         ScreenRowArgs r{};
         r.in = inter;
         r.screens = d_screens + (size_t)g0 * px;
@@ -255,10 +257,24 @@ int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
         r.tw = tw;
         if (int rc = launch_screen_row(ctx, N, r)) return rc;
     }
+    if (fused) { fused->ycol = ycol_out; fused->sh_coef = coef; fused->sh_mean = mean; fused->ex = d_ex; fused->n_sh = n_sh; }
     return SSP_OK;
 }
 
 } // namespace
+
+int ssp::evolve_to_ycol(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, int B, int S, const double *cn2,
+                        const double *dz, int n_sh, double a, double vx, double vy, double T, const float *d_noise,
+                        const float *d_noise_sh, float *d_spectrum, float *d_sh_coef, float *d_ycol, void *d_ws,
+                        size_t ws_bytes, FusedScreens *out)
+{
+    if (int rc = check_screens(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, d_noise, d_noise_sh, d_ycol, d_ws, ws_bytes)) return rc;
+    if (!(a >= 0.0 && a <= 1.0)) return ctx->fail(SSP_EINVAL, "a must be in [0, 1]");
+    if (!d_spectrum || !aligned16(d_spectrum)) return ctx->fail(SSP_EINVAL, "d_spectrum (in-out) is required");
+    if (n_sh > 0 && !d_sh_coef) return ctx->fail(SSP_EINVAL, "d_sh_coef (in-out) is required when n_sh > 0");
+    return screens_impl(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, true, a, vx, vy, T, d_noise, d_noise_sh, d_spectrum,
+                        d_sh_coef, nullptr, d_ws, nullptr, reinterpret_cast<float2 *>(d_ycol), out);
+}
 
 int ssp::check_screen_args(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, int B, int S, const double *cn2,
                            const double *dz, int n_sh, const void *noise, const void *noise_sh, const void *screens,

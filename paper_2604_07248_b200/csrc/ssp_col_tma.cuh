@@ -81,7 +81,10 @@ struct ColTmaCfg {
     static constexpr size_t SMEM = NBUF * sizeof(float2) * BUF_ELEMS + 32;   // + two mbarriers + the TMEM address slot
     static constexpr unsigned TILE_BYTES = (unsigned)(sizeof(float2) * C * N);
     // packed fp32 pairs: measured 2048 +3.6 %, 4096 +1.3 %; 1024 -1 % and 512 +1 % (within noise) stay scalar
-    static constexpr bool PACKED = (N >= 2048);
+#ifndef SSP_COL1024_PK
+#define SSP_COL1024_PK 0
+#endif
+    static constexpr bool PACKED = (N >= 2048) || (N == 1024 && SSP_COL1024_PK);
     // first-stage twiddles and the hy table kept per thread in tensor memory (128 columns per CTA): persistent CTAs only
 #ifndef SSP_COL1024_TMEM
 #define SSP_COL1024_TMEM 1

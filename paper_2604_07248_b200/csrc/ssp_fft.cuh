@@ -290,8 +290,12 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 
     fft_line<N, V, DIR_REV, INV, TAIL_SYNC, PK>(v, t, sm, TwGlobal{tw});
 }
 
-template <int N, int V, bool DIR_REV, bool INV, bool TAIL_SYNC = false, bool PK = false, class SM, class TWP>
-__device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const TWP twp)
+// HOOK: called once, right after the last exchange of the transform has been read (where TAIL_SYNC synchronises):
+// the place from which a persistent kernel starts the asynchronous copy of its next line into the exchange buffer.
+struct NoHook { __device__ __forceinline__ void operator()() const {} };
+
+template <int N, int V, bool DIR_REV, bool INV, bool TAIL_SYNC = false, bool PK = false, class SM, class TWP, class HOOK = NoHook>
+__device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const TWP twp, HOOK hook = HOOK{})
 {
     const float2 *__restrict__ tw = twp.table();
     constexpr bool TW_TMEM = std::is_same<TWP, TwTmem>::value;
@@ -339,6 +343,7 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const TWP twp
 #pragma unroll
         for (int n = 0; n < Rc; ++n) v[n] = sm.ld(k1 * P1 + k2 * P2 + n);
         if constexpr (TAIL_SYNC) sm.sync();
+        hook();
         radix<Rc, INV, PK>(v);
         return;
     }
@@ -383,6 +388,7 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const TWP twp
             }
         }
         if constexpr (TAIL_SYNC) sm.sync();
+        hook();
 #pragma unroll
         for (int i = 0; i < E / Rb; ++i) radix<Rb, INV, PK>(v + i * Rb);
     } else {
@@ -416,6 +422,7 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const TWP twp
             for (int n = 0; n < Rc; ++n) w[n] = sm.ld(base + n);
         }
         if constexpr (TAIL_SYNC) sm.sync();
+        hook();
 #pragma unroll
         for (int i = 0; i < E / Rc; ++i) radix<Rc, INV, PK>(v + i * Rc);
     }

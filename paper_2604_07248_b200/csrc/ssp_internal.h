@@ -156,6 +156,13 @@ struct RowArgs {
     const float2 *pre_line;      // per-line factor pre_line[iy] multiplying the whole line, or null
     int in_swapped;              // the input holds (im, re) pairs: written by launch_col_prop when mid_swapped(N)
     const float2 *tw;
+    // fused screen synthesis (k_row<.., FUSE>): column-transformed spectra [nscr][N][N] of the screen
+    // generator instead of phi; the screen of field b is number scr0 + b * scr_stride
+    const float2 *ycol;
+    int scr0, scr_stride, n_sh;
+    const float2 *sh_coef;       // [nscr][n_sh][3][3]
+    const float *sh_mean;        // [nscr][2]
+    const float2 *ex;            // [n_sh][N]
     // statistics epilogue of the LAST row kernel (first && !second): partial sums of the nine accumulators of
     // ssp_stats.cuh, stats_acc[field][row_stats_records(N)][ACC_N] (null: none); ROI = [roi_lo, roi_hi)^2
     double *stats_acc;
@@ -253,6 +260,20 @@ struct ScreenRowArgs {
 int check_screen_args(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, int B, int S, const double *cn2,
                       const double *dz, int n_sh, const void *noise, const void *noise_sh, const void *screens,
                       const void *ws, size_t ws_bytes);
+// Fused screen synthesis: the AR step of ssp_evolve_screens up to and including the column pass; every
+// screen's column-transformed spectrum goes to d_ycol (c64 [B][S][N][N]) and the row pass is left to the propagation's
+// row kernels, which need the tables returned in `out` (they live in the caller's workspace).
+struct FusedScreens {
+    const float2 *ycol;
+    const float2 *sh_coef;
+    const float *sh_mean;
+    const float2 *ex;
+    int n_sh;
+};
+int evolve_to_ycol(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, int B, int S, const double *cn2,
+                   const double *dz, int n_sh, double a, double vx, double vy, double T, const float *d_noise,
+                   const float *d_noise_sh, float *d_spectrum, float *d_sh_coef, float *d_ycol, void *d_ws, size_t ws_bytes,
+                   FusedScreens *out);
 int launch_screen_col(ssp_ctx *ctx, int N, const ScreenColArgs &a);
 int screen_col_plan_variant(int N);   // plan variant (ssp_fft.cuh) whose twiddles launch_screen_col expects in a.tw
 int launch_screen_row(ssp_ctx *ctx, int N, const ScreenRowArgs &a);

@@ -117,9 +117,15 @@ __device__ __forceinline__ void row_pointwise(float2 *v, const RowArgs &a, const
     }
 }
 
-template <int N, bool FIRST, bool SECOND, bool GENERIC>
+// FUSE (SURVEY 8(f)-1, K3 fused into K6; forward-only temporal frames): the screen row is not read from HBM but
+// synthesised here from the column-transformed spectrum row a.ycol (8 B/px instead of the 12 B/px row pass of the
+// generator plus 4 B/px here) -- a third in-register transform through the same rolled forward body (IFFT_x as forward
+// code on swapped data; its real part lands in .y), the subharmonic sum of k_screen_row, the result into the shared
+// screen-row buffer the pointwise stage reads anyway.
+template <int N, bool FIRST, bool SECOND, bool GENERIC, bool FUSE = false>
 __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_row(const RowArgs a)
 {
+    static_assert(!FUSE || (FIRST && !GENERIC && SYM_PLAN<N>::value && PlanInfo<N, 0>::T == 32), "fused screens: one warp per row");
     using PI = PlanInfo<N, 0>;
     using CFG = RowCfg<N>;
     constexpr int E = PI::E, T = PI::T, R1 = PI::R1, RL = PI::RL;
@@ -135,6 +141,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
     // twiddle pairs W_N^(t k) and the 32 hx values of its output points do not change from row to row and are read
     // from the thread's own tensor-memory lane (tcgen05.ld) instead of through the LSU data pipe.
     constexpr bool TM = RowCfg<N>::TMEM && FIRST && SECOND && !GENERIC;
+    static_assert(!FUSE || MidSwapped<N>::value, "fused screens: the column kernel hands the field over swapped");
     unsigned taddr = 0;
     if constexpr (TM) {
         static_assert(!TM || (CFG::THREADS == 128 && T == 32 && SYM_PLAN<N>::value), "one warp per row, four rows per CTA");
@@ -162,7 +169,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
 
     // the screen row is streamed from HBM: fetch it asynchronously now, use it after the first transform
     float *phis = reinterpret_cast<float *>(smem_raw + CFG::SMEM_X) + (size_t)lib * N;
-    if (!GENERIC || a.phi) {
+    if (!FUSE && (!GENERIC || a.phi)) {
         const float *g = a.phi + b * a.phi_batch_stride + (long long)iy * N;
 #pragma unroll
         for (int i = 0; i < E / 4; ++i) cp_async16(phis + 4 * (t + T * i), g + 4 * (t + T * i));
@@ -192,7 +199,33 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
                 v[i * RIN + q] = swap_if<SW>(x);
             }
     };
-    if constexpr (SWAP_IN && MID) {
+    if constexpr (FUSE) {
+        // ---- K3 here: Y row -> IFFT_x -> Re + subharmonics - mean -> screen-row buffer (ssp_screens.cu: k_screen_row)
+        const int scr = a.scr0 + b * a.scr_stride;
+        if (TM && blk != (long long)blockIdx.x) {
+            cp_async_wait_all();                                  // this row of Y was copied into the exchange buffer meanwhile
+            sm.sync();
+#pragma unroll
+            for (int q = 0; q < E; ++q) v[q] = swap_if<true>(sm.base[line_index<N, 0, R1>(t, 0, q)]);
+            sm.sync();
+        } else {
+            const float2 *ysrc = a.ycol + ((size_t)scr * N + iy) * N;
+#pragma unroll
+            for (int q = 0; q < E; ++q) v[q] = swap_if<true>(ysrc[line_index<N, 0, R1>(t, 0, q)]);
+        }
+    } else
+    if (TM && blk != (long long)blockIdx.x) {
+        // persistent form: this row was copied into the warp's exchange buffer (cp.async, raw order) while the previous
+        // row finished its second transform and its stores; the group committed after it is this row's screen
+        if constexpr (TM) {
+            cp_async_wait_group<1>();
+            sm.sync();
+            constexpr bool SW = SWAP_IN && !MID;
+#pragma unroll
+            for (int q = 0; q < RIN; ++q) v[q] = swap_if<SW>(sm.base[line_index<N, 0, RIN>(t, 0, q)]);
+            sm.sync();
+        }
+    } else if constexpr (SWAP_IN && MID) {
         // the column kernel has left the field swapped (always so on the common path; a run-time flag otherwise)
         if (!GENERIC || a.in_swapped) load_line(std::false_type{});
         else load_line(std::true_type{});
@@ -205,6 +238,63 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
     };
 
     constexpr int ROUT = SYM ? R1 : (SECOND ? R1 : RL);
+    if constexpr (FUSE) {
+        // pass -1: the screen row (v holds swap(Y)); pass 0: IFFT_x of the field; pass 1 (SECOND): FFT_x
+        auto prefetch_next_y = [&](int pass) {
+            if constexpr (TM) {
+                if (pass == 1) {
+                    const long long nl = line + (long long)gridDim.x * CFG::LPB;
+                    if (blk + gridDim.x < nblk) {
+                        sm.sync();
+                        const float2 *nxt = a.ycol + ((size_t)(a.scr0 + (int)(nl / N) * a.scr_stride) * N + (int)(nl % N)) * N;
+#pragma unroll
+                        for (int i = 0; i < E / 2; ++i) cp_async16(sm.base + 2 * (t + T * i), nxt + 2 * (t + T * i));
+                    }
+                    cp_async_commit();
+                }
+            }
+        };
+#pragma unroll 1
+        for (int pass = -1; pass < (SECOND ? 2 : 1); ++pass) {
+            auto hook = [&]() { prefetch_next_y(pass); };
+            if constexpr (TM) fft_line<N, 0, false, false, false, PK>(v, t, sm, TwTmem{a.tw, taddr}, hook);
+            else fft_line<N, 0, false, false, false, PK>(v, t, sm, a.tw);
+            if (pass == -1) {
+                const int scr = a.scr0 + b * a.scr_stride;
+                float cst = 0.f;
+                if (a.n_sh > 0) {
+                    cst = -__ldg(a.sh_mean + 2 * scr);
+                    for (int p = 0; p < a.n_sh; ++p) {
+                        const float2 *cf = a.sh_coef + ((size_t)scr * a.n_sh + p) * 9;
+                        const float2 ey = __ldg(a.ex + (size_t)p * N + iy);
+                        float2 d[3];
+#pragma unroll
+                        for (int bb = 0; bb < 3; ++bb) {
+                            const float2 c0 = __ldg(cf + bb), c1 = __ldg(cf + 3 + bb), c2 = __ldg(cf + 6 + bb);
+                            const float2 lo = cmul_conj(c0, ey), hi = cmul(c2, ey);
+                            d[bb] = make_float2(lo.x + c1.x + hi.x, lo.y + c1.y + hi.y);
+                        }
+                        const float ca = d[0].x + d[2].x, sa = d[0].y - d[2].y;
+                        cst += d[1].x;
+                        const float2 *exp_ = a.ex + (size_t)p * N + t;
+#pragma unroll
+                        for (int q = 0; q < E; ++q) {
+                            const float2 ex = __ldg(exp_ + (line_index<N, 0, RL>(t, 0, q) - t));
+                            v[q].y = fmaf(ca, ex.x, fmaf(sa, ex.y, v[q].y));
+                        }
+                    }
+                }
+                sm.sync();
+#pragma unroll
+                for (int q = 0; q < E; ++q) phis[line_index<N, 0, RL>(t, 0, q)] = v[q].y + cst;
+                sm.sync();
+                load_line(std::false_type{});                     // the field row, as the column kernel left it (swapped)
+            } else if (pass == 0) {
+                row_pointwise<N, RL, E, T, false, true, PK>(v, a, phis, t, b, iy);
+                sm.sync();
+            }
+        }
+    } else
     if constexpr (SYM) {
         if constexpr (FIRST && SECOND) {
 #pragma unroll 1
@@ -212,8 +302,22 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
                 // the exchange buffer is reused by the next pass: a row spanning several warps synchronises
                 // right after its last exchange read (TAIL), a warp-local row after the pointwise stage
                 constexpr bool TAIL = (T > 32);
-                if constexpr (TM) fft_line<N, 0, false, false, TAIL, PK>(v, t, sm, TwTmem{a.tw, taddr});
-                else fft_line<N, 0, false, false, TAIL, PK>(v, t, sm, a.tw);
+                if constexpr (TM) {
+                    // after the second transform's exchange has been read the buffer is idle until the next row's first
+                    // transform: the next row of this warp is copied into it now, under the last butterflies and the stores
+                    auto prefetch_next = [&]() {
+                        if (pass == 1) {
+                            if (blk + gridDim.x < nblk) {
+                                sm.sync();
+                                const float2 *nxt = a.in + (line + (long long)gridDim.x * CFG::LPB) * N;
+#pragma unroll
+                                for (int i = 0; i < E / 2; ++i) cp_async16(sm.base + 2 * (t + T * i), nxt + 2 * (t + T * i));
+                            }
+                            cp_async_commit();
+                        }
+                    };
+                    fft_line<N, 0, false, false, TAIL, PK>(v, t, sm, TwTmem{a.tw, taddr}, prefetch_next);
+                } else fft_line<N, 0, false, false, TAIL, PK>(v, t, sm, a.tw);
                 if (pass == 0) {
                     wait_phi();
                     row_pointwise<N, RL, E, T, GENERIC, true, PK>(v, a, phis, t, b, iy);

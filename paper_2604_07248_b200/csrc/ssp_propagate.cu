@@ -22,16 +22,17 @@ static int set_smem(ssp_ctx *ctx, K kernel, size_t bytes)
     return SSP_OK;
 }
 
-template <int N, bool FIRST, bool SECOND, bool GENERIC>
+template <int N, bool FIRST, bool SECOND, bool GENERIC, bool FUSE = false>
 static int launch_row_x(ssp_ctx *ctx, const RowArgs &a)
 {
     using CFG = RowCfg<N>;
     if (a.n_lines % CFG::LPB) return ctx->fail(SSP_EINVAL, "row launch: %d lines not a multiple of %d", a.n_lines, CFG::LPB);
-    auto kern = k_row<N, FIRST, SECOND, GENERIC>;
+    auto kern = k_row<N, FIRST, SECOND, GENERIC, FUSE>;
     if (int rc = set_smem(ctx, kern, CFG::SMEM + 16)) return rc;
     // algorithmic bytes: field in + out, + the screen, + saved / read planes and the gradient
-    const double bpp = 16.0 + (a.phi ? 4.0 : 0.0) + (a.plane_out ? 8.0 : 0.0) + (a.grad ? 12.0 : 0.0);
-    ctx->prof_begin(FIRST ? (SECOND ? "row_ifft_pw_fft" : "row_ifft_pw") : "row_pw_fft", bpp * (double)a.n_lines * N);
+    const double bpp = 16.0 + (a.phi ? 4.0 : 0.0) + (FUSE ? 8.0 : 0.0) + (a.plane_out ? 8.0 : 0.0) + (a.grad ? 12.0 : 0.0);
+    ctx->prof_begin(FUSE ? (SECOND ? "row_fused_screen_fft" : "row_fused_screen")
+                         : (FIRST ? (SECOND ? "row_ifft_pw_fft" : "row_ifft_pw") : "row_pw_fft"), bpp * (double)a.n_lines * N);
     constexpr bool TM = CFG::TMEM && FIRST && SECOND && !GENERIC;           // persistent form (ssp_kernels.cuh)
     int grid = a.n_lines / CFG::LPB;
     if (TM) {
@@ -55,6 +56,14 @@ static int launch_row_n(ssp_ctx *ctx, const RowArgs &a)
     if (a.in_swapped && !MID) return ctx->fail(SSP_EINVAL, "swapped row input for a kernel that does not take it");
     if (a.in_swapped && a.pre) return ctx->fail(SSP_EINVAL, "pre-multiply on a swapped row input");
     if (a.stats_acc && !(FIRST && !SECOND)) return ctx->fail(SSP_EINVAL, "statistics epilogue on a row kernel that is not the last");
+    if (a.ycol) {                                                 // fused screen synthesis: the common 1024^2 kernels only
+        if constexpr (N == 1024 && FIRST) {
+            const bool ok = !a.phi && a.win_on && !a.grad && !a.plane_out && !a.pre && a.in_swapped &&
+                            ((a.win_map != nullptr) == WinMap<N>::value) && (!SECOND || a.hx);
+            if (!ok) return ctx->fail(SSP_EUNSUPPORTED, "fused screen synthesis needs the common split step (window on, Fresnel H, nothing saved)");
+            return launch_row_x<N, FIRST, SECOND, false, true>(ctx, a);
+        } else return ctx->fail(SSP_EUNSUPPORTED, "fused screen synthesis is built for N = 1024");
+    }
     // (the persistent tensor-memory form of the common kernel caches hx per thread: without hx -- angular spectrum --
     // the generic kernel runs)
     const bool common = a.phi && a.win_on && !a.grad && !a.plane_out && !a.pre && (!MID || a.in_swapped) &&

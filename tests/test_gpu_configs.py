@@ -272,3 +272,74 @@ def test_full_size_configs_properties(ssp, cid):
         assert abs(ip1[b, 0] - ip2[b, 0]) < 2e-6 * S * ip1[b, 0], (b, ip1[b], ip2[b])
         assert abs(ip2[b, 1]) < 2e-6 * S * ip1[b, 0]
         assert ip1[b, 2] <= p0[b] * (1 + 1e-5)
+
+
+@pytest.mark.parametrize("n_sh,wind", [(3, False), (2, True), (0, False)])
+def test_fused_screen_synthesis_frame(ssp, orc, n_sh, wind):
+    """ssp_evolve_propagate (the generator's row pass fused into the split step's row kernel, forward-only
+    temporal frames at 1024^2): two successive AR frames of 3 stacks x 4 von Karman screens.  Against the oracle
+    (evolve_screens + propagate on the same noise), against the unfused GPU calls (same AR state bit for bit, fields to
+    fp32 rounding), statistics included; odd batch, wind, with and without subharmonics."""
+    import torch
+    from paper_2604_07248_b200 import api
+    wl = synth.CONFIGS[3]
+    N, S, B = wl.N, 4, 3
+    po, pg = _psd(wl, orc)
+    cn2, dz = list(wl.cn2_list[:S] * np.array([1.0, 2.0, 0.5, 1.5])), list(wl.dz[:S] * np.array([1.0, 0.7, 1.3, 1.0]))
+    a, T = 0.97, 0.01
+    vx, vy = (2.3 * wl.dx / T, -0.7 * wl.dx / T) if wind else (0.0, 0.0)
+    frames = [synth.noise(33, n_sh, b, S, N, n_sh, frames=3) for b in range(B)]
+    hi = lambda t: np.stack([frames[b][t][0] for b in range(B)])
+    sh = lambda t: np.stack([frames[b][t][1] for b in range(B)])
+    _, spec_ref, shc_ref = oracle_screens_parallel(orc, N, wl.dx, po, wl.lam, cn2, dz, n_sh, hi(0), sh(0), keep_spectrum=True)
+    spec_ref = np.ascontiguousarray(spec_ref)
+    shc_ref = np.ascontiguousarray(shc_ref) if n_sh else None
+    spec = torch.empty((B, S, N, N), dtype=torch.complex64, device="cuda")
+    shc = torch.zeros((B, S, max(n_sh, 1), 3, 3), dtype=torch.complex64, device="cuda")
+    ssp.make_screens(N, wl.dx, pg, wl.lam, cn2, dz, n_sh, cu(c64(hi(0))), cu(c64(sh(0))) if n_sh else None,
+                     spectrum=spec, sh_coef=shc if n_sh else None)
+    spec_u, shc_u = spec.clone(), shc.clone()                       # the unfused GPU path's AR state
+    ycol = torch.empty((B, S, N, N), dtype=torch.complex64, device="cuda")
+    u0 = synth.input_field(wl, B)
+    kw = dict(win_order=wl.win_order, win_sigma_frac=wl.win_sigma_frac)
+    for t in (1, 2):
+        h_t, s_t = hi(t), sh(t)
+        d_h, d_s = cu(c64(h_t)), (cu(c64(s_t)) if n_sh else None)
+        stats = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+        l0 = ssp.launch_count()
+        out = ssp.evolve_propagate(N, wl.dx, pg, wl.lam, cn2, dz, n_sh, a, vx, vy, T, d_h, d_s, spec, shc if n_sh else None,
+                                   cu(u0), ycol, stats=stats, roi_frac=0.25, **kw)
+        n_fused = ssp.launch_count() - l0
+        # unfused GPU path
+        scr_u = ssp.evolve_screens(N, wl.dx, pg, wl.lam, cn2, dz, n_sh, a, vx, vy, T, d_h, d_s, spec_u, shc_u if n_sh else None)
+        stats_u = torch.zeros(B * api.STATS_BYTES, dtype=torch.uint8, device="cuda")
+        out_u = ssp.propagate(N, wl.dx, wl.lam, dz, cu(u0), scr_u, stats=stats_u, roi_frac=0.25, **kw)
+        assert torch.equal(spec, spec_u) and torch.equal(shc, shc_u)
+        e_gpu = rel_l2(out.cpu().numpy(), out_u.cpu().numpy().astype(np.complex128)).max()
+        assert e_gpu < 2e-6 * S, e_gpu
+        # oracle
+        def evolve_one(bs):
+            b, j = divmod(bs, S)
+            sp = np.ascontiguousarray(spec_ref[b:b + 1, j:j + 1])
+            sc = np.ascontiguousarray(shc_ref[b:b + 1, j:j + 1]) if n_sh else None
+            o = orc.evolve_screens(N, wl.dx, po, wl.lam, [cn2[j]], [dz[j]], n_sh, a, vx, vy, T, h_t[b:b + 1, j:j + 1],
+                                   s_t[b:b + 1, j:j + 1] if n_sh else None, sp, sc)
+            return o[0, 0], sp[0, 0], (sc[0, 0] if n_sh else None)
+        res = pmap(evolve_one, range(B * S))
+        scr_ref = np.stack([r[0] for r in res]).reshape(B, S, N, N)
+        spec_ref = np.stack([r[1] for r in res]).reshape(B, S, N, N)
+        if n_sh:
+            shc_ref = np.stack([r[2] for r in res]).reshape(B, S, n_sh, 3, 3)
+        # the oracle propagates through ITS fp64 screens: the fused path never rounds a screen to fp32 in memory
+        ref = np.concatenate(pmap(lambda b: orc.propagate(N, wl.dx, wl.lam, dz, u0[b:b + 1], scr_ref[b:b + 1], **kw), range(B)))
+        e_f = rel_l2(out.cpu().numpy(), ref).max()
+        record("fused_frame", n_sh=n_sh, wind=wind, frame=t, vs_unfused=float(e_gpu), field=float(e_f), bound=tol(N, S + t + 1),
+               launches=int(n_fused))
+        assert e_f < tol(N, S + t + 1), (t, e_f)
+        _check_stats(api.stats_to_dicts(stats), orc.beam_stats(N, wl.dx, ref, roi_frac=0.25), wl)
+    # argument errors: other grids are refused, not silently run unfused
+    with pytest.raises(api.SspError) as ei:
+        small = torch.zeros((1, 1, 512, 512), dtype=torch.complex64, device="cuda")
+        ssp.evolve_propagate(512, wl.dx, pg, wl.lam, [cn2[0]], [dz[0]], 0, a, 0, 0, 0, small, None, small.clone(), None,
+                             small[0].clone(), small.clone(), **kw)
+    assert ei.value.code == api.EUNSUPPORTED
