@@ -52,21 +52,29 @@ __device__ __forceinline__ float2 cmul_c(float2 a, float2 b)
     return CONJ ? cmul_conj(a, b) : cmul(a, b);
 }
 
-// cos(2 pi k / 32), k = 0..31
-__host__ __device__ constexpr float cos32(int k)
+// cos(2 pi k / 64), k = 0..63 (double-precision values rounded once to fp32)
+__host__ __device__ constexpr float cos64(int k)
 {
-    constexpr float t[32] = {
-        1.0f, 0.98078528040323043f, 0.92387953251128674f, 0.83146961230254524f,
-        0.70710678118654752f, 0.55557023301960218f, 0.38268343236508977f, 0.19509032201612825f,
-        0.0f, -0.19509032201612825f, -0.38268343236508977f, -0.55557023301960218f,
-        -0.70710678118654752f, -0.83146961230254524f, -0.92387953251128674f, -0.98078528040323043f,
-        -1.0f, -0.98078528040323043f, -0.92387953251128674f, -0.83146961230254524f,
-        -0.70710678118654752f, -0.55557023301960218f, -0.38268343236508977f, -0.19509032201612825f,
-        0.0f, 0.19509032201612825f, 0.38268343236508977f, 0.55557023301960218f,
-        0.70710678118654752f, 0.83146961230254524f, 0.92387953251128674f, 0.98078528040323043f};
-    return t[k & 31];
+    constexpr float t[64] = {
+        1.0f, 0.9951847266721969f, 0.9807852804032304f, 0.9569403357322088f,
+        0.9238795325112867f, 0.881921264348355f, 0.8314696123025452f, 0.773010453362737f,
+        0.7071067811865476f, 0.6343932841636455f, 0.5555702330196023f, 0.4713967368259978f,
+        0.38268343236508984f, 0.29028467725446233f, 0.19509032201612833f, 0.09801714032956077f,
+        6.123233995736766e-17f, -0.09801714032956065f, -0.1950903220161282f, -0.29028467725446216f,
+        -0.3826834323650897f, -0.4713967368259977f, -0.555570233019602f, -0.6343932841636454f,
+        -0.7071067811865475f, -0.773010453362737f, -0.8314696123025453f, -0.8819212643483549f,
+        -0.9238795325112867f, -0.9569403357322088f, -0.9807852804032304f, -0.9951847266721968f,
+        -1.0f, -0.9951847266721969f, -0.9807852804032304f, -0.9569403357322089f,
+        -0.9238795325112868f, -0.881921264348355f, -0.8314696123025455f, -0.7730104533627371f,
+        -0.7071067811865477f, -0.6343932841636459f, -0.5555702330196022f, -0.47139673682599786f,
+        -0.38268343236509034f, -0.29028467725446244f, -0.19509032201612866f, -0.09801714032956045f,
+        -1.8369701987210297e-16f, 0.09801714032956009f, 0.1950903220161283f, 0.29028467725446205f,
+        0.38268343236509f, 0.4713967368259976f, 0.5555702330196018f, 0.6343932841636456f,
+        0.7071067811865474f, 0.7730104533627367f, 0.8314696123025452f, 0.8819212643483548f,
+        0.9238795325112865f, 0.9569403357322088f, 0.9807852804032303f, 0.9951847266721969f};
+    return t[k & 63];
 }
-__host__ __device__ constexpr float sin32(int k) { return cos32(k - 8); }
+__host__ __device__ constexpr float sin64(int k) { return cos64(k - 16); }
 
 // ---- radix-R butterflies in registers: decimation in time, FMA form ----------------------------------
 // One DIT butterfly (a, b) -> (a + w b, a - w b) with w = W_L^J = exp(-/+ i 2 pi J / L) (forward / inverse),
@@ -78,34 +86,35 @@ __host__ __device__ constexpr float sin32(int k) { return cos32(k - 8); }
 template <int L, int J, bool INV, bool PK>
 __device__ __forceinline__ void bfly_dit(float2 &a, float2 &b)
 {
-    constexpr int k32 = (J * (32 / L)) & 31;                      // w = W_32^k32, k32 < 16 since J < L/2
+    static_assert(L <= 64, "butterfly constants are tabulated for radices up to 64");
+    constexpr int k64 = (J * (64 / L)) & 63;                      // w = W_64^k64, k64 < 32 since J < L/2
     if constexpr (PK) {
-    if constexpr (k32 == 0) {
+    if constexpr (k64 == 0) {
         const float2 x = f2add(a, b), y = f2sub(a, b);
         a = x; b = y;
-    } else if constexpr (k32 == 8) {                              // w = -i (forward), +i (inverse): w b = -/+ (-b.y, b.x)
+    } else if constexpr (k64 == 16) {                              // w = -i (forward), +i (inverse): w b = -/+ (-b.y, b.x)
         constexpr float s = INV ? 1.f : -1.f;
         const float2 ib = make_float2(-b.y, b.x);
         const float2 x = f2fma(make_float2(s, s), ib, a), y = f2fma(make_float2(-s, -s), ib, a);
         a = x; b = y;
     } else {
-        constexpr float wr = cos32(k32);
-        constexpr float wi = INV ? sin32(k32) : -sin32(k32);
+        constexpr float wr = cos64(k64);
+        constexpr float wi = INV ? sin64(k64) : -sin64(k64);
         const float2 x = f2fma(make_float2(wi, wi), make_float2(-b.y, b.x), f2fma(make_float2(wr, wr), b, a));
         const float2 y = f2fma(make_float2(2.f, 2.f), a, make_float2(-x.x, -x.y));
         a = x; b = y;
     }
     } else {
-    if constexpr (k32 == 0) {
+    if constexpr (k64 == 0) {
         const float2 x = make_float2(a.x + b.x, a.y + b.y), y = make_float2(a.x - b.x, a.y - b.y);
         a = x; b = y;
-    } else if constexpr (k32 == 8) {                              // w = -i (forward), +i (inverse)
+    } else if constexpr (k64 == 16) {                              // w = -i (forward), +i (inverse)
         const float2 wb = INV ? make_float2(-b.y, b.x) : make_float2(b.y, -b.x);
         const float2 x = make_float2(a.x + wb.x, a.y + wb.y), y = make_float2(a.x - wb.x, a.y - wb.y);
         a = x; b = y;
     } else {
-        constexpr float wr = cos32(k32);
-        constexpr float wi = INV ? sin32(k32) : -sin32(k32);
+        constexpr float wr = cos64(k64);
+        constexpr float wi = INV ? sin64(k64) : -sin64(k64);
         const float2 x = make_float2(fmaf(wr, b.x, fmaf(-wi, b.y, a.x)), fmaf(wr, b.y, fmaf(wi, b.x, a.y)));
         const float2 y = make_float2(fmaf(2.f, a.x, -x.x), fmaf(2.f, a.y, -x.y));
         a = x; b = y;
@@ -148,7 +157,7 @@ __device__ __forceinline__ void dit_levels(float2 *v)
     }
 }
 
-// Radix-R DFT of v[0..R) in registers, natural order in and out.  R in {1,2,4,8,16,32}.
+// Radix-R DFT of v[0..R) in registers, natural order in and out.  R in {1,2,4,8,16,32,64}.
 template <int R, bool INV, bool PK = false>
 __device__ __forceinline__ void radix(float2 *v)
 {
@@ -177,7 +186,22 @@ SSP_PLAN(256, 0, 16, 16, 1, 16);   SSP_PLAN(256, 1, 16, 16, 1, 16);
 SSP_PLAN(512, 0, 16, 2, 16, 16);   SSP_PLAN(512, 1, 32, 16, 1, 32);
 SSP_PLAN(1024, 0, 32, 32, 1, 32);   SSP_PLAN(1024, 1, 32, 32, 1, 32);
 SSP_PLAN(2048, 0, 32, 2, 32, 32);   SSP_PLAN(2048, 1, 32, 2, 32, 32);
-SSP_PLAN(4096, 0, 32, 4, 32, 32);  SSP_PLAN(4096, 1, 32, 4, 32, 32);
+#ifndef SSP_P4096_COL64
+#define SSP_P4096_COL64 1
+#endif
+#ifndef SSP_P4096_ROW64
+#define SSP_P4096_ROW64 0
+#endif
+#if SSP_P4096_ROW64
+SSP_PLAN(4096, 0, 64, 64, 1, 64);
+#else
+SSP_PLAN(4096, 0, 32, 4, 32, 32);
+#endif
+#if SSP_P4096_COL64
+SSP_PLAN(4096, 1, 64, 64, 1, 64);
+#else
+SSP_PLAN(4096, 1, 32, 4, 32, 32);
+#endif
 // V = 2 ("screen column" variant): what the register-load screen generator k_screen_col runs.  Equal to V = 1
 //   except at N = 4096, where the single inverse transform measured faster with short last radices than with
 //   (32,4,32); at 2048 it is the shuffle plan (32,2,32) like V = 1 (4216 vs 3430 GB/s with (32,8,8)).  The TMA

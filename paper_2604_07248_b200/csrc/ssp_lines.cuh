@@ -30,8 +30,16 @@ struct RowTune<2048> {
     static constexpr int MAX_THREADS = 64;
     static constexpr int MIN_BLOCKS = 6;
 };
+#if SSP_P4096_ROW64
+template <>
+struct RowTune<4096> {                                           // (64,64), 64 points per thread: two rows per CTA, 255 registers
+    static constexpr int MAX_THREADS = 128;
+    static constexpr int MIN_BLOCKS = 2;
+};
+#else
 template <>
 struct RowTune<4096> : RowTune<1024> {};
+#endif
 
 template <int N>
 struct RowCfg {
