@@ -4,14 +4,17 @@ the adjoint split step.  Written twice: once on the CPU oracle's calls (fp64), o
 Test infrastructure only; holds no kernel code.
 
   V1 = A(U0);  V2 = e^{i th1} V1;  V3 = F_c V2;  V4 = e^{i th2} V3;  V5 = F_c^-1 V4
-  loss = 1 - |c|^2 / (P_T P_V),  c = sum conj(T) V5,  T = free-space-propagated input beam
+  loss = 1 - |c|^2 / (P_T P_V),  c = sum conj(T) V5,  T = free-space-propagated input beam   ("overlap", config 4)
   G5 = -(2 / (P_T P_V)) [c T - (|c|^2 / P_V) V5];  G4 = F_c G5;  dl/dth2 = Im(G4 conj V4)
+  loss = (1/N^2) sum |V5 - T|   ("mae": the paper's D2NN loss, "mean absolute error" between the
+         processed field and the free-space result; read as the mean modulus of the complex difference, which is what
+         an L1 loss on complex tensors computes);  G5 = (1/N^2) (V5 - T) / |V5 - T|  (0 where V5 = T)
   G2 = F_c^-1 (e^{-i th2} G4);  dl/dth1 = Im(G2 conj V2);  G1 = e^{-i th1} G2;  G0 = A^H G1 (+ dl/dphi_j)
 """
 import numpy as np
 
 
-def oracle_chain(orc, N, dx, lam, dz, u0, scr32, th1, th2, kw, aperture_radius=None, parallel=False):
+def oracle_chain(orc, N, dx, lam, dz, u0, scr32, th1, th2, kw, aperture_radius=None, parallel=False, loss_kind="overlap"):
     """All quantities for ONE batch of fields on the oracle.  Returns a dict of float64 / complex128 arrays.
     aperture_radius: optional circular aperture applied to A(U0) and to the target; a real 0/1
     mask, so the adjoint applies it again.  parallel: issue the two independent propagations (through the screens,
@@ -34,10 +37,16 @@ def oracle_chain(orc, N, dx, lam, dz, u0, scr32, th1, th2, kw, aperture_radius=N
     c = np.array([np.vdot(T[b], V5[b]) for b in range(B)])
     PT = np.array([np.vdot(T[b], T[b]).real for b in range(B)])
     PV = np.array([np.vdot(V5[b], V5[b]).real for b in range(B)])
-    loss = 1.0 - np.abs(c) ** 2 / (PT * PV)
-    al = -2.0 * c / (PT * PV)
-    be = 2.0 * np.abs(c) ** 2 / (PT * PV * PV)
-    G5 = al[:, None, None] * T + be[:, None, None] * V5
+    if loss_kind == "mae":
+        D = V5 - T
+        mod = np.abs(D)
+        loss = mod.mean(axis=(1, 2))
+        G5 = np.where(mod > 0, D / np.where(mod > 0, mod, 1.0), 0.0) / (N * N)
+    else:
+        loss = 1.0 - np.abs(c) ** 2 / (PT * PV)
+        al = -2.0 * c / (PT * PV)
+        be = 2.0 * np.abs(c) ** 2 / (PT * PV * PV)
+        G5 = al[:, None, None] * T + be[:, None, None] * V5
     G4 = orc.dft2_centered(N, G5)
     g_th2 = orc.phase_grad(N, G4, V4)
     G2 = orc.dft2_centered(N, orc.phase_mul(N, th2, G4, sign=-1.0), inverse=True)
