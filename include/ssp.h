@@ -346,6 +346,12 @@ int ssp_phase_grad(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_g, const f
  * <a,b> = sum conj(a) b.  d_out: dev double [B][4]. */
 int ssp_inner_products(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_a, const float *d_b,
                        double *d_out);
+/* The D2NN training loss of PAPER.md:113 (mean absolute error between the processed field v and the free-space
+ * result t, read as the mean modulus of the complex difference) and its gradient with respect to v:
+ *   d_loss[b] = (1/N^2) sum |v - t|,   d_grad[b] = (v - t) / (N^2 |v - t|)   (0 where v == t; real-pair convention
+ * G = dl/dRe v + i dl/dIm v as everywhere in this library).  d_v, d_t, d_grad: dev complex64 [B][N][N] (d_grad may
+ * alias d_v); d_loss: dev double [B]. */
+int ssp_mae_loss(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_v, const float *d_t, double *d_loss, float *d_grad);
 /* out[b] = alpha[b] a[b] + beta[b] b[b] with per-field complex scalars; h_alpha, h_beta:
  * host double [B][2]; out may alias a or b. */
 int ssp_lincomb(ssp_ctx *ctx, ssp_grid grid, int B, const double *h_alpha, const float *d_a,

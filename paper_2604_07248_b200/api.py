@@ -27,7 +27,7 @@ SYMBOLS = (
     "ssp_create", "ssp_destroy", "ssp_last_error", "ssp_version", "ssp_launch_count",
     "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_make_screens_pair", "ssp_evolve_screens_pair", "ssp_propagate",
     "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_propagate_host", "ssp_phase_mul",
-    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path", "ssp_dz_max", "ssp_place_screens", "ssp_fill_noise", "ssp_philox_words", "ssp_evolve_propagate", "ssp_frame_chunk", "ssp_frame_host",
+    "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path", "ssp_dz_max", "ssp_place_screens", "ssp_fill_noise", "ssp_philox_words", "ssp_evolve_propagate", "ssp_mae_loss", "ssp_frame_chunk", "ssp_frame_host",
     "ssp_profile_enable", "ssp_profile_report",
 )
 
@@ -121,6 +121,7 @@ def load():
     lib.ssp_place_screens.argtypes = [P, P, I, P, I, D, D, D, I, P, P, P, P]
     lib.ssp_adam_update.argtypes = [P, Grid, I, P, D, D, D, D, I, P, P, P]
     lib.ssp_inner_products.argtypes = [P, Grid, I, P, P, P]
+    lib.ssp_mae_loss.argtypes = [P, Grid, I, P, P, P, P]
     lib.ssp_lincomb.argtypes = [P, Grid, I, P, P, P, P, P]
     lib.ssp_profile_enable.argtypes = [P, I]
     lib.ssp_profile_report.argtypes = [P, C.c_char_p, C.c_size_t]
@@ -459,6 +460,15 @@ class Context:
         self._chk(self._lib.ssp_phase_grad(self._h, Grid(N, dx), g.shape[0], _dev(g, torch.complex64),
                                            _dev(u, torch.complex64), _dev(out, torch.float32)))
         return out
+
+    def mae_loss(self, N, dx, v, t, grad=None):
+        """(loss float64 [B] on the device, gradient complex64 [B][N][N]) of mean |v - t|."""
+        B = v.shape[0]
+        loss = torch.empty(B, dtype=torch.float64, device=v.device)
+        grad = torch.empty_like(v) if grad is None else grad
+        self._chk(self._lib.ssp_mae_loss(self._h, Grid(N, dx), B, _dev(v, torch.complex64), _dev(t, torch.complex64),
+                                         _dev(loss, torch.float64), _dev(grad, torch.complex64)))
+        return loss, grad
 
     def inner_products(self, N, dx, a, b, out=None):
         out = torch.empty((a.shape[0], 4), dtype=torch.float64, device=a.device) if out is None else out

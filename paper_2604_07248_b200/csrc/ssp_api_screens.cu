@@ -429,6 +429,15 @@ int ssp_inner_products(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_a, con
     return launch_inner(ctx, grid.N, B, reinterpret_cast<const float2 *>(d_a), reinterpret_cast<const float2 *>(d_b), d_out);
 }
 
+int ssp_mae_loss(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_v, const float *d_t, double *d_loss, float *d_grad)
+{
+    if (!ctx) return SSP_EINVAL;
+    if (!valid_N(grid.N) || B < 1 || !d_v || !d_t || !d_loss || !d_grad) return ctx->fail(SSP_EINVAL, "bad arguments");
+    SSP_CUDA(ctx, cudaSetDevice(ctx->device));
+    return launch_mae(ctx, grid.N, B, reinterpret_cast<const float2 *>(d_v), reinterpret_cast<const float2 *>(d_t), d_loss,
+                      reinterpret_cast<float2 *>(d_grad));
+}
+
 int ssp_lincomb(ssp_ctx *ctx, ssp_grid grid, int B, const double *h_alpha, const float *d_a,
                 const double *h_beta, const float *d_b, float *d_out)
 {

@@ -301,6 +301,7 @@ int launch_phase_mul(ssp_ctx *ctx, int N, int B, const float *theta, float sign,
                      const float2 *in, float2 *out);
 int launch_phase_grad(ssp_ctx *ctx, long long n, const float2 *g, const float2 *u, float *grad);
 int launch_inner(ssp_ctx *ctx, int N, int B, const float2 *a, const float2 *b, double *out);
+int launch_mae(ssp_ctx *ctx, int N, int B, const float2 *v, const float2 *t, double *loss, float2 *g);
 int launch_lincomb(ssp_ctx *ctx, int N, int B, const float2 *coef /*dev [B][2] float2*/,
                    const float2 *a, const float2 *b, float2 *out);
 

@@ -335,6 +335,43 @@ __global__ void __launch_bounds__(256) k_inner(const float2 *__restrict__ A, con
     }
 }
 
+// Mean-absolute-error loss of the D2NN and its field gradient: loss[b] = (1/N^2) sum |v - t|,
+// g = (v - t) / (N^2 |v - t|) (0 where v == t).  Per-block partial sums in double, then one atomic per block.
+__global__ void __launch_bounds__(256) k_mae(const float2 *__restrict__ V, const float2 *__restrict__ Tg, size_t px,
+                                              float inv_px, double *__restrict__ loss, float2 *__restrict__ G)
+{
+    const int b = blockIdx.y;
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < px; i += (size_t)gridDim.x * blockDim.x) {
+        const float2 v = __ldg(V + (size_t)b * px + i), t = __ldg(Tg + (size_t)b * px + i);
+        const float dx = v.x - t.x, dy = v.y - t.y;
+        const float m = sqrtf(fmaf(dx, dx, dy * dy));
+        acc += (double)m;
+        const float s = m > 0.f ? inv_px / m : 0.f;
+        G[(size_t)b * px + i] = make_float2(dx * s, dy * s);
+    }
+    acc = warp_sum(acc);
+    __shared__ double part[8];
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += part[w];
+        atomicAdd(loss + b, s * (double)inv_px);
+    }
+}
+
+int launch_mae(ssp_ctx *ctx, int N, int B, const float2 *v, const float2 *t, double *loss, float2 *g)
+{
+    const size_t px = (size_t)N * N;
+    SSP_CUDA(ctx, cudaMemsetAsync(loss, 0, sizeof(double) * (size_t)B, ctx->stream));
+    int bpf = (int)((px + 256 * 8 - 1) / (256 * 8));
+    k_mae<<<dim3(bpf, B), 256, 0, ctx->stream>>>(v, t, px, (float)(1.0 / (double)px), loss, g);
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
+}
+
 int launch_inner(ssp_ctx *ctx, int N, int B, const float2 *a, const float2 *b, double *out)
 {
     const size_t px = (size_t)N * N;

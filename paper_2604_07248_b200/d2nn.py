@@ -1,7 +1,8 @@
 """Two-mask diffractive receiver trained through the adjoint split step (O9).
 
     V1 = aperture(A(U0));  V2 = e^{i th1} V1;  V3 = F_c V2;  V4 = e^{i th2} V3;  V5 = F_c^-1 V4
-    loss = 1 - |<T, V5>|^2 / (|T|^2 |V5|^2),   T = aperture(A_vacuum(U0))        (Gaussian-overlap loss, Q21)
+    loss = mean |V5 - T|,   T = aperture(A_vacuum(U0))      ("mae": the paper's mean-absolute-error loss; default)
+    loss = 1 - |<T, V5>|^2 / (|T|^2 |V5|^2)                 ("overlap": BASELINE.json config 4's Gaussian-overlap loss, Q21)
 
 A is the split-step propagation through one realisation of the screen stack per field.  Every array operation is
 a call into libssp (propagation, lens transforms, mask multiplies, inner products, gradients, Adam update); this
@@ -32,6 +33,7 @@ class TwoMaskReceiver:
     win_order: int = 16
     win_sigma_frac: float = 0.47
     h_kind: int = api.H_FRESNEL
+    loss: str = "mae"                             # "mae" or "overlap" (config 4)
     lr: float = 0.01
     total_steps: int = 1000                       # length of the one-cycle schedule
     theta: list = field(default_factory=list)     # two fp32 [N][N] masks (constant-phase initialisation)
@@ -70,13 +72,19 @@ class TwoMaskReceiver:
         c, N, dx = self.ctx, self.N, self.dx
         T = self.target(u0) if T is None else T
         V2, V4, V5 = self.forward(u0, screens)
-        ip = c.inner_products(N, dx, T, V5).cpu().numpy()           # <T, V5>, |T|^2, |V5|^2 (fp64)
-        cc = ip[:, 0] + 1j * ip[:, 1]
-        PT, PV = ip[:, 2], ip[:, 3]
-        loss = 1.0 - np.abs(cc) ** 2 / (PT * PV)
-        al = -2.0 * cc / (PT * PV)
-        be = 2.0 * np.abs(cc) ** 2 / (PT * PV * PV)
-        G5 = c.lincomb(N, dx, list(al), T, list(be.astype(complex)), V5)
+        if self.loss == "mae":
+            d_loss, G5 = c.mae_loss(N, dx, V5, T)                    # loss and dl/dV5 in one kernel, nothing on the host
+            loss = d_loss.cpu().numpy()
+        elif self.loss == "overlap":
+            ip = c.inner_products(N, dx, T, V5).cpu().numpy()       # <T, V5>, |T|^2, |V5|^2 (fp64)
+            cc = ip[:, 0] + 1j * ip[:, 1]
+            PT, PV = ip[:, 2], ip[:, 3]
+            loss = 1.0 - np.abs(cc) ** 2 / (PT * PV)
+            al = -2.0 * cc / (PT * PV)
+            be = 2.0 * np.abs(cc) ** 2 / (PT * PV * PV)
+            G5 = c.lincomb(N, dx, list(al), T, list(be.astype(complex)), V5)
+        else:
+            raise ValueError(f"unknown loss {self.loss!r}")
         G4 = c.dft2_centered(N, dx, G5)
         g2 = c.phase_grad(N, dx, G4, V4)
         G2 = c.dft2_centered(N, dx, c.phase_mul(N, dx, self.theta[1], G4, sign=-1.0), inverse=True)
