@@ -461,7 +461,7 @@ def run_ours(args):
         c1.record()
         torch.cuda.synchronize()
         ms = c0.elapsed_time(c1) / n_rep
-        ours_fwd = sum(v["ms"] for k, v in prof.items() if k.startswith(("col_fft", "row_", "small_"))) / args.steps / 2
+        ours_fwd = sum(v["ms"] for k, v in prof.items() if k.startswith(("col_fft", "row_", "small_"))) / n_prof / 2
         cufft = {"what": "forward split steps with torch.fft (cuFFT) + elementwise torch kernels, same batch; comparison only",
                  "screen_steps_per_s": B * S / (ms * 1e-3), "ms_per_forward": ms,
                  "ours_ms_per_forward": ours_fwd, "speedup": ms / ours_fwd if ours_fwd else None}

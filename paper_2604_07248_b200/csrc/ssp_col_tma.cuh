@@ -154,7 +154,8 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
     // Tensor memory as a per-thread constant cache: this thread's 16 twiddle pairs W_N^(t k) and the 32 hy values of
     // its points never change while the CTA walks its tiles, so they are read from the thread's own TMEM lane
     // (tcgen05.ld) instead of through the LSU data pipe, which this kernel saturates first.
-    constexpr bool TM = CFG::TMEM && !H2D;
+    constexpr bool TM = CFG::TMEM;                                  // twiddles; the multiplier too when it is the 1-D table hy
+    constexpr bool TMH = CFG::TMEM && !H2D;
     unsigned &tmem_slot = *reinterpret_cast<unsigned *>(full + 2);     // (a static __shared__ would shift the TMA buffers)
     unsigned taddr = 0;
     if constexpr (TM) {
@@ -168,10 +169,12 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
         const float4 *tw4 = reinterpret_cast<const float4 *>(a.tw + PI::TW1) + t;
 #pragma unroll
         for (int p = 0; p < R1 / 2; ++p) tmem_st4(taddr + 4 * p, __ldg(tw4 + p * (N / R1)));
+        if constexpr (TMH) {
 #pragma unroll
-        for (int q = 0; q < RL; q += 2) {
-            const float2 h0 = __ldg(a.hy + line_index<N, 1, RL>(t, 0, q)), h1 = __ldg(a.hy + line_index<N, 1, RL>(t, 0, q + 1));
-            tmem_st4(taddr + 64 + 2 * q, make_float4(h0.x, h0.y, h1.x, h1.y));
+            for (int q = 0; q < RL; q += 2) {
+                const float2 h0 = __ldg(a.hy + line_index<N, 1, RL>(t, 0, q)), h1 = __ldg(a.hy + line_index<N, 1, RL>(t, 0, q + 1));
+                tmem_st4(taddr + 64 + 2 * q, make_float4(h0.x, h0.y, h1.x, h1.y));
+            }
         }
         tmem_wait_st();
     }
@@ -202,7 +205,7 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
                 if constexpr (TM) fft_line<N, 1, false, false, true, PK>(v, t, sm, TwTmem{a.tw, taddr});
                 else fft_line<N, 1, false, false, true, PK>(v, t, sm, a.tw);
                 if (pass == 0) {
-                    if constexpr (TM) {
+                    if constexpr (TMH) {
 #pragma unroll
                         for (int q = 0; q < RL; q += 4) {
                             float4 ha, hb;

@@ -156,7 +156,10 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
         for (int p = 0; p < PI::R1 / 2; ++p) tmem_st4(taddr + 4 * p, __ldg(tw4 + p * (N / PI::R1)));
 #pragma unroll
         for (int q = 0; q < PI::R1; q += 2) {
-            const float2 h0 = __ldg(a.hx + line_index<N, 0, PI::R1>(t, 0, q)), h1 = __ldg(a.hx + line_index<N, 0, PI::R1>(t, 0, q + 1));
+            // (no hx -- angular spectrum: the column kernel applies the whole H -- caches the factor 1)
+            const float2 one = make_float2(1.f, 0.f);
+            const float2 h0 = a.hx ? __ldg(a.hx + line_index<N, 0, PI::R1>(t, 0, q)) : one;
+            const float2 h1 = a.hx ? __ldg(a.hx + line_index<N, 0, PI::R1>(t, 0, q + 1)) : one;
             tmem_st4(taddr + 64 + 2 * q, make_float4(h0.x, h0.y, h1.x, h1.y));
         }
         tmem_wait_st();

@@ -36,7 +36,6 @@ static int launch_row_x(ssp_ctx *ctx, const RowArgs &a)
     constexpr bool TM = CFG::TMEM && FIRST && SECOND && !GENERIC;           // persistent form (ssp_kernels.cuh)
     int grid = a.n_lines / CFG::LPB;
     if (TM) {
-        if (!a.hx) return ctx->fail(SSP_EINVAL, "persistent row kernel without hx");
         const int resident = ctx->num_sms * CFG::MIN_BLOCKS;
         if (grid > resident) grid = resident;
     }
@@ -59,16 +58,13 @@ static int launch_row_n(ssp_ctx *ctx, const RowArgs &a)
     if (a.ycol) {                                                 // fused screen synthesis: the common 1024^2 kernels only
         if constexpr (N == 1024 && FIRST) {
             const bool ok = !a.phi && a.win_on && !a.grad && !a.plane_out && !a.pre && a.in_swapped &&
-                            ((a.win_map != nullptr) == WinMap<N>::value) && (!SECOND || a.hx);
+                            ((a.win_map != nullptr) == WinMap<N>::value);
             if (!ok) return ctx->fail(SSP_EUNSUPPORTED, "fused screen synthesis needs the common split step (window on, Fresnel H, nothing saved)");
             return launch_row_x<N, FIRST, SECOND, false, true>(ctx, a);
         } else return ctx->fail(SSP_EUNSUPPORTED, "fused screen synthesis is built for N = 1024");
     }
-    // (the persistent tensor-memory form of the common kernel caches hx per thread: without hx -- angular spectrum --
-    // the generic kernel runs)
     const bool common = a.phi && a.win_on && !a.grad && !a.plane_out && !a.pre && (!MID || a.in_swapped) &&
-                        ((a.win_map != nullptr) == WinMap<N>::value) &&
-                        (!(RowCfg<N>::TMEM && FIRST && SECOND) || a.hx);
+                        ((a.win_map != nullptr) == WinMap<N>::value);
     if (common) return launch_row_x<N, FIRST, SECOND, false>(ctx, a);
     return launch_row_x<N, FIRST, SECOND, true>(ctx, a);
 }
