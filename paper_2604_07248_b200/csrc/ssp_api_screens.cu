@@ -229,6 +229,19 @@ int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
         flt.eta = (float)(psd->eta > 0 ? psd->eta : pow(1e-18 / psd->eps, 0.25));
         flt.w = (float)psd->w;
     }
+    // warp-uniform half of the subharmonic phasors (ScreenRowArgs::e2), in double like the other tables
+    ScreenRowArgs rproto{};
+    {
+        const int RLr = row_last_radix(N);
+        double dfp = df;
+        for (int p = 0; p < n_sh; ++p) {
+            dfp /= 3.0;
+            for (int q = 0; q < RLr && q < 32; ++q) {
+                const double ang = 2.0 * kPi * dfp * (double)q * (double)(N / RLr) * grid.dx;
+                rproto.e2[p][q] = make_float2((float)cos(ang), (float)sin(ang));
+            }
+        }
+    }
     float2 *inter = reinterpret_cast<float2 *>(ws + L.inter);
     const int nscr = B * S;
     for (int g0 = 0; g0 < nscr; g0 += L.chunk) {
@@ -246,7 +259,7 @@ int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
         c.tw = twc;
         if (int rc = launch_screen_col(ctx, N, c)) return rc;
         if (ycol_out) continue;                                   // K3 runs inside the propagation's row kernels
-        ScreenRowArgs r{};
+        ScreenRowArgs r = rproto;
         r.in = inter;
         r.screens = d_screens + (size_t)g0 * px;
         r.nscr = n; r.n_sh = n_sh;

@@ -254,7 +254,12 @@ struct ScreenRowArgs {
     const float *sh_mean;     // [nscr][2]: analytic mean of phi_lo of the real-part and imaginary-part screens
     const float2 *ex;         // [n_sh][N] exp(i 2 pi df_p x)
     const float2 *tw;
+    // exp(i 2 pi df_p q (N / RL) dx), q < RL (the row plan's last radix): pixel ix = q N/RL + m of a thread splits into
+    // a per-thread phasor ex[p][m] and this warp-uniform one, read from the constant bank of the kernel arguments
+    // instead of one table value per level and pixel through the LSU (the pipe this kernel saturates first)
+    float2 e2[8][32];
 };
+int row_last_radix(int N);    // RL of the row plan at grid N
 // argument checks of ssp_make_screens / ssp_evolve_screens (ssp_api_screens.cu), for callers that must validate
 // before they queue anything (ssp_frame_host)
 int check_screen_args(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda, int B, int S, const double *cn2,

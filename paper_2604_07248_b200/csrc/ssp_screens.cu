@@ -232,15 +232,22 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS + (N
             const float ci = d[0].y + d[2].y, si = d[2].x - d[0].x;
             cst += d[1].x;
             if constexpr (PAIR) cst_im += d[1].y;
-            const float2 *exp_ = a.ex + (size_t)p * N + t;
+            // ca cos(al + be) + sa sin(al + be) = cos(be) (ca cos al + sa sin al) + sin(be) (sa cos al - ca sin al): al from the
+            // thread's own phasor ex[p][m], be = the warp-uniform phasor e2[p][q] (constant bank): still 2 FMAs per level
+            // and pixel, but no per-pixel table read
+            static_assert(RL <= 32, "e2 holds 32 phasors per level");
 #pragma unroll
-            for (int i = 0; i < E / RL; ++i)
+            for (int i = 0; i < E / RL; ++i) {
+                const float2 e1 = __ldg(a.ex + (size_t)p * N + t + T * i);
+                const float A = fmaf(ca, e1.x, sa * e1.y), Bq = fmaf(sa, e1.x, -ca * e1.y);
+                const float Ai = fmaf(ci, e1.x, si * e1.y), Bi = fmaf(si, e1.x, -ci * e1.y);
 #pragma unroll
                 for (int q = 0; q < RL; ++q) {
-                    const float2 ex = __ldg(exp_ + (line_index<N, 0, RL>(t, i, q) - t));
-                    v[i * RL + q].x = fmaf(ca, ex.x, fmaf(sa, ex.y, v[i * RL + q].x));
-                    if constexpr (PAIR) v[i * RL + q].y = fmaf(ci, ex.x, fmaf(si, ex.y, v[i * RL + q].y));
+                    const float2 e = a.e2[p][q];
+                    v[i * RL + q].x = fmaf(A, e.x, fmaf(Bq, e.y, v[i * RL + q].x));
+                    if constexpr (PAIR) v[i * RL + q].y = fmaf(Ai, e.x, fmaf(Bi, e.y, v[i * RL + q].y));
                 }
+            }
         }
     }
     float *dst = a.screens + line * N;
@@ -374,6 +381,23 @@ int launch_screen_col(ssp_ctx *ctx, int N, const ScreenColArgs &a)
     }
     SSP_DISPATCH_N(N, (launch_screen_col_n<NN>(ctx, a)));
 }
+int row_last_radix(int N)
+{
+    switch (N) {
+    case 8: return PlanInfo<8, 0>::RL;
+    case 16: return PlanInfo<16, 0>::RL;
+    case 32: return PlanInfo<32, 0>::RL;
+    case 64: return PlanInfo<64, 0>::RL;
+    case 128: return PlanInfo<128, 0>::RL;
+    case 256: return PlanInfo<256, 0>::RL;
+    case 512: return PlanInfo<512, 0>::RL;
+    case 1024: return PlanInfo<1024, 0>::RL;
+    case 2048: return PlanInfo<2048, 0>::RL;
+    case 4096: return PlanInfo<4096, 0>::RL;
+    default: return 1;
+    }
+}
+
 int launch_screen_row(ssp_ctx *ctx, int N, const ScreenRowArgs &a)
 {
     SSP_DISPATCH_N(N, (launch_screen_row_n<NN>(ctx, a)));
