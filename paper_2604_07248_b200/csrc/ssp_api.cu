@@ -146,6 +146,15 @@ int run_small(ssp_ctx *ctx, int N, int B, const std::vector<SmallStep> &steps, i
     a.win_on = win.win_on; a.win_qs = win.win_qs; a.win_half_order = win.win_half_order;
     a.tw_row = tw; a.tw_col = twc;
     if (st && st->stats) { a.stats = st->stats; a.roi_lo = st->lo; a.roi_hi = st->hi; a.roi_n = st->n; a.dx = st->dx; }
+    if (cluster_path_available(N, B)) {                           // one field over a cluster of 8 CTAs
+        if (a.stats) {
+            if (int rc = ensure_scratch(ctx, sizeof(double) * 9 * (size_t)B * N)) return rc;
+            a.stats_acc = reinterpret_cast<double *>(ctx->scratch);
+        }
+        if (int rc = launch_cluster(ctx, N, B, a)) return rc;
+        if (a.stats) return launch_stats_final(ctx, B, N, a.dx, a.roi_n, a.stats_acc, a.stats);
+        return SSP_OK;
+    }
     return launch_small(ctx, N, B, a);
 }
 
@@ -162,9 +171,9 @@ int drain_pipeline(ssp_ctx *ctx, int rc)
     return rc;
 }
 
-bool small_ok(int N, int h_kind, int n_steps, const void *planes)
+bool small_ok(int N, int B, int h_kind, int n_steps, const void *planes)
 {
-    return small_path_available(N) && h_kind == SSP_H_FRESNEL && !planes &&
+    return (small_path_available(N) || cluster_path_available(N, B)) && h_kind == SSP_H_FRESNEL && !planes &&
            sizeof(SmallStep) * (size_t)(n_steps + 1) <= kSmallStepBytes;
 }
 
@@ -198,7 +207,7 @@ int propagate_core(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0, int h_
     long long roi_n = 0;
     if (d_stats) stats_roi(N, roi_frac, &roi_lo, &roi_hi, &roi_n);
 
-    if (!fused && small_ok(N, h_kind, n_steps, d_planes)) { // whole stack in one kernel, field resident in shared memory
+    if (!fused && small_ok(N, B, h_kind, n_steps, d_planes)) { // whole stack in one kernel, field resident in shared memory
         std::vector<SmallStep> ops(n_steps + 1);
         RowArgs w{};
         fill_window(w, win, N);
@@ -340,7 +349,7 @@ int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0,
     if (int rc = get_twiddles(ctx, N, 1, &twc)) return rc;
     float2 *g = reinterpret_cast<float2 *>(d_g_in);
 
-    if (small_ok(N, h_kind, n_steps, d_planes)) { // on-chip: op 0 = plane n_steps, then (column pass, plane j-1) for j = n_steps..1
+    if (small_ok(N, B, h_kind, n_steps, d_planes)) { // on-chip: op 0 = plane n_steps, then (column pass, plane j-1) for j = n_steps..1
         std::vector<SmallStep> ops(n_steps + 1);
         RowArgs w{};
         fill_window(w, win, N);

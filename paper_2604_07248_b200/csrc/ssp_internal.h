@@ -207,7 +207,8 @@ struct SmallStep {               // one row pass, preceded (except op 0) by the 
 struct SmallArgs {
     const float2 *in;
     float2 *out;
-    ssp_stats *stats;            // optional: beam statistics of the output fields, finished inside the kernel
+    ssp_stats *stats;            // optional: beam statistics of the output fields, finished inside the kernel (k_small)
+    double *stats_acc;           // optional (k_cluster): one record of the nine accumulators per row, [B][N][ACC_N]
     int roi_lo, roi_hi;
     long long roi_n;
     double dx;
@@ -220,6 +221,9 @@ struct SmallArgs {
 };
 bool small_path_available(int N);
 int launch_small(ssp_ctx *ctx, int N, int B, const SmallArgs &a);
+// the same with one field split over a cluster of 8 CTAs through distributed shared memory (ssp_cluster.cu)
+bool cluster_path_available(int N, int B);
+int launch_cluster(ssp_ctx *ctx, int N, int B, const SmallArgs &a);
 
 // ---- screens (ssp_screens.cu) ------------------------------------------------------
 struct ScreenFilter {
