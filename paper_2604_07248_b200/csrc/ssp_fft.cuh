@@ -209,7 +209,8 @@ SSP_PLAN(4096, 1, 32, 4, 32, 32);
 SSP_PLAN(8, 2, 8, 1, 1, 8);        SSP_PLAN(16, 2, 16, 1, 1, 16);     SSP_PLAN(32, 2, 32, 1, 1, 32);
 SSP_PLAN(64, 2, 8, 8, 1, 8);       SSP_PLAN(128, 2, 16, 8, 1, 16);    SSP_PLAN(256, 2, 16, 16, 1, 16);
 SSP_PLAN(512, 2, 32, 16, 1, 32);   SSP_PLAN(1024, 2, 32, 32, 1, 32);
-SSP_PLAN(2048, 2, 32, 2, 32, 32);   SSP_PLAN(4096, 2, 32, 16, 8, 32);
+SSP_PLAN(2048, 2, 32, 2, 32, 32);
+SSP_PLAN(4096, 2, 32, 16, 8, 32);   // ((64,64) measured here: 3387 -> 1894 GB/s: this kernel lives on resident warps)
 #undef SSP_PLAN
 
 template <int N, int V>

@@ -98,7 +98,7 @@ struct ColCfg {
     static constexpr int THREADS = T * C;
     static constexpr size_t SMEM = (PlanInfo<N, V_>::NSTAGE == 1) ? 0
         : sizeof(float2) * (size_t)C * PlanInfo<N, V_>::LINE_ELEMS;
-    static constexpr int MIN_BLOCKS = (THREADS <= 256) ? 2 : 1;
+    static constexpr int MIN_BLOCKS = (THREADS <= 256 && PlanInfo<N, V_>::E <= 32) ? 2 : 1;   // 64 points per thread: 255 registers
 };
 
 // ---- shared-memory exchange accessors -------------------------------------------------
