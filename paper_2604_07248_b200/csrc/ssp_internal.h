@@ -46,6 +46,9 @@ struct ssp_ctx {
     size_t scratch_bytes = 0;
     std::vector<void *> owned;                   // misc device allocations freed at destroy
     void *encode_tiled = nullptr;                // cuTensorMapEncodeTiled, resolved through the runtime
+    // TMA descriptors by (base pointer, columns, rows, box): a split step re-launches the column kernel on the same
+    // buffers n_steps times, so the host-side encode runs once per buffer and shape; dropped at 256 entries
+    std::map<std::tuple<const void *, size_t, size_t, int, int>, CUtensorMap> tmaps;
     void *small_steps = nullptr;                 // device list of step descriptors of the on-chip path (16 KB)
     // ssp_propagate_host: copy streams and events of the chunked host <-> device pipeline (created on first use)
     cudaStream_t copy_in = nullptr, copy_out = nullptr;
@@ -126,7 +129,9 @@ int get_h2d_table(ssp_ctx *ctx, const HKey &key, const float2 **out);
 int get_sign_table(ssp_ctx *ctx, int N, const float2 **out);
 int ensure_scratch(ssp_ctx *ctx, size_t bytes);
 // TMA descriptor of a row-major buffer of complex64: `cols` elements per row, `rows` rows, boxes of
-// box_cols x box_rows elements (no swizzle).  Encoded on the host for every call: the buffers are the caller's.
+// box_cols x box_rows elements (no swizzle).  Encoded on the host once per (buffer, shape, box) and cached in the context
+// (the descriptor holds only the address and the geometry, so a caller who frees and re-allocates the same address with
+// the same shape gets the same, still valid, descriptor).
 int make_tmap_c64(ssp_ctx *ctx, const void *base, size_t cols, size_t rows, int box_cols, int box_rows,
                   CUtensorMap *out);
 bool valid_N(int N);

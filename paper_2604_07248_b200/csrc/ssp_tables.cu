@@ -171,6 +171,10 @@ int make_tmap_c64(ssp_ctx *ctx, const void *base, size_t cols, size_t rows, int 
             return ctx->fail(SSP_EUNSUPPORTED, "the driver does not export cuTensorMapEncodeTiled");
         ctx->encode_tiled = p;
     }
+    const auto key = std::make_tuple(base, cols, rows, box_cols, box_rows);
+    auto it = ctx->tmaps.find(key);
+    if (it != ctx->tmaps.end()) { *out = it->second; return SSP_OK; }
+    if (ctx->tmaps.size() >= 256) ctx->tmaps.clear();             // descriptors are values: nothing to free
     // complex64 as pairs of fp32: the inner dimension counts floats
     const cuuint64_t dims[2] = {(cuuint64_t)cols * 2, (cuuint64_t)rows};
     const cuuint64_t strides[1] = {(cuuint64_t)cols * sizeof(float2)};
@@ -181,6 +185,7 @@ int make_tmap_c64(ssp_ctx *ctx, const void *base, size_t cols, size_t rows, int 
         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return ctx->fail(SSP_ECUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    ctx->tmaps[key] = *out;
     return SSP_OK;
 }
 

@@ -66,15 +66,16 @@ class TwoMaskReceiver:
         V5 = c.dft2_centered(N, dx, V4, inverse=True)
         return V2, V4, V5
 
-    def loss_and_grads(self, u0, screens, T=None, input_grad=False):
-        """Per-field losses (numpy fp64 [B]) and d loss / d theta_1, d theta_2 per field (fp32 [B][N][N]);
-        with input_grad also G0 = A^H(...) (the adjoint split step through the screen stack)."""
+    def loss_and_grads(self, u0, screens, T=None, input_grad=False, device_loss=False):
+        """Per-field losses (numpy fp64 [B]; with device_loss and the "mae" loss: the fp64 CUDA tensor, no host
+        synchronisation) and d loss / d theta_1, d theta_2 per field (fp32 [B][N][N]); with input_grad also
+        G0 = A^H(...) (the adjoint split step through the screen stack)."""
         c, N, dx = self.ctx, self.N, self.dx
         T = self.target(u0) if T is None else T
         V2, V4, V5 = self.forward(u0, screens)
         if self.loss == "mae":
             d_loss, G5 = c.mae_loss(N, dx, V5, T)                    # loss and dl/dV5 in one kernel, nothing on the host
-            loss = d_loss.cpu().numpy()
+            loss = d_loss if device_loss else d_loss.cpu().numpy()
         elif self.loss == "overlap":
             ip = c.inner_products(N, dx, T, V5).cpu().numpy()       # <T, V5>, |T|^2, |V5|^2 (fp64)
             cc = ip[:, 0] + 1j * ip[:, 1]
@@ -103,11 +104,14 @@ class TwoMaskReceiver:
             return self.lr / 25 + (self.lr - self.lr / 25) * 0.5 * (1 - math.cos(math.pi * s / up))
         return self.lr / 2500 + (self.lr - self.lr / 2500) * 0.5 * (1 + math.cos(math.pi * min(1.0, (s - up) / max(1, n - up))))
 
-    def train_step(self, u0, screens, T=None):
-        """One epoch: a batch of fresh turbulence realisations, gradients of the mean loss, one Adam step per mask."""
-        loss, g1, g2, _ = self.loss_and_grads(u0, screens, T)
+    def train_step(self, u0, screens, T=None, sync=True):
+        """One epoch: a batch of fresh turbulence realisations, gradients of the mean loss, one Adam step per mask.
+        sync=False (mean-absolute-error loss): nothing of the epoch touches the host -- the mean loss comes back as a
+        CUDA tensor to be read whenever the caller wants a progress figure."""
+        dev = (not sync) and self.loss == "mae"
+        loss, g1, g2, _ = self.loss_and_grads(u0, screens, T, device_loss=dev)
         lr = self.one_cycle_lr()
         self.t += 1
         for th, m, v, g in zip(self.theta, self._m, self._v, (g1, g2)):
             self.ctx.adam_update(self.N, self.dx, g, lr, self.t, m, v, th)
-        return float(loss.mean())
+        return loss.mean() if dev else float(loss.mean())
