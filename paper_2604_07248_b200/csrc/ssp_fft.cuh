@@ -349,7 +349,9 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const TWP twp
         constexpr int P2 = Rc, P1 = 2 * Rc + 1;
 #pragma unroll
         for (int k = 0; k < Ra; k += 2) {
-            const float4 w = __ldg(tw4 + (k / 2) * (N / Ra));
+            float4 w;
+            if constexpr (TW_TMEM) w = tmem_ld4(twp.taddr + 2 * k);
+            else w = __ldg(tw4 + (k / 2) * (N / Ra));
             float2 x[2] = {v[k], v[k + 1]};
             if (k > 0) x[0] = cmul_c<INV, PK>(x[0], make_float2(w.x, w.y));
             x[1] = cmul_c<INV, PK>(x[1], make_float2(w.z, w.w));

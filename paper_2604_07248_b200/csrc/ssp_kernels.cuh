@@ -28,6 +28,19 @@ __device__ __forceinline__ float2 swap_if(float2 x) { return SWAP ? make_float2(
 template <int N>
 struct SYM_PLAN { static constexpr bool value = PlanInfo<N, 0>::SYM && PlanInfo<N, 0>::NSTAGE == 2 && PlanInfo<N, 0>::E == PlanInfo<N, 0>::R1; };
 
+// Tensor-memory layout of the persistent row kernel: a thread's lane holds 2E words of twiddle pairs, then 2E words of hx;
+// warps w and w + 4 of a CTA share a lane quadrant and take consecutive column blocks of 4E.
+template <int N>
+struct RowTmem {
+    using PI = PlanInfo<N, 0>;
+    static constexpr int E = PI::E;
+    static constexpr int HXOFF = 2 * E, CW = 4 * E;
+    static constexpr int GROUPS = (RowCfg<N>::THREADS + 127) / 128;
+    static constexpr int NEED = GROUPS * CW;
+    static constexpr int COLS = NEED <= 32 ? 32 : (NEED <= 64 ? 64 : (NEED <= 128 ? 128 : (NEED <= 256 ? 256 : 512)));
+    static constexpr bool OK = PI::SYM && PI::E == PI::R1 && PI::NSTAGE >= 2 && (RowCfg<N>::THREADS % 32 == 0);
+};
+
 // Pointwise stage in real space on a line held in the layout strided by RL.  SWAPPED: the registers
 // hold the field re/im-swapped (it came out of an inverse transform run by the forward code); the
 // result is in plain form either way.  GENERIC = false is the common split step (screen and window
@@ -144,13 +157,13 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
     static_assert(!FUSE || MidSwapped<N>::value, "fused screens: the column kernel hands the field over swapped");
     unsigned taddr = 0;
     if constexpr (TM) {
-        static_assert(!TM || (CFG::THREADS == 128 && T == 32 && SYM_PLAN<N>::value), "one warp per row, four rows per CTA");
+        static_assert(!TM || RowTmem<N>::OK, "symmetric plan with one first-stage butterfly per thread");
         unsigned *slot = reinterpret_cast<unsigned *>(smem_raw + CFG::SMEM);
-        if (tid < 32) tmem_alloc(slot, 128);
+        if (tid < 32) tmem_alloc(slot, RowTmem<N>::COLS);
         tmem_fence_before_sync();
         __syncthreads();
         tmem_fence_after_sync();
-        taddr = *slot + ((unsigned)(tid & ~31) << 16);
+        taddr = *slot + ((unsigned)(tid & 96) << 16) + (unsigned)(tid / 128) * RowTmem<N>::CW;
         const float4 *tw4 = reinterpret_cast<const float4 *>(a.tw + PI::TW1) + t;
 #pragma unroll
         for (int p = 0; p < PI::R1 / 2; ++p) tmem_st4(taddr + 4 * p, __ldg(tw4 + p * (N / PI::R1)));
@@ -160,7 +173,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
             const float2 one = make_float2(1.f, 0.f);
             const float2 h0 = a.hx ? __ldg(a.hx + line_index<N, 0, PI::R1>(t, 0, q)) : one;
             const float2 h1 = a.hx ? __ldg(a.hx + line_index<N, 0, PI::R1>(t, 0, q + 1)) : one;
-            tmem_st4(taddr + 64 + 2 * q, make_float4(h0.x, h0.y, h1.x, h1.y));
+            tmem_st4(taddr + RowTmem<N>::HXOFF + 2 * q, make_float4(h0.x, h0.y, h1.x, h1.y));
         }
         tmem_wait_st();
     }
@@ -367,7 +380,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
 #pragma unroll
         for (int q = 0; q < ROUT; q += 4) {
             float4 ha, hb;
-            tmem_ld8(taddr + 64 + 2 * q, ha, hb);
+            tmem_ld8(taddr + RowTmem<N>::HXOFF + 2 * q, ha, hb);
             const float2 h[4] = {make_float2(ha.x, ha.y), make_float2(ha.z, ha.w), make_float2(hb.x, hb.y), make_float2(hb.z, hb.w)};
 #pragma unroll
             for (int e = 0; e < 4; ++e) dst[line_index<N, 0, ROUT>(t, 0, q + e)] = cmul_c<false, PK>(v[q + e], h[e]);
@@ -390,7 +403,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
     if constexpr (TM) {
         tmem_fence_before_sync();
         __syncthreads();
-        if (tid < 32) tmem_dealloc(*reinterpret_cast<unsigned *>(smem_raw + CFG::SMEM), 128);
+        if (tid < 32) tmem_dealloc(*reinterpret_cast<unsigned *>(smem_raw + CFG::SMEM), RowTmem<N>::COLS);
     }
 }
 

@@ -25,6 +25,9 @@ struct RowTune<1024> {
     static constexpr int MAX_THREADS = 128;
     static constexpr int MIN_BLOCKS = 3;
 };
+#ifndef SSP_ROW512_TMEM
+#define SSP_ROW512_TMEM 1
+#endif
 template <>
 struct RowTune<2048> {
     static constexpr int MAX_THREADS = 64;
@@ -61,7 +64,9 @@ struct RowCfg {
 #ifndef SSP_ROW1024_TMEM
 #define SSP_ROW1024_TMEM 1
 #endif
-    static constexpr bool TMEM = (N == 1024) && SSP_ROW1024_TMEM;
+    // measured: 1024 +4 % (+1.3 % more with the next-row prefetch), 512 +12 % (3907 -> 4381 GB/s); 2048 as two rows per
+    // 128-thread CTA -4 % and 4096 -10 % (both spill at 168 registers), so those keep the one-row-per-CTA kernels
+    static constexpr bool TMEM = (N == 1024 && SSP_ROW1024_TMEM) || (N == 512 && SSP_ROW512_TMEM);
 };
 
 // Between the column kernel and the row kernel of a split step the field may stay re/im-swapped: the column
