@@ -89,8 +89,23 @@ struct ColTmaCfg {
 #ifndef SSP_COL1024_TMEM
 #define SSP_COL1024_TMEM 1
 #endif
-    static constexpr bool TMEM = (N == 1024) && SSP_COL1024_TMEM && NBUF == 2 && PlanInfo<N, 1>::NSTAGE == 2 && PlanInfo<N, 1>::SYM;
-    static constexpr int TMEM_COLS = 128;                             // 64: twiddle pairs, 64: hy of this thread's 32 points
+// measured at 2048 / 4096 (one tile buffer, so the persistent loop reloads it only after its own store has drained):
+// 3735 -> 3375 GB/s and 3161 -> 2590 GB/s -- fresh CTAs overlap one tile's store with the next one's load better than
+// the single-buffer loop does, and that outweighs the LSU relief; off
+#ifndef SSP_COL2048_TMEM
+#define SSP_COL2048_TMEM 0
+#endif
+#ifndef SSP_COL4096_TMEM
+#define SSP_COL4096_TMEM 0
+#endif
+    static constexpr bool TMEM = ((N == 1024 && SSP_COL1024_TMEM) || (N == 2048 && SSP_COL2048_TMEM) || (N == 4096 && SSP_COL4096_TMEM)) &&
+                                 PlanInfo<N, 1>::SYM && PlanInfo<N, 1>::E == PlanInfo<N, 1>::R1 && (THREADS % 128 == 0);
+    // per thread: 2E words of twiddle pairs, then 2E words of hy; warps w and w + 4 take consecutive column blocks of 4E
+    static constexpr int TM_HOFF = 2 * PlanInfo<N, 1>::E, TM_CW = 4 * PlanInfo<N, 1>::E;
+    static constexpr int TM_NEED = (THREADS / 128) * TM_CW;
+    static constexpr int TMEM_COLS = TM_NEED <= 128 ? 128 : (TM_NEED <= 256 ? 256 : 512);
+    // persistent even with one buffer (the tile loop reloads the buffer after its store has drained) when TMEM is on
+    static constexpr bool PERSIST = (NBUF == 2) || TMEM;
 };
 
 // Screen generator (K1+K2): one tile per CTA, one buffer (noise -> exchange -> result) plus a second one only
@@ -165,7 +180,7 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
     __syncthreads();
     if constexpr (TM) {
         tmem_fence_after_sync();
-        taddr = tmem_slot + ((unsigned)(tid & ~31) << 16);            // lanes 32 w .. 32 w + 31 belong to warp w
+        taddr = tmem_slot + ((unsigned)(tid & 96) << 16) + (unsigned)(tid / 128) * CFG::TM_CW;   // lane quadrant w % 4, column block w / 4
         const float4 *tw4 = reinterpret_cast<const float4 *>(a.tw + PI::TW1) + t;
 #pragma unroll
         for (int p = 0; p < R1 / 2; ++p) tmem_st4(taddr + 4 * p, __ldg(tw4 + p * (N / R1)));
@@ -173,7 +188,7 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
 #pragma unroll
             for (int q = 0; q < RL; q += 2) {
                 const float2 h0 = __ldg(a.hy + line_index<N, 1, RL>(t, 0, q)), h1 = __ldg(a.hy + line_index<N, 1, RL>(t, 0, q + 1));
-                tmem_st4(taddr + 64 + 2 * q, make_float4(h0.x, h0.y, h1.x, h1.y));
+                tmem_st4(taddr + CFG::TM_HOFF + 2 * q, make_float4(h0.x, h0.y, h1.x, h1.y));
             }
         }
         tmem_wait_st();
@@ -209,7 +224,7 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
 #pragma unroll
                         for (int q = 0; q < RL; q += 4) {
                             float4 ha, hb;
-                            tmem_ld8(taddr + 64 + 2 * q, ha, hb);
+                            tmem_ld8(taddr + CFG::TM_HOFF + 2 * q, ha, hb);
                             const float2 h[4] = {make_float2(ha.x, ha.y), make_float2(ha.z, ha.w), make_float2(hb.x, hb.y),
                                                  make_float2(hb.z, hb.w)};
 #pragma unroll
@@ -257,6 +272,10 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
             for (int j = 0; j < CFG::BOXES; ++j)
                 tma_store_2d(&tm_out, 2 * col0, b * N + j * CFG::BOX_ROWS, tile_s + j * CFG::BOX_ROWS * C);
             tma_store_commit();
+            if (CFG::NBUF == 1 && tile + (int)gridDim.x < a.ntiles) {   // one buffer, persistent: reload it once the store has read it
+                tma_store_wait_read();
+                issue_load(tile + gridDim.x, 0);
+            }
         }
     }
     if (tid == 0) tma_store_wait_read();

@@ -128,7 +128,7 @@ static int launch_col_tma_x(ssp_ctx *ctx, const ColArgs &a)
     const int ntiles = a.B * (N / CFG::C);
     const int resident = ctx->num_sms * CFG::MIN_BLOCKS;
     // two buffers: persistent CTAs walk the tiles; one buffer: one tile per CTA
-    const int grid = (CFG::NBUF == 2 && ntiles > resident) ? resident : ntiles;
+    const int grid = (CFG::PERSIST && ntiles > resident) ? resident : ntiles;
     ColTmaArgs ta{a.hy, a.h2d, a.tw, ntiles};
     ctx->prof_begin("col_fft_h_ifft", 16.0 * (double)a.B * N * N);
     kern<<<grid, CFG::THREADS, CFG::SMEM, ctx->stream>>>(tm_in, tm_out, ta);
