@@ -257,6 +257,21 @@ int ssp_propagate_adjoint(ssp_ctx *ctx, ssp_grid grid, double lambda, double n0,
 int ssp_beam_stats(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_field, double roi_frac,
                    ssp_stats *d_stats, float *d_mean, float *d_M2, long long *count);
 
+/* ssp_beam_stats without any allocation, for callers that may not call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  Same statistics (O8; PAPER.md:423 S25) of B fields
+ * d_field (dev c64 [B][N][N], 16-byte aligned) into d_stats (dev ssp_stats[B], required); no ensemble accumulation.
+ * The block partials live in a file-scope device array of SSP_STATS_STATIC_BYTES that every GPU loading the library
+ * holds until the process exits, instead of the context's growable scratch: the call performs no cudaMalloc,
+ * cudaFree or allocating library call.  Limit: B <= SSP_STATS_STATIC_MAX_FIELDS per call (SSP_EINVAL with a message
+ * beyond it: split the batch, or use ssp_beam_stats); any N the library supports.  One kernel, enqueued on the
+ * context's stream after a memset of the array's ticket counters; sums and their order are those of ssp_beam_stats.
+ * The array is shared by ALL contexts and streams of the process on that GPU: calls that overlap on the GPU race on it
+ * (serialise them on one stream or with events). */
+#define SSP_STATS_STATIC_MAX_FIELDS 1024
+#define SSP_STATS_STATIC_BYTES (2 * SSP_STATS_STATIC_MAX_FIELDS * 9 * 8 + SSP_STATS_STATIC_MAX_FIELDS * 4)   /* 148 KiB */
+int ssp_beam_stats_static(ssp_ctx *ctx, ssp_grid grid, int B, const float *d_field, double roi_frac,
+                          ssp_stats *d_stats);
+
 /* End-to-end form of ssp_propagate with HOST buffers: copies field and screens to the
  * device buffers given (d_field [B][N][N] c64, d_screens as above), propagates, copies
  * the output field and statistics back, and synchronises the stream.  h_* pointers are

@@ -26,7 +26,7 @@ OK, EINVAL, EUNSUPPORTED, EWORKSPACE, ECUDA = 0, -1, -2, -3, -4
 SYMBOLS = (
     "ssp_create", "ssp_destroy", "ssp_last_error", "ssp_version", "ssp_launch_count",
     "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_make_screens_pair", "ssp_evolve_screens_pair", "ssp_propagate",
-    "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_propagate_host", "ssp_phase_mul",
+    "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_beam_stats_static", "ssp_propagate_host", "ssp_phase_mul",
     "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path", "ssp_dz_max", "ssp_place_screens", "ssp_fill_noise", "ssp_philox_words", "ssp_evolve_propagate", "ssp_mae_loss", "ssp_frame_chunk", "ssp_frame_host",
     "ssp_profile_enable", "ssp_profile_report",
 )
@@ -68,6 +68,7 @@ class Stats(C.Structure):
 
 STATS_BYTES = C.sizeof(Stats)
 STAT_FIELDS = tuple(n for n, _ in Stats._fields_)
+STATS_STATIC_MAX_FIELDS = 1024     # SSP_STATS_STATIC_MAX_FIELDS of include/ssp.h
 
 _lib = None
 
@@ -102,6 +103,7 @@ def load():
                                          P, D, P, P, C.c_size_t]
     lib.ssp_propagate_adjoint.argtypes = [P, Grid, D, D, I, I, I, P, P, L, I, Window, P, P, P, P, P, C.c_size_t]
     lib.ssp_beam_stats.argtypes = [P, Grid, I, P, D, P, P, P, C.POINTER(L)]
+    lib.ssp_beam_stats_static.argtypes = [P, Grid, I, P, D, P]
     lib.ssp_propagate_host.argtypes = [P, Grid, D, D, I, I, I, P, P, L, I, Window, P, P, P, D, P, P, P, P,
                                        C.c_size_t]
     lib.ssp_frame_chunk.argtypes = [I]
@@ -386,6 +388,13 @@ class Context:
             self._h, Grid(N, dx), B, _dev(field, torch.complex64), roi_frac, _dev(stats),
             _dev(mean, torch.float32), _dev(M2, torch.float32), C.byref(cnt) if mean is not None else None))
         return stats, cnt.value
+
+    def beam_stats_static(self, N, dx, field, stats, roi_frac=0.5):
+        """ssp_beam_stats without allocation (library-resident scratch; B <= STATS_STATIC_MAX_FIELDS): fills the
+        caller's stats tensor (uint8 [B*STATS_BYTES], CUDA) and returns it."""
+        self._chk(self._lib.ssp_beam_stats_static(
+            self._h, Grid(N, dx), field.shape[0], _dev(field, torch.complex64), roi_frac, _dev(stats)))
+        return stats
 
     def propagate_host(self, N, dx, lam, dz, h_field_in, h_field_out, h_screens, shared_screens, S,
                        win_order, win_sigma_frac, h_stats, roi_frac, d_field, d_screens, d_stats,
