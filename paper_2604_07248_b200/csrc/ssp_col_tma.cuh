@@ -50,35 +50,52 @@ __device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.b
 // ---- CTA shape ---------------------------------------------------------------------------------
 // C columns per tile (TMA rows of 8 C bytes, at least 16), NBUF shared-memory buffers per CTA (2: persistent
 // CTAs, the load of the next tile overlaps the transform; 1: one tile per CTA), resident CTAs per SM.
+// NG = 2 (with NBUF = 3, one CTA per SM): two groups of T C threads work on two tiles at once, each on its own
+// named barrier, and share three tile buffers -- tile n of the CTA goes to group n % 2 in buffer n % 3, and the load of
+// tile n + 3 is issued into a buffer as soon as the store of tile n has read it.  A tall tile (N >= 2048: 64 KB) then
+// always has its successor landed or in flight, which two independent one-buffer CTAs per SM cannot arrange.
 template <int N>
-struct ColTmaTune { static constexpr int C = 4, NBUF = 2, MIN_BLOCKS = 3; static constexpr bool ENABLED = false; };
-template <> struct ColTmaTune<512> { static constexpr int C = 8, NBUF = 2, MIN_BLOCKS = 3; static constexpr bool ENABLED = true; };
-template <> struct ColTmaTune<1024> { static constexpr int C = 4, NBUF = 2, MIN_BLOCKS = 3; static constexpr bool ENABLED = true; };
+struct ColTmaTune { static constexpr int C = 4, NBUF = 2, MIN_BLOCKS = 3, NG = 1; static constexpr bool ENABLED = false; };
+template <> struct ColTmaTune<512> { static constexpr int C = 8, NBUF = 2, MIN_BLOCKS = 3, NG = 1; static constexpr bool ENABLED = true; };
+#ifndef SSP_T1024_C
+#define SSP_T1024_C 4
+#define SSP_T1024_NBUF 2
+#define SSP_T1024_MINB 3
+#define SSP_T1024_NG 1
+#endif
+// 2048^2 (64 KB tiles of 4 columns), measured: one tile per CTA, 2 CTAs/SM 3749 GB/s; two groups on three buffers
+// 2997 (200 KB of shared memory leave no L1 for the twiddle / hy reads), the same with those in tensor memory 4015
 #ifndef SSP_T2048_C
 #define SSP_T2048_C 4
-#define SSP_T2048_NBUF 1
-#define SSP_T2048_MINB 2
+#define SSP_T2048_NBUF 3
+#define SSP_T2048_MINB 1
+#define SSP_T2048_NG 2
 #endif
 #ifndef SSP_T4096_C
 #define SSP_T4096_C 2
 #define SSP_T4096_NBUF 1
 #define SSP_T4096_MINB 2
+#define SSP_T4096_NG 1
 #endif
-template <int C_, int NBUF_, int MINB_> struct ColTmaTuneV { static constexpr int C = C_, NBUF = NBUF_, MIN_BLOCKS = MINB_; static constexpr bool ENABLED = true; };
-template <> struct ColTmaTune<2048> : ColTmaTuneV<SSP_T2048_C, SSP_T2048_NBUF, SSP_T2048_MINB> {};
-template <> struct ColTmaTune<4096> : ColTmaTuneV<SSP_T4096_C, SSP_T4096_NBUF, SSP_T4096_MINB> {};
+template <int C_, int NBUF_, int MINB_, int NG_> struct ColTmaTuneV { static constexpr int C = C_, NBUF = NBUF_, MIN_BLOCKS = MINB_, NG = NG_; static constexpr bool ENABLED = true; };
+template <> struct ColTmaTune<1024> : ColTmaTuneV<SSP_T1024_C, SSP_T1024_NBUF, SSP_T1024_MINB, SSP_T1024_NG> {};
+template <> struct ColTmaTune<2048> : ColTmaTuneV<SSP_T2048_C, SSP_T2048_NBUF, SSP_T2048_MINB, SSP_T2048_NG> {};
+template <> struct ColTmaTune<4096> : ColTmaTuneV<SSP_T4096_C, SSP_T4096_NBUF, SSP_T4096_MINB, SSP_T4096_NG> {};
 
 template <int N>
 struct ColTmaCfg {
     static constexpr int T = PlanInfo<N, 1>::T;
     static constexpr int C = ColTmaTune<N>::C;
     static constexpr int NBUF = ColTmaTune<N>::NBUF;
-    static constexpr int THREADS = T * C;
+    static constexpr int NG = ColTmaTune<N>::NG;                      // tiles in work at once (groups of GT threads)
+    static constexpr int GT = T * C;
+    static constexpr int THREADS = NG * GT;
+    static_assert(NG == 1 || (NG == 2 && NBUF == 3 && GT % 32 == 0), "two groups rotate through three buffers");
     static constexpr int MIN_BLOCKS = ColTmaTune<N>::MIN_BLOCKS;
     static constexpr int BOX_ROWS = (N < 256) ? N : 256;              // TMA box dimensions are <= 256
     static constexpr int BOXES = N / BOX_ROWS;
     static constexpr int BUF_ELEMS = C * PlanInfo<N, 1>::LINE_ELEMS;  // float2 per buffer (padded exchange)
-    static constexpr size_t SMEM = NBUF * sizeof(float2) * BUF_ELEMS + 32;   // + two mbarriers + the TMEM address slot
+    static constexpr size_t SMEM = NBUF * sizeof(float2) * BUF_ELEMS + 64;   // + six mbarriers + the TMEM address slot
     static constexpr unsigned TILE_BYTES = (unsigned)(sizeof(float2) * C * N);
     // packed fp32 pairs: measured 2048 +3.6 %, 4096 +1.3 %; 1024 -1 % and 512 +1 % (within noise) stay scalar
 #ifndef SSP_COL1024_PK
@@ -89,11 +106,12 @@ struct ColTmaCfg {
 #ifndef SSP_COL1024_TMEM
 #define SSP_COL1024_TMEM 1
 #endif
-// measured at 2048 / 4096 (one tile buffer, so the persistent loop reloads it only after its own store has drained):
+// measured at 2048 / 4096 with ONE tile buffer (the persistent loop reloads it only after its own store has drained):
 // 3735 -> 3375 GB/s and 3161 -> 2590 GB/s -- fresh CTAs overlap one tile's store with the next one's load better than
-// the single-buffer loop does, and that outweighs the LSU relief; off
+// the single-buffer loop does; 2048 runs two groups on three buffers (ColTmaTune) and keeps the cache, 4096 stays off
+// (two groups there: 3164 -> 2464, with the cache 2499: 16-byte TMA rows are the limit, profiles/r02_tma_rows.md)
 #ifndef SSP_COL2048_TMEM
-#define SSP_COL2048_TMEM 0
+#define SSP_COL2048_TMEM 1
 #endif
 #ifndef SSP_COL4096_TMEM
 #define SSP_COL4096_TMEM 0
@@ -105,7 +123,7 @@ struct ColTmaCfg {
     static constexpr int TM_NEED = (THREADS / 128) * TM_CW;
     static constexpr int TMEM_COLS = TM_NEED <= 128 ? 128 : (TM_NEED <= 256 ? 256 : 512);
     // persistent even with one buffer (the tile loop reloads the buffer after its store has drained) when TMEM is on
-    static constexpr bool PERSIST = (NBUF == 2) || TMEM;
+    static constexpr bool PERSIST = (NBUF >= 2) || TMEM;
 };
 
 // Screen generator (K1+K2): one tile per CTA, one buffer (noise -> exchange -> result) plus a second one only
@@ -150,28 +168,40 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *sbuf = reinterpret_cast<float2 *>(smem_raw);
     unsigned long long *full = reinterpret_cast<unsigned long long *>(smem_raw + CFG::NBUF * sizeof(float2) * CFG::BUF_ELEMS);
-    const int tid = threadIdx.x, c = tid % C, t = fft_logical_t<N, 1, C>(tid / C);
+    constexpr int NG = CFG::NG, GT = CFG::GT;
+    const int tid = threadIdx.x, grp = tid / GT, ltid = tid % GT, c = ltid % C, t = fft_logical_t<N, 1, C>(ltid / C);
+    auto group_sync = [&]() {                                     // the threads working on one tile
+        if constexpr (NG == 1) __syncthreads();
+        else asm volatile("bar.sync %0, %1;" ::"r"(1 + grp), "n"(GT) : "memory");
+    };
 
-    auto issue_load = [&](int tile, int buf) {
+    // bar: the mbarrier that announces this fill.  Two groups: fill k of a buffer uses the buffer's barrier k & 1, so
+    // that a group waiting for fill k + 1 while the other group has not yet seen fill k complete never meets a barrier
+    // whose previous phase has the parity it waits for.
+    auto issue_load = [&](int tile, int buf, int bar) {
         const int b = tile / GROUPS, col0 = (tile % GROUPS) * C;
-        mbar_expect_tx(&full[buf], CFG::TILE_BYTES);
+        mbar_expect_tx(&full[bar], CFG::TILE_BYTES);
 #pragma unroll
         for (int j = 0; j < CFG::BOXES; ++j)
             tma_load_2d(sbuf + buf * CFG::BUF_ELEMS + j * CFG::BOX_ROWS * C, &tm_in, 2 * col0, b * N + j * CFG::BOX_ROWS,
-                        &full[buf]);
+                        &full[bar]);
     };
     if (tid == 0) {
-        mbar_init(&full[0], 1);
-        mbar_init(&full[1], 1);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) mbar_init(&full[i], 1);
         fence_mbar_init();
-        if ((int)blockIdx.x < a.ntiles) issue_load(blockIdx.x, 0);
+        if ((int)blockIdx.x < a.ntiles) issue_load(blockIdx.x, 0, 0);
+        if constexpr (NG == 2) {                                  // all three buffers start empty: fill 0 of buffers 1 and 2
+            if ((int)(blockIdx.x + gridDim.x) < a.ntiles) issue_load(blockIdx.x + gridDim.x, 1, 2);
+            if ((int)(blockIdx.x + 2 * gridDim.x) < a.ntiles) issue_load(blockIdx.x + 2 * gridDim.x, 2, 4);
+        }
     }
     // Tensor memory as a per-thread constant cache: this thread's 16 twiddle pairs W_N^(t k) and the 32 hy values of
     // its points never change while the CTA walks its tiles, so they are read from the thread's own TMEM lane
     // (tcgen05.ld) instead of through the LSU data pipe, which this kernel saturates first.
     constexpr bool TM = CFG::TMEM;                                  // twiddles; the multiplier too when it is the 1-D table hy
     constexpr bool TMH = CFG::TMEM && !H2D;
-    unsigned &tmem_slot = *reinterpret_cast<unsigned *>(full + 2);     // (a static __shared__ would shift the TMA buffers)
+    unsigned &tmem_slot = *reinterpret_cast<unsigned *>(full + 6);     // (a static __shared__ would shift the TMA buffers)
     unsigned taddr = 0;
     if constexpr (TM) {
         if (tid < 32) tmem_alloc(&tmem_slot, CFG::TMEM_COLS);
@@ -194,24 +224,27 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
         tmem_wait_st();
     }
 
-    int it = 0;
-    for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x, ++it) {
-        const int cur = (CFG::NBUF == 2) ? (it & 1) : 0;          // NBUF == 1: one tile per CTA (grid = tiles)
+    // the CTA's n-th tile is blockIdx.x + n gridDim.x; with two groups, group grp takes n = grp, grp + 2, ..
+    int it = (NG == 2) ? grp : 0;
+    for (int tile = blockIdx.x + it * gridDim.x; tile < a.ntiles; tile += NG * gridDim.x, it += NG) {
+        const int cur = (CFG::NBUF == 1) ? 0 : it % CFG::NBUF;    // NBUF == 1: one tile per CTA (grid = tiles)
         float2 *tile_s = sbuf + cur * CFG::BUF_ELEMS;
-        ColSmem<C> sm{tile_s + c};
-        mbar_wait(&full[cur], (CFG::NBUF == 2) ? ((it >> 1) & 1) : (it & 1));
+        ColSmem<C, NG == 1 ? 0 : GT> sm{tile_s + c, 1 + grp};
+        const int fill = (CFG::NBUF == 1) ? it : it / CFG::NBUF;  // how often this buffer has been filled before
+        const int bar = (NG == 2) ? 2 * cur + (fill & 1) : cur;
+        mbar_wait(&full[bar], (NG == 2) ? ((fill >> 1) & 1) : (fill & 1));
         float2 v[E];
 #pragma unroll
         for (int i = 0; i < E / R1; ++i)
 #pragma unroll
             for (int q = 0; q < R1; ++q) v[i * R1 + q] = tile_s[line_index<N, 1, R1>(t, i, q) * C + c];
-        __syncthreads();                                          // the tile is in registers: the buffer is free
+        group_sync();                                             // the tile is in registers: the buffer is free
         // multiplier of element (ky, this thread's column): hy[ky], or H(ky,kx) read through L1/L2
         const float2 *hcol = H2D ? a.h2d + (size_t)(tile % GROUPS) * N * C + c : a.hy;
         constexpr int HS = H2D ? C : 1;                           // stride of ky in the multiplier table
         if (CFG::NBUF == 2 && tid == 0 && tile + (int)gridDim.x < a.ntiles) {
             tma_store_wait_read();                                // the store of tile it-1 has released the other buffer
-            issue_load(tile + gridDim.x, cur ^ 1);
+            issue_load(tile + gridDim.x, cur ^ 1, cur ^ 1);
         }
         if constexpr (SYM) {
             // pass 0: forward; * hy, leaving the product re/im-swapped; pass 1: forward on swapped data = inverse
@@ -265,20 +298,22 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
                 for (int q = 0; q < R1; ++q) tile_s[line_index<N, 1, R1>(t, i, q) * C + c] = v[i * R1 + q];
         }
         fence_proxy_async();                                      // generic-proxy writes visible to the TMA store
-        __syncthreads();
-        if (tid == 0) {
+        group_sync();
+        if (ltid == 0) {
             const int b = tile / GROUPS, col0 = (tile % GROUPS) * C;
 #pragma unroll
             for (int j = 0; j < CFG::BOXES; ++j)
                 tma_store_2d(&tm_out, 2 * col0, b * N + j * CFG::BOX_ROWS, tile_s + j * CFG::BOX_ROWS * C);
             tma_store_commit();
-            if (CFG::NBUF == 1 && tile + (int)gridDim.x < a.ntiles) {   // one buffer, persistent: reload it once the store has read it
+            // one buffer, persistent / two groups on three buffers: reload this buffer once the store has read it
+            constexpr int AHEAD = (NG == 2) ? CFG::NBUF : 1;
+            if ((CFG::NBUF == 1 || NG == 2) && tile + AHEAD * (int)gridDim.x < a.ntiles) {
                 tma_store_wait_read();
-                issue_load(tile + gridDim.x, 0);
+                issue_load(tile + AHEAD * gridDim.x, cur, (NG == 2) ? 2 * cur + ((fill + 1) & 1) : cur);
             }
         }
     }
-    if (tid == 0) tma_store_wait_read();
+    if (ltid == 0) tma_store_wait_read();
     if constexpr (TM) {
         tmem_fence_before_sync();
         __syncthreads();

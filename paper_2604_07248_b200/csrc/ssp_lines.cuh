@@ -65,7 +65,8 @@ struct RowCfg {
 #define SSP_ROW1024_TMEM 1
 #endif
     // measured: 1024 +4 % (+1.3 % more with the next-row prefetch), 512 +12 % (3907 -> 4381 GB/s); 2048 as two rows per
-    // 128-thread CTA -4 % and 4096 -10 % (both spill at 168 registers), so those keep the one-row-per-CTA kernels
+    // 128-thread CTA -4 % and 4096 -10 % (both spill at 168 registers; 4096 with 255 registers at 2 or 3 CTAs/SM:
+    // 3805 -> 3458 / 3427 GB/s), so those keep the one-row-per-CTA kernels
     static constexpr bool TMEM = (N == 1024 && SSP_ROW1024_TMEM) || (N == 512 && SSP_ROW512_TMEM);
 };
 
@@ -130,14 +131,21 @@ struct RowSmem {
     }
 };
 
-template <int C>
+// GT > 0: the CTA holds several tiles at once, each worked on by its own group of GT threads that synchronises on
+// its own named barrier (bar_id) instead of the CTA-wide one.
+template <int C, int GT = 0>
 struct ColSmem {
     static constexpr int PAD = 1;
     static constexpr int LANE_STRIDE = C;       // lanes per thread step of a line (ssp_fft.cuh: fft_logical_t)
     float2 *base; // tile base + this thread's column
+    int bar_id = 0;
     __device__ __forceinline__ void st(int p, float2 x) { base[p * C] = x; }
     __device__ __forceinline__ float2 ld(int p) const { return base[p * C]; }
-    __device__ __forceinline__ void sync() { __syncthreads(); }
+    __device__ __forceinline__ void sync()
+    {
+        if constexpr (GT == 0) __syncthreads();
+        else asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "n"(GT) : "memory");
+    }
 };
 
 // ---- tensor-memory allocation (tcgen05.alloc / dealloc; one warp, address through shared memory) ----------------
