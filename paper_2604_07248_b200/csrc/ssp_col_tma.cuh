@@ -321,4 +321,153 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
     }
 }
 
+// ---- wide tiles for the tallest grid ------------------------------------------------------------------------------
+// The TMA engine moves about 0.5-0.7 tile ROWS per clock and SM whatever their width (profiles/r02_tma_rows.md): with
+// the 16-byte rows of a two-column tile -- all that fits twice into shared memory at N = 4096 -- a plain TMA copy stops
+// near 3 TB/s, and k_col_tma<4096> runs at that.  This kernel moves FOUR-column tiles (32-byte rows, 128 KB) and still
+// overlaps every load with the transform: one persistent CTA per SM; the landing buffer L holds the tile only until it
+// is in registers (64 points per thread), then takes the next tile's load at once; the transform's exchange runs in a
+// separate buffer X of HALF a tile, which the two column pairs (warps 0-3: columns 0-1, warps 4-7: columns 2-3) use in
+// turn -- pair g waits for the other pair's release before its first exchange write (fft_line's PRE hook) and releases
+// X right after its last exchange read (HOOK), named barriers 3 / 4 counting arrivals -- and the result leaves through
+// X as two half tiles of 2048 rows.  Twiddles and hy come from tensor memory (the 200 KB of buffers leave no L1).
+#ifndef SSP_COL4096_WIDE
+#define SSP_COL4096_WIDE 1
+#endif
+template <int N>
+struct ColWideCfg {
+    using PI = PlanInfo<N, 1>;
+    static constexpr bool ENABLED = (N == 4096) && SSP_COL4096_WIDE;
+    static constexpr int C = 4, CP = 2, NPAIR = C / CP;               // columns per tile / per pair
+    static constexpr int T = PI::T, E = PI::E;
+    static constexpr int GT = T * CP, THREADS = NPAIR * GT;           // 128 threads per pair, 256 per CTA
+    static constexpr int BOX_ROWS = 256, BOXES = N / BOX_ROWS;
+    static constexpr size_t L_BYTES = sizeof(float2) * (size_t)N * C;
+    static constexpr int X_ELEMS = CP * PI::LINE_ELEMS;               // padded exchange of one pair >= half a dense tile
+    static constexpr size_t SMEM = L_BYTES + sizeof(float2) * X_ELEMS + 64;
+    static constexpr unsigned TILE_BYTES = (unsigned)L_BYTES;
+    static constexpr bool PACKED = ColTmaCfg<N>::PACKED;
+    static constexpr int TM_HOFF = 2 * E, TM_CW = 4 * E, TMEM_COLS = 512;
+    static constexpr bool OK = PI::SYM && PI::NSTAGE == 2 && E == PI::R1 && N / PI::R1 == T && GT == 128 && NPAIR == 2 &&
+                               (THREADS / 128) * TM_CW <= 512 && X_ELEMS >= (N / 2) * C && (sizeof(float2) * X_ELEMS) % 128 == 0;
+};
+
+template <int N, bool H2D>
+__global__ void __launch_bounds__(ColWideCfg<N>::THREADS, 1)
+k_col_tma_wide(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_out, const ColTmaArgs a)
+{
+    using PI = PlanInfo<N, 1>;
+    using CFG = ColWideCfg<N>;
+    static_assert(CFG::OK, "two-stage symmetric plan with one first-stage butterfly per thread, two pairs of 128 threads");
+    constexpr int E = PI::E, T = PI::T, C = CFG::C, CP = CFG::CP, GT = CFG::GT;
+    constexpr bool PK = CFG::PACKED;
+    constexpr int GROUPS = N / C;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float2 *L = reinterpret_cast<float2 *>(smem_raw);
+    float2 *X = reinterpret_cast<float2 *>(smem_raw + CFG::L_BYTES);
+    unsigned long long *full = reinterpret_cast<unsigned long long *>(smem_raw + CFG::L_BYTES + sizeof(float2) * CFG::X_ELEMS);
+    unsigned &tmem_slot = *reinterpret_cast<unsigned *>(full + 1);
+    const int tid = threadIdx.x, pair = tid / GT, ltid = tid % GT, cp = ltid % CP, t = ltid / CP, c = pair * CP + cp;
+
+    auto issue_load = [&](int tile) {
+        const int b = tile / GROUPS, col0 = (tile % GROUPS) * C;
+        mbar_expect_tx(full, CFG::TILE_BYTES);
+#pragma unroll
+        for (int j = 0; j < CFG::BOXES; ++j) tma_load_2d(L + j * CFG::BOX_ROWS * C, &tm_in, 2 * col0, b * N + j * CFG::BOX_ROWS, full);
+    };
+    if (tid == 0) {
+        mbar_init(full, 1);
+        fence_mbar_init();
+        if ((int)blockIdx.x < a.ntiles) issue_load(blockIdx.x);
+    }
+    if (tid < 32) tmem_alloc(&tmem_slot, CFG::TMEM_COLS);
+    tmem_fence_before_sync();
+    __syncthreads();
+    tmem_fence_after_sync();
+    // per thread in its own TMEM lane: E twiddle pairs W_N^(t k), then (separable H) the E hy values of its points
+    const unsigned taddr = tmem_slot + ((unsigned)(tid & 96) << 16) + (unsigned)(tid / 128) * CFG::TM_CW;
+    {
+        const float4 *tw4 = reinterpret_cast<const float4 *>(a.tw + PI::TW1) + t;
+#pragma unroll
+        for (int p = 0; p < E / 2; ++p) tmem_st4(taddr + 4 * p, __ldg(tw4 + p * (N / E)));
+        if constexpr (!H2D) {
+#pragma unroll
+            for (int q = 0; q < E; q += 2) {
+                const float2 h0 = __ldg(a.hy + line_index<N, 1, E>(t, 0, q)), h1 = __ldg(a.hy + line_index<N, 1, E>(t, 0, q + 1));
+                tmem_st4(taddr + CFG::TM_HOFF + 2 * q, make_float4(h0.x, h0.y, h1.x, h1.y));
+            }
+        }
+        tmem_wait_st();
+    }
+    // X hand-over between the pairs: barrier 3 = "pair 0 has read its exchange", 4 = "pair 1 has read its exchange"
+    auto release = [&]() { asm volatile("bar.arrive %0, %1;" ::"r"(3 + pair), "n"(2 * GT) : "memory"); };
+    auto wait_other = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(4 - pair), "n"(2 * GT) : "memory"); };
+
+    int it = 0;
+    for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x, ++it) {
+        mbar_wait(full, it & 1);
+        float2 v[E];
+#pragma unroll
+        for (int q = 0; q < E; ++q) v[q] = L[line_index<N, 1, E>(t, 0, q) * C + c];
+        if (tid == 0) tma_store_wait_read();                      // the previous tile's second half has left X meanwhile
+        __syncthreads();                                          // the tile is in registers, X is free
+        if (tid == 0 && tile + (int)gridDim.x < a.ntiles) issue_load(tile + gridDim.x);
+        ColSmem<CP, GT> sm{X + cp, 1 + pair};
+        const float2 *hcol = a.h2d + (size_t)(tile % GROUPS) * N * C + c;
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+            // pass 0: forward, * hy leaving the product re/im-swapped; pass 1: forward on swapped data = inverse.
+            // Turns on X: pair 0, pair 1, pair 0, pair 1; pair 0's first turn of a tile has nothing to wait for.
+            auto pre = [&]() { if (pair == 1 || pass == 1) wait_other(); };
+            fft_line<N, 1, false, false, false, PK>(v, t, sm, TwTmem{a.tw, taddr}, release, pre);
+            if (pass == 0) {
+                if constexpr (!H2D) {
+#pragma unroll
+                    for (int q = 0; q < E; q += 4) {
+                        float4 ha, hb;
+                        tmem_ld8(taddr + CFG::TM_HOFF + 2 * q, ha, hb);
+                        const float2 h[4] = {make_float2(ha.x, ha.y), make_float2(ha.z, ha.w), make_float2(hb.x, hb.y), make_float2(hb.z, hb.w)};
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            const float2 x = v[q + e];
+                            v[q + e] = make_float2(fmaf(x.x, h[e].y, x.y * h[e].x), fmaf(x.x, h[e].x, -x.y * h[e].y));
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int q = 0; q < E; ++q) {
+                        const float2 h = __ldg(hcol + (size_t)line_index<N, 1, E>(t, 0, q) * C), x = v[q];
+                        v[q] = make_float2(fmaf(x.x, h.y, x.y * h.x), fmaf(x.x, h.x, -x.y * h.y));
+                    }
+                }
+            }
+        }
+        if (pair == 0) wait_other();                              // pair 1's last turn: every arrival on 3 / 4 is now matched
+        // the result leaves through X as two dense half tiles [N/2][C]
+        const int b = tile / GROUPS, col0 = (tile % GROUPS) * C;
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            __syncthreads();                                      // X is free: exchanges done / the first half's store has read it
+#pragma unroll
+            for (int q = 0; q < E / 2; ++q) {
+                const float2 x = half ? v[q + E / 2] : v[q];
+                X[line_index<N, 1, E>(t, 0, q) * C + c] = MidSwapped<N>::value ? x : make_float2(x.y, x.x);
+            }
+            fence_proxy_async();
+            __syncthreads();
+            if (tid == 0) {
+#pragma unroll
+                for (int j = 0; j < CFG::BOXES / 2; ++j)
+                    tma_store_2d(&tm_out, 2 * col0, b * N + half * (N / 2) + j * CFG::BOX_ROWS, X + j * CFG::BOX_ROWS * C);
+                tma_store_commit();
+                if (half == 0) tma_store_wait_read();
+            }
+        }
+    }
+    if (tid == 0) tma_store_wait_read();
+    tmem_fence_before_sync();
+    __syncthreads();
+    if (tid < 32) tmem_dealloc(tmem_slot, CFG::TMEM_COLS);
+}
+
 } // namespace ssp

@@ -319,8 +319,11 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const float2 
 // the place from which a persistent kernel starts the asynchronous copy of its next line into the exchange buffer.
 struct NoHook { __device__ __forceinline__ void operator()() const {} };
 
-template <int N, int V, bool DIR_REV, bool INV, bool TAIL_SYNC = false, bool PK = false, class SM, class TWP, class HOOK = NoHook>
-__device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const TWP twp, HOOK hook = HOOK{})
+// PRE: called once, after the first butterflies and before the first write to the exchange buffer: where a kernel whose
+// thread groups take turns on one exchange buffer waits for its turn (HOOK then hands the buffer on).
+template <int N, int V, bool DIR_REV, bool INV, bool TAIL_SYNC = false, bool PK = false, class SM, class TWP, class HOOK = NoHook,
+          class PRE = NoHook>
+__device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const TWP twp, HOOK hook = HOOK{}, PRE pre = PRE{})
 {
     const float2 *__restrict__ tw = twp.table();
     constexpr bool TW_TMEM = std::is_same<TWP, TwTmem>::value;
@@ -342,6 +345,7 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const TWP twp
         static_assert(E == Ra && Ra == Rc && Rb == 2, "(R, 2, R) plans with one first-stage butterfly per thread");
         const int n2 = t / Rc, n3 = t % Rc;
         radix<Ra, INV, PK>(v);
+        pre();
         const float4 *tw4 = reinterpret_cast<const float4 *>(tw1) + t;
         const float2 w2 = __ldg(tw2 + Rc + n3);                    // W_N^(Ra n3) for the k2 = 1 output
         // exchange pitches of k1 and k2: a half-warp owns one k2 and consecutive n3 (writes) / consecutive k1 (reads),
@@ -380,6 +384,7 @@ __device__ __forceinline__ void fft_line(float2 *v, int t, SM &sm, const TWP twp
 #pragma unroll
     for (int i = 0; i < E / Ra; ++i) {
         radix<Ra, INV, PK>(v + i * Ra);
+        if (i == 0) pre();
         if constexpr (NS >= 2) {
             const int m = t + T * i;
             const float4 *tw4 = reinterpret_cast<const float4 *>(tw1) + m;

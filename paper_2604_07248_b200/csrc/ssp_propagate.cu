@@ -138,14 +138,39 @@ static int launch_col_tma_x(ssp_ctx *ctx, const ColArgs &a)
     return SSP_OK;
 }
 
-template <int N>
-static int launch_col_tma_n(ssp_ctx *ctx, const ColArgs &a)
+// wide tiles, one persistent CTA per SM (ssp_col_tma.cuh: k_col_tma_wide)
+template <int N, bool H2D>
+static int launch_col_wide_x(ssp_ctx *ctx, const ColArgs &a)
 {
-    return a.h2d ? launch_col_tma_x<N, true>(ctx, a) : launch_col_tma_x<N, false>(ctx, a);
+    using CFG = ColWideCfg<N>;
+    auto kern = k_col_tma_wide<N, H2D>;
+    CUtensorMap tm_in, tm_out;
+    if (int rc = make_tmap_c64(ctx, a.in, N, (size_t)a.B * N, CFG::C, CFG::BOX_ROWS, &tm_in)) return rc;
+    if (int rc = make_tmap_c64(ctx, a.out, N, (size_t)a.B * N, CFG::C, CFG::BOX_ROWS, &tm_out)) return rc;
+    if (int rc = set_smem(ctx, kern, CFG::SMEM)) return rc;
+    const int ntiles = a.B * (N / CFG::C);
+    const int grid = ntiles > ctx->num_sms ? ctx->num_sms : ntiles;
+    ColTmaArgs ta{a.hy, a.h2d, a.tw, ntiles};
+    ctx->prof_begin("col_fft_h_ifft", 16.0 * (double)a.B * N * N);
+    kern<<<grid, CFG::THREADS, CFG::SMEM, ctx->stream>>>(tm_in, tm_out, ta);
+    ctx->prof_end();
+    ctx->launches++;
+    SSP_CUDA(ctx, cudaGetLastError());
+    return SSP_OK;
 }
 
 template <int N>
-static constexpr int col_tile_width_n() { return ColTmaTune<N>::ENABLED ? ColTmaCfg<N>::C : ColCfg<N>::C; }
+static int launch_col_tma_n(ssp_ctx *ctx, const ColArgs &a)
+{
+    if constexpr (ColWideCfg<N>::ENABLED) return a.h2d ? launch_col_wide_x<N, true>(ctx, a) : launch_col_wide_x<N, false>(ctx, a);
+    else return a.h2d ? launch_col_tma_x<N, true>(ctx, a) : launch_col_tma_x<N, false>(ctx, a);
+}
+
+template <int N>
+static constexpr int col_tile_width_n()
+{
+    return ColWideCfg<N>::ENABLED ? ColWideCfg<N>::C : (ColTmaTune<N>::ENABLED ? ColTmaCfg<N>::C : ColCfg<N>::C);
+}
 
 int col_tile_width(int N)
 {
