@@ -69,6 +69,20 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_probe() -> str:
+    """Compile the stand-alone TMA row-rate probe (csrc/probe/tma_rows.cu) -> csrc/build/tma_rows."""
+    os.makedirs(OBJ, exist_ok=True)
+    src, exe = os.path.join(CSRC, "probe", "tma_rows.cu"), os.path.join(OBJ, "tma_rows")
+    if _stale(exe, [src]):
+        r = subprocess.run([NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
+                            "-o", exe, src, "-lcuda"], capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("nvcc failed on the probe:\n%s\n%s" % (r.stdout, r.stderr))
+    return exe
+
+
 if __name__ == "__main__":
-    path = build(force="--force" in sys.argv, verbose="-v" in sys.argv)
-    print(path)
+    if "--probe" in sys.argv:
+        print(build_probe())
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
