@@ -568,12 +568,22 @@ int ssp_frame_host(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambd
     for (int c = 0; c < n_chunks; ++c) {
         const int b0 = c * Bc, nb = (B - b0 < Bc) ? B - b0 : Bc;
         const size_t off = (size_t)b0 * S * px;                   // in screens; complex arrays: 2 floats per element
-        if (int rc = ssp_fill_noise(ctx, ar->seed, 2 * ar->frame, off, (unsigned long long)nb * S * px, d_noise)) return rc;
-        if (int rc = ssp_evolve_screens(ctx, grid, psd, lambda, nb, S, cn2, dz, n_sh, ar->a, ar->vx, ar->vy, ar->T, d_noise,
-                                        n_sh > 0 ? d_noise_sh + 2 * (size_t)b0 * sh_per_field : nullptr, d_spectrum + 2 * off,
-                                        n_sh > 0 ? d_sh_coef + 2 * (size_t)b0 * sh_per_field : nullptr, d_screens + off,
-                                        d_ws, ws_bytes))
-            return rc;
+        if (screen_col_seeded_supported(grid.N)) {
+            // the generator draws the chunk's noise itself (same draws, bit for bit): no 8 B/px fill, no 8 B/px read
+            if (int rc = ssp_evolve_screens_seeded(ctx, grid, psd, lambda, nb, S, cn2, dz, n_sh, ar->a, ar->vx, ar->vy, ar->T,
+                                                   ar->seed, 2 * ar->frame, off,
+                                                   n_sh > 0 ? d_noise_sh + 2 * (size_t)b0 * sh_per_field : nullptr, d_spectrum + 2 * off,
+                                                   n_sh > 0 ? d_sh_coef + 2 * (size_t)b0 * sh_per_field : nullptr, d_screens + off,
+                                                   d_ws, ws_bytes))
+                return rc;
+        } else {
+            if (int rc = ssp_fill_noise(ctx, ar->seed, 2 * ar->frame, off, (unsigned long long)nb * S * px, d_noise)) return rc;
+            if (int rc = ssp_evolve_screens(ctx, grid, psd, lambda, nb, S, cn2, dz, n_sh, ar->a, ar->vx, ar->vy, ar->T, d_noise,
+                                            n_sh > 0 ? d_noise_sh + 2 * (size_t)b0 * sh_per_field : nullptr, d_spectrum + 2 * off,
+                                            n_sh > 0 ? d_sh_coef + 2 * (size_t)b0 * sh_per_field : nullptr, d_screens + off,
+                                            d_ws, ws_bytes))
+                return rc;
+        }
         if (c + 1 < group_end) continue;
         // fields of chunks group_begin .. c
         const int g0 = group_begin * Bc, gn = (b0 + nb) - g0;

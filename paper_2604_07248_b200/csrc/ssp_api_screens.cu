@@ -125,7 +125,7 @@ int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
                  const double *cn2, const double *dz, int n_sh, bool ar, double a, double vx, double vy, double T,
                  const float *d_noise, const float *d_noise_sh, float *d_spectrum, float *d_sh_coef,
                  float *d_screens, void *d_ws, float *d_screens_im = nullptr, float2 *ycol_out = nullptr,
-                 ssp::FusedScreens *fused = nullptr)
+                 ssp::FusedScreens *fused = nullptr, const ssp::NoiseSeed *seeded = nullptr)
 {
     SSP_CUDA(ctx, cudaSetDevice(ctx->device));
     const int N = grid.N;
@@ -247,7 +247,12 @@ int screens_impl(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
     for (int g0 = 0; g0 < nscr; g0 += L.chunk) {
         const int n = (nscr - g0 < L.chunk) ? nscr - g0 : L.chunk;
         ScreenColArgs c{};
-        c.noise = reinterpret_cast<const float2 *>(d_noise) + (size_t)g0 * px;
+        c.noise = seeded ? nullptr : reinterpret_cast<const float2 *>(d_noise) + (size_t)g0 * px;
+        if (seeded) {                                             // the generator draws element e of the batch as draw first + e
+            c.keys = key_schedule(seeded->seed);
+            c.stream_lo = (uint32_t)seeded->stream; c.stream_hi = (uint32_t)(seeded->stream >> 32);
+            c.first_draw = seeded->first + (unsigned long long)g0 * px;
+        }
         c.old_spec = ar ? reinterpret_cast<const float2 *>(d_spectrum) + (size_t)g0 * px : nullptr;
         c.spec_out = d_spectrum ? reinterpret_cast<float2 *>(d_spectrum) + (size_t)g0 * px : nullptr;
         c.out = ycol_out ? ycol_out + (size_t)g0 * px : inter;   // fused synthesis: every screen's column-transformed spectrum is kept
@@ -331,6 +336,27 @@ int ssp_evolve_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double l
     if (n_sh > 0 && !d_sh_coef) return ctx->fail(SSP_EINVAL, "d_sh_coef (in-out) is required when n_sh > 0");
     return screens_impl(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, true, a, vx, vy, T,
                         d_fresh_noise, d_fresh_noise_sh, d_spectrum, d_sh_coef, d_screens, d_ws);
+}
+
+int ssp_evolve_screens_seeded(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
+                              int B, int S, const double *cn2, const double *dz, int n_sh,
+                              double a, double vx, double vy, double T,
+                              unsigned long long seed, unsigned long long stream, unsigned long long first,
+                              const float *d_fresh_noise_sh, float *d_spectrum, float *d_sh_coef, float *d_screens,
+                              void *d_ws, size_t ws_bytes)
+{
+    // (the screens pointer stands in for the absent noise array in the shared checks)
+    if (int rc = check_screens(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, d_screens, d_fresh_noise_sh, d_screens, d_ws, ws_bytes))
+        return rc;
+    if (!(a >= 0.0 && a <= 1.0)) return ctx->fail(SSP_EINVAL, "a must be in [0, 1]");
+    if (!d_spectrum || !aligned16(d_spectrum)) return ctx->fail(SSP_EINVAL, "d_spectrum (in-out) is required");
+    if (n_sh > 0 && !d_sh_coef) return ctx->fail(SSP_EINVAL, "d_sh_coef (in-out) is required when n_sh > 0");
+    if (first & 1ull) return ctx->fail(SSP_EINVAL, "the first draw index must be even");
+    if (!screen_col_seeded_supported(grid.N))
+        return ctx->fail(SSP_EUNSUPPORTED, "seeded evolution is built for N = 512 and 1024 (use ssp_fill_noise + ssp_evolve_screens)");
+    const ssp::NoiseSeed ns{seed, stream, first};
+    return screens_impl(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, true, a, vx, vy, T, nullptr, d_fresh_noise_sh,
+                        d_spectrum, d_sh_coef, d_screens, d_ws, nullptr, nullptr, nullptr, &ns);
 }
 
 int ssp_make_screens_pair(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,

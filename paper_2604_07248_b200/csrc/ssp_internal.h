@@ -240,8 +240,14 @@ struct ScreenFilter {
     // ocean
     float eta, w, two_pi;
 };
+struct NoiseSeed { unsigned long long seed, stream, first; };   // fresh noise drawn in the generator: draw index = first + element index
+struct RoundKeys { uint32_t k[10][2]; };   // Philox key schedule (key + r * Weyl constants), computed once on the host
+RoundKeys key_schedule(unsigned long long seed);
 struct ScreenColArgs {
-    const float2 *noise;      // [nscr][N][N]
+    const float2 *noise;      // [nscr][N][N]; null: drawn in the kernel (seeded), element e of this launch = draw first_draw + e
+    RoundKeys keys;           // seeded: key schedule, stream words and the draw index of this launch's first element (even)
+    uint32_t stream_lo, stream_hi;
+    unsigned long long first_draw;
     const float2 *old_spec;   // AR: previous spectrum (may alias spec_out), or null
     float2 *spec_out;         // optional stored spectrum
     float2 *out;              // column-transformed intermediate [nscr][N][N]
@@ -289,6 +295,7 @@ int evolve_to_ycol(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambd
                    const float *d_noise_sh, float *d_spectrum, float *d_sh_coef, float *d_ycol, void *d_ws, size_t ws_bytes,
                    FusedScreens *out);
 int launch_screen_col(ssp_ctx *ctx, int N, const ScreenColArgs &a);
+bool screen_col_seeded_supported(int N);   // grids whose generator can draw the fresh noise itself (ScreenColArgs::noise == null)
 int screen_col_plan_variant(int N);   // plan variant (ssp_fft.cuh) whose twiddles launch_screen_col expects in a.tw
 int launch_screen_row(ssp_ctx *ctx, int N, const ScreenRowArgs &a);
 // subharmonic coefficient update + analytic mean, one block per screen

@@ -7,6 +7,7 @@
 #include "ssp_internal.h"
 #include "ssp_lines.cuh"
 #include "ssp_col_tma.cuh"
+#include "ssp_philox.cuh"
 
 namespace ssp {
 
@@ -104,7 +105,11 @@ __global__ void __launch_bounds__(ColCfg<N, 2>::THREADS, ColCfg<N, 2>::MIN_BLOCK
 // shared-memory buffers, the new spectrum leaves from the buffer the old one came in, the column
 // transform exchanges through the noise buffer and its result leaves from there.  Same arithmetic,
 // element for element, as k_screen_col; no global load or store is issued by the threads.
-template <int N, bool OCEAN, bool AR, bool TILT>
+// SEEDED: the fresh noise is not read but drawn here (ssp_philox.cuh: the generator and Box-Muller of ssp_fill_noise,
+// draw index = first_draw + element index), so one of the kernel's four 8 B/px streams -- and the 8 B/px write of the
+// separate noise fill -- disappears.  A Philox block makes the draws of two adjacent columns: the two lanes that own them
+// (c, c ^ 1: adjacent lanes, same rows) each compute the blocks of every other row of the pair and swap halves by shuffle.
+template <int N, bool OCEAN, bool AR, bool TILT, bool SEEDED = false>
 __global__ void __launch_bounds__(ScreenColTmaCfg<N>::THREADS, ScreenColTmaCfg<N>::MIN_BLOCKS)
 k_screen_col_tma(const __grid_constant__ CUtensorMap tm_noise, const __grid_constant__ CUtensorMap tm_spec,
                  const __grid_constant__ CUtensorMap tm_out, const ScreenColArgs a)
@@ -124,10 +129,13 @@ k_screen_col_tma(const __grid_constant__ CUtensorMap tm_noise, const __grid_cons
     if (tid == 0) {
         mbar_init(full, 1);
         fence_mbar_init();
-        mbar_expect_tx(full, ar ? 2 * CFG::TILE_BYTES : CFG::TILE_BYTES);
+        static_assert(!SEEDED || AR, "the seeded form is built for the evolution");
+        mbar_expect_tx(full, (ar && !SEEDED) ? 2 * CFG::TILE_BYTES : CFG::TILE_BYTES);
+        if constexpr (!SEEDED) {
 #pragma unroll
-        for (int j = 0; j < CFG::BOXES; ++j)
-            tma_load_2d(buf_x + j * CFG::BOX_ROWS * C, &tm_noise, 2 * col0, scr * N + j * CFG::BOX_ROWS, full);
+            for (int j = 0; j < CFG::BOXES; ++j)
+                tma_load_2d(buf_x + j * CFG::BOX_ROWS * C, &tm_noise, 2 * col0, scr * N + j * CFG::BOX_ROWS, full);
+        }
         if (ar) {
 #pragma unroll
             for (int j = 0; j < CFG::BOXES; ++j)
@@ -140,15 +148,32 @@ k_screen_col_tma(const __grid_constant__ CUtensorMap tm_noise, const __grid_cons
     float2 tx = make_float2(1.f, 0.f);
     if constexpr (TILT) tx = __ldg(a.taux + kx);
     __syncthreads();
+    float2 v[E];
+    if constexpr (SEEDED) {
+        // the draws of this thread's points, made before the spectrum tile is waited for (they need no memory)
+        static_assert(!SEEDED || (E == R1 && C % 2 == 0), "one first-stage butterfly per thread, column pairs in adjacent lanes");
+        const unsigned long long e0 = a.first_draw + (unsigned long long)scr * N * N + (unsigned)(kx & ~1);
+        const int odd = c & 1;
+#pragma unroll
+        for (int q = 0; q < E; q += 2) {
+            const int ky_m = line_index<N, 1, R1>(t, 0, q + odd);     // the row whose block this lane computes
+            uint32_t w[4];
+            philox_block(a.keys, (e0 + (unsigned long long)ky_m * N) >> 1, a.stream_lo, a.stream_hi, w);
+            const float2 z0 = box_muller(w[0], w[1]), z1 = box_muller(w[2], w[3]);   // columns kx & ~1 and (kx & ~1) + 1
+            const float2 keep = odd ? z1 : z0, give = odd ? z0 : z1;
+            const float2 recv = make_float2(__shfl_xor_sync(0xffffffffu, give.x, 1), __shfl_xor_sync(0xffffffffu, give.y, 1));
+            v[q] = odd ? recv : keep;
+            v[q + 1] = odd ? keep : recv;
+        }
+    }
     mbar_wait(full, 0);
 
-    float2 v[E];
 #pragma unroll
     for (int i = 0; i < E / R1; ++i)
 #pragma unroll
         for (int q = 0; q < R1; ++q) {
             const int ky = line_index<N, 1, R1>(t, i, q);
-            const float2 nz = buf_x[ky * C + c];
+            const float2 nz = SEEDED ? v[i * R1 + q] : buf_x[ky * C + c];
             const float kys = (float)((ky < N / 2) ? ky : ky - N);
             const float f2 = (kxs * kxs + kys * kys) * df2;
             const float amp = (kx == 0 && ky == 0) ? 0.f : amp_s * psd_shape_sqrt_k<OCEAN>(a.flt, f2);
@@ -316,21 +341,22 @@ static int launch_screen_col_n(ssp_ctx *ctx, const ScreenColArgs &a)
     return SSP_OK;
 }
 
-template <int N, bool OCEAN, bool AR, bool TILT>
+template <int N, bool OCEAN, bool AR, bool TILT, bool SEEDED = false>
 static int launch_screen_col_tma_x(ssp_ctx *ctx, const ScreenColArgs &a)
 {
     using CFG = ScreenColTmaCfg<N>;
-    auto kern = k_screen_col_tma<N, OCEAN, AR, TILT>;
+    auto kern = k_screen_col_tma<N, OCEAN, AR, TILT, SEEDED>;
     const size_t smem = CFG::smem((a.old_spec || a.spec_out) ? 2 : 1);
     const size_t rows = (size_t)a.nscr * N;
     CUtensorMap tm_noise, tm_spec, tm_out;
-    if (int rc = make_tmap_c64(ctx, a.noise, N, rows, CFG::C, CFG::BOX_ROWS, &tm_noise)) return rc;
+    // (seeded: no noise array; the descriptor is not used by the kernel)
+    if (int rc = make_tmap_c64(ctx, SEEDED ? (const void *)a.out : (const void *)a.noise, N, rows, CFG::C, CFG::BOX_ROWS, &tm_noise)) return rc;
     const void *spec = a.spec_out ? (const void *)a.spec_out : (const void *)a.old_spec;
     if (int rc = make_tmap_c64(ctx, spec ? spec : (const void *)a.noise, N, rows, CFG::C, CFG::BOX_ROWS, &tm_spec)) return rc;
     if (int rc = make_tmap_c64(ctx, a.out, N, rows, CFG::C, CFG::BOX_ROWS, &tm_out)) return rc;
     SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::smem(2)));
-    const double bpp = 16.0 + (a.old_spec ? 8.0 : 0.0) + (a.spec_out ? 8.0 : 0.0);
-    ctx->prof_begin("screen_col", bpp * (double)a.nscr * N * N);
+    const double bpp = (SEEDED ? 8.0 : 16.0) + (a.old_spec ? 8.0 : 0.0) + (a.spec_out ? 8.0 : 0.0);
+    ctx->prof_begin(SEEDED ? "screen_col_seeded" : "screen_col", bpp * (double)a.nscr * N * N);
     kern<<<a.nscr * (N / CFG::C), CFG::THREADS, smem, ctx->stream>>>(tm_noise, tm_spec, tm_out, a);
     ctx->prof_end();
     ctx->launches++;
@@ -342,6 +368,11 @@ template <int N>
 static int launch_screen_col_tma_n(ssp_ctx *ctx, const ScreenColArgs &a)
 {
     const bool ocean = a.flt.kind == SSP_PSD_OCEAN_NIKISHOV, ar = a.old_spec != nullptr, tilt = ar && a.taux;
+    if (!a.noise) {                                               // seeded: the fresh noise is drawn in the kernel
+        if (!ar) return ctx->fail(SSP_EUNSUPPORTED, "seeded noise is built for the screen evolution");
+        if (ocean) return tilt ? launch_screen_col_tma_x<N, true, true, true, true>(ctx, a) : launch_screen_col_tma_x<N, true, true, false, true>(ctx, a);
+        return tilt ? launch_screen_col_tma_x<N, false, true, true, true>(ctx, a) : launch_screen_col_tma_x<N, false, true, false, true>(ctx, a);
+    }
     if (ocean) {
         if (!ar) return launch_screen_col_tma_x<N, true, false, false>(ctx, a);
         return tilt ? launch_screen_col_tma_x<N, true, true, true>(ctx, a) : launch_screen_col_tma_x<N, true, true, false>(ctx, a);
@@ -370,6 +401,8 @@ static int launch_screen_row_n(ssp_ctx *ctx, const ScreenRowArgs &a)
 
 
 // the TMA generator runs the column plan (V = 1), the register-load one its own (V = 2); they differ at N >= 2048
+bool screen_col_seeded_supported(int N) { return N == 512 || N == 1024; }
+
 int screen_col_plan_variant(int N) { return (N == 512 || N == 1024) ? 1 : 2; }
 
 int launch_screen_col(ssp_ctx *ctx, int N, const ScreenColArgs &a)
@@ -379,6 +412,7 @@ int launch_screen_col(ssp_ctx *ctx, int N, const ScreenColArgs &a)
         if (N == 512) return launch_screen_col_tma_n<512>(ctx, a);
         if (N == 1024) return launch_screen_col_tma_n<1024>(ctx, a);
     }
+    if (!a.noise) return ctx->fail(SSP_EUNSUPPORTED, "seeded noise needs the TMA generator (N = 512, 1024; spectrum kept in place)");
     SSP_DISPATCH_N(N, (launch_screen_col_n<NN>(ctx, a)));
 }
 int row_last_radix(int N)

@@ -186,3 +186,65 @@ def test_frame_host_rejects_bad_arguments_before_any_copy(ssp):
     spec.copy_(spec0); shc.copy_(shc0)
     run(dz, 0.97)
     assert torch.equal(got, h_out) and torch.all(torch.isfinite(torch.view_as_real(h_out)))
+
+
+@pytest.mark.parametrize("N,kind,wind,n_sh,first", [
+    (512, "vk", False, 3, 0), (512, "ocean", True, 2, 1 << 33), (1024, "vk", True, 3, 6 * 1024 * 1024), (1024, "ocean", False, 0, 2)])
+def test_seeded_evolution_equals_fill_noise_plus_evolve(ssp, orc, N, kind, wind, n_sh, first):
+    """ssp_evolve_screens_seeded draws the fresh noise inside the generator's column kernel (Philox blocks shared by the
+    two lanes that own adjacent columns): screens and the advanced spectrum must be the very bytes of ssp_fill_noise +
+    ssp_evolve_screens, over two frames (the second starts from the first's spectrum), with and without wind, both PSD
+    code paths, a draw offset past 2^32 blocks; at 512 the result is also checked against the oracle fed with the
+    oracle's own draws."""
+    from paper_2604_07248_b200 import api
+    B, S, dx, lam = 2, 3, 2e-3, 1.0e-6
+    psd_kw = dict(kind=api.PSD_VON_KARMAN, L0=10.0, l0=5e-3) if kind == "vk" else \
+        dict(kind=api.PSD_OCEAN_NIKISHOV, eps=1e-5, chi_T=1e-7, w=-2.0, eta=1e-3)
+    psd = api.PsdParams(**psd_kw)
+    cn2, dz = [2e-14, 1e-14, 3e-14], [80.0, 120.0, 100.0]
+    a, (vx, vy, T) = 0.97, ((0.8, -0.4, 5e-3) if wind else (0.0, 0.0, 0.0))
+    seed = 2604 + N
+    gen = torch.Generator(device="cuda").manual_seed(N + n_sh)
+    noise0 = torch.view_as_complex(torch.randn(B, S, N, N, 2, device="cuda", generator=gen))
+    nsh = [torch.view_as_complex(torch.randn(B, S, max(n_sh, 1), 3, 3, 2, device="cuda", generator=gen)) for _ in range(3)]
+    state = []
+    for _ in range(2):                                         # the same initial spectrum for both paths
+        spec = torch.empty((B, S, N, N), dtype=torch.complex64, device="cuda")
+        shc = torch.zeros((B, S, max(n_sh, 1), 3, 3), dtype=torch.complex64, device="cuda")
+        ssp.make_screens(N, dx, psd, lam, cn2, dz, n_sh, noise0, nsh[0], spectrum=spec, sh_coef=shc)
+        state.append((spec, shc))
+    fresh = torch.empty((B, S, N, N), dtype=torch.complex64, device="cuda")
+    for frame in (1, 2):
+        off = first + (frame - 1) * B * S * N * N
+        ssp.fill_noise(seed, 2 * frame, fresh, first=off)
+        ref = ssp.evolve_screens(N, dx, psd, lam, cn2, dz, n_sh, a, vx, vy, T, fresh, nsh[frame], state[0][0], state[0][1])
+        got = ssp.evolve_screens_seeded(N, dx, psd, lam, cn2, dz, n_sh, a, vx, vy, T, seed, 2 * frame, off, nsh[frame],
+                                        state[1][0], state[1][1])
+        assert torch.equal(got, ref), (frame, float((got - ref).abs().max()))
+        assert torch.equal(state[1][0], state[0][0]) and torch.equal(state[1][1], state[0][1]), frame
+    if N == 512:
+        # against the oracle: its own generator for the draws, its own evolution (one frame from a zero spectrum)
+        spec = torch.zeros((B, S, N, N), dtype=torch.complex64, device="cuda")
+        shc = torch.zeros((B, S, max(n_sh, 1), 3, 3), dtype=torch.complex64, device="cuda")
+        got = ssp.evolve_screens_seeded(N, dx, psd, lam, cn2, dz, n_sh, 0.0, vx, vy, T, seed, 7, first, nsh[0], spec, shc)
+        hi = orc.noise(seed, 7, B * S * N * N, first=first).reshape(B, S, N, N)
+        sh = nsh[0].cpu().numpy().astype(np.complex128)[:, :, :n_sh]
+        ref, _, _ = orc.make_screens(N, dx, orc.Psd(**{k: v for k, v in psd_kw.items()}), lam, cn2, dz, n_sh,
+                                     np.stack([hi.real, hi.imag], -1), np.stack([sh.real, sh.imag], -1), keep_spectrum=False)
+        err = np.sqrt(np.sum((got.cpu().numpy() - ref) ** 2, axis=(-2, -1)) / np.sum(ref ** 2, axis=(-2, -1)))
+        assert err.max() < 2e-5 * np.log2(N), err.max()
+
+
+def test_seeded_evolution_rejects_grids_without_the_tma_generator(ssp):
+    from paper_2604_07248_b200 import api
+    psd = api.PsdParams(kind=api.PSD_VON_KARMAN, L0=10.0, l0=5e-3)
+    for N in (256, 2048):
+        spec = torch.zeros((1, 1, N, N), dtype=torch.complex64, device="cuda")
+        shc = torch.zeros((1, 1, 1, 3, 3), dtype=torch.complex64, device="cuda")
+        with pytest.raises(api.SspError) as e:
+            ssp.evolve_screens_seeded(N, 1e-3, psd, 1e-6, [1e-14], [100.0], 0, 0.9, 0, 0, 0, 1, 2, 0, None, spec, shc)
+        assert e.value.code == api.EUNSUPPORTED
+    spec = torch.zeros((1, 1, 512, 512), dtype=torch.complex64, device="cuda")
+    with pytest.raises(api.SspError) as e:                     # odd first draw
+        ssp.evolve_screens_seeded(512, 1e-3, psd, 1e-6, [1e-14], [100.0], 0, 0.9, 0, 0, 0, 1, 2, 3, None, spec, None)
+    assert e.value.code == api.EINVAL
