@@ -268,10 +268,20 @@ def run_ours(args):
     ctx.make_screens(N, wl.dx, psd, wl.lam, cn2, dz, n_sh, noise[0], noise_sh[0] if n_sh else None,
                      spectrum=spectrum, sh_coef=sh_coef if n_sh else None, screens=screens, ws=ws)
 
-    def frame(i):
-        ctx.evolve_screens(N, wl.dx, psd, wl.lam, cn2, dz, n_sh, a, 0.0, 0.0, 0.0, noise[i & 1],
-                           noise_sh[i & 1] if n_sh else None, spectrum, sh_coef if n_sh else None,
-                           screens=screens, ws=ws)
+    # The frame's fresh grid noise: drawn inside the generator's column kernel from (seed, frame) where that form exists
+    # (ssp_evolve_screens_seeded, N = 512 / 1024: the paper's pipeline draws its noise on the GPU every frame),
+    # read from one of the two resident noise frames elsewhere.  `resident_noise` times the second form on every grid.
+    seeded = N in (512, 1024)
+
+    def frame(i, resident=not seeded):
+        if resident:
+            ctx.evolve_screens(N, wl.dx, psd, wl.lam, cn2, dz, n_sh, a, 0.0, 0.0, 0.0, noise[i & 1],
+                               noise_sh[i & 1] if n_sh else None, spectrum, sh_coef if n_sh else None,
+                               screens=screens, ws=ws)
+        else:
+            ctx.evolve_screens_seeded(N, wl.dx, psd, wl.lam, cn2, dz, n_sh, a, 0.0, 0.0, 0.0, 1234 + rank, 2 * i, 0,
+                                      noise_sh[i & 1] if n_sh else None, spectrum, sh_coef if n_sh else None,
+                                      screens=screens, ws=ws)
         ctx.propagate(N, wl.dx, wl.lam, dz, u0, screens, out=out, stats=stats, **kw)
         ctx.propagate_adjoint(N, wl.dx, wl.lam, dz, out, screens, out=gin, **kw)
 
@@ -322,6 +332,23 @@ def run_ours(args):
     prof = ctx.profile_report()
     ctx.profile_enable(False)
     ms_prof_total = p0.elapsed_time(p1)
+
+    # ---- the same step with the fresh noise read from a resident array instead of drawn in the kernel (reference figure)
+    resident_noise = None
+    if seeded:
+        n_res = args.steps                                 # as many steps as the timed region: the same sustained clocks
+        for i in range(args.warmup):
+            frame(i, resident=True)
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record()
+        for i in range(n_res):
+            frame(args.warmup + i, resident=True)
+        r1.record()
+        sync_all()
+        ms_res = r0.elapsed_time(r1) / n_res
+        resident_noise = {"what": "the step with ssp_evolve_screens reading the frame's fresh noise from a resident array "
+                                  "(8 B/px more traffic, no draws)", "ms_per_step": ms_res,
+                          "value": units_step / world / (ms_res * 1e-3), "steps": n_res}
 
     # ---- roofline of the dominant kernel class (by device time inside the timed region)
     peak, peak_src = peaks()
@@ -490,12 +517,14 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": wl.name, "N": N, "B_per_gpu": B, "S": S, "n_sh": n_sh, "ar_a": a, "h_kind": args.h_kind,
-                       "step": "evolve_screens + propagate + beam_stats + propagate_adjoint",
+                       "step": ("evolve_screens_seeded (fresh noise drawn in the generator)" if seeded else "evolve_screens")
+                               + " + propagate + beam_stats + propagate_adjoint",
                        "timing": "CUDA events around the K steps, library profiling off; kernels / roofline / split_step from a separate profiled pass",
                        "units_per_step": units_step,
                        "l2": "inputs larger than L2 (no flush): each step streams > 10 GB"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches) * world, "roofline": roof,
-            "cpu_baseline": cpu, "kernels": kernels, "split_step": split_step, "forward_frame": fwd_frame, "cufft_comparison": cufft,
+            "cpu_baseline": cpu, "kernels": kernels, "split_step": split_step, "resident_noise": resident_noise,
+            "forward_frame": fwd_frame, "cufft_comparison": cufft,
         }
         print(json.dumps(line))
     ctx.close()

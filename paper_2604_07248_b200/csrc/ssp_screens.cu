@@ -9,6 +9,15 @@
 #include "ssp_col_tma.cuh"
 #include "ssp_philox.cuh"
 
+// unroll factor of the seeded kernel's draw loop (16 Philox blocks per thread), measured per config-3 frame: 1: 3.61 ms,
+// 2: 3.43, 4: 3.37, 8: 4.18, 16 (full, draws kept in registers and swapped by shuffle): 4.60 -- the last two miss the
+// instruction cache (ncu: no_instruction 1.7 stalled warps per issue)
+#ifndef SSP_SEED_UNROLL
+#define SSP_SEED_UNROLL 4
+#endif
+#define SSP_SEED_PRAGMA_(x) _Pragma(#x)
+#define SSP_SEED_PRAGMA(x) SSP_SEED_PRAGMA_(x)
+
 namespace ssp {
 
 // sqrt of the frequency-dependent part of Phi^f at squared frequency f2 (cycles/m)^2.
@@ -108,7 +117,8 @@ __global__ void __launch_bounds__(ColCfg<N, 2>::THREADS, ColCfg<N, 2>::MIN_BLOCK
 // SEEDED: the fresh noise is not read but drawn here (ssp_philox.cuh: the generator and Box-Muller of ssp_fill_noise,
 // draw index = first_draw + element index), so one of the kernel's four 8 B/px streams -- and the 8 B/px write of the
 // separate noise fill -- disappears.  A Philox block makes the draws of two adjacent columns: the two lanes that own them
-// (c, c ^ 1: adjacent lanes, same rows) each compute the blocks of every other row of the pair and swap halves by shuffle.
+// (c, c ^ 1: adjacent lanes, same rows) each compute the blocks of every other row and hand the other half over through
+// the (otherwise unused) noise buffer.
 template <int N, bool OCEAN, bool AR, bool TILT, bool SEEDED = false>
 __global__ void __launch_bounds__(ScreenColTmaCfg<N>::THREADS, ScreenColTmaCfg<N>::MIN_BLOCKS)
 k_screen_col_tma(const __grid_constant__ CUtensorMap tm_noise, const __grid_constant__ CUtensorMap tm_spec,
@@ -150,21 +160,22 @@ k_screen_col_tma(const __grid_constant__ CUtensorMap tm_noise, const __grid_cons
     __syncthreads();
     float2 v[E];
     if constexpr (SEEDED) {
-        // the draws of this thread's points, made before the spectrum tile is waited for (they need no memory)
-        static_assert(!SEEDED || (E == R1 && C % 2 == 0), "one first-stage butterfly per thread, column pairs in adjacent lanes");
+        // the draws of this thread's points, made before the spectrum tile is waited for (they need no memory): written
+        // into the noise buffer where the TMA load of the reading kernel would have put them, one 16-byte store per
+        // block (two adjacent columns); the partner lane reads its half after a __syncwarp.  The loop stays rolled: fully
+        // unrolled, the 16 blocks of ten rounds pushed the kernel past the instruction cache (ncu: no_instruction 1.7 per issue)
+        static_assert(!SEEDED || (E == R1 && C % 2 == 0 && E % 2 == 0), "one first-stage butterfly per thread, column pairs in adjacent lanes");
         const unsigned long long e0 = a.first_draw + (unsigned long long)scr * N * N + (unsigned)(kx & ~1);
         const int odd = c & 1;
-#pragma unroll
+SSP_SEED_PRAGMA(unroll SSP_SEED_UNROLL)
         for (int q = 0; q < E; q += 2) {
             const int ky_m = line_index<N, 1, R1>(t, 0, q + odd);     // the row whose block this lane computes
             uint32_t w[4];
             philox_block(a.keys, (e0 + (unsigned long long)ky_m * N) >> 1, a.stream_lo, a.stream_hi, w);
             const float2 z0 = box_muller(w[0], w[1]), z1 = box_muller(w[2], w[3]);   // columns kx & ~1 and (kx & ~1) + 1
-            const float2 keep = odd ? z1 : z0, give = odd ? z0 : z1;
-            const float2 recv = make_float2(__shfl_xor_sync(0xffffffffu, give.x, 1), __shfl_xor_sync(0xffffffffu, give.y, 1));
-            v[q] = odd ? recv : keep;
-            v[q + 1] = odd ? keep : recv;
+            *reinterpret_cast<float4 *>(buf_x + ky_m * C + (c & ~1)) = make_float4(z0.x, z0.y, z1.x, z1.y);
         }
+        __syncwarp();
     }
     mbar_wait(full, 0);
 
@@ -173,7 +184,7 @@ k_screen_col_tma(const __grid_constant__ CUtensorMap tm_noise, const __grid_cons
 #pragma unroll
         for (int q = 0; q < R1; ++q) {
             const int ky = line_index<N, 1, R1>(t, i, q);
-            const float2 nz = SEEDED ? v[i * R1 + q] : buf_x[ky * C + c];
+            const float2 nz = buf_x[ky * C + c];
             const float kys = (float)((ky < N / 2) ? ky : ky - N);
             const float f2 = (kxs * kxs + kys * kys) * df2;
             const float amp = (kx == 0 && ky == 0) ? 0.f : amp_s * psd_shape_sqrt_k<OCEAN>(a.flt, f2);
