@@ -153,8 +153,8 @@ int ssp_evolve_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double l
  * the [B][S][N][N] batch takes draw `first + e` of stream `stream` of ssp_fill_noise's generator under `seed` (Philox-4x32-10
  * and Box-Muller, same arithmetic), so the call equals ssp_fill_noise(seed, stream, first, B S N^2, noise) followed by
  * ssp_evolve_screens(.., noise, ..) bit for bit, without the 8 B/px write and the 8 B/px read of that array (and without
- * the array).  The subharmonic noise (tiny) stays an input.  `first` even.  Built where the TMA generator runs: N = 512 and
- * 1024 (SSP_EUNSUPPORTED otherwise: draw the noise with ssp_fill_noise and call ssp_evolve_screens). */
+ * the array).  The subharmonic noise (tiny) stays an input.  `first` even.  Built for N >= 512 (SSP_EUNSUPPORTED below:
+ * draw the noise with ssp_fill_noise and call ssp_evolve_screens). */
 int ssp_evolve_screens_seeded(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
                               int B, int S, const double *cn2, const double *dz, int n_sh,
                               double a, double vx, double vy, double T,

@@ -324,7 +324,7 @@ class Context:
     def evolve_screens_seeded(self, N, dx, psd: PsdParams, lam, cn2, dz, n_sh, a, vx, vy, T, seed, stream, first,
                               fresh_sh, spectrum, sh_coef, screens=None, ws=None):
         """evolve_screens with the fresh grid noise drawn inside the generator (draw first + element index of stream
-        (seed, stream)): equals fill_noise + evolve_screens bit for bit; N = 512, 1024 (EUNSUPPORTED otherwise)."""
+        (seed, stream)): equals fill_noise + evolve_screens bit for bit; N >= 512 (EUNSUPPORTED below)."""
         B, S = spectrum.shape[0], spectrum.shape[1]
         if screens is None:
             screens = torch.empty((B, S, N, N), dtype=torch.float32, device=spectrum.device)

@@ -353,7 +353,7 @@ int ssp_evolve_screens_seeded(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, d
     if (n_sh > 0 && !d_sh_coef) return ctx->fail(SSP_EINVAL, "d_sh_coef (in-out) is required when n_sh > 0");
     if (first & 1ull) return ctx->fail(SSP_EINVAL, "the first draw index must be even");
     if (!screen_col_seeded_supported(grid.N))
-        return ctx->fail(SSP_EUNSUPPORTED, "seeded evolution is built for N = 512 and 1024 (use ssp_fill_noise + ssp_evolve_screens)");
+        return ctx->fail(SSP_EUNSUPPORTED, "seeded evolution is built for N >= 512 (use ssp_fill_noise + ssp_evolve_screens)");
     const ssp::NoiseSeed ns{seed, stream, first};
     return screens_impl(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, true, a, vx, vy, T, nullptr, d_fresh_noise_sh,
                         d_spectrum, d_sh_coef, d_screens, d_ws, nullptr, nullptr, nullptr, &ns);

@@ -42,7 +42,9 @@ __device__ __forceinline__ float psd_shape_sqrt(const ScreenFilter &f, float f2)
     return (f.kind == SSP_PSD_OCEAN_NIKISHOV) ? psd_shape_sqrt_k<true>(f, f2) : psd_shape_sqrt_k<false>(f, f2);
 }
 
-template <int N>
+// SEEDED: the fresh noise is drawn here instead of loaded (see k_screen_col_tma below); the draws pass through the
+// exchange buffer, which is idle until the transform.
+template <int N, bool SEEDED = false>
 __global__ void __launch_bounds__(ColCfg<N, 2>::THREADS, ColCfg<N, 2>::MIN_BLOCKS) k_screen_col(const ScreenColArgs a)
 {
     using PI = PlanInfo<N, 2>;
@@ -65,11 +67,29 @@ __global__ void __launch_bounds__(ColCfg<N, 2>::THREADS, ColCfg<N, 2>::MIN_BLOCK
     if (ar && a.taux) tx = __ldg(a.taux + kx);
 
     float2 v[E];
+    if constexpr (SEEDED) {
+        static_assert(!SEEDED || (E == R1 && C % 2 == 0 && E % 2 == 0), "one first-stage butterfly per thread, column pairs in adjacent lanes");
+        const unsigned long long e0 = a.first_draw + (unsigned long long)scr * N * N + (unsigned)(kx & ~1);
+        const int odd = c & 1;
+SSP_SEED_PRAGMA(unroll SSP_SEED_UNROLL)
+        for (int q = 0; q < E; q += 2) {
+            const int ky_m = line_index<N, 2, R1>(t, 0, q + odd);     // the row whose block this lane computes
+            uint32_t w[4];
+            philox_block(a.keys, (e0 + (unsigned long long)ky_m * N) >> 1, a.stream_lo, a.stream_hi, w);
+            const float2 z0 = box_muller(w[0], w[1]), z1 = box_muller(w[2], w[3]);
+            *reinterpret_cast<float4 *>(smem + ky_m * C + (c & ~1)) = make_float4(z0.x, z0.y, z1.x, z1.y);
+        }
+        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < E; ++q) v[q] = smem[line_index<N, 2, R1>(t, 0, q) * C + c];
+        __syncthreads();                                          // the exchange buffer is the transform's from here on
+    } else {
     // all noise loads first (independent, in flight together), then filter in registers
 #pragma unroll
     for (int i = 0; i < E / R1; ++i)
 #pragma unroll
         for (int q = 0; q < R1; ++q) v[i * R1 + q] = __ldg(a.noise + base + (size_t)line_index<N, 2, R1>(t, i, q) * N);
+    }
 #pragma unroll
     for (int i = 0; i < E / R1; ++i)
 #pragma unroll
@@ -340,11 +360,14 @@ template <int N>
 static int launch_screen_col_n(ssp_ctx *ctx, const ScreenColArgs &a)
 {
     using CFG = ColCfg<N, 2>;
-    auto kern = k_screen_col<N>;
+    constexpr bool CAN_SEED = (N >= 2048);                        // the seeded instance is built for the tall grids only
+    const bool seeded = !a.noise;
+    if (seeded && !CAN_SEED) return ctx->fail(SSP_EUNSUPPORTED, "no seeded generator for N=%d", N);
+    auto kern = (seeded && CAN_SEED) ? k_screen_col<N, CAN_SEED> : k_screen_col<N, false>;
     if (CFG::SMEM > 48 * 1024)
         SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::SMEM));
-    const double bpp = 16.0 + (a.old_spec ? 8.0 : 0.0) + (a.spec_out ? 8.0 : 0.0);
-    ctx->prof_begin("screen_col", bpp * (double)a.nscr * N * N);
+    const double bpp = (seeded ? 8.0 : 16.0) + (a.old_spec ? 8.0 : 0.0) + (a.spec_out ? 8.0 : 0.0);
+    ctx->prof_begin(seeded ? "screen_col_seeded" : "screen_col", bpp * (double)a.nscr * N * N);
     kern<<<a.nscr * (N / CFG::C), CFG::THREADS, CFG::SMEM, ctx->stream>>>(a);
     ctx->prof_end();
     ctx->launches++;
@@ -412,7 +435,7 @@ static int launch_screen_row_n(ssp_ctx *ctx, const ScreenRowArgs &a)
 
 
 // the TMA generator runs the column plan (V = 1), the register-load one its own (V = 2); they differ at N >= 2048
-bool screen_col_seeded_supported(int N) { return N == 512 || N == 1024; }
+bool screen_col_seeded_supported(int N) { return N >= 512; }
 
 int screen_col_plan_variant(int N) { return (N == 512 || N == 1024) ? 1 : 2; }
 
@@ -423,7 +446,8 @@ int launch_screen_col(ssp_ctx *ctx, int N, const ScreenColArgs &a)
         if (N == 512) return launch_screen_col_tma_n<512>(ctx, a);
         if (N == 1024) return launch_screen_col_tma_n<1024>(ctx, a);
     }
-    if (!a.noise) return ctx->fail(SSP_EUNSUPPORTED, "seeded noise needs the TMA generator (N = 512, 1024; spectrum kept in place)");
+    if (!a.noise && (N < 2048 || !a.old_spec))
+        return ctx->fail(SSP_EUNSUPPORTED, "the seeded generator is built for the evolution at N >= 512 (512 / 1024: spectrum kept in place)");
     SSP_DISPATCH_N(N, (launch_screen_col_n<NN>(ctx, a)));
 }
 int row_last_radix(int N)
