@@ -345,10 +345,13 @@ def run_ours(args):
             frame(args.warmup + i, resident=True)
         r1.record()
         sync_all()
-        ms_res = r0.elapsed_time(r1) / n_res
+        t_res = torch.tensor([r0.elapsed_time(r1)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t_res, op=dist.ReduceOp.MAX)
+        ms_res = float(t_res.item()) / n_res
         resident_noise = {"what": "the step with ssp_evolve_screens reading the frame's fresh noise from a resident array "
                                   "(8 B/px more traffic, no draws)", "ms_per_step": ms_res,
-                          "value": units_step / world / (ms_res * 1e-3), "steps": n_res}
+                          "value": units_step / (ms_res * 1e-3), "steps": n_res}
 
     # ---- roofline of the dominant kernel class (by device time inside the timed region)
     peak, peak_src = peaks()
