@@ -190,6 +190,7 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
 #pragma unroll
         for (int i = 0; i < 6; ++i) mbar_init(&full[i], 1);
         fence_mbar_init();
+        pdl_wait();                                               // (ssp_internal.h) the tiles are the previous kernel's output
         if ((int)blockIdx.x < a.ntiles) issue_load(blockIdx.x, 0, 0);
         if constexpr (NG == 2) {                                  // all three buffers start empty: fill 0 of buffers 1 and 2
             if ((int)(blockIdx.x + gridDim.x) < a.ntiles) issue_load(blockIdx.x + gridDim.x, 1, 2);
@@ -223,6 +224,7 @@ k_col_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUt
         }
         tmem_wait_st();
     }
+    pdl_wait();                                                   // every thread: the H2D multiplier map may be the previous kernel's output
 
     // the CTA's n-th tile is blockIdx.x + n gridDim.x; with two groups, group grp takes n = grp, grp + 2, ..
     int it = (NG == 2) ? grp : 0;
@@ -378,6 +380,7 @@ k_col_tma_wide(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
     if (tid == 0) {
         mbar_init(full, 1);
         fence_mbar_init();
+        pdl_wait();                                               // (ssp_internal.h) the tiles are the previous kernel's output
         if ((int)blockIdx.x < a.ntiles) issue_load(blockIdx.x);
     }
     if (tid < 32) tmem_alloc(&tmem_slot, CFG::TMEM_COLS);
@@ -400,6 +403,7 @@ k_col_tma_wide(const __grid_constant__ CUtensorMap tm_in, const __grid_constant_
         tmem_wait_st();
     }
     // X hand-over between the pairs: barrier 3 = "pair 0 has read its exchange", 4 = "pair 1 has read its exchange"
+    pdl_wait();                                                   // every thread: the H2D multiplier map may be the previous kernel's output
     auto release = [&]() { asm volatile("bar.arrive %0, %1;" ::"r"(3 + pair), "n"(2 * GT) : "memory"); };
     auto wait_other = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(4 - pair), "n"(2 * GT) : "memory"); };
 

@@ -177,6 +177,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS) k_r
         }
         tmem_wait_st();
     }
+    pdl_wait();                                                   // (ssp_internal.h) everything above read constant tables only
     const long long nblk = TM ? (long long)(a.n_lines / CFG::LPB) : (long long)blockIdx.x + 1;
     for (long long blk = blockIdx.x; blk < nblk; blk += gridDim.x) {
     const long long line = blk * CFG::LPB + lib;
@@ -422,6 +423,7 @@ __global__ void __launch_bounds__(ColCfg<N>::THREADS, ColCfg<N>::MIN_BLOCKS) k_c
     constexpr int GROUPS = N / C;
     const int b = blockIdx.x / GROUPS, col = (blockIdx.x % GROUPS) * C + c;
     ColSmem<C> sm{smem + c};
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
 
     float2 v[E];
     constexpr int R1 = PI::R1, RL = PI::RL;

@@ -39,7 +39,7 @@ static int launch_row_x(ssp_ctx *ctx, const RowArgs &a)
         const int resident = ctx->num_sms * CFG::MIN_BLOCKS;
         if (grid > resident) grid = resident;
     }
-    kern<<<grid, CFG::THREADS, CFG::SMEM + (TM ? 16 : 0), ctx->stream>>>(a);
+    SSP_CUDA(ctx, launch_pdl(kern, dim3(grid), dim3(CFG::THREADS), CFG::SMEM + (TM ? 16 : 0), ctx->stream, pdl_enabled(), a));
     ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
@@ -85,7 +85,7 @@ static int launch_col_n(ssp_ctx *ctx, const ColArgs &a)
     auto kern = k_col<N, MODE>;
     if (int rc = set_smem(ctx, kern, CFG::SMEM)) return rc;
     ctx->prof_begin(MODE == 0 ? "col_fft_h_ifft" : "col_single", 16.0 * (double)a.B * N * N);
-    kern<<<a.B * (N / CFG::C), CFG::THREADS, CFG::SMEM, ctx->stream>>>(a);
+    SSP_CUDA(ctx, launch_pdl(kern, dim3(a.B * (N / CFG::C)), dim3(CFG::THREADS), CFG::SMEM, ctx->stream, pdl_enabled(), a));
     ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
@@ -131,7 +131,7 @@ static int launch_col_tma_x(ssp_ctx *ctx, const ColArgs &a)
     const int grid = (CFG::PERSIST && ntiles > resident) ? resident : ntiles;
     ColTmaArgs ta{a.hy, a.h2d, a.tw, ntiles};
     ctx->prof_begin("col_fft_h_ifft", 16.0 * (double)a.B * N * N);
-    kern<<<grid, CFG::THREADS, CFG::SMEM, ctx->stream>>>(tm_in, tm_out, ta);
+    SSP_CUDA(ctx, launch_pdl(kern, dim3(grid), dim3(CFG::THREADS), CFG::SMEM, ctx->stream, pdl_enabled(), tm_in, tm_out, ta));
     ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
@@ -152,7 +152,7 @@ static int launch_col_wide_x(ssp_ctx *ctx, const ColArgs &a)
     const int grid = ntiles > ctx->num_sms ? ctx->num_sms : ntiles;
     ColTmaArgs ta{a.hy, a.h2d, a.tw, ntiles};
     ctx->prof_begin("col_fft_h_ifft", 16.0 * (double)a.B * N * N);
-    kern<<<grid, CFG::THREADS, CFG::SMEM, ctx->stream>>>(tm_in, tm_out, ta);
+    SSP_CUDA(ctx, launch_pdl(kern, dim3(grid), dim3(CFG::THREADS), CFG::SMEM, ctx->stream, pdl_enabled(), tm_in, tm_out, ta));
     ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());

@@ -57,6 +57,7 @@ __global__ void __launch_bounds__(ColCfg<N, 2>::THREADS, ColCfg<N, 2>::MIN_BLOCK
     constexpr int GROUPS = N / C;
     const int scr = blockIdx.x / GROUPS, kx = (blockIdx.x % GROUPS) * C + c;
     ColSmem<C> sm{smem + c};
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
 
     const float amp_s = __ldg(a.amp + (a.g0 + scr) % a.S);
     const float kxs = (float)((kx < N / 2) ? kx : kx - N);
@@ -155,6 +156,7 @@ k_screen_col_tma(const __grid_constant__ CUtensorMap tm_noise, const __grid_cons
     const int tid = threadIdx.x, c = tid % C, t = fft_logical_t<N, 1, C>(tid / C);
     const int scr = blockIdx.x / GROUPS, col0 = (blockIdx.x % GROUPS) * C, kx = col0 + c;
     constexpr bool ar = AR;
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
 
     if (tid == 0) {
         mbar_init(full, 1);
@@ -257,6 +259,7 @@ __global__ void __launch_bounds__(RowCfg<N>::THREADS, RowCfg<N>::MIN_BLOCKS + (N
     const long long line = (long long)blockIdx.x * CFG::LPB + lib;
     const int scr = (int)(line / N), iy = (int)(line % N);
     RowSmem<T, CFG::WIDE> sm{smem + (size_t)lib * CFG::LINE_ELEMS, 1 + lib};
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
 
     float2 v[E];
     const float2 *src = a.in + line * N;
@@ -368,7 +371,7 @@ static int launch_screen_col_n(ssp_ctx *ctx, const ScreenColArgs &a)
         SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::SMEM));
     const double bpp = (seeded ? 8.0 : 16.0) + (a.old_spec ? 8.0 : 0.0) + (a.spec_out ? 8.0 : 0.0);
     ctx->prof_begin(seeded ? "screen_col_seeded" : "screen_col", bpp * (double)a.nscr * N * N);
-    kern<<<a.nscr * (N / CFG::C), CFG::THREADS, CFG::SMEM, ctx->stream>>>(a);
+    SSP_CUDA(ctx, launch_pdl(kern, dim3(a.nscr * (N / CFG::C)), dim3(CFG::THREADS), CFG::SMEM, ctx->stream, pdl_enabled(), a));
     ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
@@ -391,7 +394,7 @@ static int launch_screen_col_tma_x(ssp_ctx *ctx, const ScreenColArgs &a)
     SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::smem(2)));
     const double bpp = (SEEDED ? 8.0 : 16.0) + (a.old_spec ? 8.0 : 0.0) + (a.spec_out ? 8.0 : 0.0);
     ctx->prof_begin(SEEDED ? "screen_col_seeded" : "screen_col", bpp * (double)a.nscr * N * N);
-    kern<<<a.nscr * (N / CFG::C), CFG::THREADS, smem, ctx->stream>>>(tm_noise, tm_spec, tm_out, a);
+    SSP_CUDA(ctx, launch_pdl(kern, dim3(a.nscr * (N / CFG::C)), dim3(CFG::THREADS), smem, ctx->stream, pdl_enabled(), tm_noise, tm_spec, tm_out, a));
     ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
@@ -426,7 +429,7 @@ static int launch_screen_row_n(ssp_ctx *ctx, const ScreenRowArgs &a)
     if (smem > 48 * 1024)
         SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ctx->prof_begin("screen_row", (a.screens_im ? 16.0 : 12.0) * (double)a.nscr * N * N);
-    kern<<<(unsigned)((long long)a.nscr * N / CFG::LPB), CFG::THREADS, smem, ctx->stream>>>(a);
+    SSP_CUDA(ctx, launch_pdl(kern, dim3((unsigned)((long long)a.nscr * N / CFG::LPB)), dim3(CFG::THREADS), smem, ctx->stream, pdl_enabled(), a));
     ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());

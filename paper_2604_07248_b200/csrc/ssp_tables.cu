@@ -5,9 +5,17 @@
 #include <cmath>
 
 #include "ssp_fft.cuh"
+#include <cstdlib>
+
 #include "ssp_internal.h"
 
 namespace ssp {
+
+bool pdl_enabled()
+{
+    static const bool off = getenv("SSP_NO_PDL") != nullptr;
+    return !off;
+}
 
 bool valid_N(int N) { return N >= 8 && N <= 4096 && (N & (N - 1)) == 0; }
 
