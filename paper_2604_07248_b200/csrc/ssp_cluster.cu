@@ -59,6 +59,7 @@ __global__ void __launch_bounds__(ClusterCfg<N>::THREADS, 1) k_cluster(const Sma
     const int tid = threadIdx.x, b = blockIdx.x / CS;
     const int ll = tid / T, t = tid % T;                           // local line, thread within the line
     const int gl = rank * L + ll;                                  // global row (row pass) / column (column pass)
+    pdl_wait();                                                    // (ssp_internal.h: programmatic dependent launch)
 
     const float2 *src = a.in + ((size_t)b * N + (size_t)rank * L) * N;
     for (int i = tid; i < L * N; i += CFG::THREADS) A[(i / N) * PITCH + i % N] = src[i];
@@ -173,13 +174,15 @@ static int launch_cluster_n(ssp_ctx *ctx, int B, const SmallArgs &a)
     cfg.blockDim = dim3(CFG::THREADS);
     cfg.dynamicSmemBytes = CFG::SMEM;
     cfg.stream = ctx->stream;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = CFG::CS;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = pdl_enabled() ? 2 : 1;
     ctx->prof_begin("cluster_on_chip", (16.0 + 4.0 * a.n_screens) * (double)B * N * N);
     SSP_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, a));
     ctx->prof_end();

@@ -95,6 +95,7 @@ __global__ void __launch_bounds__(256) k_stats_final(const double *__restrict__ 
                                                       ssp_stats *__restrict__ out)
 {
     const int b = blockIdx.x, tid = threadIdx.x;
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
     double a[ACC_N];
 #pragma unroll
     for (int i = 0; i < ACC_N; ++i) a[i] = 0.0;
@@ -133,7 +134,7 @@ void stats_roi(int N, double roi_frac, int *lo_out, int *hi_out, long long *roi_
 
 int launch_stats_final(ssp_ctx *ctx, int B, int bpf, double dx, long long roi_n, const double *acc, ssp_stats *d_stats)
 {
-    k_stats_final<<<B, 256, 0, ctx->stream>>>(acc, bpf, dx, roi_n, d_stats);
+    SSP_CUDA(ctx, launch_pdl(k_stats_final, dim3(B), dim3(256), 0, ctx->stream, pdl_enabled(), acc, bpf, dx, roi_n, d_stats));
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;

@@ -331,6 +331,7 @@ __global__ void __launch_bounds__(96) k_sh_prep(int S, int n_sh, const float2 *_
 {
     __shared__ float red[96], red_im[96];
     const int scr = blockIdx.x, i = threadIdx.x, s = scr % S;
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
     float contrib = 0.f, contrib_im = 0.f;
     if (i < 9 * n_sh) {
         const size_t idx = (size_t)scr * n_sh * 9 + i;
@@ -479,8 +480,8 @@ int launch_sh_prep(ssp_ctx *ctx, int nscr, int S, int n_sh, const float2 *noise_
                    const float2 *tau_sh, float ar_a, float ar_g, const float2 *old_coef, float2 *coef_out,
                    const float2 *mfac, float *mean_out)
 {
-    k_sh_prep<<<nscr, 96, 0, ctx->stream>>>(S, n_sh, noise_sh, amp_sh, tau_sh, ar_a, ar_g, old_coef, coef_out,
-                                            mfac, mean_out);
+    SSP_CUDA(ctx, launch_pdl(k_sh_prep, dim3(nscr), dim3(96), 0, ctx->stream, pdl_enabled(), S, n_sh, noise_sh, amp_sh, tau_sh,
+                             ar_a, ar_g, old_coef, coef_out, mfac, mean_out));
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;

@@ -56,6 +56,7 @@ __global__ void __launch_bounds__(SmallCfg<N>::THREADS, 1) k_small(const SmallAr
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *F = reinterpret_cast<float2 *>(smem_raw);
     const int tid = threadIdx.x, b = blockIdx.x;
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
 
     // field -> shared memory, coalesced
     const float2 *src = a.in + (size_t)b * N * N;
@@ -168,7 +169,7 @@ static int launch_small_n(ssp_ctx *ctx, int B, const SmallArgs &a)
     SSP_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CFG::SMEM));
     // algorithmic bytes of the on-chip schedule: field in + out once, one screen per step
     ctx->prof_begin("small_on_chip", (16.0 + 4.0 * a.n_screens) * (double)B * N * N);
-    kern<<<B, CFG::THREADS, CFG::SMEM, ctx->stream>>>(a);
+    SSP_CUDA(ctx, launch_pdl(kern, dim3(B), dim3(CFG::THREADS), CFG::SMEM, ctx->stream, pdl_enabled(), a));
     ctx->prof_end();
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
