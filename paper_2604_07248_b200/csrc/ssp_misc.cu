@@ -197,6 +197,7 @@ int launch_welford(ssp_ctx *ctx, int N, int B, const float2 *field, float *mean,
 __global__ void __launch_bounds__(256) k_phase_mul(const float *__restrict__ theta, float sign, size_t px, int B,
                                                     const float2 *in, float2 *out)
 {
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= px) return;
     float s, c;
@@ -249,6 +250,7 @@ __global__ void __launch_bounds__(256) k_adam(size_t n, int B, const float *__re
                                                float eps, float c1, float c2, float o1, float o2, float *__restrict__ m,
                                                float *__restrict__ v, float *__restrict__ theta)
 {
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     float g = 0.f;
@@ -264,7 +266,7 @@ __global__ void __launch_bounds__(256) k_adam(size_t n, int B, const float *__re
 int launch_adam(ssp_ctx *ctx, long long n, int B, const float *grad, float lr, float b1, float b2, float eps,
                 float c1, float c2, float o1, float o2, float *m, float *v, float *theta)
 {
-    k_adam<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>((size_t)n, B, grad, lr, b1, b2, eps, c1, c2, o1, o2, m, v, theta);
+    SSP_CUDA(ctx, launch_pdl(k_adam, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, ctx->stream, pdl_enabled(), (size_t)n, B, grad, lr, b1, b2, eps, c1, c2, o1, o2, m, v, theta));
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;
@@ -273,6 +275,7 @@ int launch_adam(ssp_ctx *ctx, long long n, int B, const float *grad, float lr, f
 // circular aperture: integer test against a host-decided threshold
 __global__ void __launch_bounds__(256) k_aperture(int N, long long r2max, const float2 *__restrict__ in, float2 *__restrict__ out)
 {
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
     const int ix = blockIdx.x * blockDim.x + threadIdx.x, iy = blockIdx.y, b = blockIdx.z;
     if (ix >= N) return;
     const long long x = ix - N / 2, y = iy - N / 2;
@@ -282,7 +285,7 @@ __global__ void __launch_bounds__(256) k_aperture(int N, long long r2max, const 
 
 int launch_aperture(ssp_ctx *ctx, int N, int B, long long r2max_px, const float2 *in, float2 *out)
 {
-    k_aperture<<<dim3((N + 255) / 256, N, B), 256, 0, ctx->stream>>>(N, r2max_px, in, out);
+    SSP_CUDA(ctx, launch_pdl(k_aperture, dim3((N + 255) / 256, N, B), dim3(256), 0, ctx->stream, pdl_enabled(), N, r2max_px, in, out));
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;
@@ -291,7 +294,7 @@ int launch_aperture(ssp_ctx *ctx, int N, int B, long long r2max_px, const float2
 int launch_phase_mul(ssp_ctx *ctx, int N, int B, const float *theta, float sign, const float2 *in, float2 *out)
 {
     const size_t px = (size_t)N * N;
-    k_phase_mul<<<(unsigned)((px + 255) / 256), 256, 0, ctx->stream>>>(theta, sign, px, B, in, out);
+    SSP_CUDA(ctx, launch_pdl(k_phase_mul, dim3((unsigned)((px + 255) / 256)), dim3(256), 0, ctx->stream, pdl_enabled(), theta, sign, px, B, in, out));
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;
@@ -300,6 +303,7 @@ int launch_phase_mul(ssp_ctx *ctx, int N, int B, const float *theta, float sign,
 __global__ void __launch_bounds__(256) k_phase_grad(const float2 *__restrict__ g, const float2 *__restrict__ u,
                                                      size_t n, float *__restrict__ grad)
 {
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float2 a = g[i], b = u[i];
@@ -308,7 +312,7 @@ __global__ void __launch_bounds__(256) k_phase_grad(const float2 *__restrict__ g
 
 int launch_phase_grad(ssp_ctx *ctx, long long n, const float2 *g, const float2 *u, float *grad)
 {
-    k_phase_grad<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(g, u, (size_t)n, grad);
+    SSP_CUDA(ctx, launch_pdl(k_phase_grad, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, ctx->stream, pdl_enabled(), g, u, (size_t)n, grad));
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;
@@ -318,6 +322,7 @@ int launch_phase_grad(ssp_ctx *ctx, long long n, const float2 *g, const float2 *
 __global__ void __launch_bounds__(256) k_inner(const float2 *__restrict__ A, const float2 *__restrict__ Bf,
                                                 size_t px, double *__restrict__ out)
 {
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
     const int b = blockIdx.y;
     double r = 0, im = 0, na = 0, nb = 0;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < px; i += (size_t)gridDim.x * blockDim.x) {
@@ -341,6 +346,7 @@ __global__ void __launch_bounds__(256) k_inner(const float2 *__restrict__ A, con
 __global__ void __launch_bounds__(256) k_mae(const float2 *__restrict__ V, const float2 *__restrict__ Tg, size_t px,
                                               float inv_px, double *__restrict__ loss, float2 *__restrict__ G)
 {
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
     const int b = blockIdx.y;
     double acc = 0.0;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < px; i += (size_t)gridDim.x * blockDim.x) {
@@ -367,7 +373,7 @@ int launch_mae(ssp_ctx *ctx, int N, int B, const float2 *v, const float2 *t, dou
     const size_t px = (size_t)N * N;
     SSP_CUDA(ctx, cudaMemsetAsync(loss, 0, sizeof(double) * (size_t)B, ctx->stream));
     int bpf = (int)((px + 256 * 8 - 1) / (256 * 8));
-    k_mae<<<dim3(bpf, B), 256, 0, ctx->stream>>>(v, t, px, (float)(1.0 / (double)px), loss, g);
+    SSP_CUDA(ctx, launch_pdl(k_mae, dim3(bpf, B), dim3(256), 0, ctx->stream, pdl_enabled(), v, t, px, (float)(1.0 / (double)px), loss, g));
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;
@@ -378,7 +384,7 @@ int launch_inner(ssp_ctx *ctx, int N, int B, const float2 *a, const float2 *b, d
     const size_t px = (size_t)N * N;
     SSP_CUDA(ctx, cudaMemsetAsync(out, 0, sizeof(double) * 4 * (size_t)B, ctx->stream));
     int bpf = (int)((px + 256 * 16 - 1) / (256 * 16));
-    k_inner<<<dim3(bpf, B), 256, 0, ctx->stream>>>(a, b, px, out);
+    SSP_CUDA(ctx, launch_pdl(k_inner, dim3(bpf, B), dim3(256), 0, ctx->stream, pdl_enabled(), a, b, px, out));
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;
@@ -387,6 +393,7 @@ int launch_inner(ssp_ctx *ctx, int N, int B, const float2 *a, const float2 *b, d
 __global__ void __launch_bounds__(256) k_lincomb(const float2 *__restrict__ coef, const float2 *a, const float2 *b,
                                                   size_t px, float2 *out)
 {
+    pdl_wait();                                                   // (ssp_internal.h: programmatic dependent launch)
     const int f = blockIdx.y;
     const float2 al = coef[2 * f], be = coef[2 * f + 1];
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < px; i += (size_t)gridDim.x * blockDim.x) {
@@ -400,7 +407,7 @@ int launch_lincomb(ssp_ctx *ctx, int N, int B, const float2 *coef, const float2 
 {
     const size_t px = (size_t)N * N;
     int bpf = (int)((px + 256 * 4 - 1) / (256 * 4));
-    k_lincomb<<<dim3(bpf, B), 256, 0, ctx->stream>>>(coef, a, b, px, out);
+    SSP_CUDA(ctx, launch_pdl(k_lincomb, dim3(bpf, B), dim3(256), 0, ctx->stream, pdl_enabled(), coef, a, b, px, out));
     ctx->launches++;
     SSP_CUDA(ctx, cudaGetLastError());
     return SSP_OK;
