@@ -137,7 +137,8 @@ int ensure_scratch(ssp_ctx *ctx, size_t bytes);
 // launch_pdl() MUST call pdl_wait() on every path.  Measured (forward + adjoint, profiler off): 1024^2 B = 32 9.49 -> 9.36
 // ms, 2048^2 3.50 -> 3.44, 256^2 B = 8 (launch-bound) 0.161 -> 0.119.  An EARLY trigger (griddepcontrol.launch_dependents
 // at the top of each kernel, so that the next kernel's CTAs move in as this one's retire and run their prologue under its
-// tail) measured much slower on the persistent kernels -- 1024^2 12.46 ms, 2048^2 3.81 -- and is not used.
+// tail) measured much slower on the persistent kernels -- 1024^2 12.46 ms, 2048^2 3.81 --, a LATE one (at the start of a CTA's
+// last tile) no better than none (1024^2 9.57 against 9.50 ms, 2048^2 3.87 against 3.52): no trigger is issued.
 #ifdef __CUDACC__
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 template <class... KA, class... A>
