@@ -249,3 +249,27 @@ def test_seeded_evolution_rejects_small_grids_and_odd_offsets(ssp):
     with pytest.raises(api.SspError) as e:                     # odd first draw
         ssp.evolve_screens_seeded(512, 1e-3, psd, 1e-6, [1e-14], [100.0], 0, 0.9, 0, 0, 0, 1, 2, 3, None, spec, None)
     assert e.value.code == api.EINVAL
+
+
+def test_seeded_evolution_across_generator_chunks(ssp):
+    """The generator works through B x S screens in chunks of 512 MB of column-transformed spectra (256 screens at 512^2);
+    the seeded kernel's draw index must continue across the chunk boundary: 300 screens, one frame, bytes of fill + evolve."""
+    from paper_2604_07248_b200 import api
+    N, B, S, dx, lam, n_sh = 512, 30, 10, 2e-3, 1.0e-6, 1
+    psd = api.PsdParams(kind=api.PSD_VON_KARMAN, L0=10.0, l0=5e-3)
+    cn2, dz = [1e-14] * S, [100.0] * S
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    nsh = torch.view_as_complex(torch.randn(B, S, n_sh, 3, 3, 2, device="cuda", generator=gen))
+    fresh = torch.empty((B, S, N, N), dtype=torch.complex64, device="cuda")
+    ssp.fill_noise(11, 4, fresh, first=2 * N * N)
+    out = []
+    for seeded in (False, True):
+        spec = torch.zeros((B, S, N, N), dtype=torch.complex64, device="cuda")
+        shc = torch.zeros((B, S, n_sh, 3, 3), dtype=torch.complex64, device="cuda")
+        if seeded:
+            scr = ssp.evolve_screens_seeded(N, dx, psd, lam, cn2, dz, n_sh, 0.5, 0.3, 0.1, 1e-2, 11, 4, 2 * N * N, nsh, spec, shc)
+        else:
+            scr = ssp.evolve_screens(N, dx, psd, lam, cn2, dz, n_sh, 0.5, 0.3, 0.1, 1e-2, fresh, nsh, spec, shc)
+        out.append((scr, spec))
+    assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1])
+    assert float(out[1][0][-1].abs().max()) > 0                # the last chunk was written
