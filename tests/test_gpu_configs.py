@@ -193,7 +193,7 @@ def test_config5_ocean_all_screens(ssp, orc):
 
 def test_bench_launch_configuration_full_size(ssp, orc):
     """The launch configuration bench.py times (config 3 in full: 1024^2, B = 32 stacks of 20 screens, one AR
-    frame): realisation 17 of the batch is checked against the oracle run on that realisation alone (screens,
+    frame with the seeded generator): realisation 17 of the batch is checked against the oracle run on that realisation alone (screens,
     received field, adjoint field); properties that hold at any size cover the rest of the batch."""
     import torch
     from paper_2604_07248_b200 import api
@@ -208,7 +208,10 @@ def test_bench_launch_configuration_full_size(ssp, orc):
     shc = torch.zeros((B, S, wl.n_sh, 3, 3), dtype=torch.complex64, device="cuda")
     cn2, dz = list(wl.cn2_list), list(wl.dz)
     ssp.make_screens(N, wl.dx, pg, wl.lam, cn2, dz, wl.n_sh, noise[0], noise_sh[0], spectrum=spec, sh_coef=shc)
-    scr = ssp.evolve_screens(N, wl.dx, pg, wl.lam, cn2, dz, wl.n_sh, wl.ar_a, 0, 0, 0, noise[1], noise_sh[1], spec, shc)
+    # as bench.py does it: the frame's fresh grid noise is drawn inside the generator (ssp_evolve_screens_seeded); the same
+    # draws are written out by ssp_fill_noise for the oracle (tests/test_gpu_noise.py: the two are the same bytes)
+    ssp.fill_noise(1234, 2, noise[1])
+    scr = ssp.evolve_screens_seeded(N, wl.dx, pg, wl.lam, cn2, dz, wl.n_sh, wl.ar_a, 0, 0, 0, 1234, 2, 0, noise_sh[1], spec, shc)
     # the oracle consumes the same white noise (as drawn on the device, copied back) for realisation b_s
     f2 = lambda t: np.ascontiguousarray(torch.view_as_real(t[b_s:b_s + 1]).cpu().numpy())
     _, spec_ref, shc_ref = orc.make_screens(N, wl.dx, po, wl.lam, wl.cn2_list, wl.dz, wl.n_sh, f2(noise[0]), f2(noise_sh[0]))
