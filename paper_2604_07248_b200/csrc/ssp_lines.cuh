@@ -66,7 +66,8 @@ struct RowCfg {
 #endif
     // measured: 1024 +4 % (+1.3 % more with the next-row prefetch), 512 +12 % (3907 -> 4381 GB/s); 2048 as two rows per
     // 128-thread CTA -4 % and 4096 -10 % (both spill at 168 registers; 4096 with 255 registers at 2 or 3 CTAs/SM:
-    // 3805 -> 3458 / 3427 GB/s), so those keep the one-row-per-CTA kernels
+    // 3805 -> 3458 / 3427 GB/s; without the next-row prefetch, 168 registers: 3788 -> 3482), so those keep the
+    // one-row-per-CTA kernels
     static constexpr bool TMEM = (N == 1024 && SSP_ROW1024_TMEM) || (N == 512 && SSP_ROW512_TMEM);
 };
 
