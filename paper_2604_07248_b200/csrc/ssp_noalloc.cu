@@ -108,7 +108,10 @@ __global__ void __launch_bounds__(256) k_stats_static(const float2 *__restrict__
         __threadfence();                                   // the record is visible device-wide before the ticket is
     }
     __syncthreads();
-    if (tid == 0) last = atomicAdd(tickets + b, 1u) == (unsigned)(bpf - 1);
+    if (tid == 0) {
+        __threadfence();                                   // cumulative: the nine writers' records (seen through the barrier) before the ticket
+        last = atomicAdd(tickets + b, 1u) == (unsigned)(bpf - 1);
+    }
     __syncthreads();
     if (!last) return;
     __threadfence();                                       // ... and the last block sees every other block's record
