@@ -155,6 +155,14 @@ int ssp_evolve_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double l
  * ssp_evolve_screens(.., noise, ..) bit for bit, without the 8 B/px write and the 8 B/px read of that array (and without
  * the array).  The subharmonic noise (tiny) stays an input.  `first` even.  Built for N >= 512 (SSP_EUNSUPPORTED below:
  * draw the noise with ssp_fill_noise and call ssp_evolve_screens). */
+/* The first synthesis of the same kind: ssp_make_screens with the grid noise drawn in the generator (draw `first + e` for
+ * element e), equal to ssp_fill_noise + ssp_make_screens bit for bit.  With the two seeded calls a temporal simulation
+ * never holds a noise array.  N >= 512. */
+int ssp_make_screens_seeded(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
+                            int B, int S, const double *cn2, const double *dz, int n_sh,
+                            unsigned long long seed, unsigned long long stream, unsigned long long first,
+                            const float *d_noise_sh, float *d_spectrum, float *d_sh_coef, float *d_screens,
+                            void *d_ws, size_t ws_bytes);
 int ssp_evolve_screens_seeded(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
                               int B, int S, const double *cn2, const double *dz, int n_sh,
                               double a, double vx, double vy, double T,

@@ -25,7 +25,7 @@ OK, EINVAL, EUNSUPPORTED, EWORKSPACE, ECUDA = 0, -1, -2, -3, -4
 # every symbol include/ssp.h declares (tests/test_abi.py checks the header against this list)
 SYMBOLS = (
     "ssp_create", "ssp_destroy", "ssp_last_error", "ssp_version", "ssp_launch_count",
-    "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_evolve_screens_seeded", "ssp_make_screens_pair", "ssp_evolve_screens_pair", "ssp_propagate",
+    "ssp_workspace_bytes", "ssp_make_screens", "ssp_evolve_screens", "ssp_evolve_screens_seeded", "ssp_make_screens_seeded", "ssp_make_screens_pair", "ssp_evolve_screens_pair", "ssp_propagate",
     "ssp_propagate_adjoint", "ssp_beam_stats", "ssp_beam_stats_static", "ssp_propagate_host", "ssp_phase_mul",
     "ssp_dft2_centered", "ssp_phase_grad", "ssp_inner_products", "ssp_lincomb", "ssp_aperture", "ssp_adam_update", "ssp_hv57_cn2", "ssp_hv57_path", "ssp_dz_max", "ssp_place_screens", "ssp_fill_noise", "ssp_philox_words", "ssp_evolve_propagate", "ssp_mae_loss", "ssp_frame_chunk", "ssp_frame_host",
     "ssp_profile_enable", "ssp_profile_report",
@@ -98,6 +98,8 @@ def load():
                                             C.c_size_t]
     lib.ssp_evolve_screens.argtypes = [P, Grid, C.POINTER(Psd), D, I, I, P, P, I, D, D, D, D, P, P, P, P, P, P,
                                        C.c_size_t]
+    lib.ssp_make_screens_seeded.argtypes = [P, Grid, C.POINTER(Psd), D, I, I, P, P, I, C.c_ulonglong, C.c_ulonglong, C.c_ulonglong,
+                                            P, P, P, P, P, C.c_size_t]
     lib.ssp_evolve_screens_seeded.argtypes = [P, Grid, C.POINTER(Psd), D, I, I, P, P, I, D, D, D, D, C.c_ulonglong, C.c_ulonglong, C.c_ulonglong, P, P, P, P, P,
                                               C.c_size_t]
     lib.ssp_propagate.argtypes = [P, Grid, D, D, I, I, I, P, P, L, I, Window, P, P, P, P, D, P, C.c_size_t]
@@ -317,6 +319,23 @@ class Context:
         self._chk(self._lib.ssp_evolve_screens(
             self._h, Grid(N, dx), C.byref(pc), lam, B, S, _host_doubles(cn2), _host_doubles(dz), n_sh,
             a, vx, vy, T, _dev(fresh, torch.complex64), _dev(fresh_sh, torch.complex64) if n_sh > 0 else None,
+            _dev(spectrum, torch.complex64), _dev(sh_coef, torch.complex64) if n_sh > 0 else None,
+            _dev(screens, torch.float32), _dev(ws), ws.numel()))
+        return screens
+
+    def make_screens_seeded(self, N, dx, psd: PsdParams, lam, cn2, dz, n_sh, seed, stream, first, B, noise_sh=None,
+                            spectrum=None, sh_coef=None, screens=None, ws=None):
+        """make_screens with the grid noise drawn inside the generator (draw first + element index of stream (seed, stream));
+        B stacks of len(cn2) screens; N >= 512."""
+        S = len(cn2)
+        dev = torch.device("cuda", self.device)
+        if screens is None:
+            screens = torch.empty((B, S, N, N), dtype=torch.float32, device=dev)
+        ws = self.workspace(N, dx, B, S) if ws is None else ws
+        pc = psd.c()
+        self._chk(self._lib.ssp_make_screens_seeded(
+            self._h, Grid(N, dx), C.byref(pc), lam, B, S, _host_doubles(cn2), _host_doubles(dz), n_sh,
+            int(seed), int(stream), int(first), _dev(noise_sh, torch.complex64) if n_sh > 0 else None,
             _dev(spectrum, torch.complex64), _dev(sh_coef, torch.complex64) if n_sh > 0 else None,
             _dev(screens, torch.float32), _dev(ws), ws.numel()))
         return screens

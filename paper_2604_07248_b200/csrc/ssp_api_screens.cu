@@ -338,6 +338,24 @@ int ssp_evolve_screens(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double l
                         d_fresh_noise, d_fresh_noise_sh, d_spectrum, d_sh_coef, d_screens, d_ws);
 }
 
+int ssp_make_screens_seeded(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
+                            int B, int S, const double *cn2, const double *dz, int n_sh,
+                            unsigned long long seed, unsigned long long stream, unsigned long long first,
+                            const float *d_noise_sh, float *d_spectrum, float *d_sh_coef, float *d_screens,
+                            void *d_ws, size_t ws_bytes)
+{
+    // (the screens pointer stands in for the absent noise array in the shared checks)
+    if (int rc = check_screens(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, d_screens, d_noise_sh, d_screens, d_ws, ws_bytes))
+        return rc;
+    if (d_spectrum && !aligned16(d_spectrum)) return ctx->fail(SSP_EINVAL, "d_spectrum must be 16-byte aligned");
+    if (first & 1ull) return ctx->fail(SSP_EINVAL, "the first draw index must be even");
+    if (!screen_col_seeded_supported(grid.N))
+        return ctx->fail(SSP_EUNSUPPORTED, "seeded synthesis is built for N >= 512 (use ssp_fill_noise + ssp_make_screens)");
+    const ssp::NoiseSeed ns{seed, stream, first};
+    return screens_impl(ctx, grid, psd, lambda, B, S, cn2, dz, n_sh, false, 0.0, 0.0, 0.0, 0.0, nullptr, d_noise_sh,
+                        d_spectrum, d_sh_coef, d_screens, d_ws, nullptr, nullptr, nullptr, &ns);
+}
+
 int ssp_evolve_screens_seeded(ssp_ctx *ctx, ssp_grid grid, const ssp_psd *psd, double lambda,
                               int B, int S, const double *cn2, const double *dz, int n_sh,
                               double a, double vx, double vy, double T,

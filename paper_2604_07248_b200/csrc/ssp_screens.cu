@@ -161,8 +161,7 @@ k_screen_col_tma(const __grid_constant__ CUtensorMap tm_noise, const __grid_cons
     if (tid == 0) {
         mbar_init(full, 1);
         fence_mbar_init();
-        static_assert(!SEEDED || AR, "the seeded form is built for the evolution");
-        mbar_expect_tx(full, (ar && !SEEDED) ? 2 * CFG::TILE_BYTES : CFG::TILE_BYTES);
+        if constexpr (ar || !SEEDED) mbar_expect_tx(full, (ar && !SEEDED) ? 2 * CFG::TILE_BYTES : CFG::TILE_BYTES);
         if constexpr (!SEEDED) {
 #pragma unroll
             for (int j = 0; j < CFG::BOXES; ++j)
@@ -199,7 +198,7 @@ SSP_SEED_PRAGMA(unroll SSP_SEED_UNROLL)
         }
         __syncwarp();
     }
-    mbar_wait(full, 0);
+    if constexpr (ar || !SEEDED) mbar_wait(full, 0);              // (seeded first synthesis: nothing is loaded)
 
 #pragma unroll
     for (int i = 0; i < E / R1; ++i)
@@ -407,7 +406,7 @@ static int launch_screen_col_tma_n(ssp_ctx *ctx, const ScreenColArgs &a)
 {
     const bool ocean = a.flt.kind == SSP_PSD_OCEAN_NIKISHOV, ar = a.old_spec != nullptr, tilt = ar && a.taux;
     if (!a.noise) {                                               // seeded: the fresh noise is drawn in the kernel
-        if (!ar) return ctx->fail(SSP_EUNSUPPORTED, "seeded noise is built for the screen evolution");
+        if (!ar) return ocean ? launch_screen_col_tma_x<N, true, false, false, true>(ctx, a) : launch_screen_col_tma_x<N, false, false, false, true>(ctx, a);
         if (ocean) return tilt ? launch_screen_col_tma_x<N, true, true, true, true>(ctx, a) : launch_screen_col_tma_x<N, true, true, false, true>(ctx, a);
         return tilt ? launch_screen_col_tma_x<N, false, true, true, true>(ctx, a) : launch_screen_col_tma_x<N, false, true, false, true>(ctx, a);
     }
@@ -450,8 +449,8 @@ int launch_screen_col(ssp_ctx *ctx, int N, const ScreenColArgs &a)
         if (N == 512) return launch_screen_col_tma_n<512>(ctx, a);
         if (N == 1024) return launch_screen_col_tma_n<1024>(ctx, a);
     }
-    if (!a.noise && (N < 2048 || !a.old_spec))
-        return ctx->fail(SSP_EUNSUPPORTED, "the seeded generator is built for the evolution at N >= 512 (512 / 1024: spectrum kept in place)");
+    if (!a.noise && N < 2048)
+        return ctx->fail(SSP_EUNSUPPORTED, "the seeded generator is built for N >= 512 (512 / 1024: spectrum kept in place)");
     SSP_DISPATCH_N(N, (launch_screen_col_n<NN>(ctx, a)));
 }
 int row_last_radix(int N)

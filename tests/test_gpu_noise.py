@@ -273,3 +273,31 @@ def test_seeded_evolution_across_generator_chunks(ssp):
         out.append((scr, spec))
     assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1])
     assert float(out[1][0][-1].abs().max()) > 0                # the last chunk was written
+
+
+@pytest.mark.parametrize("N,kind,n_sh,keep", [(512, "vk", 3, True), (1024, "ocean", 2, False), (1024, "vk", 0, True), (2048, "vk", 1, True)])
+def test_seeded_first_synthesis_equals_fill_noise_plus_make(ssp, N, kind, n_sh, keep):
+    """ssp_make_screens_seeded (no noise array at all) against ssp_fill_noise + ssp_make_screens: screens, and the stored
+    spectrum / coefficients when kept, are the same bytes; a seeded evolution on top continues identically."""
+    from paper_2604_07248_b200 import api
+    B, S, dx, lam = 2, 2, 2e-3, 1.0e-6
+    psd = api.PsdParams(kind=api.PSD_VON_KARMAN, L0=10.0, l0=5e-3) if kind == "vk" else \
+        api.PsdParams(kind=api.PSD_OCEAN_NIKISHOV, eps=1e-5, chi_T=1e-7, w=-2.0, eta=1e-3)
+    cn2, dz = [2e-14, 1e-14], [80.0, 120.0]
+    gen = torch.Generator(device="cuda").manual_seed(N)
+    nsh = torch.view_as_complex(torch.randn(B, S, max(n_sh, 1), 3, 3, 2, device="cuda", generator=gen))
+    noise = torch.empty((B, S, N, N), dtype=torch.complex64, device="cuda")
+    ssp.fill_noise(77, 0, noise, first=4 * N)
+    mk = lambda: (torch.zeros((B, S, N, N), dtype=torch.complex64, device="cuda") if keep else None,
+                  torch.zeros((B, S, max(n_sh, 1), 3, 3), dtype=torch.complex64, device="cuda") if keep else None)
+    spec_a, shc_a = mk()
+    spec_b, shc_b = mk()
+    ref = ssp.make_screens(N, dx, psd, lam, cn2, dz, n_sh, noise, nsh, spectrum=spec_a, sh_coef=shc_a)
+    got = ssp.make_screens_seeded(N, dx, psd, lam, cn2, dz, n_sh, 77, 0, 4 * N, B, noise_sh=nsh, spectrum=spec_b, sh_coef=shc_b)
+    assert torch.equal(got, ref)
+    if keep:
+        assert torch.equal(spec_a, spec_b) and torch.equal(shc_a, shc_b)
+        ssp.fill_noise(77, 2, noise)
+        ref = ssp.evolve_screens(N, dx, psd, lam, cn2, dz, n_sh, 0.9, 0.2, 0.1, 1e-2, noise, nsh, spec_a, shc_a)
+        got = ssp.evolve_screens_seeded(N, dx, psd, lam, cn2, dz, n_sh, 0.9, 0.2, 0.1, 1e-2, 77, 2, 0, nsh, spec_b, shc_b)
+        assert torch.equal(got, ref) and torch.equal(spec_a, spec_b)
