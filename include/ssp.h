@@ -20,6 +20,12 @@
  *     and frees them in ssp_destroy.
  *   - Calls enqueue work on the context's stream and return without synchronising,
  *     except the *_host entry points, which synchronise the stream before returning.
+ *   - CUDA graphs: ssp_propagate, ssp_propagate_adjoint and ssp_beam_stats_static may be captured
+ *     (cudaStreamBeginCapture on the context's stream) after ONE call with the same arguments
+ *     outside capture: by then tables, TMA descriptors and the on-chip step list are cached and the
+ *     call issues kernels (and one memset) only.  A first-time call under capture returns
+ *     SSP_EUNSUPPORTED / SSP_ECUDA.  The screen generators upload small tables every call and are
+ *     not capturable.
  *   - Return value: 0 on success, a negative ssp_status otherwise; ssp_last_error gives
  *     the text.  After an error no output buffer is guaranteed.  No exception crosses
  *     the ABI.  A context is not thread-safe.

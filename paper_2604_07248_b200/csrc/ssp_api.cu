@@ -48,7 +48,7 @@ int ssp_destroy(ssp_ctx *ctx)
     if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
     if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
     if (ctx->scratch) cudaFree(ctx->scratch);
-    if (ctx->small_steps) cudaFree(ctx->small_steps);
+    for (auto &e : ctx->small_lists) cudaFree(e.second);
     delete ctx;
     return SSP_OK;
 }
@@ -134,15 +134,33 @@ struct SmallStats { ssp_stats *stats; int lo, hi; long long n; double dx; };
 int run_small(ssp_ctx *ctx, int N, int B, const std::vector<SmallStep> &steps, int n_screens, const RowArgs &win,
               const float2 *in, float2 *out, const float2 *tw, const float2 *twc, const SmallStats *st = nullptr)
 {
-    if (!ctx->small_steps) SSP_CUDA(ctx, cudaMalloc(&ctx->small_steps, kSmallStepBytes));
-    // pageable source: staged before cudaMemcpyAsync returns, so the vector may die afterwards
-    SSP_CUDA(ctx, cudaMemcpyAsync(ctx->small_steps, steps.data(), sizeof(SmallStep) * steps.size(), cudaMemcpyHostToDevice,
-                                  ctx->stream));
+    const size_t nbytes = sizeof(SmallStep) * steps.size();
+    if (nbytes > kSmallStepBytes) return ctx->fail(SSP_EINVAL, "too many steps for the on-chip path");
+    void *d_steps = nullptr;
+    for (auto &e : ctx->small_lists)
+        if (e.first.size() == nbytes && memcmp(e.first.data(), steps.data(), nbytes) == 0) { d_steps = e.second; break; }
+    if (!d_steps) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        SSP_CUDA(ctx, cudaStreamIsCapturing(ctx->stream, &cs));
+        if (cs != cudaStreamCaptureStatusNone)
+            return ctx->fail(SSP_EUNSUPPORTED, "stream capture: run this call once outside capture first (its step list is uploaded then)");
+        if (ctx->small_lists.size() >= 16) {                      // kernels in flight may still read the old lists
+            SSP_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+            for (auto &e : ctx->small_lists) cudaFree(e.second);
+            ctx->small_lists.clear();
+        }
+        SSP_CUDA(ctx, cudaMalloc(&d_steps, nbytes));
+        // pageable source: staged before cudaMemcpyAsync returns, so the vector may die afterwards
+        const cudaError_t ce = cudaMemcpyAsync(d_steps, steps.data(), nbytes, cudaMemcpyHostToDevice, ctx->stream);
+        if (ce != cudaSuccess) { cudaFree(d_steps); SSP_CUDA(ctx, ce); }
+        const unsigned char *pb = reinterpret_cast<const unsigned char *>(steps.data());
+        ctx->small_lists.emplace_back(std::vector<unsigned char>(pb, pb + nbytes), d_steps);
+    }
     SmallArgs a{};
     a.in = in; a.out = out;
     a.n_steps = (int)steps.size() - 1;
     a.n_screens = n_screens;
-    a.steps = reinterpret_cast<const SmallStep *>(ctx->small_steps);
+    a.steps = reinterpret_cast<const SmallStep *>(d_steps);
     a.win_on = win.win_on; a.win_qs = win.win_qs; a.win_half_order = win.win_half_order;
     a.tw_row = tw; a.tw_col = twc;
     if (st && st->stats) { a.stats = st->stats; a.roi_lo = st->lo; a.roi_hi = st->hi; a.roi_n = st->n; a.dx = st->dx; }

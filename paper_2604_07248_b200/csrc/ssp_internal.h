@@ -49,7 +49,9 @@ struct ssp_ctx {
     // TMA descriptors by (base pointer, columns, rows, box): a split step re-launches the column kernel on the same
     // buffers n_steps times, so the host-side encode runs once per buffer and shape; dropped at 256 entries
     std::map<std::tuple<const void *, size_t, size_t, int, int>, CUtensorMap> tmaps;
-    void *small_steps = nullptr;                 // device list of step descriptors of the on-chip path (16 KB)
+    // device lists of step descriptors of the on-chip path, by content: a repeated call re-uses its list without a copy
+    // (so the call can be captured into a CUDA graph once it has run outside capture); dropped at 16 entries
+    std::vector<std::pair<std::vector<unsigned char>, void *>> small_lists;
     // ssp_propagate_host: copy streams and events of the chunked host <-> device pipeline (created on first use)
     cudaStream_t copy_in = nullptr, copy_out = nullptr;
     std::vector<cudaEvent_t> pipe_events;
